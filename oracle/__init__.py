@@ -1,0 +1,32 @@
+"""fp64 CPU oracle for the BiP-PRISM on-atom contraction (arxiv/paper_2607_00756).
+
+TEST INFRASTRUCTURE -- NOT A PRODUCT PATH.  Only ``tests/``, ``__graft_entry__.smoke()``
+and ``bench.py``'s ``cpu_baseline`` / ``--impl reference`` leg may import anything from this
+package.  It shares no code with ``paper_2607_00756_b200/`` (the CUDA path); neither imports
+the other.  The only module both use is ``bip_inputs`` (seeded synthetic problem data).
+
+Everything here is a plain, slow, NumPy complex128 restatement of PAPER.md written to be checked
+against the paper by eye, one function per equation / algorithm step, each citing its passage:
+
+  beams.py       beam sets (eq. 5 / Alg. 4 l.1), probe coefficients (eq. 1), hex-ring parents
+  sibson.py      natural-neighbour weights (eq. 8) by half-plane clipping
+  multislice.py  Fresnel step (eq. 2, 6), S1 build/advance, S2 build/peel (eq. 12), Alg. 1, Alg. 3
+  bip.py         windowed reconstruction (eq. 15, eq. 11), amplitudes (eq. 13-14), output modes (§2.2.6), Alg. 5
+
+Readings of silent / ambiguous points follow SURVEY.md §8(c) and are listed in DESIGN.md §3.
+
+Pins (tests/test_oracle_*.py, all ``-m "not gpu"``):
+  whole forward model  : Alg. 5 with parents = all beams equals Alg. 1 brute force per scan
+  S2                   : reciprocity identity eq. 12 for random w at every plane; peel == rebuild
+  propagation          : Parseval for |T| = 1; vacuum closed form vs library FFT
+  normalisation        : sum |psi_0|^2 = 1 ; all-G detector => I = sum |H psi|^2
+  locality             : eq. 16-18 as equalities, eq. 17 as an inequality, Alg. 3 vs Alg. 2
+  reducers             : sum over q_par of qEELS == map == sum over d of cube
+  weights              : w >= 0, rows sum to 1, delta at parents, linear precision inside the hull, identity limit
+  hex-ring             : n_radial = 4 gives 61 parents from 365 beams (tests/golden/hexring_counts.txt)
+  MAGPHASE             : equals LINEAR for in-phase rows; exact at parents; |R|_MAGPHASE >= |R|_LINEAR
+PARITY UNPINNED: the Sibson weights for beams outside the parents' convex hull (c8) and the
+numerical value of BiP maps at parent factor f > 1 have no printed value in the paper to compare against; they are
+pinned only as "the algorithm as stated" plus their defining properties and the soft trend that the error against
+the f = 1 map falls as parents are added.
+"""

@@ -1,0 +1,177 @@
+"""Pins of hex-ring parent selection, Sibson weights and the magnitude-preserving reconstruction."""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import beams as ob
+from oracle import bip
+from oracle import sibson as osb
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def test_hexring_count_golden():
+    """n_radial = 4 reduces 365 aperture beams to 61 parents."""
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "hexring_counts.txt")) if l.strip() and not l.startswith("#")]
+    for n_radial, n_angular, n_beams, n_par in (tuple(map(int, r)) for r in rows):
+        b = ob.beams_in_disc(64, 64, 1.0, 1.0, 10.78)          # 365 lattice points with |h|^2 <= 116
+        assert b.shape[0] == n_beams
+        p = ob.hexring_parents(b, 64, 64, 1.0, 1.0, 10.78, n_radial, n_angular)
+        assert p.shape[0] == n_par == 1 + n_angular * n_radial * (n_radial + 1) // 2
+        assert np.all(np.diff(p) > 0)
+        assert any((b[i] == (0, 0)).all() for i in p)          # DC beam is a parent
+
+
+def test_hexring_geometry():
+    b = ob.beams_in_disc(64, 64, 1.0, 1.0, 10.78)
+    p = ob.hexring_parents(b, 64, 64, 1.0, 1.0, 10.78, 2)
+    hp = {tuple(h) for h in b[p]}
+    # ring 1 at |q| = 5.39, six samples from +x: (0, 5) and (0, -5) in (hy, hx); ring 2 at 10.78: (0, +-10)... snapped
+    assert (0, 5) in hp and (0, -5) in hp
+    assert (5, 3) in hp          # 60 degrees: (x, y) = (2.695, 4.668) -> (hx, hy) = (3, 5)
+    r = np.sqrt((b[p] ** 2).sum(1))
+    assert sorted(np.round(r).astype(int).tolist()).count(0) == 1
+
+
+def _grid_parents(n=5):
+    ys, xs = np.meshgrid(np.arange(n), np.arange(n), indexing="ij")
+    return np.stack([ys.ravel(), xs.ravel()], 1).astype(float)
+
+
+def test_sibson_symmetric_closed_forms():
+    P = _grid_parents(5)
+    idx, w = osb.sibson_row(np.array([2.5, 2.5]), P, 1.0)      # centre of a lattice square: 1/4 on each corner
+    assert len(idx) == 4 and np.allclose(w, 0.25, atol=1e-12)
+    idx, w = osb.sibson_row(np.array([2.0, 2.0]), P, 1.0)      # on a parent: delta
+    assert list(idx) == [12] and w[0] == 1.0
+    # mid-edge of a unit square lattice: closed form from the area-stealing construction.
+    # C(x) for x = (2, 2.5) is the hexagon with vertices (2 +- 1/2 -+ ... ) -- check by symmetry + partition of unity:
+    idx, w = osb.sibson_row(np.array([2.0, 2.5]), P, 1.0)
+    d = dict(zip(idx.tolist(), w.tolist()))
+    assert abs(d[12] - d[13]) < 1e-12                          # the two edge endpoints
+    assert abs(d[7] - d[17]) < 1e-12 and abs(d[8] - d[18]) < 1e-12 and abs(d[7] - d[8]) < 1e-12
+    assert abs(sum(w) - 1) < 1e-12 and d[12] > d[7] > 0
+
+
+def test_sibson_vs_discrete_brute_force():
+    """Brute force on a tiny input: rasterise the plane, count pixels whose nearest site changes to x."""
+    rng = np.random.default_rng(11)
+    P = rng.uniform(-1, 1, (12, 2))
+    P = np.concatenate([P, 3.0 * np.array([[np.cos(t), np.sin(t)] for t in np.linspace(0, 2 * np.pi, 9)[:-1]])])
+    x = np.array([0.1, -0.05])
+    idx, w = osb.sibson_row(x, P, 1.0)
+    g = np.linspace(-3, 3, 1501)
+    Y, X = np.meshgrid(g, g, indexing="ij")
+    pts = np.stack([Y.ravel(), X.ravel()], 1)
+    d2 = ((pts[:, None, :] - P[None, :, :]) ** 2).sum(-1)
+    owner = d2.argmin(1)
+    stolen = ((pts - x) ** 2).sum(1) < d2.min(1)
+    counts = np.bincount(owner[stolen], minlength=len(P)).astype(float)
+    wd = counts / counts.sum()
+    dense = np.zeros(len(P)); dense[idx] = w
+    assert np.abs(dense - wd).max() < 5e-3
+    assert set(np.nonzero(wd > 5e-3)[0]) <= set(idx.tolist())
+
+
+@pytest.fixture(scope="module")
+def cfg1_tables():
+    from bip_inputs import electron_wavelength
+    lam = electron_wavelength(200.0)
+    L, N = 15.62, 128
+    qa = 20e-3 / lam
+    ap = ob.beams_in_disc(N, N, L, L, qa)
+    n1 = ob.n_radial_from_factor(ap.shape[0], 2.0)
+    p1 = ob.hexring_parents(ap, N, N, L, L, qa, n1)
+    tab = osb.natural_neighbour_weights(ap, p1, L, L, qa)
+    return ap, p1, tab, L, qa
+
+
+def test_weight_table_properties(cfg1_tables):
+    """w >= 0, rows sum to 1, delta at parents, local support, linear precision inside the hull."""
+    ap, p1, tab, L, qa = cfg1_tables
+    assert ap.shape[0] == 489 and p1.shape[0] == 127           # SURVEY §8 size table, cfg 1
+    Wd = osb.to_dense(tab, len(p1))
+    assert Wd.min() >= 0.0
+    assert np.abs(Wd.sum(1) - 1).max() < 1e-14
+    for k, b in enumerate(p1):                                  # exact at the parents
+        assert Wd[b, k] == 1.0 and Wd[b].sum() == 1.0
+    assert max(len(i) for i, _ in tab) <= 8
+    q = ap / L
+    pq = q[p1]
+    from scipy.spatial import ConvexHull
+    hull = ConvexHull(pq)
+    # strictly inside the parents' convex hull (a beam ON a hull edge has an unbounded cell, clipped by the c8 box)
+    inside = -(hull.equations[:, :2] @ q.T + hull.equations[:, 2:3]).max(0) > 1e-9
+    # local support ("nonzero only for parents surrounding h_b"): every neighbour of an interior beam lies within
+    # 2.5 parent spacings; a hull-exterior beam reaches the two ends of its hull edge (< 4 spacings)
+    spacing = qa / 6
+    for b, (idx, w) in enumerate(tab):
+        assert np.all(np.linalg.norm(pq[idx] - q[b], axis=1) < (2.5 if inside[b] else 4.0) * spacing)
+    # Sibson's local-coordinates property: sum_p w_p h_p = h_b for beams inside the parents' convex hull
+    err = np.abs(Wd @ pq - q).max(1)
+    assert inside.sum() > 400
+    assert err[inside].max() < 1e-12
+    # hull-exterior beams: weights still a partition of unity on hull parents, projection error small
+    assert err[~inside].max() < 0.25 * spacing
+
+
+def test_identity_limit():
+    b = ob.beams_in_disc(32, 32, 1.0, 1.0, 4.2)
+    tab = osb.natural_neighbour_weights(b, np.arange(len(b)), 1.0, 1.0, 4.2)
+    assert np.array_equal(osb.to_dense(tab, len(b)), np.eye(len(b)))
+
+
+def test_magphase_properties():
+    """eq. 11: equals LINEAR when the de-tilted parents of a row are in phase; exact at parents;
+    |R|_MAGPHASE >= |R|_LINEAR pointwise."""
+    rng = np.random.default_rng(5)
+    ny = nx = 16
+    b = ob.beams_in_disc(ny, nx, 1.0, 1.0, 3.3)
+    p = ob.hexring_parents(b, ny, nx, 1.0, 1.0, 3.3, 2)
+    Wd = osb.to_dense(osb.natural_neighbour_weights(b, p, 1.0, 1.0, 3.3), len(p))
+    S = rng.normal(size=(len(p), ny, nx)) + 1j * rng.normal(size=(len(p), ny, nx))
+    args = (b[p], b, Wd, (3, 14), 8, ny, nx, +1)
+    Rl = bip.reconstruct_window(S, *args, "linear")
+    Rm = bip.reconstruct_window(S, *args, "magphase")
+    assert np.all(np.abs(Rm) >= np.abs(Rl) * (1 - 1e-12))
+    assert np.abs(Rm[p] - Rl[p]).max() < 1e-12                 # exact at parents
+    ys, xs = bip.window_pixels((3, 14), 8, ny, nx)
+    assert np.abs(Rl[p] - S[:, ys][:, :, xs].reshape(len(p), -1)).max() < 1e-12
+    # in-phase parents: S_p = (positive magnitude) * common phase field * carrier
+    common = np.exp(1j * rng.uniform(0, 6, (ny, nx)))
+    from oracle import multislice as ms
+    S2 = np.stack([rng.uniform(0.5, 2.0, (ny, nx)) * common * ms.plane_wave(h, ny, nx, +1) for h in b[p]])
+    assert np.abs(bip.reconstruct_window(S2, *args, "magphase") - bip.reconstruct_window(S2, *args, "linear")).max() < 1e-12
+    # conjugate convention (DESIGN c18): reconstructing conj(S) with carrier -1 is the conjugate of carrier +1
+    Rc = bip.reconstruct_window(np.conj(S), b[p], b, Wd, (3, 14), 8, ny, nx, -1, "magphase")
+    assert np.abs(Rc - np.conj(Rm)).max() < 1e-12
+
+
+def test_carrier_sign_reading_c18_vacuum():
+    """DESIGN reading c18: de-tilt must REMOVE the carrier.  In vacuum the S2 columns are
+    exp(-2 pi i h.r/N) P(q)^n exactly, so the carrier-removing sign (-1 for the bilinear S2 of eq. 12 / SURVEY c1)
+    reconstructs every detector column from a sparse parent set to interpolation accuracy, while the other sign
+    (eq. 15's phases applied to this S2 without conjugating them) does not reconstruct it at all."""
+    from oracle import multislice as ms
+    ny = nx = 32
+    L, lam, dz, nzv = 8.0, 0.025, 2.0, 3
+    qd = 1.0
+    det = ob.beams_in_disc(ny, nx, L, L, qd)
+    par = ob.hexring_parents(det, ny, nx, L, L, qd, 3)
+    Wd = osb.to_dense(osb.natural_neighbour_weights(det, par, L, L, qd), len(par))
+    P = ms.fresnel_propagator(ny, nx, L, L, lam, dz)
+    Tv = np.ones((nzv, ny, nx), complex)
+    S_all = ms.build_S2(det, Tv, P)
+    # closed form of the vacuum column
+    k = len(det) // 3
+    h = det[k]
+    assert np.abs(S_all[k] - ms.plane_wave(h, ny, nx, -1) * P[h[0] % ny, h[1] % nx] ** nzv).max() < 1e-12
+    S_par = S_all[par]
+    ys, xs = bip.window_pixels((5, 9), 8, ny, nx)
+    truth = S_all[:, ys][:, :, xs].reshape(len(det), -1)
+    good = bip.reconstruct_window(S_par, det[par], det, Wd, (5, 9), 8, ny, nx, -1, "linear")
+    bad = bip.reconstruct_window(S_par, det[par], det, Wd, (5, 9), 8, ny, nx, +1, "linear")
+    rel = lambda R: np.linalg.norm(R - truth) / np.linalg.norm(truth)
+    assert rel(good) < 0.05
+    assert rel(bad) > 0.5
