@@ -1,0 +1,223 @@
+/*
+ * bip.h -- C ABI of libbip: the on-atom contraction of BiP-PRISM (arxiv/paper_2607_00756) on one B200.
+ *
+ * The library computes Algorithm 5 of the paper ("BiP-PRISM EELS map"): the probe-forming
+ * scattering matrix S1 and the adjoint detector matrix S2 are held on sparse parent beams, advanced / peeled
+ * plane by plane (eq. 6, eq. 12), and for every ionised atom both are reconstructed on the W x W window
+ * Omega_tau by natural-neighbour weights (eq. 15, or the magnitude-preserving eq. 11), combined with the
+ * illumination coefficients c_b(rho) into the probe at the atom (eq. 7), multiplied by the transition potentials
+ * H_n (eq. 3), projected on S2 (eq. 13) and reduced over detector beams into an elemental map, qEELS bins or the
+ * energy-filtered 4D cube (eq. 14, section 2.2.6).
+ *
+ * Conventions (DESIGN.md section 3 lists every reading of the paper):
+ *   - pixel r = (ry, rx), beam h = (hy, hx) signed integer index on the corner-origin DFT grid, |h| < N/2;
+ *     h.r/N = hy ry / ny + hx rx / nx.  All [.][2] arrays are (y, x).
+ *   - complex data is interleaved (re, im); "c64" = two floats.
+ *   - the DFT is unitary: a_d = G^-1/2 sum_r S2^d(r) H psi.
+ *   - every function returns a bip_status; nothing throws across the ABI.  Arguments are validated on the host
+ *     before any launch.  bip_last_error() returns a NUL-terminated description of the last failure on that
+ *     context (or of the last failed bip_create / helper call on this thread when ctx == NULL).
+ *   - pointers are HOST pointers unless the name ends in _dev.  The library copies every host array it is
+ *     given before returning; device buffers passed in are borrowed (never freed) and must stay valid as stated.
+ *   - one context per host thread; all device work is enqueued on the CUDA stream given to bip_create
+ *     (a cudaStream_t passed as void*; NULL = the legacy default stream).  Calls return after enqueueing unless
+ *     stated otherwise; the caller synchronises the stream before reading device outputs.
+ *   - there is NO CPU fallback: every entry point that touches a scattering matrix or an output needs a CUDA
+ *     device of compute capability 10.x and fails with BIP_ERR_CUDA otherwise.
+ */
+#ifndef BIP_H_
+#define BIP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define BIP_API __attribute__((visibility("default")))
+#else
+#define BIP_API
+#endif
+
+typedef enum {
+  BIP_OK = 0,
+  BIP_ERR_INVALID = 1,      /* NULL pointer, bad shape, value out of range                        */
+  BIP_ERR_STATE = 2,        /* call order (e.g. bip_map before bip_build_S1 / S2 / bip_set_scan)  */
+  BIP_ERR_OOM = 3,          /* device or host allocation failed; message states the bytes asked   */
+  BIP_ERR_CUDA = 4,         /* CUDA / cuFFT error, or no sm_100 device                            */
+  BIP_ERR_UNSUPPORTED = 5   /* valid request the build cannot serve                               */
+} bip_status;
+
+typedef enum { BIP_MODE_MAP = 0, BIP_MODE_QEELS_X = 1, BIP_MODE_QEELS_Y = 2, BIP_MODE_CUBE = 3 } bip_mode;
+typedef enum { BIP_RECON_LINEAR = 0, BIP_RECON_MAGPHASE = 1 } bip_recon;
+/* Arithmetic of the two contractions.  TF32X3: tcgen05 tensor cores, every real product as the three-term
+ * split a_hi b_hi + a_hi b_lo + a_lo b_hi of TF32 operands with fp32 accumulation in TMEM (fp32-equivalent).
+ * FP32_SIMT: the same contractions on CUDA cores in fp32 -- the A/B reference for the tensor-core kernels. */
+typedef enum { BIP_PREC_TF32X3 = 0, BIP_PREC_FP32_SIMT = 1 } bip_precision;
+
+typedef struct bip_ctx bip_ctx;
+
+/* Real-space grid, cell and slicing. lengths in Angstrom. */
+typedef struct {
+  int32_t ny, nx;     /* pixels                                     */
+  double ly, lx;      /* field of view                              */
+  int32_t nz;         /* number of slices                           */
+  double dz;          /* slice thickness                            */
+  double lambda;      /* electron wavelength                        */
+} bip_grid;
+
+/* A natural-neighbour weight table in ELL form (eq. 8): row b lists the parents
+ * surrounding beam b. nn_idx[b][j] is a parent NUMBER (position in the parent list) or -1 for padding;
+ * nn_w[b][j] >= 0 and each row sums to 1 (+-1e-5, validated). */
+typedef struct {
+  int32_t n_rows;          /* number of beams being reconstructed            */
+  int32_t max_nn;          /* row width, 1..BIP_MAX_NN                       */
+  const int32_t* nn_idx;   /* [n_rows][max_nn]                               */
+  const float* nn_w;       /* [n_rows][max_nn]                               */
+} bip_weights;
+
+#define BIP_MAX_NN 16
+
+/* Event timings of the last bip_map in milliseconds, and of the builds. */
+typedef struct {
+  float build_s1_ms;       /* bip_build_S1                                              */
+  float build_s2_ms;       /* bip_build_S2 (adjoint multislice from the exit surface)   */
+  float advance_peel_ms;   /* S1.ADVANCETO + S2.PEELTO inside the last bip_map          */
+  float contract_ms;       /* steps a1-a8 (crop .. reduce) inside the last bip_map      */
+  float gemm2_ms;          /* the detector projection kernel alone (dominant kernel)    */
+  int32_t gemm2_launches;  /* launches of that kernel in the last bip_map               */
+  int32_t kernel_launches; /* all of the library's own kernel launches in the last bip_map (cuFFT excluded) */
+  double amplitudes;       /* scan x atom x channel x detector-beam amplitudes formed   */
+  double flops;            /* algorithmic real flops of a4 + a7: 8 N_rho W^2 (atoms B + events K) */
+} bip_timing;
+
+/* ------------------------------------------------------------------------------------------------------------
+ * Geometry helpers (host only, no device needed).  They implement the readings of SURVEY.md 8(c) c5-c8.
+ * ---------------------------------------------------------------------------------------------------------- */
+
+/* Beams with |h| < N/2 and (hy/ly)^2 + (hx/lx)^2 <= qmax^2 in ascending flat corner-origin index
+ * (hy mod ny) * nx + (hx mod nx)  (eq. 5; Alg. 4 line 1).
+ * h_out [cap][2]; *n_out receives the count even when cap is too small (then BIP_ERR_INVALID). */
+BIP_API int32_t bip_beams_in_disc(const bip_grid* g, double qmax, int32_t* h_out, int32_t cap, int32_t* n_out);
+
+/* Probe coefficients c_b = exp(-i pi lambda defocus |q_b|^2) / sqrt(G n) (eq. 1), c_out [n][2]. */
+BIP_API int32_t bip_aperture_coeffs(const bip_grid* g, int32_t n, const int32_t* h, double defocus, float* c_out);
+
+/* Hex-ring parent selection: DC + n_radial rings at |q| = k qmax / n_radial with n_angular k
+ * samples from +x, snapped to the nearest beam of h[n][2] (ties: lowest flat index), deduplicated.
+ * pos_out [cap] receives ascending positions into h; *n_out the count. */
+BIP_API int32_t bip_hexring(const bip_grid* g, int32_t n, const int32_t* h, double qmax, int32_t n_radial,
+                    int32_t n_angular, int32_t* pos_out, int32_t cap, int32_t* n_out);
+
+/* n_radial = max(1, round(sqrt(n_beams / pi) / factor)) (parent spacing "factor" in beam pixels). */
+BIP_API int32_t bip_n_radial_from_factor(int32_t n_beams, double factor);
+
+/* Sibson natural-neighbour weights (eq. 8) of every beam h[n][2] on the parents parent_h[n_parent][2], in
+ * physical q coordinates, cells clipped to |q| <= 1024 qmax, delta on a parent, weights < 1e-12 dropped and the
+ * row renormalised; row entries in ascending parent number, padded with (-1, 0).
+ * nn_idx_out / nn_w_out [n][max_nn].  Fails with BIP_ERR_INVALID if a row needs more than max_nn entries. */
+BIP_API int32_t bip_sibson(const bip_grid* g, int32_t n, const int32_t* h, int32_t n_parent, const int32_t* parent_h,
+                   double qmax, int32_t max_nn, int32_t* nn_idx_out, float* nn_w_out);
+
+/* ------------------------------------------------------------------------------------------------------------
+ * Context
+ * ---------------------------------------------------------------------------------------------------------- */
+
+/* Create a context (Alg. 5 "Require").
+ *   T          transmission functions T_j = exp(i sigma V_j), c64 [nz][ny][nx].
+ *              T_on_device != 0: a device pointer, borrowed for the lifetime of the context.
+ *              T_on_device == 0: a host pointer, copied to a device buffer the context owns.
+ *   n_ap, ap_h, ap_c   aperture beams h_b [n_ap][2] and coefficients c_b [n_ap][2] (eq. 1).
+ *   n_p1, p1_h         S1 parent beams [n_p1][2] (any beams, normally a hex-ring subset of the aperture).
+ *   w1                 weights of every aperture beam on the S1 parents (n_rows == n_ap).
+ *   n_p2, p2_h         S2 parent (detector-side) beams [n_p2][2].
+ *   stream             cudaStream_t as void*.
+ * The context allocates and owns S1 (n_p1 columns) and S2 (n_p2 columns), c64 [.][ny][nx] each. */
+BIP_API int32_t bip_create(bip_ctx** out, const bip_grid* g, const void* T, int32_t T_on_device,
+                   int32_t n_ap, const int32_t* ap_h, const float* ap_c,
+                   int32_t n_p1, const int32_t* p1_h, const bip_weights* w1,
+                   int32_t n_p2, const int32_t* p2_h, void* stream);
+
+BIP_API int32_t bip_destroy(bip_ctx* ctx);
+
+BIP_API const char* bip_last_error(const bip_ctx* ctx);
+
+/* S1 parents <- unit plane waves exp(+2 pi i h_p.r/N) at plane 0 (Alg. 3 line 3). */
+BIP_API int32_t bip_build_S1(bip_ctx* ctx);
+
+/* S2 parents <- exp(-2 pi i h_p.r/N) at the exit surface, then u <- T_j . P[u] for j = nz-1 .. 0 (eq. 12,
+ * PAPER.md:209-212): the adjoint detector columns at plane 0.  cuFFT; timed separately (bip_get_timing). */
+BIP_API int32_t bip_build_S2(bip_ctx* ctx);
+
+/* Scan positions rho [n_rho][2] in pixels, any real value.  Builds the illumination matrix
+ * c_b(rho) = c_b exp(-2 pi i h_b.rho/N) on the device. */
+BIP_API int32_t bip_set_scan(bip_ctx* ctx, int32_t n_rho, const double* rho_px);
+
+/* Register an ionisation edge: its sites, transition-potential windows and detector.
+ *   slice [n_atoms]        slice index i(tau) of each site, 0 <= slice < nz
+ *   centre_px [n_atoms][2] pixel the atom sits on; the window covers centre - w/2 .. centre + w/2 - 1 (periodic)
+ *   H  c64 [n_ch][w][w]    H[n][w/2][w/2] is on the atom's pixel; w even, 8 <= w <= min(ny, nx)
+ *   det_h [n_det][2]       detector beams (eq. 5)
+ *   w2                     weights of every detector beam on the context's S2 parents (n_rows == n_det)
+ * Several edges share S1 / S2 and one plane loop.  *edge_id receives 0, 1, ... */
+BIP_API int32_t bip_add_edge(bip_ctx* ctx, int32_t n_atoms, const int32_t* slice, const int32_t* centre_px,
+                     int32_t n_ch, int32_t w, const float* H, int32_t n_det, const int32_t* det_h,
+                     const bip_weights* w2, int32_t* edge_id);
+
+/* Drop all registered edges (the scattering matrices and scan stay). */
+BIP_API int32_t bip_clear_edges(bip_ctx* ctx);
+
+/* Number of output elements of an edge in a mode: MAP n_rho (double), QEELS n_rho * n_bins (float),
+ * CUBE n_rho * n_det (float); *n_bins = distinct h_x (QEELS_X) / h_y (QEELS_Y) of the detector, ascending. */
+BIP_API int32_t bip_output_size(const bip_ctx* ctx, int32_t edge_id, int32_t mode, int64_t* n_elems, int32_t* n_bins);
+
+/* Run Algorithm 5 for one edge (edge_id >= 0): for every plane holding >= 1 site, in increasing depth,
+ * S1.ADVANCETO / S2.PEELTO (the plane cursor is moved from wherever the last call left it; both multislice
+ * steps are unitary and are undone exactly when the cursor has to move back) and the on-atom contraction of
+ * every site and channel, accumulated into out.
+ *   out_dev   MAP: double [n_rho];  QEELS_*: float [n_rho][n_bins];  CUBE: float [n_rho][n_det]
+ *             (detector-set order).  Zero-initialised by the call.  out_bytes must match bip_output_size.
+ * Returns after enqueueing on the context's stream. */
+BIP_API int32_t bip_map(bip_ctx* ctx, int32_t edge_id, int32_t mode, int32_t recon, int32_t precision,
+                void* out_dev, size_t out_bytes);
+
+/* As bip_map with a HOST output buffer: device scratch is allocated, the result copied back and the stream
+ * synchronised before returning. */
+BIP_API int32_t bip_map_host(bip_ctx* ctx, int32_t edge_id, int32_t mode, int32_t recon, int32_t precision,
+                     void* out_host, size_t out_bytes);
+
+/* Run all registered edges in ONE plane loop (multi-edge batching): outs_dev[e] / outs_bytes[e]
+ * per edge, same layout as bip_map. */
+BIP_API int32_t bip_map_all(bip_ctx* ctx, int32_t mode, int32_t recon, int32_t precision,
+                    void* const* outs_dev, const size_t* outs_bytes, int32_t n_outs);
+
+/* Window origins (centre - w/2) mod N of an edge's atoms, int32 [n_atoms][2] -- for bit-exact index checks. */
+BIP_API int32_t bip_get_windows(const bip_ctx* ctx, int32_t edge_id, int32_t* origin_out);
+
+/* qEELS bin values (signed beam index along the resolved axis, ascending), int32 [n_bins]. */
+BIP_API int32_t bip_get_qeels_bins(const bip_ctx* ctx, int32_t edge_id, int32_t mode, int32_t* bins_out);
+
+/* Move the plane cursor: S1 advanced / S2 peeled so that both sit at ionisation plane `plane` (0..nz): S1 holds
+ * slices 0..plane-1, S2 holds slices plane..nz-1.  Moving back applies the inverse steps (|T| = 1, |P| = 1). */
+BIP_API int32_t bip_seek_plane(bip_ctx* ctx, int32_t plane);
+
+/* Copy parent columns [p0, p0 + np) of S1 (which = 1) or S2 (which = 2) at the current plane to host,
+ * c64 [np][ny][nx]; synchronises the stream. */
+BIP_API int32_t bip_copy_S(bip_ctx* ctx, int32_t which, int32_t p0, int32_t np, void* out_host);
+
+/* Reconstructed windows of one atom at the current plane, for parity of steps a1-a2 / a6:
+ * which = 1: S1^b|Omega c64 [n_ap][w*w]; which = 2: S2^d|Omega c64 [n_det][w*w].  Host output; synchronises. */
+BIP_API int32_t bip_debug_reconstruct(bip_ctx* ctx, int32_t edge_id, int32_t atom, int32_t which, int32_t recon,
+                              void* out_host);
+
+BIP_API int32_t bip_get_timing(const bip_ctx* ctx, bip_timing* out);
+
+/* Library / device description ("libbip <version>; device <name> sm_XY; SMs n"); never NULL. */
+BIP_API const char* bip_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BIP_H_ */

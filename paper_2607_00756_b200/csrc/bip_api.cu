@@ -1,0 +1,595 @@
+// C ABI of libbip (include/bip.h) and the plane-loop driver of Algorithm 5.
+#include <algorithm>
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <map>
+#include <mutex>
+
+#include "bip_internal.h"
+
+namespace bip {
+
+void ms_release(bip_ctx* ctx);
+
+static thread_local std::string g_err;
+
+int32_t fail(bip_ctx* ctx, int32_t status, const char* fmt, ...) {
+  char buf[1024];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  if (ctx) ctx->err = buf;
+  g_err = buf;
+  return status;
+}
+
+int32_t dev_alloc(bip_ctx* ctx, void** p, size_t bytes, const char* what) {
+  *p = nullptr;
+  if (bytes == 0) bytes = 16;
+  cudaError_t e = cudaMalloc(p, bytes);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    return fail(ctx, e == cudaErrorMemoryAllocation ? BIP_ERR_OOM : BIP_ERR_CUDA, "cudaMalloc of %zu bytes for %s failed: %s",
+                bytes, what, cudaGetErrorString(e));
+  }
+  return BIP_OK;
+}
+
+int32_t ensure(bip_ctx* ctx, DevBuf& b, size_t bytes, const char* what) {
+  if (b.bytes >= bytes && b.p) return BIP_OK;
+  if (b.p) { cudaStreamSynchronize(ctx->stream); cudaFree(b.p); b.p = nullptr; b.bytes = 0; }
+  BIP_TRY(dev_alloc(ctx, &b.p, bytes, what));
+  b.bytes = bytes;
+  return BIP_OK;
+}
+
+static inline int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
+
+// Carve four planes [batch][rows][ld] out of one DevBuf (zero-filled when (re)allocated or when `zero`).
+// The kernels that fill the planes write only the valid columns; the padding up to `ld` must read as zero, so the
+// buffer is cleared whenever its layout (rows, cols, batch) changes.
+static int32_t planes_in(bip_ctx* ctx, DevBuf& buf, Planes& P, int64_t rows, int64_t cols, int64_t batch, const char* what) {
+  P.rows = rows;
+  P.ld = round_up(cols, 32);
+  P.batch_stride = rows * P.ld;
+  const int64_t plane_floats = round_up(P.batch_stride * batch, 256);   // keep plane bases 1024 B aligned
+  const void* before = buf.p;
+  BIP_TRY(ensure(ctx, buf, (size_t)plane_floats * 4 * sizeof(float), what));
+  const uint64_t sig = ((uint64_t)rows * 1000003ull + (uint64_t)cols) * 1000003ull + (uint64_t)batch;
+  if (buf.p != before || buf.sig != sig) {
+    if (P.ld != cols || buf.p != before) BIP_CUDA(ctx, cudaMemsetAsync(buf.p, 0, buf.bytes, ctx->stream));
+    buf.sig = sig;
+  }
+  for (int k = 0; k < 4; ++k) P.p[k] = reinterpret_cast<float*>(buf.p) + k * plane_floats;
+  return BIP_OK;
+}
+
+template <class T>
+static int32_t upload(bip_ctx* ctx, T** dst, const T* src, size_t n, const char* what) {
+  BIP_TRY(dev_alloc(ctx, (void**)dst, n * sizeof(T), what));
+  BIP_CUDA(ctx, cudaMemcpyAsync(*dst, src, n * sizeof(T), cudaMemcpyHostToDevice, ctx->stream));
+  return BIP_OK;
+}
+
+static int32_t check_weights(bip_ctx* ctx, const bip_weights* w, int32_t n_rows, int32_t n_parent, const char* what) {
+  if (!w || !w->nn_idx || !w->nn_w) return fail(ctx, BIP_ERR_INVALID, "%s: weight table is NULL", what);
+  if (w->n_rows != n_rows) return fail(ctx, BIP_ERR_INVALID, "%s: weight table has %d rows, expected %d", what, w->n_rows, n_rows);
+  if (w->max_nn < 1 || w->max_nn > BIP_MAX_NN) return fail(ctx, BIP_ERR_INVALID, "%s: max_nn %d outside 1..%d", what, w->max_nn, BIP_MAX_NN);
+  for (int32_t b = 0; b < n_rows; ++b) {
+    double s = 0;
+    bool ended = false;
+    for (int j = 0; j < w->max_nn; ++j) {
+      const int32_t p = w->nn_idx[(size_t)b * w->max_nn + j];
+      const float v = w->nn_w[(size_t)b * w->max_nn + j];
+      if (p < 0) { ended = true; continue; }
+      if (ended) return fail(ctx, BIP_ERR_INVALID, "%s: row %d has an entry after the -1 padding", what, b);
+      if (p >= n_parent) return fail(ctx, BIP_ERR_INVALID, "%s: row %d names parent %d >= %d", what, b, p, n_parent);
+      if (!(v >= 0.f)) return fail(ctx, BIP_ERR_INVALID, "%s: row %d has a negative or NaN weight", what, b);
+      s += v;
+    }
+    if (std::fabs(s - 1.0) > 1e-5) return fail(ctx, BIP_ERR_INVALID, "%s: row %d sums to %.8f, not 1", what, b, s);
+  }
+  return BIP_OK;
+}
+
+static int32_t check_beams(bip_ctx* ctx, const bip_grid& g, int32_t n, const int32_t* h, const char* what) {
+  if (n <= 0 || !h) return fail(ctx, BIP_ERR_INVALID, "%s: empty beam list", what);
+  for (int32_t i = 0; i < n; ++i)
+    if (2 * std::abs(h[2 * i]) >= g.ny || 2 * std::abs(h[2 * i + 1]) >= g.nx)
+      return fail(ctx, BIP_ERR_INVALID, "%s: beam %d = (%d, %d) violates |h| < N/2", what, i, h[2 * i], h[2 * i + 1]);
+  return BIP_OK;
+}
+
+struct EventPool {
+  std::vector<cudaEvent_t> all;
+  size_t used = 0;
+  cudaEvent_t get() {
+    if (used == all.size()) { cudaEvent_t e; cudaEventCreate(&e); all.push_back(e); }
+    return all[used++];
+  }
+  void reset() { used = 0; }
+  void destroy() { for (auto e : all) cudaEventDestroy(e); all.clear(); used = 0; }
+};
+
+struct Spans {
+  EventPool pool_map, pool_b1, pool_b2;
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> adv, contract, gemm2, build1, build2;
+};
+static std::map<const bip_ctx*, Spans>& spans() { static std::map<const bip_ctx*, Spans> m; return m; }
+
+struct Span {
+  bip_ctx* ctx; std::vector<std::pair<cudaEvent_t, cudaEvent_t>>* v; cudaEvent_t a, b;
+  Span(bip_ctx* c, EventPool& pool, std::vector<std::pair<cudaEvent_t, cudaEvent_t>>& vec) : ctx(c), v(&vec) {
+    a = pool.get(); b = pool.get(); cudaEventRecord(a, c->stream);
+  }
+  ~Span() { cudaEventRecord(b, ctx->stream); v->push_back({a, b}); }
+};
+
+static float sum_ms(std::vector<std::pair<cudaEvent_t, cudaEvent_t>>& v) {
+  float t = 0;
+  for (auto& p : v) { float ms = 0; if (cudaEventElapsedTime(&ms, p.first, p.second) == cudaSuccess) t += ms; }
+  return t;
+}
+
+static int32_t seek(bip_ctx* ctx, int32_t plane) {
+  if (!ctx->s1_built || !ctx->s2_built) return fail(ctx, BIP_ERR_STATE, "bip_build_S1 and bip_build_S2 must run before the plane loop");
+  if (plane < 0 || plane > ctx->g.nz) return fail(ctx, BIP_ERR_INVALID, "plane %d outside 0..%d", plane, ctx->g.nz);
+  while (ctx->plane1 < plane) { BIP_TRY(ms_step_S1(ctx, ctx->plane1, +1)); ctx->plane1++; }
+  while (ctx->plane1 > plane) { ctx->plane1--; BIP_TRY(ms_step_S1(ctx, ctx->plane1, -1)); }
+  while (ctx->plane2 < plane) { BIP_TRY(ms_step_S2(ctx, ctx->plane2, +1)); ctx->plane2++; }
+  while (ctx->plane2 > plane) { ctx->plane2--; BIP_TRY(ms_step_S2(ctx, ctx->plane2, -1)); }
+  return BIP_OK;
+}
+
+struct EdgeDev { int32_t* origin_dev = nullptr; };
+static std::map<const bip_ctx*, std::vector<EdgeDev>>& edge_dev() { static std::map<const bip_ctx*, std::vector<EdgeDev>> m; return m; }
+
+static size_t scratch_budget() {
+  const char* e = std::getenv("BIP_SCRATCH_GB");
+  double gb = e ? std::atof(e) : 12.0;
+  if (!(gb > 0.05)) gb = 0.05;
+  return (size_t)(gb * (double)(1ull << 30));
+}
+
+// Steps a1-a8 for atoms [a0, a0 + nb) of one edge, all sitting in the current plane.
+static int32_t contract_batch(bip_ctx* ctx, Edge& e, const int32_t* origin_dev, int32_t a0, int32_t nb, int mode, int recon,
+                              int precision, void* out) {
+  auto& sp = spans()[ctx];
+  const int w2 = e.w * e.w;
+  const int32_t* org = origin_dev + 2 * (int64_t)a0;
+  Planes R1t, R2, Phi;
+  BIP_TRY(ensure(ctx, ctx->D1, (size_t)nb * ctx->n_p1 * w2 * sizeof(float2), "D1 (de-tilted S1 windows)"));
+  BIP_TRY(ensure(ctx, ctx->D2, (size_t)nb * ctx->n_p2 * w2 * sizeof(float2), "D2 (de-tilted S2 windows)"));
+  BIP_TRY(planes_in(ctx, ctx->R1, R1t, w2, ctx->n_ap, nb, "R1 (reconstructed S1 windows)"));
+  BIP_TRY(planes_in(ctx, ctx->R2, R2, e.n_det, w2, nb, "R2 (reconstructed S2 windows)"));
+  const int64_t rho_rows = ctx->n_rho;
+  BIP_TRY(planes_in(ctx, ctx->Phi, Phi, rho_rows * e.n_ch, w2, nb, "Phi (H_n psi)"));
+
+  // a1-a2: S1 windows -> R1^T[s][b]
+  BIP_TRY(launch_crop_detilt(ctx, ctx->S1, ctx->p1_h_dev, ctx->n_p1, +1, org, nb, e.w, (float2*)ctx->D1.p));
+  BIP_TRY(launch_recon(ctx, (const float2*)ctx->D1.p, ctx->n_p1, ctx->ap_h_dev, ctx->n_ap, ctx->w1_idx_dev, ctx->w1_w_dev,
+                       ctx->nn1, +1, recon, org, nb, e.w, /*transpose=*/true, R1t));
+  // a3-a5: probe at the atom, times H_n
+  Gemm1Args g1;
+  g1.A = ctx->A; g1.R1t = R1t; g1.H = e.H_dev; g1.Phi = Phi; g1.phi_ch_stride = rho_rows * Phi.ld;
+  g1.n_rho = ctx->n_rho; g1.n_ap = ctx->n_ap; g1.w2 = w2; g1.n_ch = e.n_ch; g1.n_atoms = nb;
+  BIP_TRY(precision == BIP_PREC_TF32X3 ? launch_gemm1_tc(ctx, g1) : launch_gemm1_simt(ctx, g1));
+  // a6: S2 windows -> R2[d][s]
+  BIP_TRY(launch_crop_detilt(ctx, ctx->S2, ctx->p2_h_dev, ctx->n_p2, -1, org, nb, e.w, (float2*)ctx->D2.p));
+  BIP_TRY(launch_recon(ctx, (const float2*)ctx->D2.p, ctx->n_p2, e.det_h_dev, e.n_det, e.nn_idx_dev, e.nn_w_dev, e.max_nn, -1,
+                       recon, org, nb, e.w, /*transpose=*/false, R2));
+  // a7-a8: detector projection and reduction
+  Gemm2Args g2;
+  g2.Phi = Phi; g2.phi_ch_stride = g1.phi_ch_stride; g2.R2 = R2;
+  g2.n_rho = ctx->n_rho; g2.n_det = e.n_det; g2.w2 = w2; g2.n_ch = e.n_ch; g2.n_atoms = nb;
+  g2.inv_G = (float)(1.0 / ((double)ctx->g.ny * ctx->g.nx));
+  g2.mode = mode;
+  g2.bin_of_det = mode == BIP_MODE_QEELS_X ? e.bin_of_det_x_dev : e.bin_of_det_y_dev;
+  g2.n_bins = mode == BIP_MODE_QEELS_X ? (int)e.binx.size() : (int)e.biny.size();
+  g2.out = out;
+  {
+    Span s(ctx, sp.pool_map, sp.gemm2);
+    BIP_TRY(precision == BIP_PREC_TF32X3 ? launch_gemm2_tc(ctx, g2) : launch_gemm2_simt(ctx, g2));
+  }
+  ctx->timing.gemm2_launches++;
+  ctx->timing.amplitudes += (double)ctx->n_rho * nb * e.n_ch * e.n_det;
+  ctx->timing.flops += 8.0 * ctx->n_rho * w2 * ((double)nb * ctx->n_ap + (double)nb * e.n_ch * e.n_det);
+  return BIP_OK;
+}
+
+static int32_t out_elems(const bip_ctx* ctx, const Edge& e, int mode, int64_t* n, int32_t* nbins, size_t* bytes) {
+  int64_t ne = 0; int32_t nb = 0; size_t by = 0;
+  switch (mode) {
+    case BIP_MODE_MAP: ne = ctx->n_rho; by = ne * sizeof(double); break;
+    case BIP_MODE_QEELS_X: nb = (int32_t)e.binx.size(); ne = (int64_t)ctx->n_rho * nb; by = ne * sizeof(float); break;
+    case BIP_MODE_QEELS_Y: nb = (int32_t)e.biny.size(); ne = (int64_t)ctx->n_rho * nb; by = ne * sizeof(float); break;
+    case BIP_MODE_CUBE: ne = (int64_t)ctx->n_rho * e.n_det; by = ne * sizeof(float); break;
+    default: return BIP_ERR_INVALID;
+  }
+  if (n) *n = ne;
+  if (nbins) *nbins = nb;
+  if (bytes) *bytes = by;
+  return BIP_OK;
+}
+
+static int32_t run_edges(bip_ctx* ctx, const std::vector<int32_t>& ids, int mode, int recon, int precision, void* const* outs,
+                         const size_t* outs_bytes) {
+  if (!ctx->s1_built || !ctx->s2_built) return fail(ctx, BIP_ERR_STATE, "bip_map: call bip_build_S1 and bip_build_S2 first");
+  if (ctx->n_rho <= 0) return fail(ctx, BIP_ERR_STATE, "bip_map: call bip_set_scan first");
+  if (mode < BIP_MODE_MAP || mode > BIP_MODE_CUBE) return fail(ctx, BIP_ERR_INVALID, "bip_map: unknown mode %d", mode);
+  if (recon != BIP_RECON_LINEAR && recon != BIP_RECON_MAGPHASE) return fail(ctx, BIP_ERR_INVALID, "bip_map: unknown recon %d", recon);
+  if (precision != BIP_PREC_TF32X3 && precision != BIP_PREC_FP32_SIMT) return fail(ctx, BIP_ERR_INVALID, "bip_map: unknown precision %d", precision);
+  if (precision == BIP_PREC_TF32X3 && !tc_available()) return fail(ctx, BIP_ERR_UNSUPPORTED, "bip_map: the tensor-core path is not built");
+  for (size_t k = 0; k < ids.size(); ++k) {
+    if (ids[k] < 0 || ids[k] >= (int)ctx->edges.size()) return fail(ctx, BIP_ERR_INVALID, "bip_map: edge %d does not exist", ids[k]);
+    size_t need = 0;
+    out_elems(ctx, ctx->edges[ids[k]], mode, nullptr, nullptr, &need);
+    if (!outs[k]) return fail(ctx, BIP_ERR_INVALID, "bip_map: output %zu is NULL", k);
+    if (outs_bytes[k] != need) return fail(ctx, BIP_ERR_INVALID, "bip_map: output %zu has %zu bytes, expected %zu", k, outs_bytes[k], need);
+  }
+  auto& sp = spans()[ctx];
+  sp.adv.clear(); sp.contract.clear(); sp.gemm2.clear();
+  sp.pool_map.reset();
+  ctx->timing.gemm2_launches = 0; ctx->timing.kernel_launches = 0; ctx->timing.amplitudes = 0; ctx->timing.flops = 0;
+  for (size_t k = 0; k < ids.size(); ++k) BIP_CUDA(ctx, cudaMemsetAsync(outs[k], 0, outs_bytes[k], ctx->stream));
+
+  std::vector<int32_t> planes;
+  for (int32_t id : ids) for (int32_t s : ctx->edges[id].slice) planes.push_back(s);
+  std::sort(planes.begin(), planes.end());
+  planes.erase(std::unique(planes.begin(), planes.end()), planes.end());
+  const size_t budget = scratch_budget();
+  for (int32_t plane : planes) {                                         // Alg. 5 line 3
+    { Span s(ctx, sp.pool_map, sp.adv); BIP_TRY(seek(ctx, plane)); }                  // line 4: ADVANCETO / PEELTO
+    for (size_t k = 0; k < ids.size(); ++k) {
+      Edge& e = ctx->edges[ids[k]];
+      const int32_t* origin_dev = edge_dev()[ctx][ids[k]].origin_dev;
+      // atoms are sorted by slice: contiguous range for this plane
+      auto lo = std::lower_bound(e.slice.begin(), e.slice.end(), plane) - e.slice.begin();
+      auto hi = std::upper_bound(e.slice.begin(), e.slice.end(), plane) - e.slice.begin();
+      if (lo == hi) continue;
+      const int64_t w2 = (int64_t)e.w * e.w;
+      const size_t per_atom = (size_t)((ctx->n_p1 + ctx->n_p2) * w2 * 8 + 16 * (w2 * round_up(ctx->n_ap, 32) + (int64_t)e.n_det * round_up(w2, 32) +
+                                                                                (int64_t)ctx->n_rho * e.n_ch * round_up(w2, 32)));
+      const int32_t nb_max = (int32_t)std::max<size_t>(1, std::min<size_t>(budget / std::max<size_t>(per_atom, 1), 4096));
+      Span s(ctx, sp.pool_map, sp.contract);
+      for (int32_t a0 = (int32_t)lo; a0 < (int32_t)hi; a0 += nb_max)     // lines 5-8
+        BIP_TRY(contract_batch(ctx, e, origin_dev, a0, std::min<int32_t>(nb_max, (int32_t)hi - a0), mode, recon, precision, outs[k]));
+    }
+  }
+  return BIP_OK;
+}
+
+}  // namespace bip
+
+using namespace bip;
+
+extern "C" {
+
+const char* bip_version(void) {
+  static char buf[256];
+  static std::once_flag once;
+  std::call_once(once, [] {
+    int dev = 0, n = 0;
+    cudaDeviceProp p{};
+    if (cudaGetDeviceCount(&n) == cudaSuccess && n > 0 && cudaGetDevice(&dev) == cudaSuccess && cudaGetDeviceProperties(&p, dev) == cudaSuccess)
+      snprintf(buf, sizeof buf, "libbip 0.1 (sm_100a); device %s sm_%d%d; SMs %d; L2 %d MB", p.name, p.major, p.minor, p.multiProcessorCount, p.l2CacheSize >> 20);
+    else { cudaGetLastError(); snprintf(buf, sizeof buf, "libbip 0.1 (sm_100a); no CUDA device"); }
+  });
+  return buf;
+}
+
+const char* bip_last_error(const bip_ctx* ctx) { return ctx ? ctx->err.c_str() : g_err.c_str(); }
+
+int32_t bip_create(bip_ctx** out, const bip_grid* g, const void* T, int32_t T_on_device, int32_t n_ap, const int32_t* ap_h,
+                   const float* ap_c, int32_t n_p1, const int32_t* p1_h, const bip_weights* w1, int32_t n_p2,
+                   const int32_t* p2_h, void* stream) {
+  if (!out) return fail(nullptr, BIP_ERR_INVALID, "bip_create: out is NULL");
+  *out = nullptr;
+  if (!g || g->ny < 8 || g->nx < 8 || g->ny > 8192 || g->nx > 8192 || g->nz < 1 || !(g->ly > 0) || !(g->lx > 0) || !(g->dz > 0) || !(g->lambda > 0))
+    return fail(nullptr, BIP_ERR_INVALID, "bip_create: bad grid");
+  if (!T) return fail(nullptr, BIP_ERR_INVALID, "bip_create: T is NULL");
+  if (!ap_c) return fail(nullptr, BIP_ERR_INVALID, "bip_create: aperture coefficients are NULL");
+  BIP_TRY(check_beams(nullptr, *g, n_ap, ap_h, "bip_create: aperture"));
+  BIP_TRY(check_beams(nullptr, *g, n_p1, p1_h, "bip_create: S1 parents"));
+  BIP_TRY(check_beams(nullptr, *g, n_p2, p2_h, "bip_create: S2 parents"));
+  BIP_TRY(check_weights(nullptr, w1, n_ap, n_p1, "bip_create: w1"));
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return fail(nullptr, BIP_ERR_CUDA, "bip_create: no CUDA device (libbip has no CPU path)"); }
+  int dev = 0;
+  cudaDeviceProp prop{};
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return fail(nullptr, BIP_ERR_CUDA, "bip_create: cannot query the device");
+  if (prop.major != 10) return fail(nullptr, BIP_ERR_CUDA, "bip_create: device %s is sm_%d%d; libbip is built for sm_100a only", prop.name, prop.major, prop.minor);
+
+  bip_ctx* ctx = new (std::nothrow) bip_ctx();
+  if (!ctx) return fail(nullptr, BIP_ERR_OOM, "bip_create: host allocation failed");
+  ctx->g = *g;
+  ctx->stream = (cudaStream_t)stream;
+  ctx->sm_count = prop.multiProcessorCount;
+  ctx->n_ap = n_ap; ctx->n_p1 = n_p1; ctx->n_p2 = n_p2; ctx->nn1 = w1->max_nn;
+  ctx->ap_h.assign(ap_h, ap_h + 2 * (size_t)n_ap);
+  ctx->p1_h.assign(p1_h, p1_h + 2 * (size_t)n_p1);
+  ctx->p2_h.assign(p2_h, p2_h + 2 * (size_t)n_p2);
+  const size_t G = (size_t)g->ny * g->nx;
+  auto build = [&]() -> int32_t {
+    if (T_on_device) ctx->T_dev = (const float2*)T;
+    else {
+      float2* t = nullptr;
+      BIP_TRY(dev_alloc(ctx, (void**)&t, G * g->nz * sizeof(float2), "transmission functions"));
+      ctx->T_dev = t; ctx->T_owned = true;
+      BIP_CUDA(ctx, cudaMemcpyAsync(t, T, G * g->nz * sizeof(float2), cudaMemcpyHostToDevice, ctx->stream));
+    }
+    BIP_TRY(upload(ctx, &ctx->ap_h_dev, ap_h, 2 * (size_t)n_ap, "aperture beams"));
+    BIP_TRY(upload(ctx, &ctx->p1_h_dev, p1_h, 2 * (size_t)n_p1, "S1 parents"));
+    BIP_TRY(upload(ctx, &ctx->p2_h_dev, p2_h, 2 * (size_t)n_p2, "S2 parents"));
+    BIP_TRY(upload(ctx, (float**)&ctx->ap_c_dev, ap_c, 2 * (size_t)n_ap, "aperture coefficients"));
+    BIP_TRY(upload(ctx, &ctx->w1_idx_dev, w1->nn_idx, (size_t)n_ap * w1->max_nn, "w1 indices"));
+    BIP_TRY(upload(ctx, &ctx->w1_w_dev, w1->nn_w, (size_t)n_ap * w1->max_nn, "w1 weights"));
+    BIP_TRY(dev_alloc(ctx, (void**)&ctx->S1, (size_t)n_p1 * G * sizeof(float2), "S1 parent columns"));
+    BIP_TRY(dev_alloc(ctx, (void**)&ctx->S2, (size_t)n_p2 * G * sizeof(float2), "S2 parent columns"));
+    BIP_TRY(ms_init(ctx));
+    BIP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return BIP_OK;
+  };
+  int32_t st = build();
+  if (st != BIP_OK) { std::string m = ctx->err; bip_destroy(ctx); g_err = m; return st; }
+  *out = ctx;
+  return BIP_OK;
+}
+
+int32_t bip_clear_edges(bip_ctx* ctx) {
+  if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
+  cudaStreamSynchronize(ctx->stream);
+  auto& ed = edge_dev()[ctx];
+  for (size_t k = 0; k < ctx->edges.size(); ++k) {
+    Edge& e = ctx->edges[k];
+    cudaFree(e.H_dev); cudaFree(e.det_h_dev); cudaFree(e.nn_idx_dev); cudaFree(e.nn_w_dev);
+    cudaFree(e.bin_of_det_x_dev); cudaFree(e.bin_of_det_y_dev);
+    if (k < ed.size()) cudaFree(ed[k].origin_dev);
+  }
+  ctx->edges.clear();
+  ed.clear();
+  return BIP_OK;
+}
+
+int32_t bip_destroy(bip_ctx* ctx) {
+  if (!ctx) return BIP_OK;
+  cudaStreamSynchronize(ctx->stream);
+  bip_clear_edges(ctx);
+  edge_dev().erase(ctx);
+  ms_release(ctx);
+  auto it = spans().find(ctx);
+  if (it != spans().end()) { it->second.pool_map.destroy(); it->second.pool_b1.destroy(); it->second.pool_b2.destroy(); spans().erase(it); }
+  if (ctx->T_owned) cudaFree((void*)ctx->T_dev);
+  void* ptrs[] = {ctx->ap_h_dev, ctx->p1_h_dev, ctx->p2_h_dev, ctx->ap_c_dev, ctx->w1_idx_dev, ctx->w1_w_dev, ctx->rooty_dev,
+                  ctx->rootx_dev, ctx->P_dev, ctx->S1, ctx->S2, ctx->D1.p, ctx->D2.p, ctx->R1.p, ctx->R2.p, ctx->Psi.p,
+                  ctx->Phi.p, ctx->A.p[0]};
+  for (void* p : ptrs) if (p) cudaFree(p);
+  cudaGetLastError();
+  delete ctx;
+  return BIP_OK;
+}
+
+int32_t bip_build_S1(bip_ctx* ctx) {
+  if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
+  auto& sp = spans()[ctx];
+  sp.build1.clear(); sp.pool_b1.reset();
+  { Span s(ctx, sp.pool_b1, sp.build1); BIP_TRY(ms_plane_waves(ctx, ctx->S1, ctx->p1_h_dev, ctx->n_p1, +1)); }
+  ctx->plane1 = 0;
+  ctx->s1_built = true;
+  return BIP_OK;
+}
+
+int32_t bip_build_S2(bip_ctx* ctx) {
+  if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
+  auto& sp = spans()[ctx];
+  sp.build2.clear(); sp.pool_b2.reset();
+  {
+    Span s(ctx, sp.pool_b2, sp.build2);
+    BIP_TRY(ms_plane_waves(ctx, ctx->S2, ctx->p2_h_dev, ctx->n_p2, -1));
+    ctx->plane2 = ctx->g.nz;
+    while (ctx->plane2 > 0) { ctx->plane2--; BIP_TRY(ms_step_S2(ctx, ctx->plane2, -1)); }
+  }
+  ctx->s2_built = true;
+  return BIP_OK;
+}
+
+int32_t bip_set_scan(bip_ctx* ctx, int32_t n_rho, const double* rho_px) {
+  if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
+  if (n_rho <= 0 || !rho_px) return fail(ctx, BIP_ERR_INVALID, "bip_set_scan: empty scan");
+  for (int32_t i = 0; i < 2 * n_rho; ++i) if (!std::isfinite(rho_px[i])) return fail(ctx, BIP_ERR_INVALID, "bip_set_scan: non-finite position");
+  cudaStreamSynchronize(ctx->stream);
+  if (ctx->A.p[0]) { cudaFree(ctx->A.p[0]); ctx->A = Planes(); }
+  Planes A;
+  A.rows = n_rho; A.ld = round_up(ctx->n_ap, 32); A.batch_stride = 0;
+  const int64_t plane_floats = round_up(A.rows * A.ld, 256);
+  float* base = nullptr;
+  BIP_TRY(dev_alloc(ctx, (void**)&base, (size_t)plane_floats * 4 * sizeof(float), "illumination matrix"));
+  BIP_CUDA(ctx, cudaMemsetAsync(base, 0, (size_t)plane_floats * 4 * sizeof(float), ctx->stream));
+  for (int k = 0; k < 4; ++k) A.p[k] = base + k * plane_floats;
+  double* rho_dev = nullptr;
+  BIP_TRY(dev_alloc(ctx, (void**)&rho_dev, sizeof(double) * 2 * n_rho, "scan positions"));
+  BIP_CUDA(ctx, cudaMemcpyAsync(rho_dev, rho_px, sizeof(double) * 2 * n_rho, cudaMemcpyHostToDevice, ctx->stream));
+  ctx->A = A;
+  ctx->n_rho = n_rho;
+  int32_t st = launch_illumination(ctx, rho_dev, n_rho, A);
+  cudaStreamSynchronize(ctx->stream);
+  cudaFree(rho_dev);
+  return st;
+}
+
+int32_t bip_add_edge(bip_ctx* ctx, int32_t n_atoms, const int32_t* slice, const int32_t* centre_px, int32_t n_ch, int32_t w,
+                     const float* H, int32_t n_det, const int32_t* det_h, const bip_weights* w2, int32_t* edge_id) {
+  if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
+  if (n_atoms < 0 || (n_atoms > 0 && (!slice || !centre_px))) return fail(ctx, BIP_ERR_INVALID, "bip_add_edge: bad site list");
+  if (n_ch < 1 || n_ch > 1024 || !H) return fail(ctx, BIP_ERR_INVALID, "bip_add_edge: bad channel count or H is NULL");
+  if (w < 8 || (w & 1) || w > std::min(ctx->g.ny, ctx->g.nx)) return fail(ctx, BIP_ERR_INVALID, "bip_add_edge: window %d must be even and in 8..min(ny, nx)", w);
+  BIP_TRY(check_beams(ctx, ctx->g, n_det, det_h, "bip_add_edge: detector"));
+  BIP_TRY(check_weights(ctx, w2, n_det, ctx->n_p2, "bip_add_edge: w2"));
+  Edge e;
+  e.n_atoms = n_atoms; e.n_ch = n_ch; e.w = w; e.n_det = n_det; e.max_nn = w2->max_nn;
+  // sort sites by slice (stable): the plane loop takes contiguous ranges
+  std::vector<int32_t> order(n_atoms);
+  for (int i = 0; i < n_atoms; ++i) order[i] = i;
+  for (int i = 0; i < n_atoms; ++i) {
+    if (slice[i] < 0 || slice[i] >= ctx->g.nz) return fail(ctx, BIP_ERR_INVALID, "bip_add_edge: site %d in slice %d outside 0..%d", i, slice[i], ctx->g.nz - 1);
+    if (centre_px[2 * i] < 0 || centre_px[2 * i] >= ctx->g.ny || centre_px[2 * i + 1] < 0 || centre_px[2 * i + 1] >= ctx->g.nx)
+      return fail(ctx, BIP_ERR_INVALID, "bip_add_edge: site %d centre outside the grid", i);
+  }
+  std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return slice[a] < slice[b]; });
+  e.slice.resize(n_atoms); e.origin.resize(2 * (size_t)n_atoms);
+  for (int i = 0; i < n_atoms; ++i) {
+    const int a = order[i];
+    e.slice[i] = slice[a];
+    e.origin[2 * i] = ((centre_px[2 * a] - w / 2) % ctx->g.ny + ctx->g.ny) % ctx->g.ny;
+    e.origin[2 * i + 1] = ((centre_px[2 * a + 1] - w / 2) % ctx->g.nx + ctx->g.nx) % ctx->g.nx;
+  }
+  e.det_h.assign(det_h, det_h + 2 * (size_t)n_det);
+  // qEELS bins: distinct signed indices along the resolved axis, ascending
+  std::vector<int32_t> bx(n_det), by(n_det);
+  for (int d = 0; d < n_det; ++d) { by[d] = det_h[2 * d]; bx[d] = det_h[2 * d + 1]; }
+  e.binx = bx; std::sort(e.binx.begin(), e.binx.end()); e.binx.erase(std::unique(e.binx.begin(), e.binx.end()), e.binx.end());
+  e.biny = by; std::sort(e.biny.begin(), e.biny.end()); e.biny.erase(std::unique(e.biny.begin(), e.biny.end()), e.biny.end());
+  for (int d = 0; d < n_det; ++d) {
+    bx[d] = (int32_t)(std::lower_bound(e.binx.begin(), e.binx.end(), bx[d]) - e.binx.begin());
+    by[d] = (int32_t)(std::lower_bound(e.biny.begin(), e.biny.end(), by[d]) - e.biny.begin());
+  }
+  EdgeDev ed;
+  BIP_TRY(upload(ctx, (float**)&e.H_dev, H, 2 * (size_t)n_ch * w * w, "H windows"));
+  BIP_TRY(upload(ctx, &e.det_h_dev, det_h, 2 * (size_t)n_det, "detector beams"));
+  BIP_TRY(upload(ctx, &e.nn_idx_dev, w2->nn_idx, (size_t)n_det * w2->max_nn, "w2 indices"));
+  BIP_TRY(upload(ctx, &e.nn_w_dev, w2->nn_w, (size_t)n_det * w2->max_nn, "w2 weights"));
+  BIP_TRY(upload(ctx, &e.bin_of_det_x_dev, bx.data(), (size_t)n_det, "qEELS bins"));
+  BIP_TRY(upload(ctx, &e.bin_of_det_y_dev, by.data(), (size_t)n_det, "qEELS bins"));
+  BIP_TRY(upload(ctx, &ed.origin_dev, e.origin.data(), std::max<size_t>(2 * (size_t)n_atoms, 2), "window origins"));
+  BIP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));     // host sources may go away after return
+  ctx->edges.push_back(std::move(e));
+  edge_dev()[ctx].push_back(ed);
+  if (edge_id) *edge_id = (int32_t)ctx->edges.size() - 1;
+  return BIP_OK;
+}
+
+int32_t bip_output_size(const bip_ctx* ctx, int32_t edge_id, int32_t mode, int64_t* n_elems, int32_t* n_bins) {
+  if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
+  if (edge_id < 0 || edge_id >= (int)ctx->edges.size()) return fail(const_cast<bip_ctx*>(ctx), BIP_ERR_INVALID, "edge %d does not exist", edge_id);
+  if (ctx->n_rho <= 0) return fail(const_cast<bip_ctx*>(ctx), BIP_ERR_STATE, "bip_output_size: call bip_set_scan first");
+  if (out_elems(ctx, ctx->edges[edge_id], mode, n_elems, n_bins, nullptr) != BIP_OK) return fail(const_cast<bip_ctx*>(ctx), BIP_ERR_INVALID, "unknown mode %d", mode);
+  return BIP_OK;
+}
+
+int32_t bip_map(bip_ctx* ctx, int32_t edge_id, int32_t mode, int32_t recon, int32_t precision, void* out_dev, size_t out_bytes) {
+  if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
+  std::vector<int32_t> ids{edge_id};
+  void* outs[1] = {out_dev};
+  size_t by[1] = {out_bytes};
+  return run_edges(ctx, ids, mode, recon, precision, outs, by);
+}
+
+int32_t bip_map_all(bip_ctx* ctx, int32_t mode, int32_t recon, int32_t precision, void* const* outs_dev, const size_t* outs_bytes,
+                    int32_t n_outs) {
+  if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
+  if (n_outs != (int32_t)ctx->edges.size() || !outs_dev || !outs_bytes) return fail(ctx, BIP_ERR_INVALID, "bip_map_all: need one output per edge (%zu)", ctx->edges.size());
+  std::vector<int32_t> ids(n_outs);
+  for (int i = 0; i < n_outs; ++i) ids[i] = i;
+  return run_edges(ctx, ids, mode, recon, precision, outs_dev, outs_bytes);
+}
+
+int32_t bip_map_host(bip_ctx* ctx, int32_t edge_id, int32_t mode, int32_t recon, int32_t precision, void* out_host, size_t out_bytes) {
+  if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
+  if (!out_host) return fail(ctx, BIP_ERR_INVALID, "bip_map_host: output is NULL");
+  void* d = nullptr;
+  BIP_TRY(dev_alloc(ctx, &d, out_bytes, "host-call output staging"));
+  int32_t st = bip_map(ctx, edge_id, mode, recon, precision, d, out_bytes);
+  if (st == BIP_OK) {
+    cudaError_t e = cudaMemcpyAsync(out_host, d, out_bytes, cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) st = fail(ctx, BIP_ERR_CUDA, "bip_map_host: %s", cudaGetErrorString(e));
+  }
+  cudaStreamSynchronize(ctx->stream);
+  cudaFree(d);
+  return st;
+}
+
+int32_t bip_get_windows(const bip_ctx* ctx, int32_t edge_id, int32_t* origin_out) {
+  if (!ctx || !origin_out) return fail(nullptr, BIP_ERR_INVALID, "bip_get_windows: NULL argument");
+  if (edge_id < 0 || edge_id >= (int)ctx->edges.size()) return fail(const_cast<bip_ctx*>(ctx), BIP_ERR_INVALID, "edge %d does not exist", edge_id);
+  const Edge& e = ctx->edges[edge_id];
+  std::copy(e.origin.begin(), e.origin.end(), origin_out);
+  return BIP_OK;
+}
+
+int32_t bip_get_qeels_bins(const bip_ctx* ctx, int32_t edge_id, int32_t mode, int32_t* bins_out) {
+  if (!ctx || !bins_out) return fail(nullptr, BIP_ERR_INVALID, "bip_get_qeels_bins: NULL argument");
+  if (edge_id < 0 || edge_id >= (int)ctx->edges.size()) return fail(const_cast<bip_ctx*>(ctx), BIP_ERR_INVALID, "edge %d does not exist", edge_id);
+  const Edge& e = ctx->edges[edge_id];
+  if (mode == BIP_MODE_QEELS_X) std::copy(e.binx.begin(), e.binx.end(), bins_out);
+  else if (mode == BIP_MODE_QEELS_Y) std::copy(e.biny.begin(), e.biny.end(), bins_out);
+  else return fail(const_cast<bip_ctx*>(ctx), BIP_ERR_INVALID, "mode %d has no bins", mode);
+  return BIP_OK;
+}
+
+int32_t bip_seek_plane(bip_ctx* ctx, int32_t plane) {
+  if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
+  return seek(ctx, plane);
+}
+
+int32_t bip_copy_S(bip_ctx* ctx, int32_t which, int32_t p0, int32_t np, void* out_host) {
+  if (!ctx || !out_host) return fail(ctx, BIP_ERR_INVALID, "bip_copy_S: NULL argument");
+  const int32_t n = which == 1 ? ctx->n_p1 : which == 2 ? ctx->n_p2 : -1;
+  if (n < 0) return fail(ctx, BIP_ERR_INVALID, "bip_copy_S: which must be 1 or 2");
+  if ((which == 1 && !ctx->s1_built) || (which == 2 && !ctx->s2_built)) return fail(ctx, BIP_ERR_STATE, "bip_copy_S: matrix not built");
+  if (p0 < 0 || np < 0 || p0 + np > n) return fail(ctx, BIP_ERR_INVALID, "bip_copy_S: columns %d..%d outside 0..%d", p0, p0 + np, n);
+  const size_t G = (size_t)ctx->g.ny * ctx->g.nx;
+  const float2* S = which == 1 ? ctx->S1 : ctx->S2;
+  BIP_CUDA(ctx, cudaMemcpyAsync(out_host, S + (size_t)p0 * G, (size_t)np * G * sizeof(float2), cudaMemcpyDeviceToHost, ctx->stream));
+  BIP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+  return BIP_OK;
+}
+
+int32_t bip_debug_reconstruct(bip_ctx* ctx, int32_t edge_id, int32_t atom, int32_t which, int32_t recon, void* out_host) {
+  if (!ctx || !out_host) return fail(ctx, BIP_ERR_INVALID, "bip_debug_reconstruct: NULL argument");
+  if (edge_id < 0 || edge_id >= (int)ctx->edges.size()) return fail(ctx, BIP_ERR_INVALID, "edge %d does not exist", edge_id);
+  Edge& e = ctx->edges[edge_id];
+  if (atom < 0 || atom >= e.n_atoms) return fail(ctx, BIP_ERR_INVALID, "atom %d does not exist", atom);
+  if (which != 1 && which != 2) return fail(ctx, BIP_ERR_INVALID, "which must be 1 or 2");
+  if (!ctx->s1_built || !ctx->s2_built) return fail(ctx, BIP_ERR_STATE, "matrices not built");
+  const int w2 = e.w * e.w;
+  const int32_t* org = edge_dev()[ctx][edge_id].origin_dev + 2 * (int64_t)atom;
+  const int n_par = which == 1 ? ctx->n_p1 : ctx->n_p2;
+  const int n_beams = which == 1 ? ctx->n_ap : e.n_det;
+  DevBuf& D = which == 1 ? ctx->D1 : ctx->D2;
+  BIP_TRY(ensure(ctx, D, (size_t)n_par * w2 * sizeof(float2), "D"));
+  float2* R = nullptr;
+  BIP_TRY(dev_alloc(ctx, (void**)&R, (size_t)n_beams * w2 * sizeof(float2), "debug reconstruction"));
+  int32_t st = launch_crop_detilt(ctx, which == 1 ? ctx->S1 : ctx->S2, which == 1 ? ctx->p1_h_dev : ctx->p2_h_dev, n_par,
+                                  which == 1 ? +1 : -1, org, 1, e.w, (float2*)D.p);
+  if (st == BIP_OK)
+    st = launch_recon_c64(ctx, (const float2*)D.p, n_par, which == 1 ? ctx->ap_h_dev : e.det_h_dev, n_beams,
+                          which == 1 ? ctx->w1_idx_dev : e.nn_idx_dev, which == 1 ? ctx->w1_w_dev : e.nn_w_dev,
+                          which == 1 ? ctx->nn1 : e.max_nn, which == 1 ? +1 : -1, recon, org, 0, e.w, R);
+  if (st == BIP_OK) {
+    cudaError_t er = cudaMemcpyAsync(out_host, R, (size_t)n_beams * w2 * sizeof(float2), cudaMemcpyDeviceToHost, ctx->stream);
+    if (er == cudaSuccess) er = cudaStreamSynchronize(ctx->stream);
+    if (er != cudaSuccess) st = fail(ctx, BIP_ERR_CUDA, "bip_debug_reconstruct: %s", cudaGetErrorString(er));
+  }
+  cudaStreamSynchronize(ctx->stream);
+  cudaFree(R);
+  return st;
+}
+
+int32_t bip_get_timing(const bip_ctx* cctx, bip_timing* out) {
+  if (!cctx || !out) return fail(nullptr, BIP_ERR_INVALID, "bip_get_timing: NULL argument");
+  bip_ctx* ctx = const_cast<bip_ctx*>(cctx);
+  cudaStreamSynchronize(ctx->stream);
+  auto& sp = spans()[ctx];
+  ctx->timing.build_s1_ms = sum_ms(sp.build1);
+  ctx->timing.build_s2_ms = sum_ms(sp.build2);
+  ctx->timing.advance_peel_ms = sum_ms(sp.adv);
+  ctx->timing.contract_ms = sum_ms(sp.contract);
+  ctx->timing.gemm2_ms = sum_ms(sp.gemm2);
+  *out = ctx->timing;
+  return BIP_OK;
+}
+
+}  // extern "C"

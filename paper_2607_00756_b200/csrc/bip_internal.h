@@ -1,0 +1,168 @@
+// Internal declarations of libbip (not part of the ABI).
+#ifndef BIP_INTERNAL_H_
+#define BIP_INTERNAL_H_
+
+#include <cstdarg>
+#include <cstdint>
+#include <cstdio>
+#include <string>
+#include <vector>
+
+#include "../../include/bip.h"
+
+namespace bip {
+
+// Records the message on the context (or a thread-local slot when ctx == nullptr) and returns `status`.
+int32_t fail(bip_ctx* ctx, int32_t status, const char* fmt, ...) __attribute__((format(printf, 3, 4)));
+
+}  // namespace bip
+
+#ifdef __CUDACC__
+#include <cuda_runtime.h>
+#include <cufft.h>
+
+namespace bip {
+
+// Split-plane operand: a complex matrix [rows][ld] stored as four fp32 planes
+//   re_hi, re_lo, im_hi, im_lo  with hi = tf32(x) (round-to-nearest, ties away) and lo = x - hi (exact in fp32).
+// The tensor-core kernels feed the planes to tcgen05 kind::tf32 as they are (3xTF32 split); the fp32 SIMT
+// reference kernels read hi + lo.  `ld` is a multiple of 32 floats (128 B) and plane bases are 1024 B aligned.
+struct Planes {
+  float* p[4] = {nullptr, nullptr, nullptr, nullptr};   // re_hi, re_lo, im_hi, im_lo
+  int64_t rows = 0;      // rows per batch item (padded to a multiple of 128)
+  int64_t ld = 0;        // floats per row
+  int64_t batch_stride = 0;   // floats between batch items inside one plane (0 = shared)
+};
+
+struct DevBuf {
+  void* p = nullptr;
+  size_t bytes = 0;
+  uint64_t sig = 0;      // layout signature of the planes last carved out of it
+};
+
+struct Edge {
+  int32_t n_atoms = 0, n_ch = 0, w = 0, n_det = 0, max_nn = 0;
+  std::vector<int32_t> slice;          // [n_atoms]
+  std::vector<int32_t> origin;         // [n_atoms][2] window origin (centre - w/2) mod N
+  std::vector<int32_t> det_h;          // [n_det][2]
+  std::vector<int32_t> binx, biny;     // distinct h_x / h_y ascending
+  float2* H_dev = nullptr;             // [n_ch][w*w]
+  int32_t* det_h_dev = nullptr;        // [n_det][2]
+  int32_t* nn_idx_dev = nullptr;       // [n_det][max_nn]
+  float* nn_w_dev = nullptr;           // [n_det][max_nn]
+  int32_t* bin_of_det_x_dev = nullptr; // [n_det] bin number along x
+  int32_t* bin_of_det_y_dev = nullptr;
+};
+
+}  // namespace bip
+
+struct bip_ctx {
+  bip_grid g{};
+  cudaStream_t stream = nullptr;
+  int sm_count = 0;
+  std::string err;
+
+  const float2* T_dev = nullptr;   // [nz][ny][nx]
+  bool T_owned = false;
+
+  // aperture / parents
+  int32_t n_ap = 0, n_p1 = 0, n_p2 = 0, nn1 = 0;
+  std::vector<int32_t> ap_h, p1_h, p2_h;
+  int32_t *ap_h_dev = nullptr, *p1_h_dev = nullptr, *p2_h_dev = nullptr;
+  float2* ap_c_dev = nullptr;
+  int32_t* w1_idx_dev = nullptr;
+  float* w1_w_dev = nullptr;
+
+  // roots of unity exp(2 pi i k / N), k = 0..N-1 (exact phases for tilt / de-tilt)
+  float2 *rooty_dev = nullptr, *rootx_dev = nullptr;
+  float2* P_dev = nullptr;         // Fresnel propagator / G  (forward step)
+  float2 *S1 = nullptr, *S2 = nullptr;
+  bool s1_built = false, s2_built = false;
+  int32_t plane1 = 0, plane2 = 0;  // S1 holds slices 0..plane1-1; S2 holds slices plane2..nz-1
+  cufftHandle plan = 0;
+  int32_t plan_batch = 0;
+  bool plan_ok = false;
+
+  // scan
+  int32_t n_rho = 0;
+  bip::Planes A;                   // illumination [n_rho][n_ap] split planes (K-major over b)
+
+  std::vector<bip::Edge> edges;
+
+  // scratch, grown on demand
+  bip::DevBuf D1, D2, R1, R2, Psi, Phi;
+
+  bip_timing timing{};
+  cudaEvent_t ev[8] = {};
+};
+
+namespace bip {
+
+#define BIP_CUDA(ctx, call)                                                                          \
+  do {                                                                                               \
+    cudaError_t e_ = (call);                                                                         \
+    if (e_ != cudaSuccess)                                                                           \
+      return bip::fail((ctx), e_ == cudaErrorMemoryAllocation ? BIP_ERR_OOM : BIP_ERR_CUDA,          \
+                       "%s:%d %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_));           \
+  } while (0)
+
+#define BIP_TRY(call)                  \
+  do {                                 \
+    int32_t s_ = (call);               \
+    if (s_ != BIP_OK) return s_;       \
+  } while (0)
+
+int32_t dev_alloc(bip_ctx* ctx, void** p, size_t bytes, const char* what);
+int32_t ensure(bip_ctx* ctx, DevBuf& b, size_t bytes, const char* what);
+
+// ---- multislice (bip_multislice.cu) ----
+int32_t ms_init(bip_ctx* ctx);                       // propagator, roots of unity, cuFFT plan
+int32_t ms_plane_waves(bip_ctx* ctx, float2* S, const int32_t* h_dev, int32_t n, int sign);
+// forward: S <- P[T_j S] (dir=+1) ; inverse: S <- T_j* P*[S] (dir=-1)               (S1, eq. 6)
+int32_t ms_step_S1(bip_ctx* ctx, int32_t j, int dir);
+// build/un-peel: S <- T_j P[S] (dir=-1, towards the entrance) ; peel: S <- P*[T_j* S] (dir=+1)   (S2, eq. 12)
+int32_t ms_step_S2(bip_ctx* ctx, int32_t j, int dir);
+
+// ---- reconstruction (bip_recon.cu) ----
+// a1: D[a][p][s] = S_p(r) * exp(-carrier 2 pi i h_p.r/N) on the atoms' windows
+int32_t launch_crop_detilt(bip_ctx* ctx, const float2* S, const int32_t* ph_dev, int32_t n_par, int carrier,
+                           const int32_t* origin_dev, int32_t n_atoms, int32_t w, float2* D);
+// a2/a6: R[a][beam][s] (or transposed [a][s][beam]) split planes from D with ELL weights, re-tilted
+int32_t launch_recon(bip_ctx* ctx, const float2* D, int32_t n_par, const int32_t* bh_dev, int32_t n_beams,
+                     const int32_t* nn_idx, const float* nn_w, int32_t max_nn, int carrier, int recon,
+                     const int32_t* origin_dev, int32_t n_atoms, int32_t w, bool transpose, Planes out);
+int32_t launch_recon_c64(bip_ctx* ctx, const float2* D, int32_t n_par, const int32_t* bh_dev, int32_t n_beams,
+                         const int32_t* nn_idx, const float* nn_w, int32_t max_nn, int carrier, int recon,
+                         const int32_t* origin_dev, int32_t atom, int32_t w, float2* out);
+// a3: illumination planes A[rho][b] = c_b exp(-2 pi i h_b.rho/N)
+int32_t launch_illumination(bip_ctx* ctx, const double* rho_dev, int32_t n_rho, Planes out);
+
+// ---- contractions ----
+struct Gemm1Args {       // a4 + a5: Psi = A . R1 ; Phi_n = H_n . Psi -> split planes [atom][n][rho][s]
+  Planes A;              // [n_rho][n_ap]
+  Planes R1t;            // [atom][s][b]   (K-major over b)
+  const float2* H;       // [n_ch][w*w]
+  Planes Phi;            // [atom][n][n_rho][w*w]: batch_stride per atom, rows = n_ch * rows_per_ch
+  int64_t phi_ch_stride; // floats between channels inside one atom
+  int32_t n_rho, n_ap, w2, n_ch, n_atoms;
+};
+struct Gemm2Args {       // a7 + a8: a_n = g Phi_n . R2^T ; |a|^2 reduced per mode
+  Planes Phi;
+  int64_t phi_ch_stride;
+  Planes R2;             // [atom][d][s]
+  int32_t n_rho, n_det, w2, n_ch, n_atoms;
+  float inv_G;           // 1 / (ny nx): |a|^2 scale of the unitary DFT
+  int32_t mode;
+  const int32_t* bin_of_det;   // QEELS
+  int32_t n_bins;
+  void* out;             // MAP double[n_rho]; QEELS float[n_rho][n_bins]; CUBE float[n_rho][n_det]
+};
+int32_t launch_gemm1_simt(bip_ctx* ctx, const Gemm1Args& a);
+int32_t launch_gemm2_simt(bip_ctx* ctx, const Gemm2Args& a);
+int32_t launch_gemm1_tc(bip_ctx* ctx, const Gemm1Args& a);
+int32_t launch_gemm2_tc(bip_ctx* ctx, const Gemm2Args& a);
+bool tc_available();
+
+}  // namespace bip
+#endif  // __CUDACC__
+#endif  // BIP_INTERNAL_H_

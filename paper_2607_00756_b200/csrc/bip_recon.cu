@@ -1,0 +1,246 @@
+// Windowed column reconstruction (eq. 15; eq. 11) and illumination
+// coefficients: steps a1, a2, a3, a6 of SURVEY.md 8(a).
+#include "bip_internal.h"
+
+namespace bip {
+
+namespace {
+
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) {
+  return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+
+__device__ __forceinline__ float tf32_hi(float x) {
+  uint32_t r;
+  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
+  return __uint_as_float(r);
+}
+
+// exp(+2 pi i h.r/N) for non-negative reduced beam index (hyp, hxp) at global pixel (ry, rx): exact phase from the
+// root tables, (h r mod N) reduced in integers (SURVEY "Phases exactly").
+__device__ __forceinline__ float2 tilt(const float2* __restrict__ rooty, const float2* __restrict__ rootx,
+                                       int hyp, int hxp, int ry, int rx, int ny, int nx) {
+  return cmul(rooty[(hyp * ry) % ny], rootx[(hxp * rx) % nx]);
+}
+
+// a1: D[a][p][s] = S_p(r) exp(-carrier 2 pi i h_p.r/N), r = (origin_a + s) mod N
+__global__ void k_crop_detilt(const float2* __restrict__ S, const int32_t* __restrict__ ph, int carrier,
+                              const int32_t* __restrict__ origin, int w, int ny, int nx,
+                              const float2* __restrict__ rooty, const float2* __restrict__ rootx,
+                              float2* __restrict__ D, int n_par) {
+  const int a = blockIdx.z, p = blockIdx.y;
+  const int w2 = w * w;
+  const int oy = origin[2 * a], ox = origin[2 * a + 1];
+  const int hyp = ((ph[2 * p] % ny) + ny) % ny, hxp = ((ph[2 * p + 1] % nx) + nx) % nx;
+  const float2* col = S + (int64_t)p * ny * nx;
+  float2* out = D + ((int64_t)a * n_par + p) * w2;
+  for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < w2; s += gridDim.x * blockDim.x) {
+    const int sy = s / w, sx = s - sy * w;
+    int ry = oy + sy; if (ry >= ny) ry -= ny;
+    int rx = ox + sx; if (rx >= nx) rx -= nx;
+    float2 t = tilt(rooty, rootx, hyp, hxp, ry, rx, ny, nx);
+    if (carrier > 0) t.y = -t.y;                       // remove the carrier: multiply by its conjugate
+    out[s] = cmul(col[(int64_t)ry * nx + rx], t);
+  }
+}
+
+// One reconstructed element: sum_j w_j D[idx_j][s], optional magnitude-preserving form, re-tilt.
+__device__ __forceinline__ float2 recon_elem(const float2* __restrict__ Da, const int32_t* __restrict__ idx,
+                                             const float* __restrict__ wt, int max_nn, int w2, int s, int recon,
+                                             float2 t) {
+  float zr = 0.f, zi = 0.f, mag = 0.f;
+  for (int j = 0; j < max_nn; ++j) {
+    const int p = idx[j];
+    if (p < 0) break;
+    const float wj = wt[j];
+    const float2 d = Da[(int64_t)p * w2 + s];
+    zr = fmaf(wj, d.x, zr);
+    zi = fmaf(wj, d.y, zi);
+    if (recon == BIP_RECON_MAGPHASE) mag = fmaf(wj, sqrtf(d.x * d.x + d.y * d.y), mag);
+  }
+  if (recon == BIP_RECON_MAGPHASE) {
+    const float az = sqrtf(zr * zr + zi * zi);
+    const float sc = az >= 1e-30f ? mag / az : 0.f;   // eq. 11; |z| < 1e-30 -> 0
+    zr *= sc; zi *= sc;
+  }
+  return cmul(make_float2(zr, zi), t);
+}
+
+// a2 / a6 (row-major output [a][beam][s], K-major over s): grid (s-chunks, beams, atoms)
+__global__ void k_recon_rows(const float2* __restrict__ D, int n_par, const int32_t* __restrict__ bh, int n_beams,
+                             const int32_t* __restrict__ nn_idx, const float* __restrict__ nn_w, int max_nn,
+                             int carrier, int recon, const int32_t* __restrict__ origin, int w, int ny, int nx,
+                             const float2* __restrict__ rooty, const float2* __restrict__ rootx, Planes out) {
+  const int a = blockIdx.z, b = blockIdx.y;
+  const int w2 = w * w;
+  __shared__ int32_t s_idx[BIP_MAX_NN];
+  __shared__ float s_w[BIP_MAX_NN];
+  if (threadIdx.x < max_nn) {
+    s_idx[threadIdx.x] = nn_idx[(int64_t)b * max_nn + threadIdx.x];
+    s_w[threadIdx.x] = nn_w[(int64_t)b * max_nn + threadIdx.x];
+  }
+  __syncthreads();
+  const int oy = origin[2 * a], ox = origin[2 * a + 1];
+  const int hyp = ((bh[2 * b] % ny) + ny) % ny, hxp = ((bh[2 * b + 1] % nx) + nx) % nx;
+  const float2* Da = D + (int64_t)a * n_par * w2;
+  const int64_t row = (int64_t)a * out.batch_stride + (int64_t)b * out.ld;
+  for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < w2; s += gridDim.x * blockDim.x) {
+    const int sy = s / w, sx = s - sy * w;
+    int ry = oy + sy; if (ry >= ny) ry -= ny;
+    int rx = ox + sx; if (rx >= nx) rx -= nx;
+    float2 t = tilt(rooty, rootx, hyp, hxp, ry, rx, ny, nx);
+    if (carrier < 0) t.y = -t.y;                       // restore the carrier exp(carrier 2 pi i h_b.r/N)
+    const float2 v = recon_elem(Da, s_idx, s_w, max_nn, w2, s, recon, t);
+    const float rh = tf32_hi(v.x), ih = tf32_hi(v.y);
+    out.p[0][row + s] = rh; out.p[1][row + s] = v.x - rh;
+    out.p[2][row + s] = ih; out.p[3][row + s] = v.y - ih;
+  }
+}
+
+// a2 transposed output [a][s][beam] (K-major over beams, operand of the probe GEMM): 32 x 32 tiles through smem
+__global__ void k_recon_transposed(const float2* __restrict__ D, int n_par, const int32_t* __restrict__ bh, int n_beams,
+                                   const int32_t* __restrict__ nn_idx, const float* __restrict__ nn_w, int max_nn,
+                                   int carrier, int recon, const int32_t* __restrict__ origin, int w, int ny, int nx,
+                                   const float2* __restrict__ rooty, const float2* __restrict__ rootx, Planes out) {
+  __shared__ float2 tile[32][33];
+  const int a = blockIdx.z;
+  const int w2 = w * w;
+  const int b0 = blockIdx.y * 32, s0 = blockIdx.x * 32;
+  const int oy = origin[2 * a], ox = origin[2 * a + 1];
+  const float2* Da = D + (int64_t)a * n_par * w2;
+  // compute: threadIdx.x <-> s (coalesced reads of D), threadIdx.y strides over beams
+  for (int bb = threadIdx.y; bb < 32; bb += blockDim.y) {
+    const int b = b0 + bb, s = s0 + threadIdx.x;
+    float2 v = make_float2(0.f, 0.f);
+    if (b < n_beams && s < w2) {
+      const int sy = s / w, sx = s - sy * w;
+      int ry = oy + sy; if (ry >= ny) ry -= ny;
+      int rx = ox + sx; if (rx >= nx) rx -= nx;
+      const int hyp = ((bh[2 * b] % ny) + ny) % ny, hxp = ((bh[2 * b + 1] % nx) + nx) % nx;
+      float2 t = tilt(rooty, rootx, hyp, hxp, ry, rx, ny, nx);
+      if (carrier < 0) t.y = -t.y;
+      v = recon_elem(Da, nn_idx + (int64_t)b * max_nn, nn_w + (int64_t)b * max_nn, max_nn, w2, s, recon, t);
+    }
+    tile[bb][threadIdx.x] = v;
+  }
+  __syncthreads();
+  // store: threadIdx.x <-> beam (coalesced writes)
+  for (int ss = threadIdx.y; ss < 32; ss += blockDim.y) {
+    const int s = s0 + ss, b = b0 + threadIdx.x;
+    if (s < w2 && b < n_beams) {
+      const float2 v = tile[threadIdx.x][ss];
+      const int64_t o = (int64_t)a * out.batch_stride + (int64_t)s * out.ld + b;
+      const float rh = tf32_hi(v.x), ih = tf32_hi(v.y);
+      out.p[0][o] = rh; out.p[1][o] = v.x - rh;
+      out.p[2][o] = ih; out.p[3][o] = v.y - ih;
+    }
+  }
+}
+
+// plain c64 output of one atom (debug / parity of a1-a2, a6)
+__global__ void k_recon_c64(const float2* __restrict__ D, int n_par, const int32_t* __restrict__ bh, int n_beams,
+                            const int32_t* __restrict__ nn_idx, const float* __restrict__ nn_w, int max_nn,
+                            int carrier, int recon, const int32_t* __restrict__ origin, int atom, int w, int ny, int nx,
+                            const float2* __restrict__ rooty, const float2* __restrict__ rootx, float2* __restrict__ out) {
+  const int b = blockIdx.y;
+  const int w2 = w * w;
+  const int oy = origin[2 * atom], ox = origin[2 * atom + 1];
+  const int hyp = ((bh[2 * b] % ny) + ny) % ny, hxp = ((bh[2 * b + 1] % nx) + nx) % nx;
+  for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < w2; s += gridDim.x * blockDim.x) {
+    const int sy = s / w, sx = s - sy * w;
+    int ry = oy + sy; if (ry >= ny) ry -= ny;
+    int rx = ox + sx; if (rx >= nx) rx -= nx;
+    float2 t = tilt(rooty, rootx, hyp, hxp, ry, rx, ny, nx);
+    if (carrier < 0) t.y = -t.y;
+    out[(int64_t)b * w2 + s] = recon_elem(D, nn_idx + (int64_t)b * max_nn, nn_w + (int64_t)b * max_nn, max_nn, w2, s, recon, t);
+  }
+}
+
+// a3: A[rho][b] = c_b exp(-2 pi i (hy rho_y / ny + hx rho_x / nx)), phase in double (rho may be any real)
+__global__ void k_illumination(const double* __restrict__ rho, int n_rho, const int32_t* __restrict__ h,
+                               const float2* __restrict__ c, int n_ap, int ny, int nx, Planes out) {
+  const int r = blockIdx.y;
+  const double py = rho[2 * r], px = rho[2 * r + 1];
+  for (int b = blockIdx.x * blockDim.x + threadIdx.x; b < n_ap; b += gridDim.x * blockDim.x) {
+    double t = (double)h[2 * b] * py / ny + (double)h[2 * b + 1] * px / nx;
+    t -= rint(t);                                       // exact range reduction of the turn count
+    double sn, cs;
+    sincospi(-2.0 * t, &sn, &cs);
+    const float2 cb = c[b];
+    const float re = (float)((double)cb.x * cs - (double)cb.y * sn);
+    const float im = (float)((double)cb.x * sn + (double)cb.y * cs);
+    const int64_t o = (int64_t)r * out.ld + b;
+    const float rh = tf32_hi(re), ih = tf32_hi(im);
+    out.p[0][o] = rh; out.p[1][o] = re - rh;
+    out.p[2][o] = ih; out.p[3][o] = im - ih;
+  }
+}
+
+}  // namespace
+
+int32_t launch_crop_detilt(bip_ctx* ctx, const float2* S, const int32_t* ph_dev, int32_t n_par, int carrier,
+                           const int32_t* origin_dev, int32_t n_atoms, int32_t w, float2* D) {
+  dim3 grid((unsigned)((w * w + 255) / 256), (unsigned)n_par, (unsigned)n_atoms);
+  k_crop_detilt<<<grid, 256, 0, ctx->stream>>>(S, ph_dev, carrier, origin_dev, w, ctx->g.ny, ctx->g.nx,
+                                               ctx->rooty_dev, ctx->rootx_dev, D, n_par);
+  BIP_CUDA(ctx, cudaGetLastError());
+  ctx->timing.kernel_launches++;
+  return BIP_OK;
+}
+
+int32_t launch_recon(bip_ctx* ctx, const float2* D, int32_t n_par, const int32_t* bh_dev, int32_t n_beams,
+                     const int32_t* nn_idx, const float* nn_w, int32_t max_nn, int carrier, int recon,
+                     const int32_t* origin_dev, int32_t n_atoms, int32_t w, bool transpose, Planes out) {
+  const int w2 = w * w;
+  if (!transpose) {
+    for (int b0 = 0; b0 < n_beams; b0 += 65535) {     // gridDim.y limit
+      const int nb = std::min(65535, n_beams - b0);
+      Planes o = out;
+      for (int k = 0; k < 4; ++k) o.p[k] += (int64_t)b0 * out.ld;
+      dim3 grid((unsigned)((w2 + 255) / 256), (unsigned)nb, (unsigned)n_atoms);
+      k_recon_rows<<<grid, 256, 0, ctx->stream>>>(D, n_par, bh_dev + 2 * (int64_t)b0, nb, nn_idx + (int64_t)b0 * max_nn,
+                                                  nn_w + (int64_t)b0 * max_nn, max_nn, carrier, recon, origin_dev, w,
+                                                  ctx->g.ny, ctx->g.nx, ctx->rooty_dev, ctx->rootx_dev, o);
+      BIP_CUDA(ctx, cudaGetLastError());
+      ctx->timing.kernel_launches++;
+    }
+  } else {
+    dim3 grid((unsigned)((w2 + 31) / 32), (unsigned)((n_beams + 31) / 32), (unsigned)n_atoms);
+    k_recon_transposed<<<grid, dim3(32, 8), 0, ctx->stream>>>(D, n_par, bh_dev, n_beams, nn_idx, nn_w, max_nn, carrier, recon,
+                                                             origin_dev, w, ctx->g.ny, ctx->g.nx, ctx->rooty_dev,
+                                                             ctx->rootx_dev, out);
+    BIP_CUDA(ctx, cudaGetLastError());
+    ctx->timing.kernel_launches++;
+  }
+  return BIP_OK;
+}
+
+int32_t launch_recon_c64(bip_ctx* ctx, const float2* D, int32_t n_par, const int32_t* bh_dev, int32_t n_beams,
+                         const int32_t* nn_idx, const float* nn_w, int32_t max_nn, int carrier, int recon,
+                         const int32_t* origin_dev, int32_t atom, int32_t w, float2* out) {
+  for (int b0 = 0; b0 < n_beams; b0 += 65535) {
+    const int nb = std::min(65535, n_beams - b0);
+    dim3 grid((unsigned)((w * w + 255) / 256), (unsigned)nb);
+    k_recon_c64<<<grid, 256, 0, ctx->stream>>>(D, n_par, bh_dev + 2 * (int64_t)b0, nb, nn_idx + (int64_t)b0 * max_nn,
+                                               nn_w + (int64_t)b0 * max_nn, max_nn, carrier, recon, origin_dev, atom, w,
+                                               ctx->g.ny, ctx->g.nx, ctx->rooty_dev, ctx->rootx_dev,
+                                               out + (int64_t)b0 * w * w);
+    BIP_CUDA(ctx, cudaGetLastError());
+  }
+  return BIP_OK;
+}
+
+int32_t launch_illumination(bip_ctx* ctx, const double* rho_dev, int32_t n_rho, Planes out) {
+  for (int r0 = 0; r0 < n_rho; r0 += 65535) {
+    const int nr = std::min(65535, n_rho - r0);
+    Planes o = out;
+    for (int k = 0; k < 4; ++k) o.p[k] += (int64_t)r0 * out.ld;
+    dim3 grid((unsigned)((ctx->n_ap + 255) / 256), (unsigned)nr);
+    k_illumination<<<grid, 256, 0, ctx->stream>>>(rho_dev + 2 * (int64_t)r0, nr, ctx->ap_h_dev, ctx->ap_c_dev, ctx->n_ap,
+                                                  ctx->g.ny, ctx->g.nx, o);
+    BIP_CUDA(ctx, cudaGetLastError());
+  }
+  return BIP_OK;
+}
+
+}  // namespace bip
