@@ -1,0 +1,363 @@
+#!/usr/bin/env python
+"""Benchmark of the BiP-PRISM on-atom contraction on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg2] [--atoms A]
+
+A *step* is one pass of the whole hot path (plane-loop driver, crop, de-tilt, NNW
+reconstruction, probe GEMM, (.)H_n, detector GEMM, |a|^2 reduction) over one batch of ``--atoms`` ionised atoms of
+the synthetic BASELINE.json configs[1] cell (512^2 grid, 40 slices, 300 kV, 25/40 mrad, parent factor 4, 9
+channels, 48 x 48 windows, 64 x 64 scan, elemental-map output), all scan positions, channels and detector beams.
+metric = scan-pos x atom x channel x detector-beam amplitudes per second.
+
+  value   inputs resident in HBM, whole step timed on the device (CUDA events on the launching stream);
+  e2e     the same through the host-buffer entry points: per step the edge (sites, H_n windows, detector beams,
+          weight table) is copied host->device from pinned memory by bip_add_edge and the map is read back by
+          bip_map_host;
+  roofline  the detector-projection kernel (a7-a8, >= 90 % of the flops): algorithmic flops / its event time,
+          against the fp32-equivalent ceiling of the arithmetic in use;
+  cpu_baseline  the fp64 NumPy oracle, as it stands, on the host cores, on a bounded sample.
+
+With N > 1 (torchrun) every rank runs the same step on its own atoms (independent problems, no data-path
+collective): weak scaling, value = total amplitudes / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+sys.path.insert(0, os.path.join(ROOT, "tests"))
+
+METRIC = "scan-pos x atom x channel x detector-beam amplitudes/s"
+UNIT = "amplitudes/s"
+SM_COUNT, FMA_LANES, = 148, 128
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return d, "measured"
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.th.join(timeout=2)
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        pw = [float(r[2]) for r in self.rows if len(r) > 2 and r[2].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for k, n in enumerate(names) if any(len(r) > 3 + k and r[3 + k].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": reasons}
+
+
+def pinned(a: np.ndarray) -> np.ndarray:
+    """Copy of ``a`` in page-locked host memory (numpy view of a pinned torch tensor)."""
+    import torch
+    t = torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    return t.numpy()
+
+
+def build_problem(args, rank):
+    """Synthetic configs[1] cell; the edge is sampled down to --atoms sites of the first ionisation plane(s)."""
+    from bip_inputs.specimen import make_workload
+    wl = make_workload(args.workload, scale=args.scale)
+    e = wl.edges[0]
+    lo = rank * args.atoms                     # each rank takes its own atoms of the same planes (weak scaling)
+    idx = np.arange(lo, min(lo + args.atoms, e.n_atoms))
+    return wl, e.take(idx)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2607_00756_b200 as B
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (libbip has no CPU path)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    peaks, peak_src = load_peaks()
+    prec = {"tf32x3": B.PREC_TF32X3, "fp32_simt": B.PREC_FP32_SIMT}[args.precision]
+    recon = {"linear": B.RECON_LINEAR, "magphase": B.RECON_MAGPHASE}[args.recon]
+
+    wl, edge = build_problem(args, rank)
+    g = B.Grid(wl.ny, wl.nx, wl.ly, wl.lx, wl.nz, wl.dz, wl.lam)
+    geo = B.plan_geometry(g, wl.alpha_mrad, edge.det_mrad, wl.defocus, wl.parent_factor)
+    T_dev = torch.from_numpy(wl.T).cuda()
+    ctx = B.Context(g, T_dev, geo.ap_h, geo.ap_c, geo.p1_h, geo.w1, geo.p2_h)
+    ctx.build_S1()
+    ctx.build_S2()
+    ctx.set_scan(wl.scan)
+    eid = ctx.add_edge(edge.slice, edge.centre, edge.H, geo.det_h, geo.w2)
+    torch.cuda.synchronize()
+    t_build = ctx.get_timing()
+    out = torch.empty(ctx.n_rho, dtype=torch.float64, device="cuda")
+    first_plane = int(edge.slice.min())
+
+    def step():
+        ctx.seek_plane(max(first_plane - 1, 0))      # every step moves the plane cursor (ADVANCETO / PEELTO) again
+        ctx.map(eid, B.MODE_MAP, recon, prec, out=out)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    gemm2_ms, gemm2_launches, contract_ms, adv_ms, launches = 0.0, 0, 0.0, 0.0, 0
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        step()
+        t = ctx.get_timing()                         # synchronises; the spans are device event times
+        gemm2_ms += t["gemm2_ms"]; gemm2_launches += t["gemm2_launches"]; contract_ms += t["contract_ms"]
+        adv_ms += t["advance_peel_ms"]; launches += t["kernel_launches"]
+    ev1.record()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    ms_total = ev0.elapsed_time(ev1)
+    if world > 1:
+        tt = torch.tensor([ms_total], device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms_total = float(tt.item())
+    amps_step = float(ctx.n_rho) * edge.n_atoms * edge.n_ch * geo.det_h.shape[0]
+    value = amps_step * world * args.steps / (ms_total * 1e-3)
+    map_dev = out.cpu().numpy()
+
+    # ---- end to end through the host-buffer API: pinned inputs in, map out, every step ----
+    h_slice, h_centre, h_H = pinned(edge.slice), pinned(edge.centre), pinned(edge.H)
+    h_det, h_idx, h_w = pinned(geo.det_h), pinned(geo.w2[0]), pinned(geo.w2[1])
+    h2d = sum(a.nbytes for a in (h_slice, h_centre, h_H, h_det, h_idx, h_w)) + 2 * 4 * edge.n_atoms + 2 * 4 * geo.det_h.shape[0]
+    d2h = ctx.n_rho * 8
+
+    def step_e2e():
+        ctx.clear_edges()
+        e2 = ctx.add_edge(h_slice, h_centre, h_H, h_det, (h_idx, h_w))
+        ctx.seek_plane(max(first_plane - 1, 0))
+        return ctx.map_host(e2, B.MODE_MAP, recon, prec)
+
+    step_e2e()
+    barrier()
+    t0 = time.perf_counter()
+    e2e_steps = max(1, min(args.steps, 3))
+    for _ in range(e2e_steps):
+        m_host = step_e2e()
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        tt = torch.tensor([e2e_s], device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e_s = float(tt.item())
+    e2e_value = amps_step * world * e2e_steps / e2e_s
+    assert np.allclose(m_host, map_dev, rtol=1e-5, atol=0), "host-buffer path disagrees with the device path"
+
+    # ---- roofline of the dominant kernel (a7-a8) ----
+    w2 = edge.W * edge.W
+    flops_gemm2_step = 8.0 * ctx.n_rho * w2 * edge.n_atoms * edge.n_ch * geo.det_h.shape[0]
+    achieved = flops_gemm2_step * args.steps / (gemm2_ms * 1e-3) / 1e12 if gemm2_ms > 0 else 0.0
+    if args.precision == "tf32x3":
+        tf32_peak = peaks["bf16_tflops_sustained"] * (1.1 / 2.25)          # nominal tf32 : bf16 ratio (B200_PROFILING.md)
+        roof = {"bound": "tensor", "achieved": achieved, "peak": tf32_peak / 3.0, "unit": "TFLOP/s",
+                "frac": achieved / (tf32_peak / 3.0), "traffic": None, "kernel": "k_gemm2_tc",
+                "note": f"fp32-equivalent flops; 3xTF32 issues 3 tensor flops per flop: ceiling = tf32 peak {tf32_peak:.0f} / 3 "
+                        f"(bf16 sustained x 1.1/2.25, {peak_src}); issued tensor rate {3 * achieved:.1f} TFLOP/s",
+                "avg_launch_ms": gemm2_ms / max(gemm2_launches, 1), "launches": gemm2_launches}
+    else:
+        alu_peak = SM_COUNT * FMA_LANES * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
+        roof = {"bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s", "frac": achieved / alu_peak,
+                "traffic": None, "kernel": "k_gemm2_simt",
+                "note": "fp32 FMA peak = 148 SMs x 128 lanes x 2 x max SM clock (reference CUDA-core path)",
+                "avg_launch_ms": gemm2_ms / max(gemm2_launches, 1), "launches": gemm2_launches}
+    traffic_file = os.path.join(ROOT, "profiles", "gemm2_traffic.json")
+    if os.path.exists(traffic_file):
+        roof["traffic"] = json.load(open(traffic_file)).get(roof["kernel"])
+
+    line = None
+    if rank == 0:
+        cpu = cpu_baseline(args) if world == 1 and not args.no_cpu_baseline else None
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "tf32x3(c64)" if args.precision == "tf32x3" else "f32(c64)", "data": "synthetic",
+            "config": {"workload": f"BASELINE configs[1] ({wl.name}): {wl.ny}x{wl.nx} grid, {wl.nz} slices, B={geo.ap_h.shape[0]}, "
+                                   f"K={geo.det_h.shape[0]}, parents=({ctx.n_p1},{ctx.n_p2}), W={edge.W}, N_ch={edge.n_ch}, "
+                                   f"N_rho={ctx.n_rho}, map output, recon={args.recon}",
+                       "atoms_per_step_per_gpu": edge.n_atoms, "sampled": "first sites of the first B plane; the full edge has "
+                       f"{wl.edges[0].n_atoms} sites", "precision": args.precision,
+                       "l2": "per-step working set (operand planes > 5 GB per atom) far exceeds the 126 MB L2: no flush needed",
+                       "parallelism": f"atoms sharded over {world} GPU(s), no data-path collective"},
+            "clocks": clocks, "gpu_launches": launches,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                    "steps": e2e_steps},
+            "roofline": roof,
+            "phases_ms_per_step": {"contract": contract_ms / args.steps, "gemm2": gemm2_ms / args.steps,
+                                   "advance_peel": adv_ms / args.steps, "build_s1_once": t_build["build_s1_ms"],
+                                   "build_s2_once": t_build["build_s2_ms"]},
+            "fp32_equiv_tflops_contract": float(ctx.get_timing()["flops"]) * 1.0 / (contract_ms / args.steps * 1e-3) / 1e12 if contract_ms else None,
+            "cpu_baseline": cpu,
+        }
+        print(json.dumps(line))
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return line
+
+
+def oracle_sample_setup(args):
+    """The bounded sample timed on the host cores: ONE atom of the same cell geometry (same grid, beams, parents,
+    window, channels, all detector beams), a 16 x 16 subset of the scan, slab truncated to its first two slices so
+    that the (untimed) fp64 parent windows are cheap to build.  Contraction shapes per (scan, channel, beam) are
+    those of the full workload."""
+    from bip_inputs.specimen import make_workload
+    from helpers import OracleSetup
+    from oracle import bip as obip
+    from oracle import multislice as oms
+    wl = make_workload(args.workload, scale=args.scale, nz=2)
+    e = wl.edges[0].take([0])
+    orc = OracleSetup(wl, e, n_jobs=os.cpu_count())
+    T = wl.T.astype(np.complex128)
+    plane = int(e.slice[0])
+    crops = []
+    for which, par_h in ((1, orc.ap[orc.p1_pos]), (2, orc.det[orc.p2_pos])):
+        parts = []
+        for c0 in range(0, len(par_h), 256):          # parents in chunks: only the windows are kept
+            hs = par_h[c0:c0 + 256]
+            if which == 1:
+                S = oms.build_S1(hs, wl.ny, wl.nx)
+                for i in range(plane):
+                    S = oms.advance_S1(S, T[i], orc.P)
+            else:
+                S = oms.build_S2_at(hs, T, orc.P, plane)
+            parts.append(obip.crop_window(S, e.centre[0], e.W, wl.ny, wl.nx))
+        crops.append(np.concatenate(parts))
+    sy, sx = wl.scan_shape
+    sub = np.array([iy * sx + ix for iy in range(0, sy, max(1, sy // 16)) for ix in range(0, sx, max(1, sx // 16))])[:256]
+    scan = wl.scan[sub]
+    A = obip.illumination(orc.c, orc.ap, scan, wl.ny, wl.nx)
+    return wl, e, orc, crops, A
+
+
+def oracle_sample_run(wl, e, orc, crops, A, recon):
+    from oracle import bip as obip
+    a, _ = obip.atom_amplitudes(None, None, orc.ap[orc.p1_pos], orc.det[orc.p2_pos], orc.ap, orc.det, orc.w1, orc.w2, A,
+                                e.H.astype(np.complex128), e.centre[0], wl.ny, wl.nx, recon, crops=tuple(crops))
+    return obip.reduce_modes(a, orc.det)["map"]
+
+
+def _threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = [p["num_threads"] for p in threadpool_info() if p.get("user_api") == "blas"]
+        return max(n) if n else os.cpu_count()
+    except Exception:
+        return os.cpu_count()
+
+
+def cpu_baseline(args):
+    setup = oracle_sample_setup(args)
+    wl, e, orc, crops, A = setup
+    t0 = time.perf_counter()
+    m = oracle_sample_run(*setup, args.recon)
+    dt = time.perf_counter() - t0
+    amps = float(A.shape[0]) * 1 * e.n_ch * len(orc.det)
+    return {"value": amps / dt, "unit": UNIT, "cores": _threads(), "host_cpus": os.cpu_count(), "kind": "oracle", "seconds": dt,
+            "sample": f"1 atom x {A.shape[0]} scan positions x {e.n_ch} channels x {len(orc.det)} detector beams of the same cell "
+                      f"(slab truncated to 2 slices for the untimed window build); steps a1-a8, NumPy complex128",
+            "map_sum": float(m.sum())}
+
+
+def run_reference(args):
+    """The oracle as it stands, timed on the host cores (this tier's reference arm)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return None
+    setup = oracle_sample_setup(args)
+    wl, e, orc, crops, A = setup
+    for _ in range(min(args.warmup, 1)):
+        oracle_sample_run(*setup, args.recon)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_sample_run(*setup, args.recon)
+    dt = time.perf_counter() - t0
+    amps = float(A.shape[0]) * e.n_ch * len(orc.det)
+    v = amps * args.steps / dt
+    sample = (f"each step: 1 atom x {A.shape[0]} scan positions x {e.n_ch} channels x {len(orc.det)} detector beams of "
+              f"BASELINE configs[1] geometry (slab truncated to 2 slices for the untimed fp64 window build)")
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": int(os.environ.get("WORLD_SIZE", "1")),
+            "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64(c128)", "data": "synthetic",
+            "config": {"workload": f"BASELINE configs[1] ({wl.name}) sampled", "sample": sample, "recon": args.recon},
+            "cpu_baseline": {"value": v, "unit": UNIT, "kind": "oracle", "cores": _threads(), "sample": sample},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line))
+    return line
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg2")
+    ap.add_argument("--scale", type=int, default=1, help="shrink cells and grid together (debug; 1 = BASELINE size)")
+    ap.add_argument("--atoms", type=int, default=2, help="ionised atoms per step per GPU")
+    ap.add_argument("--precision", default=os.environ.get("BIP_BENCH_PRECISION", "fp32_simt"), choices=["tf32x3", "fp32_simt"])
+    ap.add_argument("--recon", default="magphase", choices=["linear", "magphase"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

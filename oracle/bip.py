@@ -28,13 +28,22 @@ def tilt_phases(h, ys, xs, ny, nx, sign):
     return np.exp(sign * 2j * np.pi * ph).reshape(h.shape[0], -1)
 
 
-def reconstruct_window(S_par, parent_h, beam_h, w, centre, W, ny, nx, carrier, recon):
+def crop_window(S_par, centre, W, ny, nx):
+    """S_p | Omega_tau for every parent column: [Bp, W*W]."""
+    ys, xs = window_pixels(centre, W, ny, nx)
+    return S_par[:, ys][:, :, xs].reshape(S_par.shape[0], -1)
+
+
+def reconstruct_window(S_par, parent_h, beam_h, w, centre, W, ny, nx, carrier, recon, crop=None):
     """Windowed column reconstruction (eq. 15; eq. 11, PAPER.md:183 for recon="magphase").
 
     crop the parent columns on Omega_tau -> de-tilt -> NNW-combine to the full beam set -> re-tilt.
-    S_par [Bp, ny, nx]; w sparse/dense [n_beams, Bp]; returns R [n_beams, W*W]."""
+    S_par [Bp, ny, nx]; w sparse/dense [n_beams, Bp]; returns R [n_beams, W*W].
+    ``crop`` may hand in the already cropped columns [Bp, W*W] (then S_par is not read): large configs keep
+    only the windows of the sampled atoms in memory (SURVEY 8(d) "Parity protocol")."""
     ys, xs = window_pixels(centre, W, ny, nx)
-    crop = S_par[:, ys][:, :, xs].reshape(S_par.shape[0], -1)                 # S_p | Omega
+    if crop is None:
+        crop = crop_window(S_par, centre, W, ny, nx)                          # S_p | Omega
     D = crop * tilt_phases(parent_h, ys, xs, ny, nx, -carrier)                # S_p^dt  (eq. 10)
     z = w @ D                                                                 # sum_p w_{b,p} S_p^dt
     if recon == "linear":
@@ -55,14 +64,15 @@ def illumination(c, beams, scan, ny, nx):
     return c[None, :] * np.exp(-2j * np.pi * ph)
 
 
-def atom_amplitudes(S1, S2, p1_h, p2_h, ap_beams, det_beams, w1, w2, A, H, centre, ny, nx, recon):
+def atom_amplitudes(S1, S2, p1_h, p2_h, ap_beams, det_beams, w1, w2, A, H, centre, ny, nx, recon, crops=None):
     """Steps a1-a7 for one ionised atom: amplitudes a[n, rho, d] (eq. 13 in the probe-first association).
 
     Psi[rho, s] = sum_b c_b(rho) S1^b|Omega (eq. 7 on the window);  Phi_n = H_n . Psi (eq. 3);
     a_d = G^-1/2 sum_s S2^d|Omega[s] Phi_n[s]  (eq. 12-13, unitary F: SURVEY c3)."""
     W = H.shape[1]
-    R1 = reconstruct_window(S1, p1_h, ap_beams, w1, centre, W, ny, nx, +1, recon)     # [B, W^2]
-    R2 = reconstruct_window(S2, p2_h, det_beams, w2, centre, W, ny, nx, -1, recon)    # [K, W^2]
+    c1, c2 = crops if crops is not None else (None, None)
+    R1 = reconstruct_window(S1, p1_h, ap_beams, w1, centre, W, ny, nx, +1, recon, c1)     # [B, W^2]
+    R2 = reconstruct_window(S2, p2_h, det_beams, w2, centre, W, ny, nx, -1, recon, c2)    # [K, W^2]
     Psi = A @ R1                                                                       # [n_rho, W^2]
     a = np.empty((H.shape[0], A.shape[0], det_beams.shape[0]), dtype=np.complex128)
     for n in range(H.shape[0]):

@@ -5,6 +5,7 @@ the *unitary* transform of PAPER.md:312 is F / sqrt(G) (c3).  No band-limit (c13
 signed; pixel r = (ry, rx); h.r/N = hy ry / ny + hx rx / nx.
 """
 import numpy as np
+from scipy import fft as _fft
 
 
 def fresnel_propagator(ny, nx, ly, lx, lam, dz):
@@ -18,8 +19,9 @@ def fresnel_propagator(ny, nx, ly, lx, lam, dz):
 
 
 def propagate(psi, P):
-    """Fresnel operator: F^-1[P . F psi] (eq. 2)."""
-    return np.fft.ifft2(P * np.fft.fft2(psi))
+    """Fresnel operator: F^-1[P . F psi] (eq. 2) on the last two axes (library FFT; stacks of columns are
+    transformed together, one thread per column)."""
+    return _fft.ifft2(P * _fft.fft2(psi, workers=-1), workers=-1)
 
 
 def slice_step(psi, T_j, P):
@@ -60,7 +62,7 @@ def build_S1(parent_h, ny, nx):
 def advance_S1(S1, T_i, P):
     """ADVANCETO by one slice: S_b <- P(T_i S_b) on every row (eq. 6).
     After advancing through slices 0..i-1 the rows are the waves entering slice i."""
-    return np.stack([slice_step(s, T_i, P) for s in S1])
+    return slice_step(S1, T_i, P)
 
 
 def build_S2(parent_h, T, P):
@@ -69,32 +71,22 @@ def build_S2(parent_h, T, P):
     S2^d := M^T chi*_d so that sum_r S2^d(r) w(r) = [F M_{i->exit} w]_{h_d} with NO conjugation in the pairing:
     start from the conjugate detector plane wave exp(-2 pi i h_d.r/N) at the exit surface and apply
     u <- T_j . P[u] for j = nz-1 .. 0 (transpose of transmit-then-propagate; P^T = P since P(q) is even)."""
-    ny, nx = T.shape[1:]
-    out = []
-    for h in parent_h:
-        u = plane_wave(h, ny, nx, -1)
-        for j in range(T.shape[0] - 1, -1, -1):
-            u = T[j] * propagate(u, P)
-        out.append(u)
-    return np.stack(out)
+    return build_S2_at(parent_h, T, P, 0)
 
 
 def build_S2_at(parent_h, T, P, i):
     """S2 at plane i built directly from the exit surface (contains slices i .. nz-1)."""
     ny, nx = T.shape[1:]
-    out = []
-    for h in parent_h:
-        u = plane_wave(h, ny, nx, -1)
-        for j in range(T.shape[0] - 1, i - 1, -1):
-            u = T[j] * propagate(u, P)
-        out.append(u)
-    return np.stack(out)
+    u = np.stack([plane_wave(h, ny, nx, -1) for h in parent_h])
+    for j in range(T.shape[0] - 1, i - 1, -1):
+        u = T[j] * propagate(u, P)
+    return u
 
 
 def peel_S2(S2, T_i, P):
     """PEELTO by one slice: S2^(i+1) = P*[T_i* . S2^(i)], exact because |T| = 1."""
     Pc = np.conj(P)
-    return np.stack([propagate(np.conj(T_i) * u, Pc) for u in S2])
+    return propagate(np.conj(T_i) * S2, Pc)
 
 
 def embed_window(Hwin, centre, ny, nx):

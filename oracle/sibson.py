@@ -64,14 +64,36 @@ def _cell(poly, site, others, tol):
     return poly, cutters
 
 
-def sibson_row(x, parents_q, qmax):
+def sibson_row(x, parents_q, qmax, prune=True):
     """Weights of one query point x (physical q, shape [2]) on the parents ([P, 2]).
-    Returns (indices ascending, weights)."""
+    Returns (indices ascending, weights).
+
+    prune: work on the nearest parents only, when that provably changes nothing.  Let R be the largest distance
+    from x to a vertex of C(x).  A parent o with |o - x| > 2R cannot bound C(x) (every y in C(x) has
+    |y - o| >= |o - x| - R > R >= |y - x|), and a parent o with |o - x| > 4R cannot bound C(x) & V_P(p) for a
+    neighbour p (|y - p| <= |y - x| + |x - p| <= 3R < |o - x| - R <= |y - o|).  So the cell is first built from
+    the k nearest parents and accepted if every other parent is farther than 4R; otherwise k is doubled."""
     parents_q = np.asarray(parents_q, dtype=np.float64)
     x = np.asarray(x, dtype=np.float64)
     hit = np.nonzero(np.all(parents_q == x[None, :], axis=1))[0]
     if hit.size:
         return hit[:1].astype(np.int64), np.ones(1)
+    if prune and parents_q.shape[0] > 64:
+        d2 = np.sum((parents_q - x[None, :]) ** 2, axis=1)
+        order = np.argsort(d2, kind="stable")
+        k = 48
+        while k < parents_q.shape[0]:
+            near = order[:k]
+            half = BOX_FACTOR * qmax
+            box = np.array([[-half, -half], [-half, half], [half, half], [half, -half]], dtype=np.float64)
+            cx, _ = _cell(box, x, parents_q[near], 1e-13 * half * half)
+            R2 = np.max(np.sum((cx - x[None, :]) ** 2, axis=1))
+            if d2[order[k]] > 16.0 * R2:                       # every excluded parent is farther than 4R
+                idx, w = sibson_row(x, parents_q[near], qmax, prune=False)
+                idx = near[idx]
+                o = np.argsort(idx)
+                return idx[o].astype(np.int64), w[o]
+            k *= 2
     half = BOX_FACTOR * qmax
     box = np.array([[-half, -half], [-half, half], [half, half], [half, -half]], dtype=np.float64)
     tol = 1e-13 * half * half

@@ -69,7 +69,7 @@ static int32_t planes_in(bip_ctx* ctx, DevBuf& buf, Planes& P, int64_t rows, int
 template <class T>
 static int32_t upload(bip_ctx* ctx, T** dst, const T* src, size_t n, const char* what) {
   BIP_TRY(dev_alloc(ctx, (void**)dst, n * sizeof(T), what));
-  BIP_CUDA(ctx, cudaMemcpyAsync(*dst, src, n * sizeof(T), cudaMemcpyHostToDevice, ctx->stream));
+  if (n) BIP_CUDA(ctx, cudaMemcpyAsync(*dst, src, n * sizeof(T), cudaMemcpyHostToDevice, ctx->stream));
   return BIP_OK;
 }
 
@@ -363,7 +363,7 @@ int32_t bip_destroy(bip_ctx* ctx) {
   if (it != spans().end()) { it->second.pool_map.destroy(); it->second.pool_b1.destroy(); it->second.pool_b2.destroy(); spans().erase(it); }
   if (ctx->T_owned) cudaFree((void*)ctx->T_dev);
   void* ptrs[] = {ctx->ap_h_dev, ctx->p1_h_dev, ctx->p2_h_dev, ctx->ap_c_dev, ctx->w1_idx_dev, ctx->w1_w_dev, ctx->rooty_dev,
-                  ctx->rootx_dev, ctx->P_dev, ctx->S1, ctx->S2, ctx->D1.p, ctx->D2.p, ctx->R1.p, ctx->R2.p, ctx->Psi.p,
+                  ctx->rootx_dev, ctx->P_dev, ctx->ms_work, ctx->S1, ctx->S2, ctx->D1.p, ctx->D2.p, ctx->R1.p, ctx->R2.p, ctx->Psi.p,
                   ctx->Phi.p, ctx->A.p[0]};
   for (void* p : ptrs) if (p) cudaFree(p);
   cudaGetLastError();
@@ -462,7 +462,7 @@ int32_t bip_add_edge(bip_ctx* ctx, int32_t n_atoms, const int32_t* slice, const 
   BIP_TRY(upload(ctx, &e.nn_w_dev, w2->nn_w, (size_t)n_det * w2->max_nn, "w2 weights"));
   BIP_TRY(upload(ctx, &e.bin_of_det_x_dev, bx.data(), (size_t)n_det, "qEELS bins"));
   BIP_TRY(upload(ctx, &e.bin_of_det_y_dev, by.data(), (size_t)n_det, "qEELS bins"));
-  BIP_TRY(upload(ctx, &ed.origin_dev, e.origin.data(), std::max<size_t>(2 * (size_t)n_atoms, 2), "window origins"));
+  BIP_TRY(upload(ctx, &ed.origin_dev, e.origin.data(), 2 * (size_t)n_atoms, "window origins"));
   BIP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));     // host sources may go away after return
   ctx->edges.push_back(std::move(e));
   edge_dev()[ctx].push_back(ed);

@@ -75,7 +75,8 @@ struct bip_ctx {
 
   // roots of unity exp(2 pi i k / N), k = 0..N-1 (exact phases for tilt / de-tilt)
   float2 *rooty_dev = nullptr, *rootx_dev = nullptr;
-  float2* P_dev = nullptr;         // Fresnel propagator / G  (forward step)
+  void* P_dev = nullptr;           // Fresnel propagator / G as double2 [ny][nx]
+  void* ms_work = nullptr;         // double2 workspace of the slice steps [plan_batch][ny][nx]
   float2 *S1 = nullptr, *S2 = nullptr;
   bool s1_built = false, s2_built = false;
   int32_t plane1 = 0, plane2 = 0;  // S1 holds slices 0..plane1-1; S2 holds slices plane2..nz-1
@@ -101,9 +102,11 @@ namespace bip {
 #define BIP_CUDA(ctx, call)                                                                          \
   do {                                                                                               \
     cudaError_t e_ = (call);                                                                         \
-    if (e_ != cudaSuccess)                                                                           \
+    if (e_ != cudaSuccess) {                                                                         \
+      (void)cudaGetLastError(); /* do not leave it for an unrelated later check */                   \
       return bip::fail((ctx), e_ == cudaErrorMemoryAllocation ? BIP_ERR_OOM : BIP_ERR_CUDA,          \
                        "%s:%d %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_));           \
+    }                                                                                                \
   } while (0)
 
 #define BIP_TRY(call)                  \

@@ -27,14 +27,50 @@ __global__ void k_plane_waves(float2* __restrict__ S, const int32_t* __restrict_
   }
 }
 
-// S[p][i] *= (conj ? conj(F[i]) : F[i]) for a batch of columns; F is a single [G] field (T_j, or P/G).
-__global__ void k_mul_field(float2* __restrict__ S, const float2* __restrict__ F, int64_t G, int conj_f) {
+// cuFFT's single-precision C2C loses ~3e-7 of the norm^2 per forward+inverse pair, systematically (measured on
+// B200, profiles/r01_notes.md); over tens of slices that alone breaks the 1e-6 summed-intensity bound.  The slice
+// steps therefore run in double precision (Z2Z) on a chunk workspace and the columns are stored back as c64:
+// the only rounding per slice is one unbiased round-to-nearest of the result.
+
+// W[p][i] = (double) S[p][i] * (mode 0: 1, 1: T[i], 2: conj T[i])
+__global__ void k_load_cols(double2* __restrict__ W, const float2* __restrict__ S, const float2* __restrict__ T,
+                            int64_t G, int mode) {
   const int64_t p = blockIdx.y;
-  float2* col = S + p * G;
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < G; i += (int64_t)gridDim.x * blockDim.x) {
-    float2 f = F[i];
-    if (conj_f) f.y = -f.y;
-    col[i] = cmul(col[i], f);
+    const float2 s = S[p * G + i];
+    double2 v = make_double2(s.x, s.y);
+    if (mode) {
+      const float2 t = T[i];
+      const double tr = t.x, ti = mode == 2 ? -(double)t.y : (double)t.y;
+      v = make_double2(v.x * tr - v.y * ti, v.x * ti + v.y * tr);
+    }
+    W[p * G + i] = v;
+  }
+}
+
+// W[p][i] *= (conj ? conj(P[i]) : P[i])   (P carries the 1/G of the unnormalised transform pair)
+__global__ void k_mul_prop(double2* __restrict__ W, const double2* __restrict__ P, int64_t G, int conj_p) {
+  const int64_t p = blockIdx.y;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < G; i += (int64_t)gridDim.x * blockDim.x) {
+    const double2 f = P[i];
+    const double fi = conj_p ? -f.y : f.y;
+    const double2 v = W[p * G + i];
+    W[p * G + i] = make_double2(v.x * f.x - v.y * fi, v.x * fi + v.y * f.x);
+  }
+}
+
+// S[p][i] = (float) (W[p][i] * (mode 0: 1, 1: T[i], 2: conj T[i]))
+__global__ void k_store_cols(float2* __restrict__ S, const double2* __restrict__ W, const float2* __restrict__ T,
+                             int64_t G, int mode) {
+  const int64_t p = blockIdx.y;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < G; i += (int64_t)gridDim.x * blockDim.x) {
+    double2 v = W[p * G + i];
+    if (mode) {
+      const float2 t = T[i];
+      const double tr = t.x, ti = mode == 2 ? -(double)t.y : (double)t.y;
+      v = make_double2(v.x * tr - v.y * ti, v.x * ti + v.y * tr);
+    }
+    S[p * G + i] = make_float2((float)v.x, (float)v.y);
   }
 }
 
@@ -52,7 +88,7 @@ int32_t get_plan(bip_ctx* ctx, int batch, cufftHandle* out) {
   if (it != pc.plans.end()) { *out = it->second; return BIP_OK; }
   cufftHandle h;
   int n[2] = {ctx->g.ny, ctx->g.nx};
-  cufftResult r = cufftPlanMany(&h, 2, n, nullptr, 1, ctx->g.ny * ctx->g.nx, nullptr, 1, ctx->g.ny * ctx->g.nx, CUFFT_C2C, batch);
+  cufftResult r = cufftPlanMany(&h, 2, n, nullptr, 1, ctx->g.ny * ctx->g.nx, nullptr, 1, ctx->g.ny * ctx->g.nx, CUFFT_Z2Z, batch);
   if (r != CUFFT_SUCCESS) return fail(ctx, r == CUFFT_ALLOC_FAILED ? BIP_ERR_OOM : BIP_ERR_CUDA, "cufftPlanMany(%dx%d, batch %d) failed: %d", ctx->g.ny, ctx->g.nx, batch, (int)r);
   r = cufftSetStream(h, ctx->stream);
   if (r != CUFFT_SUCCESS) return fail(ctx, BIP_ERR_CUDA, "cufftSetStream failed: %d", (int)r);
@@ -61,26 +97,28 @@ int32_t get_plan(bip_ctx* ctx, int batch, cufftHandle* out) {
   return BIP_OK;
 }
 
-int32_t fft_cols(bip_ctx* ctx, float2* S, int n_cols, int dir) {
+// One unitary slice operation on all columns of S:  S <- post . F^-1[ Pspec . F[ pre . S ] ]
+//   pre / post: 0 = identity, 1 = T_j, 2 = conj T_j ;  conj_p: multiply the spectrum by conj(P) instead of P
+int32_t slice_op(bip_ctx* ctx, float2* S, int n_cols, const float2* Tj, int pre, int conj_p, int post) {
   const int64_t G = (int64_t)ctx->g.ny * ctx->g.nx;
   const int chunk = ctx->plan_batch;
+  double2* W = reinterpret_cast<double2*>(ctx->ms_work);
+  const double2* P = reinterpret_cast<const double2*>(ctx->P_dev);
   for (int c0 = 0; c0 < n_cols; c0 += chunk) {
     const int nb = std::min(chunk, n_cols - c0);
     cufftHandle h;
     BIP_TRY(get_plan(ctx, nb, &h));
-    cufftComplex* p = reinterpret_cast<cufftComplex*>(S + (int64_t)c0 * G);
-    cufftResult r = cufftExecC2C(h, p, p, dir);
-    if (r != CUFFT_SUCCESS) return fail(ctx, BIP_ERR_CUDA, "cufftExecC2C failed: %d", (int)r);
+    float2* Sc = S + (int64_t)c0 * G;
+    dim3 grid((unsigned)std::min<int64_t>((G + 255) / 256, 2048), (unsigned)nb);
+    k_load_cols<<<grid, 256, 0, ctx->stream>>>(W, Sc, Tj, G, pre);
+    cufftResult r = cufftExecZ2Z(h, reinterpret_cast<cufftDoubleComplex*>(W), reinterpret_cast<cufftDoubleComplex*>(W), CUFFT_FORWARD);
+    if (r != CUFFT_SUCCESS) return fail(ctx, BIP_ERR_CUDA, "cufftExecZ2Z failed: %d", (int)r);
+    k_mul_prop<<<grid, 256, 0, ctx->stream>>>(W, P, G, conj_p);
+    r = cufftExecZ2Z(h, reinterpret_cast<cufftDoubleComplex*>(W), reinterpret_cast<cufftDoubleComplex*>(W), CUFFT_INVERSE);
+    if (r != CUFFT_SUCCESS) return fail(ctx, BIP_ERR_CUDA, "cufftExecZ2Z failed: %d", (int)r);
+    k_store_cols<<<grid, 256, 0, ctx->stream>>>(Sc, W, Tj, G, post);
+    BIP_CUDA(ctx, cudaGetLastError());
   }
-  return BIP_OK;
-}
-
-int32_t mul_field(bip_ctx* ctx, float2* S, int n_cols, const float2* F, int conj_f) {
-  const int64_t G = (int64_t)ctx->g.ny * ctx->g.nx;
-  dim3 grid((unsigned)std::min<int64_t>((G + 255) / 256, 1024), (unsigned)n_cols);
-  // gridDim.y is limited to 65535 columns, far above any parent count used here
-  k_mul_field<<<grid, 256, 0, ctx->stream>>>(S, F, G, conj_f);
-  BIP_CUDA(ctx, cudaGetLastError());
   return BIP_OK;
 }
 
@@ -106,7 +144,7 @@ int32_t ms_init(bip_ctx* ctx) {
   BIP_CUDA(ctx, cudaMemcpyAsync(ctx->rootx_dev, rx.data(), sizeof(float2) * nx, cudaMemcpyHostToDevice, ctx->stream));
   // Fresnel propagator P(q) = exp(-i pi lambda dz |q|^2) (eq. 2), no band limit, with the 1/G of the
   // unnormalised cuFFT round trip folded in.
-  std::vector<float2> P(G);
+  std::vector<double2> P(G);
   for (int ky = 0; ky < ny; ++ky) {
     const int hy = ky < (ny + 1) / 2 ? ky : ky - ny;
     const double qy = hy / ctx->g.ly;
@@ -114,15 +152,16 @@ int32_t ms_init(bip_ctx* ctx) {
       const int hx = kx < (nx + 1) / 2 ? kx : kx - nx;
       const double qx = hx / ctx->g.lx;
       const double ph = -M_PI * ctx->g.lambda * ctx->g.dz * (qy * qy + qx * qx);
-      P[(int64_t)ky * nx + kx] = make_float2((float)(std::cos(ph) / (double)G), (float)(std::sin(ph) / (double)G));
+      P[(int64_t)ky * nx + kx] = make_double2(std::cos(ph) / (double)G, std::sin(ph) / (double)G);
     }
   }
-  BIP_TRY(dev_alloc(ctx, (void**)&ctx->P_dev, sizeof(float2) * G, "propagator"));
-  BIP_CUDA(ctx, cudaMemcpyAsync(ctx->P_dev, P.data(), sizeof(float2) * G, cudaMemcpyHostToDevice, ctx->stream));
+  BIP_TRY(dev_alloc(ctx, (void**)&ctx->P_dev, sizeof(double2) * G, "propagator"));
+  BIP_CUDA(ctx, cudaMemcpyAsync(ctx->P_dev, P.data(), sizeof(double2) * G, cudaMemcpyHostToDevice, ctx->stream));
   BIP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-  // cuFFT batch: at most 256 MB of columns per call
-  const int64_t col_bytes = G * (int64_t)sizeof(float2);
-  ctx->plan_batch = (int)std::max<int64_t>(1, std::min<int64_t>(std::max(ctx->n_p1, ctx->n_p2), (256ll << 20) / col_bytes));
+  // cuFFT batch: at most 512 MB of double-precision workspace per call
+  const int64_t col_bytes = G * (int64_t)sizeof(double2);
+  ctx->plan_batch = (int)std::max<int64_t>(1, std::min<int64_t>(std::max(ctx->n_p1, ctx->n_p2), (512ll << 20) / col_bytes));
+  BIP_TRY(dev_alloc(ctx, &ctx->ms_work, (size_t)ctx->plan_batch * col_bytes, "multislice workspace"));
   ctx->plan_ok = true;
   return BIP_OK;
 }
@@ -136,37 +175,15 @@ int32_t ms_plane_waves(bip_ctx* ctx, float2* S, const int32_t* h_dev, int32_t n,
 }
 
 int32_t ms_step_S1(bip_ctx* ctx, int32_t j, int dir) {
-  const int64_t G = (int64_t)ctx->g.ny * ctx->g.nx;
-  const float2* Tj = ctx->T_dev + (int64_t)j * G;
-  if (dir > 0) {                     // S <- P[T_j S]
-    BIP_TRY(mul_field(ctx, ctx->S1, ctx->n_p1, Tj, 0));
-    BIP_TRY(fft_cols(ctx, ctx->S1, ctx->n_p1, CUFFT_FORWARD));
-    BIP_TRY(mul_field(ctx, ctx->S1, ctx->n_p1, ctx->P_dev, 0));
-    BIP_TRY(fft_cols(ctx, ctx->S1, ctx->n_p1, CUFFT_INVERSE));
-  } else {                           // inverse: S <- T_j* P*[S]   (|T| = |P| = 1)
-    BIP_TRY(fft_cols(ctx, ctx->S1, ctx->n_p1, CUFFT_FORWARD));
-    BIP_TRY(mul_field(ctx, ctx->S1, ctx->n_p1, ctx->P_dev, 1));
-    BIP_TRY(fft_cols(ctx, ctx->S1, ctx->n_p1, CUFFT_INVERSE));
-    BIP_TRY(mul_field(ctx, ctx->S1, ctx->n_p1, Tj, 1));
-  }
-  return BIP_OK;
+  const float2* Tj = ctx->T_dev + (int64_t)j * ctx->g.ny * ctx->g.nx;
+  if (dir > 0) return slice_op(ctx, ctx->S1, ctx->n_p1, Tj, /*pre=*/1, /*conj_p=*/0, /*post=*/0);   // S <- P[T_j S]   (eq. 6)
+  return slice_op(ctx, ctx->S1, ctx->n_p1, Tj, 0, 1, 2);                                             // S <- T_j* P*[S]
 }
 
 int32_t ms_step_S2(bip_ctx* ctx, int32_t j, int dir) {
-  const int64_t G = (int64_t)ctx->g.ny * ctx->g.nx;
-  const float2* Tj = ctx->T_dev + (int64_t)j * G;
-  if (dir < 0) {                     // build / un-peel: S <- T_j P[S]   (absorbs slice j)
-    BIP_TRY(fft_cols(ctx, ctx->S2, ctx->n_p2, CUFFT_FORWARD));
-    BIP_TRY(mul_field(ctx, ctx->S2, ctx->n_p2, ctx->P_dev, 0));
-    BIP_TRY(fft_cols(ctx, ctx->S2, ctx->n_p2, CUFFT_INVERSE));
-    BIP_TRY(mul_field(ctx, ctx->S2, ctx->n_p2, Tj, 0));
-  } else {                           // peel: S <- P*[T_j* S]            (sheds slice j)
-    BIP_TRY(mul_field(ctx, ctx->S2, ctx->n_p2, Tj, 1));
-    BIP_TRY(fft_cols(ctx, ctx->S2, ctx->n_p2, CUFFT_FORWARD));
-    BIP_TRY(mul_field(ctx, ctx->S2, ctx->n_p2, ctx->P_dev, 1));
-    BIP_TRY(fft_cols(ctx, ctx->S2, ctx->n_p2, CUFFT_INVERSE));
-  }
-  return BIP_OK;
+  const float2* Tj = ctx->T_dev + (int64_t)j * ctx->g.ny * ctx->g.nx;
+  if (dir < 0) return slice_op(ctx, ctx->S2, ctx->n_p2, Tj, 0, 0, 1);   // build / un-peel: S <- T_j P[S]  (eq. 12)
+  return slice_op(ctx, ctx->S2, ctx->n_p2, Tj, 2, 1, 0);                // peel: S <- P*[T_j* S]
 }
 
 }  // namespace bip

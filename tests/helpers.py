@@ -10,7 +10,7 @@ from oracle import sibson as osb
 class OracleSetup:
     """Everything the oracle derives from a workload edge: beams, parents, weights, coefficients, propagator."""
 
-    def __init__(self, wl, edge, parent_factor=None):
+    def __init__(self, wl, edge, parent_factor=None, n_jobs=1):
         f1, f2 = parent_factor if parent_factor is not None else wl.parent_factor
         ny, nx, ly, lx = wl.ny, wl.nx, wl.ly, wl.lx
         self.qa = wl.alpha_mrad * 1e-3 / wl.lam
@@ -25,7 +25,13 @@ class OracleSetup:
                 import scipy.sparse as sp
                 return np.arange(len(beams)), sp.identity(len(beams), format="csr")
             pos = ob.hexring_parents(beams, ny, nx, ly, lx, q, ob.n_radial_from_factor(len(beams), f))
-            tab = osb.natural_neighbour_weights(beams, pos, ly, lx, q)
+            if n_jobs == 1:
+                tab = osb.natural_neighbour_weights(beams, pos, ly, lx, q)
+            else:                                     # harness-level parallelism over rows; the oracle is unchanged
+                from joblib import Parallel, delayed
+                chunks = np.array_split(np.arange(len(beams)), 8 * n_jobs)
+                parts = Parallel(n_jobs=n_jobs)(delayed(osb.natural_neighbour_weights)(beams, pos, ly, lx, q, rows=c) for c in chunks)
+                tab = [r for part in parts for r in part]
             import scipy.sparse as sp
             rows = np.concatenate([np.full(len(i), b) for b, (i, _) in enumerate(tab)])
             cols = np.concatenate([i for i, _ in tab])

@@ -116,6 +116,16 @@ def test_weight_table_properties(cfg1_tables):
     assert err[~inside].max() < 0.25 * spacing
 
 
+def test_pruned_sibson_equals_unpruned(cfg1_tables):
+    """The nearest-parents shortcut of sibson_row is exact (its lemma is in the docstring)."""
+    ap, p1, tab, L, qa = cfg1_tables
+    q = ap / L
+    for b in list(range(0, len(ap), 7)) + [37, 87, 251]:           # includes hull-edge and hull-exterior beams
+        i0, w0 = osb.sibson_row(q[b], q[p1], qa, prune=False)
+        i1, w1 = osb.sibson_row(q[b], q[p1], qa, prune=True)
+        assert np.array_equal(i0, i1) and np.abs(w0 - w1).max() < 1e-11
+
+
 def test_identity_limit():
     b = ob.beams_in_disc(32, 32, 1.0, 1.0, 4.2)
     tab = osb.natural_neighbour_weights(b, np.arange(len(b)), 1.0, 1.0, 4.2)
