@@ -95,8 +95,8 @@ __global__ void __launch_bounds__(256) k_gemm1_simt(Gemm1Args g) {
         const float im = h.x * C[i][j].y + h.y * C[i][j].x;
         const int64_t o = (int64_t)atom * g.Phi.batch_stride + (int64_t)n * g.phi_ch_stride + (int64_t)rho * g.Phi.ld + s;
         const float rh = tf32_hi(re), ih = tf32_hi(im);
-        g.Phi.p[0][o] = rh; g.Phi.p[1][o] = re - rh;
-        g.Phi.p[2][o] = ih; g.Phi.p[3][o] = im - ih;
+        g.Phi.p[0][o] = rh; g.Phi.p[1][o] = tf32_hi(re - rh);
+        g.Phi.p[2][o] = ih; g.Phi.p[3][o] = tf32_hi(im - ih);
       }
     }
   }

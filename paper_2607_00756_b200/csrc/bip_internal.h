@@ -24,7 +24,8 @@ int32_t fail(bip_ctx* ctx, int32_t status, const char* fmt, ...) __attribute__((
 namespace bip {
 
 // Split-plane operand: a complex matrix [rows][ld] stored as four fp32 planes
-//   re_hi, re_lo, im_hi, im_lo  with hi = tf32(x) (round-to-nearest, ties away) and lo = x - hi (exact in fp32).
+//   re_hi, re_lo, im_hi, im_lo  with hi = tf32(x) and lo = tf32(x - hi) (cvt.rna: round-to-nearest, so the tensor
+// core's truncation of the low 13 mantissa bits never acts and the split stays unbiased; hi + lo = x to 2^-22).
 // The tensor-core kernels feed the planes to tcgen05 kind::tf32 as they are (3xTF32 split); the fp32 SIMT
 // reference kernels read hi + lo.  `ld` is a multiple of 32 floats (128 B) and plane bases are 1024 B aligned.
 struct Planes {

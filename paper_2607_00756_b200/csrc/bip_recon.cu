@@ -92,8 +92,8 @@ __global__ void k_recon_rows(const float2* __restrict__ D, int n_par, const int3
     if (carrier < 0) t.y = -t.y;                       // restore the carrier exp(carrier 2 pi i h_b.r/N)
     const float2 v = recon_elem(Da, s_idx, s_w, max_nn, w2, s, recon, t);
     const float rh = tf32_hi(v.x), ih = tf32_hi(v.y);
-    out.p[0][row + s] = rh; out.p[1][row + s] = v.x - rh;
-    out.p[2][row + s] = ih; out.p[3][row + s] = v.y - ih;
+    out.p[0][row + s] = rh; out.p[1][row + s] = tf32_hi(v.x - rh);
+    out.p[2][row + s] = ih; out.p[3][row + s] = tf32_hi(v.y - ih);
   }
 }
 
@@ -131,8 +131,8 @@ __global__ void k_recon_transposed(const float2* __restrict__ D, int n_par, cons
       const float2 v = tile[threadIdx.x][ss];
       const int64_t o = (int64_t)a * out.batch_stride + (int64_t)s * out.ld + b;
       const float rh = tf32_hi(v.x), ih = tf32_hi(v.y);
-      out.p[0][o] = rh; out.p[1][o] = v.x - rh;
-      out.p[2][o] = ih; out.p[3][o] = v.y - ih;
+      out.p[0][o] = rh; out.p[1][o] = tf32_hi(v.x - rh);
+      out.p[2][o] = ih; out.p[3][o] = tf32_hi(v.y - ih);
     }
   }
 }
@@ -171,8 +171,8 @@ __global__ void k_illumination(const double* __restrict__ rho, int n_rho, const 
     const float im = (float)((double)cb.x * sn + (double)cb.y * cs);
     const int64_t o = (int64_t)r * out.ld + b;
     const float rh = tf32_hi(re), ih = tf32_hi(im);
-    out.p[0][o] = rh; out.p[1][o] = re - rh;
-    out.p[2][o] = ih; out.p[3][o] = im - ih;
+    out.p[0][o] = rh; out.p[1][o] = tf32_hi(re - rh);
+    out.p[2][o] = ih; out.p[3][o] = tf32_hi(im - ih);
   }
 }
 
