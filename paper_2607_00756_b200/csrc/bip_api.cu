@@ -66,6 +66,55 @@ static int32_t planes_in(bip_ctx* ctx, DevBuf& buf, Planes& P, int64_t rows, int
   return BIP_OK;
 }
 
+// Carve a sliced bf16 operand [batch][rows][k] out of one DevBuf.  Producers write every k-step of every valid row;
+// the padding rows of the last row tile only have to be finite (they feed masked accumulator rows / columns), so the
+// buffer is cleared when it is (re)allocated and never again.
+static int32_t sliced_in(bip_ctx* ctx, DevBuf& buf, Sliced& S, int64_t rows, int64_t k, int64_t batch, const char* what) {
+  S.rows = rows;
+  S.rows_pad = round_up(rows, SL_ROWS);
+  S.k = k;
+  S.ksteps = (k + SL_K - 1) / SL_K;
+  S.batch_stride = S.rows_pad / SL_ROWS * S.ksteps * SL_STEP_EL;
+  const void* before = buf.p;
+  BIP_TRY(ensure(ctx, buf, (size_t)(S.batch_stride * std::max<int64_t>(batch, 1)) * sizeof(__nv_bfloat16), what));
+  if (buf.p != before) BIP_CUDA(ctx, cudaMemsetAsync(buf.p, 0, buf.bytes, ctx->stream));
+  S.base = reinterpret_cast<__nv_bfloat16*>(buf.p);
+  return BIP_OK;
+}
+
+// a3, built on first use in the format the requested arithmetic reads.
+static int32_t ensure_illumination(bip_ctx* ctx, int precision) {
+  if (precision == BIP_PREC_BF16X6) {
+    if (ctx->A_sl.base) return BIP_OK;
+    Sliced A;
+    DevBuf b;
+    BIP_TRY(sliced_in(ctx, b, A, ctx->n_rho, ctx->n_ap, 1, "illumination matrix (sliced)"));
+    A.batch_stride = 0;
+    if (dev_alloc(ctx, (void**)&A.scale, (size_t)A.rows_pad * sizeof(float), "illumination row scales") != BIP_OK) { cudaFree(b.p); return BIP_ERR_OOM; }
+    BIP_CUDA(ctx, cudaMemsetAsync(A.scale, 0, (size_t)A.rows_pad * sizeof(float), ctx->stream));
+    A.scale_batch_stride = 0;
+    int e = 0;
+    std::frexp(1.0001f * ctx->ap_c_max, &e);
+    ctx->A_sl = A;
+    return launch_illumination_sliced(ctx, ctx->rho_dev, ctx->n_rho, ctx->ap_c_max > 0.f ? std::ldexp(1.f, e) : 1.f, A);
+  }
+  if (ctx->A.p[0]) return BIP_OK;
+  Planes A;
+  A.rows = ctx->n_rho; A.ld = round_up(ctx->n_ap, 32); A.batch_stride = 0;
+  const int64_t plane_floats = round_up(A.rows * A.ld, 256);
+  float* base = nullptr;
+  BIP_TRY(dev_alloc(ctx, (void**)&base, (size_t)plane_floats * 4 * sizeof(float), "illumination matrix"));
+  BIP_CUDA(ctx, cudaMemsetAsync(base, 0, (size_t)plane_floats * 4 * sizeof(float), ctx->stream));
+  for (int k = 0; k < 4; ++k) A.p[k] = base + k * plane_floats;
+  ctx->A = A;
+  return launch_illumination(ctx, ctx->rho_dev, ctx->n_rho, A);
+}
+
+static void free_illumination(bip_ctx* ctx) {
+  if (ctx->A.p[0]) { cudaFree(ctx->A.p[0]); ctx->A = Planes(); }
+  if (ctx->A_sl.base) { cudaFree(ctx->A_sl.base); cudaFree(ctx->A_sl.scale); ctx->A_sl = Sliced(); }
+}
+
 template <class T>
 static int32_t upload(bip_ctx* ctx, T** dst, const T* src, size_t n, const char* what) {
   BIP_TRY(dev_alloc(ctx, (void**)dst, n * sizeof(T), what));
@@ -153,12 +202,66 @@ static size_t scratch_budget() {
   return (size_t)(gb * (double)(1ull << 30));
 }
 
+// Steps a1-a8 on the sliced bf16 operands (BIP_PREC_BF16X6).
+static int32_t contract_batch_bf16(bip_ctx* ctx, Edge& e, const int32_t* org, int32_t nb, int mode, int recon, void* out) {
+  auto& sp = spans()[ctx];
+  const int w2 = e.w * e.w;
+  const int64_t rho_pad = round_up(ctx->n_rho, SL_ROWS);
+  Sliced R1t, R2, Phi;
+  BIP_TRY(ensure(ctx, ctx->D1, (size_t)nb * ctx->n_p1 * w2 * sizeof(float2), "D1 (de-tilted S1 windows)"));
+  BIP_TRY(ensure(ctx, ctx->D2, (size_t)nb * ctx->n_p2 * w2 * sizeof(float2), "D2 (de-tilted S2 windows)"));
+  BIP_TRY(sliced_in(ctx, ctx->R1s, R1t, w2, ctx->n_ap, nb, "R1 (reconstructed S1 windows, sliced)"));
+  BIP_TRY(sliced_in(ctx, ctx->R2s, R2, e.n_det, w2, nb, "R2 (reconstructed S2 windows, sliced)"));
+  BIP_TRY(sliced_in(ctx, ctx->Phis, Phi, rho_pad * e.n_ch, w2, nb, "Phi (H_n psi, sliced)"));
+  const int64_t psi_ld = w2;
+  BIP_TRY(ensure(ctx, ctx->Psi, (size_t)nb * ctx->n_rho * psi_ld * sizeof(float2), "Psi (probe at the atom)"));
+  const int64_t n_scale = (int64_t)nb * (R1t.rows_pad + R2.rows_pad + Phi.rows_pad);
+  BIP_TRY(ensure(ctx, ctx->Scl, (size_t)n_scale * sizeof(float), "row scales"));
+  R1t.scale = reinterpret_cast<float*>(ctx->Scl.p);           R1t.scale_batch_stride = R1t.rows_pad;
+  R2.scale = R1t.scale + (int64_t)nb * R1t.rows_pad;          R2.scale_batch_stride = R2.rows_pad;
+  Phi.scale = R2.scale + (int64_t)nb * R2.rows_pad;           Phi.scale_batch_stride = Phi.rows_pad;
+
+  // a1-a2: S1 windows -> R1^T[s][b]
+  BIP_TRY(launch_crop_detilt(ctx, ctx->S1, ctx->p1_h_dev, ctx->n_p1, +1, org, nb, e.w, (float2*)ctx->D1.p));
+  BIP_TRY(launch_recon_t_sliced(ctx, (const float2*)ctx->D1.p, ctx->n_p1, ctx->ap_h_dev, ctx->n_ap, ctx->w1_idx_dev, ctx->w1_w_dev,
+                                ctx->nn1, +1, recon, org, nb, e.w, R1t));
+  // a3-a4: probe at the atom
+  Gemm1SlArgs g1;
+  g1.A = ctx->A_sl; g1.R1t = R1t; g1.Psi = (float2*)ctx->Psi.p; g1.psi_ld = psi_ld; g1.psi_batch_stride = (int64_t)ctx->n_rho * psi_ld;
+  g1.n_rho = ctx->n_rho; g1.w2 = w2; g1.n_atoms = nb;
+  BIP_TRY(launch_gemm1_bf16(ctx, g1));
+  // a5: times H_n, split into slices
+  BIP_TRY(launch_quantize_phi(ctx, g1.Psi, psi_ld, g1.psi_batch_stride, e.H_dev, Phi, ctx->n_rho, (int32_t)rho_pad, w2, e.n_ch, nb));
+  // a6: S2 windows -> R2[d][s]
+  BIP_TRY(launch_crop_detilt(ctx, ctx->S2, ctx->p2_h_dev, ctx->n_p2, -1, org, nb, e.w, (float2*)ctx->D2.p));
+  BIP_TRY(launch_recon_rows_sliced(ctx, (const float2*)ctx->D2.p, ctx->n_p2, e.det_h_dev, e.n_det, e.nn_idx_dev, e.nn_w_dev, e.max_nn,
+                                   -1, recon, org, nb, e.w, R2));
+  // a7-a8: detector projection and reduction
+  Gemm2SlArgs g2;
+  g2.Phi = Phi; g2.R2 = R2; g2.rows_pad = (int32_t)rho_pad;
+  g2.n_rho = ctx->n_rho; g2.n_det = e.n_det; g2.n_ch = e.n_ch; g2.n_atoms = nb;
+  g2.inv_G = (float)(1.0 / ((double)ctx->g.ny * ctx->g.nx));
+  g2.mode = mode;
+  g2.bin_of_det = mode == BIP_MODE_QEELS_X ? e.bin_of_det_x_dev : e.bin_of_det_y_dev;
+  g2.n_bins = mode == BIP_MODE_QEELS_X ? (int)e.binx.size() : (int)e.biny.size();
+  g2.out = out;
+  {
+    Span s(ctx, sp.pool_map, sp.gemm2);
+    BIP_TRY(launch_gemm2_bf16(ctx, g2));
+  }
+  ctx->timing.gemm2_launches++;
+  ctx->timing.amplitudes += (double)ctx->n_rho * nb * e.n_ch * e.n_det;
+  ctx->timing.flops += 8.0 * ctx->n_rho * w2 * ((double)nb * ctx->n_ap + (double)nb * e.n_ch * e.n_det);
+  return BIP_OK;
+}
+
 // Steps a1-a8 for atoms [a0, a0 + nb) of one edge, all sitting in the current plane.
 static int32_t contract_batch(bip_ctx* ctx, Edge& e, const int32_t* origin_dev, int32_t a0, int32_t nb, int mode, int recon,
                               int precision, void* out) {
   auto& sp = spans()[ctx];
   const int w2 = e.w * e.w;
   const int32_t* org = origin_dev + 2 * (int64_t)a0;
+  if (precision == BIP_PREC_BF16X6) return contract_batch_bf16(ctx, e, org, nb, mode, recon, out);
   Planes R1t, R2, Phi;
   BIP_TRY(ensure(ctx, ctx->D1, (size_t)nb * ctx->n_p1 * w2 * sizeof(float2), "D1 (de-tilted S1 windows)"));
   BIP_TRY(ensure(ctx, ctx->D2, (size_t)nb * ctx->n_p2 * w2 * sizeof(float2), "D2 (de-tilted S2 windows)"));
@@ -220,8 +323,8 @@ static int32_t run_edges(bip_ctx* ctx, const std::vector<int32_t>& ids, int mode
   if (ctx->n_rho <= 0) return fail(ctx, BIP_ERR_STATE, "bip_map: call bip_set_scan first");
   if (mode < BIP_MODE_MAP || mode > BIP_MODE_CUBE) return fail(ctx, BIP_ERR_INVALID, "bip_map: unknown mode %d", mode);
   if (recon != BIP_RECON_LINEAR && recon != BIP_RECON_MAGPHASE) return fail(ctx, BIP_ERR_INVALID, "bip_map: unknown recon %d", recon);
-  if (precision != BIP_PREC_TF32X3 && precision != BIP_PREC_FP32_SIMT) return fail(ctx, BIP_ERR_INVALID, "bip_map: unknown precision %d", precision);
-  if (precision == BIP_PREC_TF32X3 && !tc_available()) return fail(ctx, BIP_ERR_UNSUPPORTED, "bip_map: the tensor-core path is not built");
+  if (precision != BIP_PREC_TF32X3 && precision != BIP_PREC_FP32_SIMT && precision != BIP_PREC_BF16X6) return fail(ctx, BIP_ERR_INVALID, "bip_map: unknown precision %d", precision);
+  if (precision != BIP_PREC_FP32_SIMT && !tc_available()) return fail(ctx, BIP_ERR_UNSUPPORTED, "bip_map: the tensor-core path is not built");
   for (size_t k = 0; k < ids.size(); ++k) {
     if (ids[k] < 0 || ids[k] >= (int)ctx->edges.size()) return fail(ctx, BIP_ERR_INVALID, "bip_map: edge %d does not exist", ids[k]);
     size_t need = 0;
@@ -229,6 +332,7 @@ static int32_t run_edges(bip_ctx* ctx, const std::vector<int32_t>& ids, int mode
     if (!outs[k]) return fail(ctx, BIP_ERR_INVALID, "bip_map: output %zu is NULL", k);
     if (outs_bytes[k] != need) return fail(ctx, BIP_ERR_INVALID, "bip_map: output %zu has %zu bytes, expected %zu", k, outs_bytes[k], need);
   }
+  BIP_TRY(ensure_illumination(ctx, precision));
   auto& sp = spans()[ctx];
   sp.adv.clear(); sp.contract.clear(); sp.gemm2.clear();
   sp.pool_map.reset();
@@ -250,8 +354,10 @@ static int32_t run_edges(bip_ctx* ctx, const std::vector<int32_t>& ids, int mode
       auto hi = std::upper_bound(e.slice.begin(), e.slice.end(), plane) - e.slice.begin();
       if (lo == hi) continue;
       const int64_t w2 = (int64_t)e.w * e.w;
-      const size_t per_atom = (size_t)((ctx->n_p1 + ctx->n_p2) * w2 * 8 + 16 * (w2 * round_up(ctx->n_ap, 32) + (int64_t)e.n_det * round_up(w2, 32) +
-                                                                                (int64_t)ctx->n_rho * e.n_ch * round_up(w2, 32)));
+      const int64_t el = precision == BIP_PREC_BF16X6 ? 12 : 16;      // operand bytes per complex element
+      const size_t per_atom = (size_t)((ctx->n_p1 + ctx->n_p2) * w2 * 8 + (int64_t)ctx->n_rho * w2 * 8 +
+                                       el * (round_up(w2, 128) * round_up(ctx->n_ap, 32) + round_up(e.n_det, 128) * round_up(w2, 32) +
+                                             round_up(ctx->n_rho, 128) * e.n_ch * round_up(w2, 32)));
       const int32_t nb_max = (int32_t)std::max<size_t>(1, std::min<size_t>(budget / std::max<size_t>(per_atom, 1), 4096));
       Span s(ctx, sp.pool_map, sp.contract);
       for (int32_t a0 = (int32_t)lo; a0 < (int32_t)hi; a0 += nb_max)     // lines 5-8
@@ -308,6 +414,7 @@ int32_t bip_create(bip_ctx** out, const bip_grid* g, const void* T, int32_t T_on
   ctx->stream = (cudaStream_t)stream;
   ctx->sm_count = prop.multiProcessorCount;
   ctx->n_ap = n_ap; ctx->n_p1 = n_p1; ctx->n_p2 = n_p2; ctx->nn1 = w1->max_nn;
+  for (int32_t b = 0; b < n_ap; ++b) ctx->ap_c_max = std::max(ctx->ap_c_max, std::hypot(ap_c[2 * b], ap_c[2 * b + 1]));
   ctx->ap_h.assign(ap_h, ap_h + 2 * (size_t)n_ap);
   ctx->p1_h.assign(p1_h, p1_h + 2 * (size_t)n_p1);
   ctx->p2_h.assign(p2_h, p2_h + 2 * (size_t)n_p2);
@@ -364,7 +471,8 @@ int32_t bip_destroy(bip_ctx* ctx) {
   if (ctx->T_owned) cudaFree((void*)ctx->T_dev);
   void* ptrs[] = {ctx->ap_h_dev, ctx->p1_h_dev, ctx->p2_h_dev, ctx->ap_c_dev, ctx->w1_idx_dev, ctx->w1_w_dev, ctx->rooty_dev,
                   ctx->rootx_dev, ctx->P_dev, ctx->ms_work, ctx->S1, ctx->S2, ctx->D1.p, ctx->D2.p, ctx->R1.p, ctx->R2.p, ctx->Psi.p,
-                  ctx->Phi.p, ctx->A.p[0]};
+                  ctx->Phi.p, ctx->R1s.p, ctx->R2s.p, ctx->Phis.p, ctx->Scl.p, ctx->rho_dev};
+  free_illumination(ctx);
   for (void* p : ptrs) if (p) cudaFree(p);
   cudaGetLastError();
   delete ctx;
@@ -400,23 +508,14 @@ int32_t bip_set_scan(bip_ctx* ctx, int32_t n_rho, const double* rho_px) {
   if (n_rho <= 0 || !rho_px) return fail(ctx, BIP_ERR_INVALID, "bip_set_scan: empty scan");
   for (int32_t i = 0; i < 2 * n_rho; ++i) if (!std::isfinite(rho_px[i])) return fail(ctx, BIP_ERR_INVALID, "bip_set_scan: non-finite position");
   cudaStreamSynchronize(ctx->stream);
-  if (ctx->A.p[0]) { cudaFree(ctx->A.p[0]); ctx->A = Planes(); }
-  Planes A;
-  A.rows = n_rho; A.ld = round_up(ctx->n_ap, 32); A.batch_stride = 0;
-  const int64_t plane_floats = round_up(A.rows * A.ld, 256);
-  float* base = nullptr;
-  BIP_TRY(dev_alloc(ctx, (void**)&base, (size_t)plane_floats * 4 * sizeof(float), "illumination matrix"));
-  BIP_CUDA(ctx, cudaMemsetAsync(base, 0, (size_t)plane_floats * 4 * sizeof(float), ctx->stream));
-  for (int k = 0; k < 4; ++k) A.p[k] = base + k * plane_floats;
-  double* rho_dev = nullptr;
-  BIP_TRY(dev_alloc(ctx, (void**)&rho_dev, sizeof(double) * 2 * n_rho, "scan positions"));
-  BIP_CUDA(ctx, cudaMemcpyAsync(rho_dev, rho_px, sizeof(double) * 2 * n_rho, cudaMemcpyHostToDevice, ctx->stream));
-  ctx->A = A;
+  free_illumination(ctx);
+  if (ctx->rho_dev) { cudaFree(ctx->rho_dev); ctx->rho_dev = nullptr; }
+  ctx->n_rho = 0;
+  BIP_TRY(dev_alloc(ctx, (void**)&ctx->rho_dev, sizeof(double) * 2 * n_rho, "scan positions"));
+  BIP_CUDA(ctx, cudaMemcpyAsync(ctx->rho_dev, rho_px, sizeof(double) * 2 * n_rho, cudaMemcpyHostToDevice, ctx->stream));
+  BIP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));      // the host array may go away after return
   ctx->n_rho = n_rho;
-  int32_t st = launch_illumination(ctx, rho_dev, n_rho, A);
-  cudaStreamSynchronize(ctx->stream);
-  cudaFree(rho_dev);
-  return st;
+  return BIP_OK;                                           // the illumination matrix (a3) is built on first use
 }
 
 int32_t bip_add_edge(bip_ctx* ctx, int32_t n_atoms, const int32_t* slice, const int32_t* centre_px, int32_t n_ch, int32_t w,

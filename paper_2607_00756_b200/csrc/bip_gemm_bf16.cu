@@ -1,0 +1,440 @@
+// tcgen05 / TMEM / bulk-TMA versions of the two contractions (steps a4-a5 and a7-a8 of SURVEY.md 8(a)) on the
+// three-slice bf16 operand format of bip_sliced.cuh (precision BIP_PREC_BF16X6, fp32-equivalent).
+//
+// One persistent, warp-specialised kernel computes C[128 x 128] (complex) = X[128 x Kd] . Y[128 x Kd]^T per work item:
+//
+//   Cr = Xr Yr - Xi Yi ,  Ci = Xr Yi + Xi Yr ,   real product = x1 y1 + (x1 y2 + x2 y1) + (x1 y3 + x2 y2 + x3 y1)
+//
+// i.e. 24 tcgen05.mma.kind::f16 (bf16, M = 128, N = 128, K = 16) per 16 k-elements.  Four fp32 accumulators live in
+// TMEM (the whole 512 columns): C0r, C0i take the leading products x1 y1 -- integers / 2^14, summed EXACTLY over a
+// chunk of 256 k-elements -- and C12r, C12i take the small ones.  After every chunk the eight epilogue warps read
+// the accumulators back (tcgen05.ld) and add them to fp32 running sums in registers (round-to-nearest), so the
+// truncating accumulation of the tensor core never biases the result (bip_sliced.cuh).  Operand tiles arrive by
+// cp.async.bulk (one contiguous 24 KB block per operand and k-step) through a 4-stage mbarrier ring; one elected
+// thread issues the MMAs.  Fused epilogues:
+//
+//   GEMM1 (a4):    Psi[rho][s] = sx[rho] sy[s] C           -> c64, quantised to Phi_n = H_n Psi by k_quantize_phi (a5)
+//   GEMM2 (a7-a8): |a_n[rho][d]|^2 / G summed over channels and reduced per output mode
+//
+// Warp roles: warp 0 bulk-copy producer, warp 1 TMEM owner + MMA issuer, warps 2-9 epilogue (TMEM lane quarter =
+// warp % 4, column half = (warp - 2) / 4).
+#include <cuda.h>
+
+#include "bip_internal.h"
+
+namespace bip {
+
+namespace {
+
+constexpr int TM = 128, TN = 128;
+constexpr int STAGES = 4;
+constexpr int X_BYTES = SL_STEP_EL * 2;          // 24 KB
+constexpr int STAGE_BYTES = 2 * X_BYTES;         // X and Y of one k-step
+constexpr int PART_BYTES = SL_TILE_EL * 2;       // 4 KB
+constexpr int CHUNK_STEPS = 16;                  // 256 k-elements: 2 * 256 * 2^14 = 2^23 < 2^24, exact
+constexpr int NUM_EPI_WARPS = 8;
+constexpr int NUM_THREADS = 64 + 32 * NUM_EPI_WARPS;
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
+constexpr int DGROUP = 4;                        // column tiles per raster group (concurrent CTAs share operand tiles in L2)
+
+enum { EPI_GEMM1 = 1, EPI_GEMM2 = 2 };
+
+struct BfParams {
+  const __nv_bfloat16* X; const __nv_bfloat16* Y;
+  const float* sx; const float* sy;
+  int64_t x_batch_stride, y_batch_stride, sx_batch_stride, sy_batch_stride;
+  int ksteps;
+  int n_rt, n_ct, n_items, n_ch_loop;
+  int n_rows, n_cols;      // valid rows (rho) / columns (s or d) per atom
+  int rows_pad;            // padded rho rows per channel block of X
+  // GEMM1 epilogue
+  float2* Psi; int64_t psi_ld, psi_batch_stride;
+  // GEMM2 epilogue
+  int mode; float inv_G; const int32_t* bin_of_det; int n_bins; void* out;
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t done = 0;
+  while (!done) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred P1;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\n\t"
+        "selp.b32 %0, 1, 0, P1;\n\t"
+        "}"
+        : "=r"(done)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+  }
+}
+__device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+// K-major, no-swizzle shared-memory matrix descriptor (cute::UMMA::SmemDescriptor, LayoutType::INTERLEAVE):
+// core matrices of 8 rows x 16 bytes; LBO = 128 B between the two k halves, SBO = 256 B between 8-row groups.
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr & 0x3FFFF) >> 4);            // start address, bits [0,14)
+  d |= (uint64_t)(128 >> 4) << 16;                    // leading byte offset, bits [16,30)
+  d |= (uint64_t)(256 >> 4) << 32;                    // stride byte offset, bits [32,46)
+  d |= (uint64_t)1 << 46;                             // descriptor version (Blackwell)
+  return d;                                           // layout type 0 = no swizzle
+}
+
+// cute::UMMA::InstrDescriptor for kind::f16 with bf16 operands, fp32 accumulate, K-major A and B
+__host__ __device__ constexpr uint32_t umma_idesc(bool neg_a) {
+  return (1u << 4) | (1u << 7) | (1u << 10) | ((neg_a ? 1u : 0u) << 13) | ((uint32_t)(TN >> 3) << 17) | ((uint32_t)(TM >> 4) << 24);
+}
+
+__device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
+      "}" ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+
+__device__ __forceinline__ void umma_commit(uint64_t* bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
+        "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]),
+        "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]),
+        "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+      : "r"(taddr));
+}
+
+// item -> (atom, row tile, column tile); column tiles rasterised in groups of DGROUP.
+__device__ __forceinline__ void decode_item(const BfParams& p, int item, int& atom, int& rt, int& ct) {
+  const int per_atom = p.n_rt * p.n_ct;
+  atom = item / per_atom;
+  int idx = item - atom * per_atom;
+  const int full = p.n_ct / DGROUP;
+  const int blk = p.n_rt * DGROUP;
+  if (idx < full * blk) {
+    const int g = idx / blk, r = idx - g * blk;
+    rt = r / DGROUP;
+    ct = g * DGROUP + (r - rt * DGROUP);
+  } else {
+    idx -= full * blk;
+    const int gsz = p.n_ct - full * DGROUP;
+    rt = idx / gsz;
+    ct = full * DGROUP + (idx - rt * gsz);
+  }
+}
+
+template <int EPI>
+__global__ void __launch_bounds__(NUM_THREADS, 1) k_bf16_contract(const BfParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + STAGES * STAGE_BYTES);
+  uint64_t* full = bars;                 // [STAGES]
+  uint64_t* empty = bars + STAGES;       // [STAGES]
+  uint64_t* tmem_full = bars + 2 * STAGES;
+  uint64_t* tmem_empty = bars + 2 * STAGES + 1;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * STAGES + 2);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int n_chunks = (p.ksteps + CHUNK_STEPS - 1) / CHUNK_STEPS;
+
+  if (warp == 0 && lane == 0) {
+    for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+    mbar_init(tmem_full, 1);
+    mbar_init(tmem_empty, NUM_EPI_WARPS);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 1) {   // the whole tensor memory: 512 columns
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp == 0) {
+    // ================= bulk-copy producer =================
+    if (lane == 0) {
+      uint32_t it = 0;
+      for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
+        int atom, rt, ct;
+        decode_item(p, item, atom, rt, ct);
+        const __nv_bfloat16* ysrc = p.Y + (int64_t)atom * p.y_batch_stride + (int64_t)ct * p.ksteps * SL_STEP_EL;
+        for (int n = 0; n < p.n_ch_loop; ++n) {
+          const __nv_bfloat16* xsrc = p.X + (int64_t)atom * p.x_batch_stride + ((int64_t)n * p.n_rt + rt) * p.ksteps * SL_STEP_EL;
+          for (int ks = 0; ks < p.ksteps; ++ks, ++it) {
+            const int s = it % STAGES;
+            mbar_wait(&empty[s], ((it / STAGES) & 1) ^ 1);
+            uint8_t* st = smem + s * STAGE_BYTES;
+            mbar_expect_tx(&full[s], STAGE_BYTES);
+            bulk_load(st, xsrc + (int64_t)ks * SL_STEP_EL, X_BYTES, &full[s]);
+            bulk_load(st + X_BYTES, ysrc + (int64_t)ks * SL_STEP_EL, X_BYTES, &full[s]);
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ================= MMA issuer =================
+    if (lane == 0) {
+      uint32_t it = 0, chunk_id = 0;
+      const uint32_t id_pos = umma_idesc(false), id_neg = umma_idesc(true);
+      const uint32_t t0r = tmem_base, t0i = tmem_base + TN, t12r = tmem_base + 2 * TN, t12i = tmem_base + 3 * TN;
+      for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
+        for (int n = 0; n < p.n_ch_loop; ++n) {
+          for (int c = 0; c < n_chunks; ++c, ++chunk_id) {
+            mbar_wait(tmem_empty, (chunk_id & 1) ^ 1);        // epilogue has drained the previous chunk
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            const int ks_end = min(p.ksteps, (c + 1) * CHUNK_STEPS);
+            for (int ks = c * CHUNK_STEPS; ks < ks_end; ++ks, ++it) {
+              const int s = it % STAGES;
+              mbar_wait(&full[s], (it / STAGES) & 1);
+              asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+              const uint32_t a0 = smem_u32(smem + s * STAGE_BYTES), b0 = a0 + X_BYTES;
+              const uint64_t xr1 = umma_desc(a0), xr2 = umma_desc(a0 + PART_BYTES), xr3 = umma_desc(a0 + 2 * PART_BYTES);
+              const uint64_t xi1 = umma_desc(a0 + 3 * PART_BYTES), xi2 = umma_desc(a0 + 4 * PART_BYTES), xi3 = umma_desc(a0 + 5 * PART_BYTES);
+              const uint64_t yr1 = umma_desc(b0), yr2 = umma_desc(b0 + PART_BYTES), yr3 = umma_desc(b0 + 2 * PART_BYTES);
+              const uint64_t yi1 = umma_desc(b0 + 3 * PART_BYTES), yi2 = umma_desc(b0 + 4 * PART_BYTES), yi3 = umma_desc(b0 + 5 * PART_BYTES);
+              const uint32_t acc = ks > c * CHUNK_STEPS ? 1u : 0u;
+              // small products first: C12r = sum over (i + j in {3, 4}) of xr_i yr_j - xi_i yi_j
+              umma_bf16(t12r, xr1, yr3, id_pos, acc);
+              umma_bf16(t12r, xr2, yr2, id_pos, 1u);
+              umma_bf16(t12r, xr3, yr1, id_pos, 1u);
+              umma_bf16(t12r, xi1, yi3, id_neg, 1u);
+              umma_bf16(t12r, xi2, yi2, id_neg, 1u);
+              umma_bf16(t12r, xi3, yi1, id_neg, 1u);
+              umma_bf16(t12r, xr1, yr2, id_pos, 1u);
+              umma_bf16(t12r, xr2, yr1, id_pos, 1u);
+              umma_bf16(t12r, xi1, yi2, id_neg, 1u);
+              umma_bf16(t12r, xi2, yi1, id_neg, 1u);
+              // C12i = sum of xr_i yi_j + xi_i yr_j
+              umma_bf16(t12i, xr1, yi3, id_pos, acc);
+              umma_bf16(t12i, xr2, yi2, id_pos, 1u);
+              umma_bf16(t12i, xr3, yi1, id_pos, 1u);
+              umma_bf16(t12i, xi1, yr3, id_pos, 1u);
+              umma_bf16(t12i, xi2, yr2, id_pos, 1u);
+              umma_bf16(t12i, xi3, yr1, id_pos, 1u);
+              umma_bf16(t12i, xr1, yi2, id_pos, 1u);
+              umma_bf16(t12i, xr2, yi1, id_pos, 1u);
+              umma_bf16(t12i, xi1, yr2, id_pos, 1u);
+              umma_bf16(t12i, xi2, yr1, id_pos, 1u);
+              // leading products, exact
+              umma_bf16(t0r, xr1, yr1, id_pos, acc);
+              umma_bf16(t0r, xi1, yi1, id_neg, 1u);
+              umma_bf16(t0i, xr1, yi1, id_pos, acc);
+              umma_bf16(t0i, xi1, yr1, id_pos, 1u);
+              umma_commit(&empty[s]);                    // stage reusable once these MMAs have read it
+            }
+            umma_commit(tmem_full);                      // accumulators of this chunk complete
+          }
+        }
+      }
+    }
+  } else {
+    // ================= epilogue warps =================
+    const int quarter = warp & 3;                      // TMEM lanes [32 q, 32 q + 32) are visible to warps with warp % 4 == q
+    const int half = (warp - 2) >> 2;                  // columns [64 half, 64 half + 64) of every accumulator
+    const uint32_t t_lane = tmem_base + ((uint32_t)(quarter * 32) << 16) + half * 64;
+    uint32_t chunk_id = 0;
+    for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
+      int atom, rt, ct;
+      decode_item(p, item, atom, rt, ct);
+      const int row = rt * TM + quarter * 32 + lane;   // this thread's rho
+      const bool row_ok = row < p.n_rows;
+      const int col0 = ct * TN + half * 64;
+      const float* sy = p.sy + (int64_t)atom * p.sy_batch_stride;
+      float rowsum = 0.f;
+      for (int n = 0; n < p.n_ch_loop; ++n) {
+        float rr[64], ri[64];
+#pragma unroll
+        for (int j = 0; j < 64; ++j) { rr[j] = 0.f; ri[j] = 0.f; }
+#pragma unroll 1
+        for (int c = 0; c < n_chunks; ++c, ++chunk_id) {
+          mbar_wait(tmem_full, chunk_id & 1);
+          asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll
+          for (int g = 0; g < 2; ++g) {
+            uint32_t v[32];
+            tmem_ld32(t_lane + g * 32, v);                   // C0r
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+            for (int j = 0; j < 32; ++j) rr[g * 32 + j] += __uint_as_float(v[j]);
+            tmem_ld32(t_lane + 2 * TN + g * 32, v);          // C12r
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+            for (int j = 0; j < 32; ++j) rr[g * 32 + j] += __uint_as_float(v[j]);
+            tmem_ld32(t_lane + TN + g * 32, v);              // C0i
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+            for (int j = 0; j < 32; ++j) ri[g * 32 + j] += __uint_as_float(v[j]);
+            tmem_ld32(t_lane + 3 * TN + g * 32, v);          // C12i
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+            for (int j = 0; j < 32; ++j) ri[g * 32 + j] += __uint_as_float(v[j]);
+          }
+          asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+          __syncwarp();
+          if (lane == 0) mbar_arrive(tmem_empty);
+        }
+        // ---- end of a (tile, channel): fused epilogue on the running sums ----
+        const float sxr = row_ok ? p.sx[(int64_t)atom * p.sx_batch_stride + (int64_t)n * p.rows_pad + row] : 0.f;
+        if (EPI == EPI_GEMM2) {
+          const float sx2 = sxr * sxr;
+          if (p.mode == BIP_MODE_MAP) {
+            float acc = 0.f;
+#pragma unroll
+            for (int j = 0; j < 64; ++j) {
+              const int d = col0 + j;
+              const float s = d < p.n_cols ? __ldg(sy + d) : 0.f;
+              acc = fmaf(fmaf(rr[j], rr[j], ri[j] * ri[j]), s * s, acc);
+            }
+            rowsum = fmaf(acc, sx2, rowsum);
+          } else if (row_ok) {
+            float* out = reinterpret_cast<float*>(p.out);
+            const float f = sx2 * p.inv_G;
+#pragma unroll
+            for (int j = 0; j < 64; ++j) {
+              const int d = col0 + j;
+              if (d < p.n_cols) {
+                const float s = __ldg(sy + d);
+                const float v = fmaf(rr[j], rr[j], ri[j] * ri[j]) * (s * s) * f;
+                if (p.mode == BIP_MODE_CUBE) atomicAdd(out + (int64_t)row * p.n_cols + d, v);
+                else atomicAdd(out + (int64_t)row * p.n_bins + __ldg(p.bin_of_det + d), v);
+              }
+            }
+          }
+        } else if (row_ok) {
+          // GEMM1: Psi[atom][rho][s], c64
+          float2* dst = p.Psi + (int64_t)atom * p.psi_batch_stride + (int64_t)row * p.psi_ld;
+#pragma unroll
+          for (int j = 0; j < 64; j += 2) {
+            const int s0 = col0 + j;
+            if (s0 + 1 < p.n_cols) {
+              const float a = sxr * __ldg(sy + s0), b = sxr * __ldg(sy + s0 + 1);
+              *reinterpret_cast<float4*>(dst + s0) = make_float4(rr[j] * a, ri[j] * a, rr[j + 1] * b, ri[j + 1] * b);
+            } else if (s0 < p.n_cols) {
+              const float a = sxr * __ldg(sy + s0);
+              dst[s0] = make_float2(rr[j] * a, ri[j] * a);
+            }
+          }
+        }
+      }
+      if (EPI == EPI_GEMM2 && p.mode == BIP_MODE_MAP && row_ok)
+        atomicAdd(reinterpret_cast<double*>(p.out) + row, (double)rowsum * (double)p.inv_G);
+    }
+  }
+
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  if (warp == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
+}
+
+// a5: Phi_n[rho][s] = H_n[s] Psi[rho][s] as sliced rows (n, rho) with their power-of-two scales.
+// One warp per (rho, n, atom); lanes stride over the groups of 8 window pixels; two passes (row maximum, then split).
+__global__ void __launch_bounds__(256) k_quantize_phi(const float2* __restrict__ Psi, int64_t psi_ld, int64_t psi_batch_stride,
+                                                      const float2* __restrict__ H, Sliced Phi, int n_rho, int rows_pad, int w2) {
+  const int rho = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  const int n = blockIdx.y, atom = blockIdx.z;
+  if (rho >= n_rho) return;
+  const float2* prow = Psi + (int64_t)atom * psi_batch_stride + (int64_t)rho * psi_ld;
+  const float2* hrow = H + (int64_t)n * w2;
+  const int n_groups = 2 * (int)Phi.ksteps;
+  float m = 0.f;
+  for (int s = lane; s < w2; s += 32) {
+    const float2 a = prow[s], h = __ldg(hrow + s);
+    m = fmaxf(m, fmaxf(fabsf(h.x * a.x - h.y * a.y), fabsf(h.x * a.y + h.y * a.x)));
+  }
+#pragma unroll
+  for (int o = 16; o; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+  const float scale = sl_pow2_scale(m), inv = 1.f / scale;
+  const int64_t row = (int64_t)n * rows_pad + rho;
+  if (lane == 0) Phi.scale[(int64_t)atom * Phi.scale_batch_stride + row] = scale;
+  for (int g = lane; g < n_groups; g += 32) {
+    float re[8], im[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      const int s = g * 8 + j;
+      float2 a = make_float2(0.f, 0.f), h = a;
+      if (s < w2) { a = prow[s]; h = __ldg(hrow + s); }
+      re[j] = h.x * a.x - h.y * a.y;
+      im[j] = h.x * a.y + h.y * a.x;
+    }
+    sl_store_group(Phi, atom, row, g, re, im, inv);
+  }
+}
+
+template <int EPI>
+int32_t launch(bip_ctx* ctx, const BfParams& p) {
+  static bool attr_set = false;
+  if (!attr_set) {
+    BIP_CUDA(ctx, cudaFuncSetAttribute(k_bf16_contract<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+    attr_set = true;
+  }
+  if (p.n_items <= 0) return BIP_OK;
+  const int grid = std::max(1, std::min(p.n_items, ctx->sm_count));
+  k_bf16_contract<EPI><<<grid, NUM_THREADS, SMEM_BYTES, ctx->stream>>>(p);
+  BIP_CUDA(ctx, cudaGetLastError());
+  ctx->timing.kernel_launches++;
+  return BIP_OK;
+}
+
+}  // namespace
+
+int32_t launch_gemm1_bf16(bip_ctx* ctx, const Gemm1SlArgs& a) {
+  BfParams p{};
+  p.X = a.A.base; p.sx = a.A.scale; p.x_batch_stride = 0; p.sx_batch_stride = 0;
+  p.Y = a.R1t.base; p.sy = a.R1t.scale; p.y_batch_stride = a.R1t.batch_stride; p.sy_batch_stride = a.R1t.scale_batch_stride;
+  p.ksteps = (int)a.A.ksteps;
+  p.n_rt = (int)(a.A.rows_pad / TM);
+  p.n_ct = (int)(a.R1t.rows_pad / TN);
+  p.n_items = a.n_atoms * p.n_rt * p.n_ct;
+  p.n_ch_loop = 1;
+  p.n_rows = a.n_rho; p.n_cols = a.w2; p.rows_pad = (int)a.A.rows_pad;
+  p.Psi = a.Psi; p.psi_ld = a.psi_ld; p.psi_batch_stride = a.psi_batch_stride;
+  return launch<EPI_GEMM1>(ctx, p);
+}
+
+int32_t launch_quantize_phi(bip_ctx* ctx, const float2* Psi, int64_t psi_ld, int64_t psi_batch_stride, const float2* H,
+                            const Sliced& Phi, int32_t n_rho, int32_t rows_pad, int32_t w2, int32_t n_ch, int32_t n_atoms) {
+  dim3 grid((unsigned)((n_rho + 7) / 8), (unsigned)n_ch, (unsigned)n_atoms);
+  k_quantize_phi<<<grid, 256, 0, ctx->stream>>>(Psi, psi_ld, psi_batch_stride, H, Phi, n_rho, rows_pad, w2);
+  BIP_CUDA(ctx, cudaGetLastError());
+  ctx->timing.kernel_launches++;
+  return BIP_OK;
+}
+
+int32_t launch_gemm2_bf16(bip_ctx* ctx, const Gemm2SlArgs& a) {
+  BfParams p{};
+  p.X = a.Phi.base; p.sx = a.Phi.scale; p.x_batch_stride = a.Phi.batch_stride; p.sx_batch_stride = a.Phi.scale_batch_stride;
+  p.Y = a.R2.base; p.sy = a.R2.scale; p.y_batch_stride = a.R2.batch_stride; p.sy_batch_stride = a.R2.scale_batch_stride;
+  p.ksteps = (int)a.Phi.ksteps;
+  p.rows_pad = a.rows_pad;
+  p.n_rt = a.rows_pad / TM;
+  p.n_ct = (int)(a.R2.rows_pad / TN);
+  p.n_items = a.n_atoms * p.n_rt * p.n_ct;
+  p.n_ch_loop = a.n_ch;
+  p.n_rows = a.n_rho; p.n_cols = a.n_det;
+  p.mode = a.mode; p.inv_G = a.inv_G; p.bin_of_det = a.bin_of_det; p.n_bins = a.n_bins; p.out = a.out;
+  return launch<EPI_GEMM2>(ctx, p);
+}
+
+}  // namespace bip

@@ -9,6 +9,7 @@
 #include <vector>
 
 #include "../../include/bip.h"
+#include "bip_sliced.cuh"
 
 namespace bip {
 
@@ -71,6 +72,7 @@ struct bip_ctx {
   std::vector<int32_t> ap_h, p1_h, p2_h;
   int32_t *ap_h_dev = nullptr, *p1_h_dev = nullptr, *p2_h_dev = nullptr;
   float2* ap_c_dev = nullptr;
+  float ap_c_max = 0.f;            // max_b |c_b|
   int32_t* w1_idx_dev = nullptr;
   float* w1_w_dev = nullptr;
 
@@ -87,12 +89,15 @@ struct bip_ctx {
 
   // scan
   int32_t n_rho = 0;
-  bip::Planes A;                   // illumination [n_rho][n_ap] split planes (K-major over b)
+  double* rho_dev = nullptr;       // [n_rho][2] scan positions in pixels
+  bip::Planes A;                   // illumination [n_rho][n_ap] split planes (K-major over b); built on first use
+  bip::Sliced A_sl;                // the same as a sliced bf16 operand; built on first use
 
   std::vector<bip::Edge> edges;
 
   // scratch, grown on demand
   bip::DevBuf D1, D2, R1, R2, Psi, Phi;
+  bip::DevBuf R1s, R2s, Phis, Scl;  // sliced operands of the bf16 path and their row scales
 
   bip_timing timing{};
   cudaEvent_t ev[8] = {};
@@ -166,6 +171,37 @@ int32_t launch_gemm2_simt(bip_ctx* ctx, const Gemm2Args& a);
 int32_t launch_gemm1_tc(bip_ctx* ctx, const Gemm1Args& a);
 int32_t launch_gemm2_tc(bip_ctx* ctx, const Gemm2Args& a);
 bool tc_available();
+
+// ---- contractions on sliced bf16 operands (bip_gemm_bf16.cu) ----
+struct Gemm1SlArgs {     // a4: Psi = A . R1   (c64 [atom][rho][s])
+  Sliced A;              // rows rho, k = aperture beams
+  Sliced R1t;            // rows s, k = aperture beams, batch = atoms
+  float2* Psi;
+  int64_t psi_ld, psi_batch_stride;
+  int32_t n_rho, w2, n_atoms;
+};
+struct Gemm2SlArgs {     // a7 + a8
+  Sliced Phi;            // rows (n, rho) = n * rows_pad + rho, k = window pixels, batch = atoms
+  Sliced R2;             // rows d, k = window pixels, batch = atoms
+  int32_t rows_pad;      // padded rho rows per channel
+  int32_t n_rho, n_det, n_ch, n_atoms;
+  float inv_G;
+  int32_t mode;
+  const int32_t* bin_of_det;
+  int32_t n_bins;
+  void* out;
+};
+int32_t launch_gemm1_bf16(bip_ctx* ctx, const Gemm1SlArgs& a);
+int32_t launch_gemm2_bf16(bip_ctx* ctx, const Gemm2SlArgs& a);
+int32_t launch_quantize_phi(bip_ctx* ctx, const float2* Psi, int64_t psi_ld, int64_t psi_batch_stride, const float2* H,
+                            const Sliced& Phi, int32_t n_rho, int32_t rows_pad, int32_t w2, int32_t n_ch, int32_t n_atoms);
+int32_t launch_recon_t_sliced(bip_ctx* ctx, const float2* D, int32_t n_par, const int32_t* bh_dev, int32_t n_beams,
+                              const int32_t* nn_idx, const float* nn_w, int32_t max_nn, int carrier, int recon,
+                              const int32_t* origin_dev, int32_t n_atoms, int32_t w, Sliced out);
+int32_t launch_recon_rows_sliced(bip_ctx* ctx, const float2* D, int32_t n_par, const int32_t* bh_dev, int32_t n_beams,
+                                 const int32_t* nn_idx, const float* nn_w, int32_t max_nn, int carrier, int recon,
+                                 const int32_t* origin_dev, int32_t n_atoms, int32_t w, Sliced out);
+int32_t launch_illumination_sliced(bip_ctx* ctx, const double* rho_dev, int32_t n_rho, float scale, Sliced out);
 
 }  // namespace bip
 #endif  // __CUDACC__

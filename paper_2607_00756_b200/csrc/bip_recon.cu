@@ -176,6 +176,133 @@ __global__ void k_illumination(const double* __restrict__ rho, int n_rho, const 
   }
 }
 
+
+// ---- sliced-operand producers (precision BIP_PREC_BF16X6; layout and split in bip_sliced.cuh) ----
+
+// scale[a][s] = power of two >= max_p |D[a][p][s]|: a bound of every reconstructed beam at window pixel s, because
+// the natural-neighbour weights are a convex combination (eq. 8) in both eq. 15 and eq. 11.
+__global__ void k_parent_colmax(const float2* __restrict__ D, int n_par, int w2, float* __restrict__ scale, int64_t scale_batch_stride) {
+  const int a = blockIdx.y;
+  const int s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= w2) return;
+  const float2* Da = D + (int64_t)a * n_par * w2;
+  float m = 0.f;
+  for (int p = 0; p < n_par; ++p) {
+    const float2 d = Da[(int64_t)p * w2 + s];
+    m = fmaxf(m, d.x * d.x + d.y * d.y);
+  }
+  scale[(int64_t)a * scale_batch_stride + s] = sl_pow2_scale(1.001f * sqrtf(m));
+}
+
+// a2 as the K-major operand of the probe GEMM: rows = window pixels s, k = aperture beams b.
+// thread = (row s, group of 8 consecutive beams); lanes run over consecutive s (coalesced reads of D, 128-byte stores).
+__global__ void __launch_bounds__(256) k_recon_t_sliced(const float2* __restrict__ D, int n_par, const int32_t* __restrict__ bh, int n_beams,
+                                 const int32_t* __restrict__ nn_idx, const float* __restrict__ nn_w, int max_nn, int carrier,
+                                 int recon, const int32_t* __restrict__ origin, int w, int ny, int nx,
+                                 const float2* __restrict__ rooty, const float2* __restrict__ rootx, Sliced out) {
+  const int a = blockIdx.z;
+  const int w2 = w * w;
+  const int s = blockIdx.x * 32 + threadIdx.x, g = blockIdx.y * 8 + threadIdx.y;
+  if (s >= w2 || g >= 2 * out.ksteps) return;
+  const int oy = origin[2 * a], ox = origin[2 * a + 1];
+  const int sy = s / w, sx = s - sy * w;
+  int ry = oy + sy; if (ry >= ny) ry -= ny;
+  int rx = ox + sx; if (rx >= nx) rx -= nx;
+  const float2* Da = D + (int64_t)a * n_par * w2;
+  float re[8], im[8];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    const int b = g * 8 + j;
+    float2 v = make_float2(0.f, 0.f);
+    if (b < n_beams) {
+      const int hyp = ((bh[2 * b] % ny) + ny) % ny, hxp = ((bh[2 * b + 1] % nx) + nx) % nx;
+      float2 t = tilt(rooty, rootx, hyp, hxp, ry, rx, ny, nx);
+      if (carrier < 0) t.y = -t.y;
+      v = recon_elem(Da, nn_idx + (int64_t)b * max_nn, nn_w + (int64_t)b * max_nn, max_nn, w2, s, recon, t);
+    }
+    re[j] = v.x; im[j] = v.y;
+  }
+  sl_store_group(out, a, s, g, re, im, 1.f / out.scale[(int64_t)a * out.scale_batch_stride + s]);
+}
+
+// a6 as the K-major operand of the detector GEMM: rows = detector beams d, k = window pixels s.
+// One block per (beam, atom): pass 1 finds the row maximum, pass 2 splits and stores.
+__global__ void __launch_bounds__(128) k_recon_rows_sliced(const float2* __restrict__ D, int n_par, const int32_t* __restrict__ bh, int b0,
+                                    const int32_t* __restrict__ nn_idx, const float* __restrict__ nn_w, int max_nn, int carrier,
+                                    int recon, const int32_t* __restrict__ origin, int w, int ny, int nx,
+                                    const float2* __restrict__ rooty, const float2* __restrict__ rootx, Sliced out) {
+  const int a = blockIdx.y, b = b0 + blockIdx.x;
+  const int w2 = w * w;
+  __shared__ int32_t s_idx[BIP_MAX_NN];
+  __shared__ float s_w[BIP_MAX_NN];
+  __shared__ float s_red[4];
+  if (threadIdx.x < max_nn) {
+    s_idx[threadIdx.x] = nn_idx[(int64_t)b * max_nn + threadIdx.x];
+    s_w[threadIdx.x] = nn_w[(int64_t)b * max_nn + threadIdx.x];
+  }
+  __syncthreads();
+  const int oy = origin[2 * a], ox = origin[2 * a + 1];
+  const int hyp = ((bh[2 * b] % ny) + ny) % ny, hxp = ((bh[2 * b + 1] % nx) + nx) % nx;
+  const float2* Da = D + (int64_t)a * n_par * w2;
+  auto value = [&](int s) {
+    const int sy = s / w, sx = s - sy * w;
+    int ry = oy + sy; if (ry >= ny) ry -= ny;
+    int rx = ox + sx; if (rx >= nx) rx -= nx;
+    float2 t = tilt(rooty, rootx, hyp, hxp, ry, rx, ny, nx);
+    if (carrier < 0) t.y = -t.y;
+    return recon_elem(Da, s_idx, s_w, max_nn, w2, s, recon, t);
+  };
+  float m = 0.f;
+  for (int s = threadIdx.x; s < w2; s += blockDim.x) {
+    const float2 v = value(s);
+    m = fmaxf(m, fmaxf(fabsf(v.x), fabsf(v.y)));
+  }
+#pragma unroll
+  for (int o = 16; o; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = m;
+  __syncthreads();
+  m = fmaxf(fmaxf(s_red[0], s_red[1]), fmaxf(s_red[2], s_red[3]));
+  const float scale = sl_pow2_scale(m), inv = 1.f / scale;
+  if (threadIdx.x == 0) out.scale[(int64_t)a * out.scale_batch_stride + b] = scale;
+  const int n_groups = 2 * (int)out.ksteps;
+  for (int g = threadIdx.x; g < n_groups; g += blockDim.x) {
+    float re[8], im[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      const int s = g * 8 + j;
+      const float2 v = s < w2 ? value(s) : make_float2(0.f, 0.f);
+      re[j] = v.x; im[j] = v.y;
+    }
+    sl_store_group(out, a, b, g, re, im, inv);
+  }
+}
+
+// a3 as the K-major operand of the probe GEMM: rows = scan positions, k = aperture beams; every row has the scale
+// `scale` >= max_b |c_b|.  thread = (rho, group of 8 beams), lanes over consecutive rho.
+__global__ void __launch_bounds__(256) k_illumination_sliced(const double* __restrict__ rho, int n_rho, const int32_t* __restrict__ h,
+                                      const float2* __restrict__ c, int n_ap, int ny, int nx, float scale, Sliced out) {
+  const int r = blockIdx.x * 32 + threadIdx.x, g = blockIdx.y * 8 + threadIdx.y;
+  if (r >= n_rho || g >= 2 * out.ksteps) return;
+  const double py = rho[2 * r], px = rho[2 * r + 1];
+  float re[8], im[8];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    const int b = g * 8 + j;
+    re[j] = 0.f; im[j] = 0.f;
+    if (b < n_ap) {
+      double t = (double)h[2 * b] * py / ny + (double)h[2 * b + 1] * px / nx;
+      t -= rint(t);
+      double sn, cs;
+      sincospi(-2.0 * t, &sn, &cs);
+      const float2 cb = c[b];
+      re[j] = (float)((double)cb.x * cs - (double)cb.y * sn);
+      im[j] = (float)((double)cb.x * sn + (double)cb.y * cs);
+    }
+  }
+  if (g == 0) out.scale[r] = scale;
+  sl_store_group(out, 0, r, g, re, im, 1.f / scale);
+}
+
 }  // namespace
 
 int32_t launch_crop_detilt(bip_ctx* ctx, const float2* S, const int32_t* ph_dev, int32_t n_par, int carrier,
@@ -240,6 +367,48 @@ int32_t launch_illumination(bip_ctx* ctx, const double* rho_dev, int32_t n_rho, 
                                                   ctx->g.ny, ctx->g.nx, o);
     BIP_CUDA(ctx, cudaGetLastError());
   }
+  return BIP_OK;
+}
+
+
+int32_t launch_recon_t_sliced(bip_ctx* ctx, const float2* D, int32_t n_par, const int32_t* bh_dev, int32_t n_beams,
+                              const int32_t* nn_idx, const float* nn_w, int32_t max_nn, int carrier, int recon,
+                              const int32_t* origin_dev, int32_t n_atoms, int32_t w, Sliced out) {
+  const int w2 = w * w;
+  dim3 g0((unsigned)((w2 + 255) / 256), (unsigned)n_atoms);
+  k_parent_colmax<<<g0, 256, 0, ctx->stream>>>(D, n_par, w2, out.scale, out.scale_batch_stride);
+  BIP_CUDA(ctx, cudaGetLastError());
+  dim3 grid((unsigned)((w2 + 31) / 32), (unsigned)((2 * out.ksteps + 7) / 8), (unsigned)n_atoms);
+  k_recon_t_sliced<<<grid, dim3(32, 8), 0, ctx->stream>>>(D, n_par, bh_dev, n_beams, nn_idx, nn_w, max_nn, carrier, recon, origin_dev,
+                                                         w, ctx->g.ny, ctx->g.nx, ctx->rooty_dev, ctx->rootx_dev, out);
+  BIP_CUDA(ctx, cudaGetLastError());
+  ctx->timing.kernel_launches += 2;
+  return BIP_OK;
+}
+
+int32_t launch_recon_rows_sliced(bip_ctx* ctx, const float2* D, int32_t n_par, const int32_t* bh_dev, int32_t n_beams,
+                                 const int32_t* nn_idx, const float* nn_w, int32_t max_nn, int carrier, int recon,
+                                 const int32_t* origin_dev, int32_t n_atoms, int32_t w, Sliced out) {
+  for (int a0 = 0; a0 < n_atoms; a0 += 65535) {          // gridDim.y limit
+    const int na = std::min(65535, n_atoms - a0);
+    Sliced o = out;
+    o.base += (int64_t)a0 * out.batch_stride;
+    o.scale += (int64_t)a0 * out.scale_batch_stride;
+    dim3 grid((unsigned)n_beams, (unsigned)na);
+    k_recon_rows_sliced<<<grid, 128, 0, ctx->stream>>>(D + (int64_t)a0 * n_par * w * w, n_par, bh_dev, 0, nn_idx, nn_w, max_nn, carrier,
+                                                      recon, origin_dev + 2 * (int64_t)a0, w, ctx->g.ny, ctx->g.nx, ctx->rooty_dev,
+                                                      ctx->rootx_dev, o);
+    BIP_CUDA(ctx, cudaGetLastError());
+    ctx->timing.kernel_launches++;
+  }
+  return BIP_OK;
+}
+
+int32_t launch_illumination_sliced(bip_ctx* ctx, const double* rho_dev, int32_t n_rho, float scale, Sliced out) {
+  dim3 grid((unsigned)((n_rho + 31) / 32), (unsigned)((2 * out.ksteps + 7) / 8));
+  k_illumination_sliced<<<grid, dim3(32, 8), 0, ctx->stream>>>(rho_dev, n_rho, ctx->ap_h_dev, ctx->ap_c_dev, ctx->n_ap, ctx->g.ny,
+                                                              ctx->g.nx, scale, out);
+  BIP_CUDA(ctx, cudaGetLastError());
   return BIP_OK;
 }
 
