@@ -53,16 +53,20 @@ typedef enum {
 typedef enum { BIP_MODE_MAP = 0, BIP_MODE_QEELS_X = 1, BIP_MODE_QEELS_Y = 2, BIP_MODE_CUBE = 3 } bip_mode;
 typedef enum { BIP_RECON_LINEAR = 0, BIP_RECON_MAGPHASE = 1 } bip_recon;
 /* Arithmetic of the two contractions (all fp32-equivalent).
- * BF16X6 (the one to use): tcgen05 tensor cores on operands split into three bf16 slices per real number against a
- *   power-of-two row scale; a real product is the six-term sum x1 y1 + (x1 y2 + x2 y1) + (x1 y3 + x2 y2 + x3 y1)
- *   (the tensor time of 3xTF32).  The leading terms x1 y1 are small integers and accumulate EXACTLY in TMEM over
- *   chunks of 256 k-elements; chunk sums are added in fp32 round-to-nearest.  Meets the 1e-6 summed-intensity bound.
+ * FP16X4 (the one to use): tcgen05 tensor cores on operands split, against a power-of-two row scale, into a 9-bit
+ *   fixed-point leading slice and an fp16 residual slice (representation error 2^-21 of the row maximum); a real
+ *   product is the four-term sum x1 y1 + (x1 y2 + x2 y1 + x2 y2) -- 2/3 of the tensor time of 3xTF32.  The leading
+ *   products x1 y1 are small integers and accumulate EXACTLY in TMEM over chunks of 128 k-elements; chunk sums are
+ *   added in fp32 round-to-nearest.  Meets the 1e-6 summed-intensity bound.
+ * BF16X6: the same construction with three bf16 slices per real number (8-bit leading slice, chunks of 256
+ *   k-elements) and the six-term product x1 y1 + (x1 y2 + x2 y1) + (x1 y3 + x2 y2 + x3 y1): representation error
+ *   2^-24 of the row maximum at the tensor time of 3xTF32.
  * TF32X3: every real product as a_hi b_hi + a_hi b_lo + a_lo b_hi of TF32 operands, accumulated in one TMEM chain.
  *   The tensor core truncates on accumulation (profiles/r01_tcgen05_rounding_probe.txt): per-pixel error within
  *   1e-4 but the summed intensity is biased by ~ -1.25e-8 per accumulating MMA (-2.6e-5 at configs[0]).  Kept as the
  *   measured A/B case for that finding.
  * FP32_SIMT: the same contractions on CUDA cores in fp32 -- the A/B reference for the tensor-core kernels. */
-typedef enum { BIP_PREC_TF32X3 = 0, BIP_PREC_FP32_SIMT = 1, BIP_PREC_BF16X6 = 2 } bip_precision;
+typedef enum { BIP_PREC_TF32X3 = 0, BIP_PREC_FP32_SIMT = 1, BIP_PREC_BF16X6 = 2, BIP_PREC_FP16X4 = 3 } bip_precision;
 
 typedef struct bip_ctx bip_ctx;
 

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libbip.so")
 
 MODE_MAP, MODE_QEELS_X, MODE_QEELS_Y, MODE_CUBE = 0, 1, 2, 3
 RECON_LINEAR, RECON_MAGPHASE = 0, 1
-PREC_TF32X3, PREC_FP32_SIMT, PREC_BF16X6 = 0, 1, 2
+PREC_TF32X3, PREC_FP32_SIMT, PREC_BF16X6, PREC_FP16X4 = 0, 1, 2, 3
 MAX_NN = 16
 _STATUS = {1: "BIP_ERR_INVALID", 2: "BIP_ERR_STATE", 3: "BIP_ERR_OOM", 4: "BIP_ERR_CUDA", 5: "BIP_ERR_UNSUPPORTED"}
 
@@ -276,7 +276,7 @@ class Context:
             return (self.n_rho,), np.float64
         return (self.n_rho, n // self.n_rho), np.float32
 
-    def map(self, edge_id: int, mode: int = MODE_MAP, recon: int = RECON_LINEAR, precision: int = PREC_BF16X6, out=None):
+    def map(self, edge_id: int, mode: int = MODE_MAP, recon: int = RECON_LINEAR, precision: int = PREC_FP16X4, out=None):
         """bip_map into a torch CUDA tensor (allocated here unless given); returns it without synchronising."""
         import torch
         shape, dt = self._shape(edge_id, mode)
@@ -288,7 +288,7 @@ class Context:
                                    C.c_size_t(out.numel() * out.element_size())))
         return out
 
-    def map_all(self, mode: int = MODE_MAP, recon: int = RECON_LINEAR, precision: int = PREC_BF16X6):
+    def map_all(self, mode: int = MODE_MAP, recon: int = RECON_LINEAR, precision: int = PREC_FP16X4):
         import torch
         outs = []
         for e in range(len(self._edges)):
@@ -299,7 +299,7 @@ class Context:
         self._ck(self._lib.bip_map_all(self._ctx, mode, recon, precision, ptrs, sizes, len(outs)))
         return outs
 
-    def map_host(self, edge_id: int, mode: int = MODE_MAP, recon: int = RECON_LINEAR, precision: int = PREC_BF16X6) -> np.ndarray:
+    def map_host(self, edge_id: int, mode: int = MODE_MAP, recon: int = RECON_LINEAR, precision: int = PREC_FP16X4) -> np.ndarray:
         shape, dt = self._shape(edge_id, mode)
         out = np.empty(shape, dtype=dt)
         self._ck(self._lib.bip_map_host(self._ctx, edge_id, mode, recon, precision, C.c_void_p(out.ctypes.data), C.c_size_t(out.nbytes)))

@@ -66,29 +66,35 @@ static int32_t planes_in(bip_ctx* ctx, DevBuf& buf, Planes& P, int64_t rows, int
   return BIP_OK;
 }
 
-// Carve a sliced bf16 operand [batch][rows][k] out of one DevBuf.  Producers write every k-step of every valid row;
+// Carve a sliced 16-bit operand [batch][rows][k] of format `fmt` out of one DevBuf.  Producers write every k-step of every valid row;
 // the padding rows of the last row tile only have to be finite (they feed masked accumulator rows / columns), so the
 // buffer is cleared when it is (re)allocated and never again.
-static int32_t sliced_in(bip_ctx* ctx, DevBuf& buf, Sliced& S, int64_t rows, int64_t k, int64_t batch, const char* what) {
+static int32_t sliced_in(bip_ctx* ctx, DevBuf& buf, Sliced& S, int fmt, int64_t rows, int64_t k, int64_t batch, const char* what) {
+  S.fmt = fmt;
   S.rows = rows;
   S.rows_pad = round_up(rows, SL_ROWS);
   S.k = k;
   S.ksteps = (k + SL_K - 1) / SL_K;
-  S.batch_stride = S.rows_pad / SL_ROWS * S.ksteps * SL_STEP_EL;
+  S.batch_stride = S.rows_pad / SL_ROWS * S.ksteps * sl_step_el(fmt);
   const void* before = buf.p;
-  BIP_TRY(ensure(ctx, buf, (size_t)(S.batch_stride * std::max<int64_t>(batch, 1)) * sizeof(__nv_bfloat16), what));
+  BIP_TRY(ensure(ctx, buf, (size_t)(S.batch_stride * std::max<int64_t>(batch, 1)) * sizeof(uint16_t), what));
   if (buf.p != before) BIP_CUDA(ctx, cudaMemsetAsync(buf.p, 0, buf.bytes, ctx->stream));
-  S.base = reinterpret_cast<__nv_bfloat16*>(buf.p);
+  S.base = reinterpret_cast<uint16_t*>(buf.p);
   return BIP_OK;
 }
 
 // a3, built on first use in the format the requested arithmetic reads.
+static void free_illumination(bip_ctx* ctx);
+static inline int sliced_fmt_of(int precision) { return precision == BIP_PREC_FP16X4 ? SL_FMT_FP16X4 : precision == BIP_PREC_BF16X6 ? SL_FMT_BF16X6 : -1; }
+
 static int32_t ensure_illumination(bip_ctx* ctx, int precision) {
-  if (precision == BIP_PREC_BF16X6) {
-    if (ctx->A_sl.base) return BIP_OK;
+  const int fmt = sliced_fmt_of(precision);
+  if (fmt >= 0) {
+    if (ctx->A_sl.base && ctx->A_sl.fmt == fmt) return BIP_OK;
+    if (ctx->A_sl.base) { cudaStreamSynchronize(ctx->stream); cudaFree(ctx->A_sl.base); cudaFree(ctx->A_sl.scale); ctx->A_sl = Sliced(); }
     Sliced A;
     DevBuf b;
-    BIP_TRY(sliced_in(ctx, b, A, ctx->n_rho, ctx->n_ap, 1, "illumination matrix (sliced)"));
+    BIP_TRY(sliced_in(ctx, b, A, fmt, ctx->n_rho, ctx->n_ap, 1, "illumination matrix (sliced)"));
     A.batch_stride = 0;
     if (dev_alloc(ctx, (void**)&A.scale, (size_t)A.rows_pad * sizeof(float), "illumination row scales") != BIP_OK) { cudaFree(b.p); return BIP_ERR_OOM; }
     BIP_CUDA(ctx, cudaMemsetAsync(A.scale, 0, (size_t)A.rows_pad * sizeof(float), ctx->stream));
@@ -202,17 +208,17 @@ static size_t scratch_budget() {
   return (size_t)(gb * (double)(1ull << 30));
 }
 
-// Steps a1-a8 on the sliced bf16 operands (BIP_PREC_BF16X6).
-static int32_t contract_batch_bf16(bip_ctx* ctx, Edge& e, const int32_t* org, int32_t nb, int mode, int recon, void* out) {
+// Steps a1-a8 on the sliced 16-bit operands (BIP_PREC_FP16X4 / BIP_PREC_BF16X6).
+static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, int32_t nb, int mode, int recon, int fmt, void* out) {
   auto& sp = spans()[ctx];
   const int w2 = e.w * e.w;
   const int64_t rho_pad = round_up(ctx->n_rho, SL_ROWS);
   Sliced R1t, R2, Phi;
   BIP_TRY(ensure(ctx, ctx->D1, (size_t)nb * ctx->n_p1 * w2 * sizeof(float2), "D1 (de-tilted S1 windows)"));
   BIP_TRY(ensure(ctx, ctx->D2, (size_t)nb * ctx->n_p2 * w2 * sizeof(float2), "D2 (de-tilted S2 windows)"));
-  BIP_TRY(sliced_in(ctx, ctx->R1s, R1t, w2, ctx->n_ap, nb, "R1 (reconstructed S1 windows, sliced)"));
-  BIP_TRY(sliced_in(ctx, ctx->R2s, R2, e.n_det, w2, nb, "R2 (reconstructed S2 windows, sliced)"));
-  BIP_TRY(sliced_in(ctx, ctx->Phis, Phi, rho_pad * e.n_ch, w2, nb, "Phi (H_n psi, sliced)"));
+  BIP_TRY(sliced_in(ctx, ctx->R1s, R1t, fmt, w2, ctx->n_ap, nb, "R1 (reconstructed S1 windows, sliced)"));
+  BIP_TRY(sliced_in(ctx, ctx->R2s, R2, fmt, e.n_det, w2, nb, "R2 (reconstructed S2 windows, sliced)"));
+  BIP_TRY(sliced_in(ctx, ctx->Phis, Phi, fmt, rho_pad * e.n_ch, w2, nb, "Phi (H_n psi, sliced)"));
   const int64_t psi_ld = w2;
   BIP_TRY(ensure(ctx, ctx->Psi, (size_t)nb * ctx->n_rho * psi_ld * sizeof(float2), "Psi (probe at the atom)"));
   const int64_t n_scale = (int64_t)nb * (R1t.rows_pad + R2.rows_pad + Phi.rows_pad);
@@ -229,7 +235,7 @@ static int32_t contract_batch_bf16(bip_ctx* ctx, Edge& e, const int32_t* org, in
   Gemm1SlArgs g1;
   g1.A = ctx->A_sl; g1.R1t = R1t; g1.Psi = (float2*)ctx->Psi.p; g1.psi_ld = psi_ld; g1.psi_batch_stride = (int64_t)ctx->n_rho * psi_ld;
   g1.n_rho = ctx->n_rho; g1.w2 = w2; g1.n_atoms = nb;
-  BIP_TRY(launch_gemm1_bf16(ctx, g1));
+  BIP_TRY(launch_gemm1_sliced(ctx, g1));
   // a5: times H_n, split into slices
   BIP_TRY(launch_quantize_phi(ctx, g1.Psi, psi_ld, g1.psi_batch_stride, e.H_dev, Phi, ctx->n_rho, (int32_t)rho_pad, w2, e.n_ch, nb));
   // a6: S2 windows -> R2[d][s]
@@ -247,7 +253,7 @@ static int32_t contract_batch_bf16(bip_ctx* ctx, Edge& e, const int32_t* org, in
   g2.out = out;
   {
     Span s(ctx, sp.pool_map, sp.gemm2);
-    BIP_TRY(launch_gemm2_bf16(ctx, g2));
+    BIP_TRY(launch_gemm2_sliced(ctx, g2));
   }
   ctx->timing.gemm2_launches++;
   ctx->timing.amplitudes += (double)ctx->n_rho * nb * e.n_ch * e.n_det;
@@ -261,7 +267,7 @@ static int32_t contract_batch(bip_ctx* ctx, Edge& e, const int32_t* origin_dev, 
   auto& sp = spans()[ctx];
   const int w2 = e.w * e.w;
   const int32_t* org = origin_dev + 2 * (int64_t)a0;
-  if (precision == BIP_PREC_BF16X6) return contract_batch_bf16(ctx, e, org, nb, mode, recon, out);
+  if (sliced_fmt_of(precision) >= 0) return contract_batch_sliced(ctx, e, org, nb, mode, recon, sliced_fmt_of(precision), out);
   Planes R1t, R2, Phi;
   BIP_TRY(ensure(ctx, ctx->D1, (size_t)nb * ctx->n_p1 * w2 * sizeof(float2), "D1 (de-tilted S1 windows)"));
   BIP_TRY(ensure(ctx, ctx->D2, (size_t)nb * ctx->n_p2 * w2 * sizeof(float2), "D2 (de-tilted S2 windows)"));
@@ -323,7 +329,7 @@ static int32_t run_edges(bip_ctx* ctx, const std::vector<int32_t>& ids, int mode
   if (ctx->n_rho <= 0) return fail(ctx, BIP_ERR_STATE, "bip_map: call bip_set_scan first");
   if (mode < BIP_MODE_MAP || mode > BIP_MODE_CUBE) return fail(ctx, BIP_ERR_INVALID, "bip_map: unknown mode %d", mode);
   if (recon != BIP_RECON_LINEAR && recon != BIP_RECON_MAGPHASE) return fail(ctx, BIP_ERR_INVALID, "bip_map: unknown recon %d", recon);
-  if (precision != BIP_PREC_TF32X3 && precision != BIP_PREC_FP32_SIMT && precision != BIP_PREC_BF16X6) return fail(ctx, BIP_ERR_INVALID, "bip_map: unknown precision %d", precision);
+  if (precision != BIP_PREC_TF32X3 && precision != BIP_PREC_FP32_SIMT && precision != BIP_PREC_BF16X6 && precision != BIP_PREC_FP16X4) return fail(ctx, BIP_ERR_INVALID, "bip_map: unknown precision %d", precision);
   if (precision != BIP_PREC_FP32_SIMT && !tc_available()) return fail(ctx, BIP_ERR_UNSUPPORTED, "bip_map: the tensor-core path is not built");
   for (size_t k = 0; k < ids.size(); ++k) {
     if (ids[k] < 0 || ids[k] >= (int)ctx->edges.size()) return fail(ctx, BIP_ERR_INVALID, "bip_map: edge %d does not exist", ids[k]);
@@ -354,7 +360,7 @@ static int32_t run_edges(bip_ctx* ctx, const std::vector<int32_t>& ids, int mode
       auto hi = std::upper_bound(e.slice.begin(), e.slice.end(), plane) - e.slice.begin();
       if (lo == hi) continue;
       const int64_t w2 = (int64_t)e.w * e.w;
-      const int64_t el = precision == BIP_PREC_BF16X6 ? 12 : 16;      // operand bytes per complex element
+      const int64_t el = precision == BIP_PREC_FP16X4 ? 8 : precision == BIP_PREC_BF16X6 ? 12 : 16;      // operand bytes per complex element
       const size_t per_atom = (size_t)((ctx->n_p1 + ctx->n_p2) * w2 * 8 + (int64_t)ctx->n_rho * w2 * 8 +
                                        el * (round_up(w2, 128) * round_up(ctx->n_ap, 32) + round_up(e.n_det, 128) * round_up(w2, 32) +
                                              round_up(ctx->n_rho, 128) * e.n_ch * round_up(w2, 32)));

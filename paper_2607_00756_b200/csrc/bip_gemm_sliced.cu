@@ -1,17 +1,20 @@
-// tcgen05 / TMEM / bulk-TMA versions of the two contractions (steps a4-a5 and a7-a8 of SURVEY.md 8(a)) on the
-// three-slice bf16 operand format of bip_sliced.cuh (precision BIP_PREC_BF16X6, fp32-equivalent).
+// tcgen05 / TMEM / bulk-TMA versions of the two contractions (steps a4-a5 and a7-a8 of SURVEY.md 8(a)) on the sliced
+// 16-bit operand formats of bip_sliced.cuh (precisions BIP_PREC_FP16X4 and BIP_PREC_BF16X6, both fp32-equivalent).
 //
 // One persistent, warp-specialised kernel computes C[128 x 128] (complex) = X[128 x Kd] . Y[128 x Kd]^T per work item:
 //
-//   Cr = Xr Yr - Xi Yi ,  Ci = Xr Yi + Xi Yr ,   real product = x1 y1 + (x1 y2 + x2 y1) + (x1 y3 + x2 y2 + x3 y1)
+//   Cr = Xr Yr - Xi Yi ,  Ci = Xr Yi + Xi Yr
+//   real product = x1 y1 + (x1 y2 + x2 y1 + x2 y2)                               FP16X4: 16 MMAs per 16 k-elements
+//                = x1 y1 + (x1 y2 + x2 y1) + (x1 y3 + x2 y2 + x3 y1)             BF16X6: 24 MMAs per 16 k-elements
 //
-// i.e. 24 tcgen05.mma.kind::f16 (bf16, M = 128, N = 128, K = 16) per 16 k-elements.  Four fp32 accumulators live in
-// TMEM (the whole 512 columns): C0r, C0i take the leading products x1 y1 -- integers / 2^14, summed EXACTLY over a
-// chunk of 256 k-elements -- and C12r, C12i take the small ones.  After every chunk the eight epilogue warps read
-// the accumulators back (tcgen05.ld) and add them to fp32 running sums in registers (round-to-nearest), so the
-// truncating accumulation of the tensor core never biases the result (bip_sliced.cuh).  Operand tiles arrive by
-// cp.async.bulk (one contiguous 24 KB block per operand and k-step) through a 4-stage mbarrier ring; one elected
-// thread issues the MMAs.  Fused epilogues:
+// each a tcgen05.mma.kind::f16 (M = 128, N = 128, K = 16).  Four fp32 accumulators live in TMEM (the whole 512
+// columns): C0r, C0i take the LEADING products x1 y1 -- small integers, summed EXACTLY over a chunk of 128 (256)
+// k-elements -- and C12r, C12i take the small ones over the whole k range.  After every chunk the eight epilogue
+// warps read C0 back (tcgen05.ld) and add it to fp32 running sums in registers (round-to-nearest), so the
+// truncating accumulation of the tensor core never biases the result (bip_sliced.cuh).  The MMA issuer runs the
+// small products LAG k-steps AHEAD of the leading ones, so the tensor pipe keeps working on C12 while the epilogue
+// drains C0.  Operand tiles arrive by cp.async.bulk (one contiguous 16 / 24 KB block per operand and k-step)
+// through an mbarrier ring; one elected thread issues the MMAs.  Fused epilogues:
 //
 //   GEMM1 (a4):    Psi[rho][s] = sx[rho] sy[s] C           -> c64, quantised to Phi_n = H_n Psi by k_quantize_phi (a5)
 //   GEMM2 (a7-a8): |a_n[rho][d]|^2 / G summed over channels and reduced per output mode
@@ -20,6 +23,8 @@
 // warp % 4, column half = (warp - 2) / 4).
 #include <cuda.h>
 
+#include <cstdlib>
+
 #include "bip_internal.h"
 
 namespace bip {
@@ -27,26 +32,38 @@ namespace bip {
 namespace {
 
 constexpr int TM = 128, TN = 128;
-constexpr int STAGES = 4;
-constexpr int X_BYTES = SL_STEP_EL * 2;          // 24 KB
-constexpr int STAGE_BYTES = 2 * X_BYTES;         // X and Y of one k-step
 constexpr int PART_BYTES = SL_TILE_EL * 2;       // 4 KB
-constexpr int CHUNK_STEPS = 16;                  // 256 k-elements: 2 * 256 * 2^14 = 2^23 < 2^24, exact
 constexpr int NUM_EPI_WARPS = 8;
 constexpr int NUM_THREADS = 64 + 32 * NUM_EPI_WARPS;
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
 constexpr int DGROUP = 4;                        // column tiles per raster group (concurrent CTAs share operand tiles in L2)
+
+template <int FMT> struct Cfg;
+template <> struct Cfg<SL_FMT_FP16X4> {
+  static constexpr int PARTS = 4, STAGES = 7, LAG_MAX = 4;
+  static constexpr int CHUNK_STEPS = 8;          // 128 k-elements: 2 * 128 * 2^16 = 2^24, exact
+  static constexpr uint32_t AB_FORMAT = 0;       // fp16
+};
+template <> struct Cfg<SL_FMT_BF16X6> {
+  static constexpr int PARTS = 6, STAGES = 4, LAG_MAX = 2;
+  static constexpr int CHUNK_STEPS = 16;         // 256 k-elements: 2 * 256 * 2^14 = 2^23 < 2^24, exact
+  static constexpr uint32_t AB_FORMAT = 1;       // bf16
+};
+template <int FMT> __host__ __device__ constexpr int x_bytes() { return Cfg<FMT>::PARTS * PART_BYTES; }
+template <int FMT> __host__ __device__ constexpr int stage_bytes() { return 2 * x_bytes<FMT>(); }
+template <int FMT> __host__ __device__ constexpr int smem_bytes() { return Cfg<FMT>::STAGES * stage_bytes<FMT>() + 1024 /*align*/ + 256 /*barriers*/; }
 
 enum { EPI_GEMM1 = 1, EPI_GEMM2 = 2 };
 
-struct BfParams {
-  const __nv_bfloat16* X; const __nv_bfloat16* Y;
+struct SlParams {
+  const uint16_t* X; const uint16_t* Y;
   const float* sx; const float* sy;
   int64_t x_batch_stride, y_batch_stride, sx_batch_stride, sy_batch_stride;
   int ksteps;
   int n_rt, n_ct, n_items, n_ch_loop;
   int n_rows, n_cols;      // valid rows (rho) / columns (s or d) per atom
   int rows_pad;            // padded rho rows per channel block of X
+  int chunk_steps;         // k-steps per exactly accumulated chunk of leading products
+  int lag_max;             // the leading products may trail the small ones by up to this many k-steps (< STAGES)
   // GEMM1 epilogue
   float2* Psi; int64_t psi_ld, psi_batch_stride;
   // GEMM2 epilogue
@@ -77,6 +94,19 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         : "memory");
   }
 }
+__device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {
+  uint32_t done;
+  asm volatile(
+      "{\n\t"
+      ".reg .pred P1;\n\t"
+      "mbarrier.test_wait.parity.shared::cta.b64 P1, [%1], %2;\n\t"
+      "selp.b32 %0, 1, 0, P1;\n\t"
+      "}"
+      : "=r"(done)
+      : "r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+  return done != 0;
+}
 __device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
@@ -93,12 +123,13 @@ __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr) {
   return d;                                           // layout type 0 = no swizzle
 }
 
-// cute::UMMA::InstrDescriptor for kind::f16 with bf16 operands, fp32 accumulate, K-major A and B
-__host__ __device__ constexpr uint32_t umma_idesc(bool neg_a) {
-  return (1u << 4) | (1u << 7) | (1u << 10) | ((neg_a ? 1u : 0u) << 13) | ((uint32_t)(TN >> 3) << 17) | ((uint32_t)(TM >> 4) << 24);
+// cute::UMMA::InstrDescriptor for kind::f16 (fp16 or bf16 operands), fp32 accumulate, K-major A and B
+__host__ __device__ constexpr uint32_t umma_idesc(uint32_t ab_format, bool neg_a) {
+  return (1u << 4) | (ab_format << 7) | (ab_format << 10) | ((neg_a ? 1u : 0u) << 13) | ((uint32_t)(TN >> 3) << 17) |
+         ((uint32_t)(TM >> 4) << 24);
 }
 
-__device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+__device__ __forceinline__ void umma_f16(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
   asm volatile(
       "{\n\t"
       ".reg .pred p;\n\t"
@@ -125,7 +156,7 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
 }
 
 // item -> (atom, row tile, column tile); column tiles rasterised in groups of DGROUP.
-__device__ __forceinline__ void decode_item(const BfParams& p, int item, int& atom, int& rt, int& ct) {
+__device__ __forceinline__ void decode_item(const SlParams& p, int item, int& atom, int& rt, int& ct) {
   const int per_atom = p.n_rt * p.n_ct;
   atom = item / per_atom;
   int idx = item - atom * per_atom;
@@ -143,24 +174,93 @@ __device__ __forceinline__ void decode_item(const BfParams& p, int item, int& at
   }
 }
 
-template <int EPI>
-__global__ void __launch_bounds__(NUM_THREADS, 1) k_bf16_contract(const BfParams p) {
+// The small products of one k-step (accumulators C12r, C12i): everything except x1 y1.
+template <int FMT>
+__device__ __forceinline__ void issue_small(uint32_t t12r, uint32_t t12i, uint32_t a0, uint32_t b0, uint32_t acc) {
+  constexpr uint32_t id_pos = umma_idesc(Cfg<FMT>::AB_FORMAT, false), id_neg = umma_idesc(Cfg<FMT>::AB_FORMAT, true);
+  if (FMT == SL_FMT_FP16X4) {
+    const uint64_t xr1 = umma_desc(a0), xr2 = umma_desc(a0 + PART_BYTES), xi1 = umma_desc(a0 + 2 * PART_BYTES), xi2 = umma_desc(a0 + 3 * PART_BYTES);
+    const uint64_t yr1 = umma_desc(b0), yr2 = umma_desc(b0 + PART_BYTES), yi1 = umma_desc(b0 + 2 * PART_BYTES), yi2 = umma_desc(b0 + 3 * PART_BYTES);
+    // tiniest first: x2 y2, then x1 y2 + x2 y1
+    umma_f16(t12r, xr2, yr2, id_pos, acc);
+    umma_f16(t12r, xi2, yi2, id_neg, 1u);
+    umma_f16(t12r, xr1, yr2, id_pos, 1u);
+    umma_f16(t12r, xr2, yr1, id_pos, 1u);
+    umma_f16(t12r, xi1, yi2, id_neg, 1u);
+    umma_f16(t12r, xi2, yi1, id_neg, 1u);
+    umma_f16(t12i, xr2, yi2, id_pos, acc);
+    umma_f16(t12i, xi2, yr2, id_pos, 1u);
+    umma_f16(t12i, xr1, yi2, id_pos, 1u);
+    umma_f16(t12i, xr2, yi1, id_pos, 1u);
+    umma_f16(t12i, xi1, yr2, id_pos, 1u);
+    umma_f16(t12i, xi2, yr1, id_pos, 1u);
+  } else {
+    const uint64_t xr1 = umma_desc(a0), xr2 = umma_desc(a0 + PART_BYTES), xr3 = umma_desc(a0 + 2 * PART_BYTES);
+    const uint64_t xi1 = umma_desc(a0 + 3 * PART_BYTES), xi2 = umma_desc(a0 + 4 * PART_BYTES), xi3 = umma_desc(a0 + 5 * PART_BYTES);
+    const uint64_t yr1 = umma_desc(b0), yr2 = umma_desc(b0 + PART_BYTES), yr3 = umma_desc(b0 + 2 * PART_BYTES);
+    const uint64_t yi1 = umma_desc(b0 + 3 * PART_BYTES), yi2 = umma_desc(b0 + 4 * PART_BYTES), yi3 = umma_desc(b0 + 5 * PART_BYTES);
+    // C12r = sum over (i + j in {3, 4}) of xr_i yr_j - xi_i yi_j
+    umma_f16(t12r, xr1, yr3, id_pos, acc);
+    umma_f16(t12r, xr2, yr2, id_pos, 1u);
+    umma_f16(t12r, xr3, yr1, id_pos, 1u);
+    umma_f16(t12r, xi1, yi3, id_neg, 1u);
+    umma_f16(t12r, xi2, yi2, id_neg, 1u);
+    umma_f16(t12r, xi3, yi1, id_neg, 1u);
+    umma_f16(t12r, xr1, yr2, id_pos, 1u);
+    umma_f16(t12r, xr2, yr1, id_pos, 1u);
+    umma_f16(t12r, xi1, yi2, id_neg, 1u);
+    umma_f16(t12r, xi2, yi1, id_neg, 1u);
+    // C12i = sum of xr_i yi_j + xi_i yr_j
+    umma_f16(t12i, xr1, yi3, id_pos, acc);
+    umma_f16(t12i, xr2, yi2, id_pos, 1u);
+    umma_f16(t12i, xr3, yi1, id_pos, 1u);
+    umma_f16(t12i, xi1, yr3, id_pos, 1u);
+    umma_f16(t12i, xi2, yr2, id_pos, 1u);
+    umma_f16(t12i, xi3, yr1, id_pos, 1u);
+    umma_f16(t12i, xr1, yi2, id_pos, 1u);
+    umma_f16(t12i, xr2, yi1, id_pos, 1u);
+    umma_f16(t12i, xi1, yr2, id_pos, 1u);
+    umma_f16(t12i, xi2, yr1, id_pos, 1u);
+  }
+}
+
+// The leading products x1 y1 of one k-step (accumulators C0r, C0i): exact.
+template <int FMT>
+__device__ __forceinline__ void issue_lead(uint32_t t0r, uint32_t t0i, uint32_t a0, uint32_t b0, uint32_t acc) {
+  constexpr uint32_t id_pos = umma_idesc(Cfg<FMT>::AB_FORMAT, false), id_neg = umma_idesc(Cfg<FMT>::AB_FORMAT, true);
+  constexpr int IM = (Cfg<FMT>::PARTS / 2) * PART_BYTES;          // offset of the first imaginary slice
+  const uint64_t xr1 = umma_desc(a0), xi1 = umma_desc(a0 + IM), yr1 = umma_desc(b0), yi1 = umma_desc(b0 + IM);
+  umma_f16(t0r, xr1, yr1, id_pos, acc);
+  umma_f16(t0r, xi1, yi1, id_neg, 1u);
+  umma_f16(t0i, xr1, yi1, id_pos, acc);
+  umma_f16(t0i, xi1, yr1, id_pos, 1u);
+}
+
+template <int EPI, int FMT>
+__global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlParams p) {
+  using C = Cfg<FMT>;
+  constexpr int STAGES = C::STAGES;
+  constexpr int X_BYTES = x_bytes<FMT>(), STAGE_BYTES = stage_bytes<FMT>(), STEP_EL = sl_step_el(FMT);
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + STAGES * STAGE_BYTES);
   uint64_t* full = bars;                 // [STAGES]
   uint64_t* empty = bars + STAGES;       // [STAGES]
-  uint64_t* tmem_full = bars + 2 * STAGES;
-  uint64_t* tmem_empty = bars + 2 * STAGES + 1;
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * STAGES + 2);
+  uint64_t* c0_full = bars + 2 * STAGES;       // leading accumulators of a chunk complete
+  uint64_t* c0_empty = bars + 2 * STAGES + 1;  // ... drained by the epilogue warps
+  uint64_t* c12_full = bars + 2 * STAGES + 2;  // small-product accumulators of a (tile, channel) complete
+  uint64_t* c12_empty = bars + 2 * STAGES + 3;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * STAGES + 4);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int n_chunks = (p.ksteps + CHUNK_STEPS - 1) / CHUNK_STEPS;
+  const int n_my_items = p.n_items > (int)blockIdx.x ? (p.n_items - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
 
   if (warp == 0 && lane == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
-    mbar_init(tmem_full, 1);
-    mbar_init(tmem_empty, NUM_EPI_WARPS);
+    mbar_init(c0_full, 1);
+    mbar_init(c0_empty, NUM_EPI_WARPS);
+    mbar_init(c12_full, 1);
+    mbar_init(c12_empty, NUM_EPI_WARPS);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) {   // the whole tensor memory: 512 columns
@@ -179,82 +279,72 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_bf16_contract(const BfParams
       for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
         int atom, rt, ct;
         decode_item(p, item, atom, rt, ct);
-        const __nv_bfloat16* ysrc = p.Y + (int64_t)atom * p.y_batch_stride + (int64_t)ct * p.ksteps * SL_STEP_EL;
+        const uint16_t* ysrc = p.Y + (int64_t)atom * p.y_batch_stride + (int64_t)ct * p.ksteps * STEP_EL;
         for (int n = 0; n < p.n_ch_loop; ++n) {
-          const __nv_bfloat16* xsrc = p.X + (int64_t)atom * p.x_batch_stride + ((int64_t)n * p.n_rt + rt) * p.ksteps * SL_STEP_EL;
+          const uint16_t* xsrc = p.X + (int64_t)atom * p.x_batch_stride + ((int64_t)n * p.n_rt + rt) * p.ksteps * STEP_EL;
           for (int ks = 0; ks < p.ksteps; ++ks, ++it) {
             const int s = it % STAGES;
             mbar_wait(&empty[s], ((it / STAGES) & 1) ^ 1);
             uint8_t* st = smem + s * STAGE_BYTES;
             mbar_expect_tx(&full[s], STAGE_BYTES);
-            bulk_load(st, xsrc + (int64_t)ks * SL_STEP_EL, X_BYTES, &full[s]);
-            bulk_load(st + X_BYTES, ysrc + (int64_t)ks * SL_STEP_EL, X_BYTES, &full[s]);
+            bulk_load(st, xsrc + (int64_t)ks * STEP_EL, X_BYTES, &full[s]);
+            bulk_load(st + X_BYTES, ysrc + (int64_t)ks * STEP_EL, X_BYTES, &full[s]);
           }
         }
       }
     }
   } else if (warp == 1) {
     // ================= MMA issuer =================
+    // The k-steps of all (tile, channel) segments of this CTA form one sequence g = 0 .. total - 1.  The small
+    // products of k-step g are issued first; the leading products follow through a second cursor gl <= g.  When the
+    // leading cursor reaches a new chunk whose C0 the epilogue has not drained yet, the issuer does not block: it
+    // keeps queueing small products (up to lag_max k-steps ahead), so the tensor pipe stays busy during the drain,
+    // and the leading products catch up afterwards.  At a segment boundary the leading cursor catches up first: the
+    // epilogue cannot release C12 before it has seen every C0 chunk but the last.
     if (lane == 0) {
-      uint32_t it = 0, chunk_id = 0;
-      const uint32_t id_pos = umma_idesc(false), id_neg = umma_idesc(true);
       const uint32_t t0r = tmem_base, t0i = tmem_base + TN, t12r = tmem_base + 2 * TN, t12i = tmem_base + 3 * TN;
-      for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
-        for (int n = 0; n < p.n_ch_loop; ++n) {
-          for (int c = 0; c < n_chunks; ++c, ++chunk_id) {
-            mbar_wait(tmem_empty, (chunk_id & 1) ^ 1);        // epilogue has drained the previous chunk
-            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            const int ks_end = min(p.ksteps, (c + 1) * CHUNK_STEPS);
-            for (int ks = c * CHUNK_STEPS; ks < ks_end; ++ks, ++it) {
-              const int s = it % STAGES;
-              mbar_wait(&full[s], (it / STAGES) & 1);
-              asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-              const uint32_t a0 = smem_u32(smem + s * STAGE_BYTES), b0 = a0 + X_BYTES;
-              const uint64_t xr1 = umma_desc(a0), xr2 = umma_desc(a0 + PART_BYTES), xr3 = umma_desc(a0 + 2 * PART_BYTES);
-              const uint64_t xi1 = umma_desc(a0 + 3 * PART_BYTES), xi2 = umma_desc(a0 + 4 * PART_BYTES), xi3 = umma_desc(a0 + 5 * PART_BYTES);
-              const uint64_t yr1 = umma_desc(b0), yr2 = umma_desc(b0 + PART_BYTES), yr3 = umma_desc(b0 + 2 * PART_BYTES);
-              const uint64_t yi1 = umma_desc(b0 + 3 * PART_BYTES), yi2 = umma_desc(b0 + 4 * PART_BYTES), yi3 = umma_desc(b0 + 5 * PART_BYTES);
-              const uint32_t acc = ks > c * CHUNK_STEPS ? 1u : 0u;
-              // small products first: C12r = sum over (i + j in {3, 4}) of xr_i yr_j - xi_i yi_j
-              umma_bf16(t12r, xr1, yr3, id_pos, acc);
-              umma_bf16(t12r, xr2, yr2, id_pos, 1u);
-              umma_bf16(t12r, xr3, yr1, id_pos, 1u);
-              umma_bf16(t12r, xi1, yi3, id_neg, 1u);
-              umma_bf16(t12r, xi2, yi2, id_neg, 1u);
-              umma_bf16(t12r, xi3, yi1, id_neg, 1u);
-              umma_bf16(t12r, xr1, yr2, id_pos, 1u);
-              umma_bf16(t12r, xr2, yr1, id_pos, 1u);
-              umma_bf16(t12r, xi1, yi2, id_neg, 1u);
-              umma_bf16(t12r, xi2, yi1, id_neg, 1u);
-              // C12i = sum of xr_i yi_j + xi_i yr_j
-              umma_bf16(t12i, xr1, yi3, id_pos, acc);
-              umma_bf16(t12i, xr2, yi2, id_pos, 1u);
-              umma_bf16(t12i, xr3, yi1, id_pos, 1u);
-              umma_bf16(t12i, xi1, yr3, id_pos, 1u);
-              umma_bf16(t12i, xi2, yr2, id_pos, 1u);
-              umma_bf16(t12i, xi3, yr1, id_pos, 1u);
-              umma_bf16(t12i, xr1, yi2, id_pos, 1u);
-              umma_bf16(t12i, xr2, yi1, id_pos, 1u);
-              umma_bf16(t12i, xi1, yr2, id_pos, 1u);
-              umma_bf16(t12i, xi2, yr1, id_pos, 1u);
-              // leading products, exact
-              umma_bf16(t0r, xr1, yr1, id_pos, acc);
-              umma_bf16(t0r, xi1, yi1, id_neg, 1u);
-              umma_bf16(t0i, xr1, yi1, id_pos, acc);
-              umma_bf16(t0i, xi1, yr1, id_pos, 1u);
-              umma_commit(&empty[s]);                    // stage reusable once these MMAs have read it
-            }
-            umma_commit(tmem_full);                      // accumulators of this chunk complete
-          }
+      const uint32_t total = (uint32_t)n_my_items * (uint32_t)p.n_ch_loop * (uint32_t)p.ksteps;
+      const uint32_t chunk = (uint32_t)p.chunk_steps, lag_max = (uint32_t)p.lag_max;
+      uint32_t ks_s = 0, seg_s = 0;              // small-product cursor: k-step inside its segment, segment number
+      uint32_t gl = 0, ks_l = 0, chunk_id = 0;   // leading-product cursor
+      auto lead = [&]() {
+        const uint32_t s = gl % STAGES, in_chunk = ks_l % chunk;
+        if (in_chunk == 0) {
+          mbar_wait(c0_empty, (chunk_id & 1) ^ 1);                   // epilogue has drained the previous chunk's C0
+          asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        }
+        const uint32_t a0 = smem_u32(smem + s * STAGE_BYTES);
+        issue_lead<FMT>(t0r, t0i, a0, a0 + X_BYTES, in_chunk ? 1u : 0u);
+        umma_commit(&empty[s]);                                      // stage reusable once every MMA so far has read it
+        ++gl; ++ks_l;
+        if (in_chunk == chunk - 1 || ks_l == (uint32_t)p.ksteps) { umma_commit(c0_full); ++chunk_id; }
+        if (ks_l == (uint32_t)p.ksteps) ks_l = 0;
+      };
+      for (uint32_t g = 0; g < total; ++g) {
+        const uint32_t s = g % STAGES;
+        mbar_wait(&full[s], (g / STAGES) & 1);
+        if (ks_s == 0) {
+          while (gl < g) lead();
+          mbar_wait(c12_empty, (seg_s & 1) ^ 1);                     // epilogue has drained the previous segment's C12
+        }
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        const uint32_t a0 = smem_u32(smem + s * STAGE_BYTES);
+        issue_small<FMT>(t12r, t12i, a0, a0 + X_BYTES, ks_s ? 1u : 0u);
+        if (++ks_s == (uint32_t)p.ksteps) { umma_commit(c12_full); ks_s = 0; ++seg_s; }
+        while (gl <= g) {
+          if (ks_l % chunk == 0 && g - gl + 1 < lag_max && !mbar_test(c0_empty, (chunk_id & 1) ^ 1)) break;
+          lead();
         }
       }
+      while (gl < total) lead();
     }
   } else {
     // ================= epilogue warps =================
     const int quarter = warp & 3;                      // TMEM lanes [32 q, 32 q + 32) are visible to warps with warp % 4 == q
     const int half = (warp - 2) >> 2;                  // columns [64 half, 64 half + 64) of every accumulator
     const uint32_t t_lane = tmem_base + ((uint32_t)(quarter * 32) << 16) + half * 64;
-    uint32_t chunk_id = 0;
+    const int n_chunks = (p.ksteps + p.chunk_steps - 1) / p.chunk_steps;
+    uint32_t chunk_id = 0, seg = 0;
     for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
       int atom, rt, ct;
       decode_item(p, item, atom, rt, ct);
@@ -263,37 +353,32 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_bf16_contract(const BfParams
       const int col0 = ct * TN + half * 64;
       const float* sy = p.sy + (int64_t)atom * p.sy_batch_stride;
       float rowsum = 0.f;
-      for (int n = 0; n < p.n_ch_loop; ++n) {
+      for (int n = 0; n < p.n_ch_loop; ++n, ++seg) {
         float rr[64], ri[64];
 #pragma unroll
         for (int j = 0; j < 64; ++j) { rr[j] = 0.f; ri[j] = 0.f; }
 #pragma unroll 1
-        for (int c = 0; c < n_chunks; ++c, ++chunk_id) {
-          mbar_wait(tmem_full, chunk_id & 1);
+        for (int c = 0; c <= n_chunks; ++c) {
+          // n_chunks passes over the exact leading sums C0 and one over the small products C12, which is taken
+          // before the last C0 chunk: C12 is complete LAG k-steps earlier, and releasing it first lets the issuer
+          // start the next segment's small products while the last chunk drains
+          const bool small = c == n_chunks - 1;
+          if (small) mbar_wait(c12_full, seg & 1); else mbar_wait(c0_full, chunk_id & 1);
           asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+          const uint32_t tr = t_lane + (small ? 2 * TN : 0), ti = tr + TN;
 #pragma unroll
           for (int g = 0; g < 2; ++g) {
-            uint32_t v[32];
-            tmem_ld32(t_lane + g * 32, v);                   // C0r
+            uint32_t v[32], u[32];
+            tmem_ld32(tr + g * 32, v);
+            tmem_ld32(ti + g * 32, u);
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
-            for (int j = 0; j < 32; ++j) rr[g * 32 + j] += __uint_as_float(v[j]);
-            tmem_ld32(t_lane + 2 * TN + g * 32, v);          // C12r
-            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-            for (int j = 0; j < 32; ++j) rr[g * 32 + j] += __uint_as_float(v[j]);
-            tmem_ld32(t_lane + TN + g * 32, v);              // C0i
-            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-            for (int j = 0; j < 32; ++j) ri[g * 32 + j] += __uint_as_float(v[j]);
-            tmem_ld32(t_lane + 3 * TN + g * 32, v);          // C12i
-            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-            for (int j = 0; j < 32; ++j) ri[g * 32 + j] += __uint_as_float(v[j]);
+            for (int j = 0; j < 32; ++j) { rr[g * 32 + j] += __uint_as_float(v[j]); ri[g * 32 + j] += __uint_as_float(u[j]); }
           }
           asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
           __syncwarp();
-          if (lane == 0) mbar_arrive(tmem_empty);
+          if (lane == 0) mbar_arrive(small ? c12_empty : c0_empty);
+          if (!small) ++chunk_id;
         }
         // ---- end of a (tile, channel): fused epilogue on the running sums ----
         const float sxr = row_ok ? p.sx[(int64_t)atom * p.sx_batch_stride + (int64_t)n * p.rows_pad + row] : 0.f;
@@ -382,25 +467,36 @@ __global__ void __launch_bounds__(256) k_quantize_phi(const float2* __restrict__
   }
 }
 
-template <int EPI>
-int32_t launch(bip_ctx* ctx, const BfParams& p) {
+template <int EPI, int FMT>
+int32_t launch_fmt(bip_ctx* ctx, const SlParams& p) {
   static bool attr_set = false;
   if (!attr_set) {
-    BIP_CUDA(ctx, cudaFuncSetAttribute(k_bf16_contract<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+    BIP_CUDA(ctx, cudaFuncSetAttribute(k_sliced_contract<EPI, FMT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<FMT>()));
     attr_set = true;
   }
   if (p.n_items <= 0) return BIP_OK;
+  SlParams q = p;
+  q.chunk_steps = Cfg<FMT>::CHUNK_STEPS;
+  q.lag_max = Cfg<FMT>::LAG_MAX;
+  if (const char* e = std::getenv("BIP_TUNE_CHUNK")) q.chunk_steps = std::max(1, std::atoi(e));   // timing experiments only: breaks exactness
+  if (const char* e = std::getenv("BIP_TUNE_LAG")) q.lag_max = std::min(std::max(1, std::atoi(e)), Cfg<FMT>::STAGES - 1);
   const int grid = std::max(1, std::min(p.n_items, ctx->sm_count));
-  k_bf16_contract<EPI><<<grid, NUM_THREADS, SMEM_BYTES, ctx->stream>>>(p);
+  k_sliced_contract<EPI, FMT><<<grid, NUM_THREADS, smem_bytes<FMT>(), ctx->stream>>>(q);
   BIP_CUDA(ctx, cudaGetLastError());
   ctx->timing.kernel_launches++;
   return BIP_OK;
 }
 
+template <int EPI>
+int32_t launch(bip_ctx* ctx, const SlParams& p, int fmt) {
+  return fmt == SL_FMT_FP16X4 ? launch_fmt<EPI, SL_FMT_FP16X4>(ctx, p) : launch_fmt<EPI, SL_FMT_BF16X6>(ctx, p);
+}
+
 }  // namespace
 
-int32_t launch_gemm1_bf16(bip_ctx* ctx, const Gemm1SlArgs& a) {
-  BfParams p{};
+int32_t launch_gemm1_sliced(bip_ctx* ctx, const Gemm1SlArgs& a) {
+  if (a.A.fmt != a.R1t.fmt) return fail(ctx, BIP_ERR_INVALID, "gemm1: operand formats differ");
+  SlParams p{};
   p.X = a.A.base; p.sx = a.A.scale; p.x_batch_stride = 0; p.sx_batch_stride = 0;
   p.Y = a.R1t.base; p.sy = a.R1t.scale; p.y_batch_stride = a.R1t.batch_stride; p.sy_batch_stride = a.R1t.scale_batch_stride;
   p.ksteps = (int)a.A.ksteps;
@@ -410,7 +506,7 @@ int32_t launch_gemm1_bf16(bip_ctx* ctx, const Gemm1SlArgs& a) {
   p.n_ch_loop = 1;
   p.n_rows = a.n_rho; p.n_cols = a.w2; p.rows_pad = (int)a.A.rows_pad;
   p.Psi = a.Psi; p.psi_ld = a.psi_ld; p.psi_batch_stride = a.psi_batch_stride;
-  return launch<EPI_GEMM1>(ctx, p);
+  return launch<EPI_GEMM1>(ctx, p, a.A.fmt);
 }
 
 int32_t launch_quantize_phi(bip_ctx* ctx, const float2* Psi, int64_t psi_ld, int64_t psi_batch_stride, const float2* H,
@@ -422,8 +518,9 @@ int32_t launch_quantize_phi(bip_ctx* ctx, const float2* Psi, int64_t psi_ld, int
   return BIP_OK;
 }
 
-int32_t launch_gemm2_bf16(bip_ctx* ctx, const Gemm2SlArgs& a) {
-  BfParams p{};
+int32_t launch_gemm2_sliced(bip_ctx* ctx, const Gemm2SlArgs& a) {
+  if (a.Phi.fmt != a.R2.fmt) return fail(ctx, BIP_ERR_INVALID, "gemm2: operand formats differ");
+  SlParams p{};
   p.X = a.Phi.base; p.sx = a.Phi.scale; p.x_batch_stride = a.Phi.batch_stride; p.sx_batch_stride = a.Phi.scale_batch_stride;
   p.Y = a.R2.base; p.sy = a.R2.scale; p.y_batch_stride = a.R2.batch_stride; p.sy_batch_stride = a.R2.scale_batch_stride;
   p.ksteps = (int)a.Phi.ksteps;
@@ -434,7 +531,7 @@ int32_t launch_gemm2_bf16(bip_ctx* ctx, const Gemm2SlArgs& a) {
   p.n_ch_loop = a.n_ch;
   p.n_rows = a.n_rho; p.n_cols = a.n_det;
   p.mode = a.mode; p.inv_G = a.inv_G; p.bin_of_det = a.bin_of_det; p.n_bins = a.n_bins; p.out = a.out;
-  return launch<EPI_GEMM2>(ctx, p);
+  return launch<EPI_GEMM2>(ctx, p, a.Phi.fmt);
 }
 
 }  // namespace bip

@@ -91,13 +91,13 @@ struct bip_ctx {
   int32_t n_rho = 0;
   double* rho_dev = nullptr;       // [n_rho][2] scan positions in pixels
   bip::Planes A;                   // illumination [n_rho][n_ap] split planes (K-major over b); built on first use
-  bip::Sliced A_sl;                // the same as a sliced bf16 operand; built on first use
+  bip::Sliced A_sl;                // the same as a sliced 16-bit operand (format A_sl.fmt); built on first use
 
   std::vector<bip::Edge> edges;
 
   // scratch, grown on demand
   bip::DevBuf D1, D2, R1, R2, Psi, Phi;
-  bip::DevBuf R1s, R2s, Phis, Scl;  // sliced operands of the bf16 path and their row scales
+  bip::DevBuf R1s, R2s, Phis, Scl;  // sliced operands of the tensor-core path and their row scales
 
   bip_timing timing{};
   cudaEvent_t ev[8] = {};
@@ -172,7 +172,7 @@ int32_t launch_gemm1_tc(bip_ctx* ctx, const Gemm1Args& a);
 int32_t launch_gemm2_tc(bip_ctx* ctx, const Gemm2Args& a);
 bool tc_available();
 
-// ---- contractions on sliced bf16 operands (bip_gemm_bf16.cu) ----
+// ---- contractions on sliced 16-bit operands (bip_gemm_sliced.cu) ----
 struct Gemm1SlArgs {     // a4: Psi = A . R1   (c64 [atom][rho][s])
   Sliced A;              // rows rho, k = aperture beams
   Sliced R1t;            // rows s, k = aperture beams, batch = atoms
@@ -191,8 +191,8 @@ struct Gemm2SlArgs {     // a7 + a8
   int32_t n_bins;
   void* out;
 };
-int32_t launch_gemm1_bf16(bip_ctx* ctx, const Gemm1SlArgs& a);
-int32_t launch_gemm2_bf16(bip_ctx* ctx, const Gemm2SlArgs& a);
+int32_t launch_gemm1_sliced(bip_ctx* ctx, const Gemm1SlArgs& a);
+int32_t launch_gemm2_sliced(bip_ctx* ctx, const Gemm2SlArgs& a);
 int32_t launch_quantize_phi(bip_ctx* ctx, const float2* Psi, int64_t psi_ld, int64_t psi_batch_stride, const float2* H,
                             const Sliced& Phi, int32_t n_rho, int32_t rows_pad, int32_t w2, int32_t n_ch, int32_t n_atoms);
 int32_t launch_recon_t_sliced(bip_ctx* ctx, const float2* D, int32_t n_par, const int32_t* bh_dev, int32_t n_beams,
