@@ -123,24 +123,90 @@ __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr) {
   return d;                                           // layout type 0 = no swizzle
 }
 
-// cute::UMMA::InstrDescriptor for kind::f16 (fp16 or bf16 operands), fp32 accumulate, K-major A and B
-__host__ __device__ constexpr uint32_t umma_idesc(uint32_t ab_format, bool neg_a) {
+// cute::UMMA::InstrDescriptor for kind::f16 (fp16 or bf16 operands), fp32 accumulate, K-major A and B;
+// M = 128 (one CTA) or 256 (CTA pair, cta_group::2), N = 128
+__host__ __device__ constexpr uint32_t umma_idesc(uint32_t ab_format, bool neg_a, bool pair) {
   return (1u << 4) | (ab_format << 7) | (ab_format << 10) | ((neg_a ? 1u : 0u) << 13) | ((uint32_t)(TN >> 3) << 17) |
-         ((uint32_t)(TM >> 4) << 24);
+         ((uint32_t)((pair ? 2 * TM : TM) >> 4) << 24);
 }
 
+template <bool PAIR>
 __device__ __forceinline__ void umma_f16(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+  if (PAIR)
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t"
+        "}" ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
+        : "memory");
+  else
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
+        "}" ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+
+// tcgen05.commit: the mbarrier is arrived on once every MMA issued so far by this thread has completed; for a CTA
+// pair the arrival is multicast to the barrier at the same offset in both CTAs.
+template <bool PAIR>
+__device__ __forceinline__ void umma_commit(uint64_t* bar) {
+  if (PAIR)
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+                 ::"r"(smem_u32(bar)), "h"((uint16_t)3) : "memory");
+  else
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+// one lane of the (converged) warp: the thread that issues every tcgen05.mma / tcgen05.commit of the CTA
+__device__ __forceinline__ uint32_t elect_one() {
+  uint32_t pred;
   asm volatile(
       "{\n\t"
-      ".reg .pred p;\n\t"
-      "setp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
-      "}" ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
-      : "memory");
+      ".reg .pred P1;\n\t"
+      "elect.sync _|P1, 0xffffffff;\n\t"
+      "selp.b32 %0, 1, 0, P1;\n\t"
+      "}"
+      : "=r"(pred));
+  return pred;
 }
 
-__device__ __forceinline__ void umma_commit(uint64_t* bar) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+// ---- CTA-pair plumbing ----
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// arrive on the barrier at the same shared-memory offset in CTA `rank` of the cluster
+__device__ __forceinline__ void mbar_arrive_cluster(uint64_t* bar, uint32_t rank) {
+  asm volatile(
+      "{\n\t"
+      ".reg .b32 ra;\n\t"
+      "mapa.shared::cluster.u32 ra, %0, %1;\n\t"
+      "mbarrier.arrive.release.cluster.shared::cluster.b64 _, [ra];\n\t"
+      "}" ::"r"(smem_u32(bar)), "r"(rank)
+      : "memory");
+}
+// wait on a barrier that threads of the peer CTA arrive on
+__device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity) {
+  uint32_t done = 0;
+  while (!done) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred P1;\n\t"
+        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 P1, [%1], %2;\n\t"
+        "selp.b32 %0, 1, 0, P1;\n\t"
+        "}"
+        : "=r"(done)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+  }
 }
 
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
@@ -175,65 +241,69 @@ __device__ __forceinline__ void decode_item(const SlParams& p, int item, int& at
 }
 
 // The small products of one k-step (accumulators C12r, C12i): everything except x1 y1.
-template <int FMT>
+template <int FMT, bool PAIR>
 __device__ __forceinline__ void issue_small(uint32_t t12r, uint32_t t12i, uint32_t a0, uint32_t b0, uint32_t acc) {
-  constexpr uint32_t id_pos = umma_idesc(Cfg<FMT>::AB_FORMAT, false), id_neg = umma_idesc(Cfg<FMT>::AB_FORMAT, true);
+  constexpr uint32_t id_pos = umma_idesc(Cfg<FMT>::AB_FORMAT, false, PAIR), id_neg = umma_idesc(Cfg<FMT>::AB_FORMAT, true, PAIR);
+  constexpr int YP = PAIR ? PART_BYTES / 2 : PART_BYTES;      // a CTA of a pair holds 64 of the 128 Y rows of every part
+  auto umma = [](uint32_t d, uint64_t da, uint64_t db, uint32_t id, uint32_t ac) { umma_f16<PAIR>(d, da, db, id, ac); };
   if (FMT == SL_FMT_FP16X4) {
     const uint64_t xr1 = umma_desc(a0), xr2 = umma_desc(a0 + PART_BYTES), xi1 = umma_desc(a0 + 2 * PART_BYTES), xi2 = umma_desc(a0 + 3 * PART_BYTES);
-    const uint64_t yr1 = umma_desc(b0), yr2 = umma_desc(b0 + PART_BYTES), yi1 = umma_desc(b0 + 2 * PART_BYTES), yi2 = umma_desc(b0 + 3 * PART_BYTES);
+    const uint64_t yr1 = umma_desc(b0), yr2 = umma_desc(b0 + YP), yi1 = umma_desc(b0 + 2 * YP), yi2 = umma_desc(b0 + 3 * YP);
     // tiniest first: x2 y2, then x1 y2 + x2 y1
-    umma_f16(t12r, xr2, yr2, id_pos, acc);
-    umma_f16(t12r, xi2, yi2, id_neg, 1u);
-    umma_f16(t12r, xr1, yr2, id_pos, 1u);
-    umma_f16(t12r, xr2, yr1, id_pos, 1u);
-    umma_f16(t12r, xi1, yi2, id_neg, 1u);
-    umma_f16(t12r, xi2, yi1, id_neg, 1u);
-    umma_f16(t12i, xr2, yi2, id_pos, acc);
-    umma_f16(t12i, xi2, yr2, id_pos, 1u);
-    umma_f16(t12i, xr1, yi2, id_pos, 1u);
-    umma_f16(t12i, xr2, yi1, id_pos, 1u);
-    umma_f16(t12i, xi1, yr2, id_pos, 1u);
-    umma_f16(t12i, xi2, yr1, id_pos, 1u);
+    umma(t12r, xr2, yr2, id_pos, acc);
+    umma(t12r, xi2, yi2, id_neg, 1u);
+    umma(t12r, xr1, yr2, id_pos, 1u);
+    umma(t12r, xr2, yr1, id_pos, 1u);
+    umma(t12r, xi1, yi2, id_neg, 1u);
+    umma(t12r, xi2, yi1, id_neg, 1u);
+    umma(t12i, xr2, yi2, id_pos, acc);
+    umma(t12i, xi2, yr2, id_pos, 1u);
+    umma(t12i, xr1, yi2, id_pos, 1u);
+    umma(t12i, xr2, yi1, id_pos, 1u);
+    umma(t12i, xi1, yr2, id_pos, 1u);
+    umma(t12i, xi2, yr1, id_pos, 1u);
   } else {
     const uint64_t xr1 = umma_desc(a0), xr2 = umma_desc(a0 + PART_BYTES), xr3 = umma_desc(a0 + 2 * PART_BYTES);
     const uint64_t xi1 = umma_desc(a0 + 3 * PART_BYTES), xi2 = umma_desc(a0 + 4 * PART_BYTES), xi3 = umma_desc(a0 + 5 * PART_BYTES);
-    const uint64_t yr1 = umma_desc(b0), yr2 = umma_desc(b0 + PART_BYTES), yr3 = umma_desc(b0 + 2 * PART_BYTES);
-    const uint64_t yi1 = umma_desc(b0 + 3 * PART_BYTES), yi2 = umma_desc(b0 + 4 * PART_BYTES), yi3 = umma_desc(b0 + 5 * PART_BYTES);
+    const uint64_t yr1 = umma_desc(b0), yr2 = umma_desc(b0 + YP), yr3 = umma_desc(b0 + 2 * YP);
+    const uint64_t yi1 = umma_desc(b0 + 3 * YP), yi2 = umma_desc(b0 + 4 * YP), yi3 = umma_desc(b0 + 5 * YP);
     // C12r = sum over (i + j in {3, 4}) of xr_i yr_j - xi_i yi_j
-    umma_f16(t12r, xr1, yr3, id_pos, acc);
-    umma_f16(t12r, xr2, yr2, id_pos, 1u);
-    umma_f16(t12r, xr3, yr1, id_pos, 1u);
-    umma_f16(t12r, xi1, yi3, id_neg, 1u);
-    umma_f16(t12r, xi2, yi2, id_neg, 1u);
-    umma_f16(t12r, xi3, yi1, id_neg, 1u);
-    umma_f16(t12r, xr1, yr2, id_pos, 1u);
-    umma_f16(t12r, xr2, yr1, id_pos, 1u);
-    umma_f16(t12r, xi1, yi2, id_neg, 1u);
-    umma_f16(t12r, xi2, yi1, id_neg, 1u);
+    umma(t12r, xr1, yr3, id_pos, acc);
+    umma(t12r, xr2, yr2, id_pos, 1u);
+    umma(t12r, xr3, yr1, id_pos, 1u);
+    umma(t12r, xi1, yi3, id_neg, 1u);
+    umma(t12r, xi2, yi2, id_neg, 1u);
+    umma(t12r, xi3, yi1, id_neg, 1u);
+    umma(t12r, xr1, yr2, id_pos, 1u);
+    umma(t12r, xr2, yr1, id_pos, 1u);
+    umma(t12r, xi1, yi2, id_neg, 1u);
+    umma(t12r, xi2, yi1, id_neg, 1u);
     // C12i = sum of xr_i yi_j + xi_i yr_j
-    umma_f16(t12i, xr1, yi3, id_pos, acc);
-    umma_f16(t12i, xr2, yi2, id_pos, 1u);
-    umma_f16(t12i, xr3, yi1, id_pos, 1u);
-    umma_f16(t12i, xi1, yr3, id_pos, 1u);
-    umma_f16(t12i, xi2, yr2, id_pos, 1u);
-    umma_f16(t12i, xi3, yr1, id_pos, 1u);
-    umma_f16(t12i, xr1, yi2, id_pos, 1u);
-    umma_f16(t12i, xr2, yi1, id_pos, 1u);
-    umma_f16(t12i, xi1, yr2, id_pos, 1u);
-    umma_f16(t12i, xi2, yr1, id_pos, 1u);
+    umma(t12i, xr1, yi3, id_pos, acc);
+    umma(t12i, xr2, yi2, id_pos, 1u);
+    umma(t12i, xr3, yi1, id_pos, 1u);
+    umma(t12i, xi1, yr3, id_pos, 1u);
+    umma(t12i, xi2, yr2, id_pos, 1u);
+    umma(t12i, xi3, yr1, id_pos, 1u);
+    umma(t12i, xr1, yi2, id_pos, 1u);
+    umma(t12i, xr2, yi1, id_pos, 1u);
+    umma(t12i, xi1, yr2, id_pos, 1u);
+    umma(t12i, xi2, yr1, id_pos, 1u);
   }
 }
 
 // The leading products x1 y1 of one k-step (accumulators C0r, C0i): exact.
-template <int FMT>
+template <int FMT, bool PAIR>
 __device__ __forceinline__ void issue_lead(uint32_t t0r, uint32_t t0i, uint32_t a0, uint32_t b0, uint32_t acc) {
-  constexpr uint32_t id_pos = umma_idesc(Cfg<FMT>::AB_FORMAT, false), id_neg = umma_idesc(Cfg<FMT>::AB_FORMAT, true);
-  constexpr int IM = (Cfg<FMT>::PARTS / 2) * PART_BYTES;          // offset of the first imaginary slice
-  const uint64_t xr1 = umma_desc(a0), xi1 = umma_desc(a0 + IM), yr1 = umma_desc(b0), yi1 = umma_desc(b0 + IM);
-  umma_f16(t0r, xr1, yr1, id_pos, acc);
-  umma_f16(t0r, xi1, yi1, id_neg, 1u);
-  umma_f16(t0i, xr1, yi1, id_pos, acc);
-  umma_f16(t0i, xi1, yr1, id_pos, 1u);
+  constexpr uint32_t id_pos = umma_idesc(Cfg<FMT>::AB_FORMAT, false, PAIR), id_neg = umma_idesc(Cfg<FMT>::AB_FORMAT, true, PAIR);
+  constexpr int YP = PAIR ? PART_BYTES / 2 : PART_BYTES;
+  constexpr int IM = (Cfg<FMT>::PARTS / 2) * PART_BYTES, IMY = (Cfg<FMT>::PARTS / 2) * YP;   // first imaginary slice
+  auto umma = [](uint32_t d, uint64_t da, uint64_t db, uint32_t id, uint32_t ac) { umma_f16<PAIR>(d, da, db, id, ac); };
+  const uint64_t xr1 = umma_desc(a0), xi1 = umma_desc(a0 + IM), yr1 = umma_desc(b0), yi1 = umma_desc(b0 + IMY);
+  umma(t0r, xr1, yr1, id_pos, acc);
+  umma(t0r, xi1, yi1, id_neg, 1u);
+  umma(t0i, xr1, yi1, id_pos, acc);
+  umma(t0i, xi1, yr1, id_pos, 1u);
 }
 
 template <int EPI, int FMT>
@@ -296,48 +366,63 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
   } else if (warp == 1) {
     // ================= MMA issuer =================
     // The k-steps of all (tile, channel) segments of this CTA form one sequence g = 0 .. total - 1.  The small
-    // products of k-step g are issued first; the leading products follow through a second cursor gl <= g.  When the
-    // leading cursor reaches a new chunk whose C0 the epilogue has not drained yet, the issuer does not block: it
-    // keeps queueing small products (up to lag_max k-steps ahead), so the tensor pipe stays busy during the drain,
-    // and the leading products catch up afterwards.  At a segment boundary the leading cursor catches up first: the
-    // epilogue cannot release C12 before it has seen every C0 chunk but the last.
-    if (lane == 0) {
-      const uint32_t t0r = tmem_base, t0i = tmem_base + TN, t12r = tmem_base + 2 * TN, t12i = tmem_base + 3 * TN;
-      const uint32_t total = (uint32_t)n_my_items * (uint32_t)p.n_ch_loop * (uint32_t)p.ksteps;
-      const uint32_t chunk = (uint32_t)p.chunk_steps, lag_max = (uint32_t)p.lag_max;
-      uint32_t ks_s = 0, seg_s = 0;              // small-product cursor: k-step inside its segment, segment number
-      uint32_t gl = 0, ks_l = 0, chunk_id = 0;   // leading-product cursor
-      auto lead = [&]() {
-        const uint32_t s = gl % STAGES, in_chunk = ks_l % chunk;
-        if (in_chunk == 0) {
-          mbar_wait(c0_empty, (chunk_id & 1) ^ 1);                   // epilogue has drained the previous chunk's C0
-          asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        }
-        const uint32_t a0 = smem_u32(smem + s * STAGE_BYTES);
-        issue_lead<FMT>(t0r, t0i, a0, a0 + X_BYTES, in_chunk ? 1u : 0u);
-        umma_commit(&empty[s]);                                      // stage reusable once every MMA so far has read it
-        ++gl; ++ks_l;
-        if (in_chunk == chunk - 1 || ks_l == (uint32_t)p.ksteps) { umma_commit(c0_full); ++chunk_id; }
-        if (ks_l == (uint32_t)p.ksteps) ks_l = 0;
-      };
-      for (uint32_t g = 0; g < total; ++g) {
-        const uint32_t s = g % STAGES;
-        mbar_wait(&full[s], (g / STAGES) & 1);
-        if (ks_s == 0) {
-          while (gl < g) lead();
-          mbar_wait(c12_empty, (seg_s & 1) ^ 1);                     // epilogue has drained the previous segment's C12
-        }
+    // products of k-step g are issued first; the leading products follow through a second cursor (`pending` k-steps
+    // behind).  When the leading cursor reaches a new chunk whose C0 the epilogue has not drained yet, the issuer
+    // does not block: it keeps queueing small products (up to lag_max k-steps ahead), so the tensor pipe stays busy
+    // during the drain, and the leading products catch up afterwards.  At a segment boundary the leading cursor
+    // catches up first: the epilogue cannot release C12 before it has seen every C0 chunk but the last.
+    // The whole warp runs the control flow (converged); one elected lane issues the tcgen05 instructions -- a
+    // lane-divergent `if (lane == 0)` region makes ptxas wrap every uniform-datapath instruction in an ELECT loop,
+    // and the issuing thread, not the tensor pipe, becomes the bottleneck (profiles/r01_fp16x4_issue_bound.md).
+    const uint32_t t0r = tmem_base, t0i = tmem_base + TN, t12r = tmem_base + 2 * TN, t12i = tmem_base + 3 * TN;
+    const uint32_t total = (uint32_t)n_my_items * (uint32_t)p.n_ch_loop * (uint32_t)p.ksteps;
+    const uint32_t ksteps = (uint32_t)p.ksteps, chunk = (uint32_t)p.chunk_steps, lag_max = (uint32_t)p.lag_max;
+    const uint32_t smem_base = smem_u32(smem);
+    uint32_t s_small = 0, ph_small = 0;            // stage and phase of the small-product cursor
+    uint32_t ks_s = 0, seg_par = 0;                // its k-step inside the segment; segment parity
+    uint32_t s_lead = 0, ks_l = 0, in_chunk = 0, chunk_par = 0, pending = 0;   // leading-product cursor
+    auto lead = [&]() {
+      if (in_chunk == 0) {
+        mbar_wait(c0_empty, chunk_par ^ 1);                          // epilogue has drained the previous chunk's C0
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        const uint32_t a0 = smem_u32(smem + s * STAGE_BYTES);
-        issue_small<FMT>(t12r, t12i, a0, a0 + X_BYTES, ks_s ? 1u : 0u);
-        if (++ks_s == (uint32_t)p.ksteps) { umma_commit(c12_full); ks_s = 0; ++seg_s; }
-        while (gl <= g) {
-          if (ks_l % chunk == 0 && g - gl + 1 < lag_max && !mbar_test(c0_empty, (chunk_id & 1) ^ 1)) break;
-          lead();
-        }
       }
-      while (gl < total) lead();
+      ++ks_l;
+      const bool chunk_end = in_chunk + 1 == chunk || ks_l == ksteps;
+      if (elect_one()) {
+        const uint32_t a0 = smem_base + s_lead * STAGE_BYTES;
+        issue_lead<FMT, false>(t0r, t0i, a0, a0 + X_BYTES, in_chunk ? 1u : 0u);
+        umma_commit<false>(&empty[s_lead]);                          // stage reusable once every MMA so far has read it
+        if (chunk_end) umma_commit<false>(c0_full);
+      }
+      __syncwarp();
+      if (chunk_end) { in_chunk = 0; chunk_par ^= 1; } else ++in_chunk;
+      if (ks_l == ksteps) ks_l = 0;
+      if (++s_lead == STAGES) s_lead = 0;
+      --pending;
+    };
+    for (uint32_t g = 0; g < total; ++g) {
+      mbar_wait(&full[s_small], ph_small);
+      if (ks_s == 0) {
+        while (pending) lead();
+        mbar_wait(c12_empty, seg_par ^ 1);                           // epilogue has drained the previous segment's C12
+      }
+      asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+      const bool seg_end = ks_s + 1 == ksteps;
+      if (elect_one()) {
+        const uint32_t a0 = smem_base + s_small * STAGE_BYTES;
+        issue_small<FMT, false>(t12r, t12i, a0, a0 + X_BYTES, ks_s ? 1u : 0u);
+        if (seg_end) umma_commit<false>(c12_full);
+      }
+      __syncwarp();
+      if (seg_end) { ks_s = 0; seg_par ^= 1; } else ++ks_s;
+      if (++s_small == STAGES) { s_small = 0; ph_small ^= 1; }
+      ++pending;
+      while (pending) {
+        if (in_chunk == 0 && pending < lag_max && !mbar_test(c0_empty, chunk_par ^ 1)) break;
+        lead();
+      }
     }
+    while (pending) lead();
   } else {
     // ================= epilogue warps =================
     const int quarter = warp & 3;                      // TMEM lanes [32 q, 32 q + 32) are visible to warps with warp % 4 == q
