@@ -69,10 +69,11 @@ static int32_t planes_in(bip_ctx* ctx, DevBuf& buf, Planes& P, int64_t rows, int
 // Carve a sliced 16-bit operand [batch][rows][k] of format `fmt` out of one DevBuf.  Producers write every k-step of every valid row;
 // the padding rows of the last row tile only have to be finite (they feed masked accumulator rows / columns), so the
 // buffer is cleared when it is (re)allocated and never again.
-static int32_t sliced_in(bip_ctx* ctx, DevBuf& buf, Sliced& S, int fmt, int64_t rows, int64_t k, int64_t batch, const char* what) {
+static int32_t sliced_in(bip_ctx* ctx, DevBuf& buf, Sliced& S, int fmt, int64_t rows, int64_t k, int64_t batch, const char* what,
+                         int64_t row_align = SL_ROWS) {
   S.fmt = fmt;
   S.rows = rows;
-  S.rows_pad = round_up(rows, SL_ROWS);
+  S.rows_pad = round_up(rows, row_align);
   S.k = k;
   S.ksteps = (k + SL_K - 1) / SL_K;
   S.batch_stride = S.rows_pad / SL_ROWS * S.ksteps * sl_step_el(fmt);
@@ -94,7 +95,7 @@ static int32_t ensure_illumination(bip_ctx* ctx, int precision) {
     if (ctx->A_sl.base) { cudaStreamSynchronize(ctx->stream); cudaFree(ctx->A_sl.base); cudaFree(ctx->A_sl.scale); ctx->A_sl = Sliced(); }
     Sliced A;
     DevBuf b;
-    BIP_TRY(sliced_in(ctx, b, A, fmt, ctx->n_rho, ctx->n_ap, 1, "illumination matrix (sliced)"));
+    BIP_TRY(sliced_in(ctx, b, A, fmt, ctx->n_rho, ctx->n_ap, 1, "illumination matrix (sliced)", 2 * SL_ROWS));   // X operand: row-tile pairs
     A.batch_stride = 0;
     if (dev_alloc(ctx, (void**)&A.scale, (size_t)A.rows_pad * sizeof(float), "illumination row scales") != BIP_OK) { cudaFree(b.p); return BIP_ERR_OOM; }
     BIP_CUDA(ctx, cudaMemsetAsync(A.scale, 0, (size_t)A.rows_pad * sizeof(float), ctx->stream));
@@ -212,7 +213,7 @@ static size_t scratch_budget() {
 static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, int32_t nb, int mode, int recon, int fmt, void* out) {
   auto& sp = spans()[ctx];
   const int w2 = e.w * e.w;
-  const int64_t rho_pad = round_up(ctx->n_rho, SL_ROWS);
+  const int64_t rho_pad = round_up(ctx->n_rho, 2 * SL_ROWS);    // X operands are padded to pairs of row tiles (CTA-pair kernel)
   Sliced R1t, R2, Phi;
   BIP_TRY(ensure(ctx, ctx->D1, (size_t)nb * ctx->n_p1 * w2 * sizeof(float2), "D1 (de-tilted S1 windows)"));
   BIP_TRY(ensure(ctx, ctx->D2, (size_t)nb * ctx->n_p2 * w2 * sizeof(float2), "D2 (de-tilted S2 windows)"));
@@ -363,7 +364,7 @@ static int32_t run_edges(bip_ctx* ctx, const std::vector<int32_t>& ids, int mode
       const int64_t el = precision == BIP_PREC_FP16X4 ? 8 : precision == BIP_PREC_BF16X6 ? 12 : 16;      // operand bytes per complex element
       const size_t per_atom = (size_t)((ctx->n_p1 + ctx->n_p2) * w2 * 8 + (int64_t)ctx->n_rho * w2 * 8 +
                                        el * (round_up(w2, 128) * round_up(ctx->n_ap, 32) + round_up(e.n_det, 128) * round_up(w2, 32) +
-                                             round_up(ctx->n_rho, 128) * e.n_ch * round_up(w2, 32)));
+                                             round_up(ctx->n_rho, 256) * e.n_ch * round_up(w2, 32)));
       const int32_t nb_max = (int32_t)std::max<size_t>(1, std::min<size_t>(budget / std::max<size_t>(per_atom, 1), 4096));
       Span s(ctx, sp.pool_map, sp.contract);
       for (int32_t a0 = (int32_t)lo; a0 < (int32_t)hi; a0 += nb_max)     // lines 5-8

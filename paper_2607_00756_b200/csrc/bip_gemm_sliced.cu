@@ -39,18 +39,20 @@ constexpr int DGROUP = 4;                        // column tiles per raster grou
 
 template <int FMT> struct Cfg;
 template <> struct Cfg<SL_FMT_FP16X4> {
-  static constexpr int PARTS = 4, STAGES = 7, LAG_MAX = 4;
+  static constexpr int PARTS = 4, STAGES = 7, STAGES_PAIR = 9, LAG_MAX = 4;
   static constexpr int CHUNK_STEPS = 8;          // 128 k-elements: 2 * 128 * 2^16 = 2^24, exact
   static constexpr uint32_t AB_FORMAT = 0;       // fp16
 };
 template <> struct Cfg<SL_FMT_BF16X6> {
-  static constexpr int PARTS = 6, STAGES = 4, LAG_MAX = 2;
+  static constexpr int PARTS = 6, STAGES = 4, STAGES_PAIR = 6, LAG_MAX = 2;
   static constexpr int CHUNK_STEPS = 16;         // 256 k-elements: 2 * 256 * 2^14 = 2^23 < 2^24, exact
   static constexpr uint32_t AB_FORMAT = 1;       // bf16
 };
 template <int FMT> __host__ __device__ constexpr int x_bytes() { return Cfg<FMT>::PARTS * PART_BYTES; }
 template <int FMT> __host__ __device__ constexpr int stage_bytes() { return 2 * x_bytes<FMT>(); }
-template <int FMT> __host__ __device__ constexpr int smem_bytes() { return Cfg<FMT>::STAGES * stage_bytes<FMT>() + 1024 /*align*/ + 256 /*barriers*/; }
+template <int FMT, bool PAIR> __host__ __device__ constexpr int smem_bytes() {
+  return (PAIR ? Cfg<FMT>::STAGES_PAIR * (x_bytes<FMT>() * 3 / 2) : Cfg<FMT>::STAGES * stage_bytes<FMT>()) + 1024 /*align*/ + 512 /*barriers*/;
+}
 
 enum { EPI_GEMM1 = 1, EPI_GEMM2 = 2 };
 
@@ -59,7 +61,8 @@ struct SlParams {
   const float* sx; const float* sy;
   int64_t x_batch_stride, y_batch_stride, sx_batch_stride, sy_batch_stride;
   int ksteps;
-  int n_rt, n_ct, n_items, n_ch_loop;
+  int n_rt, n_ct, n_items, n_ch_loop;   // row work tiles (pairs of 128-row tiles in pair mode), column tiles per atom
+  int n_rt_x;              // 128-row tiles per channel block of X
   int n_rows, n_cols;      // valid rows (rho) / columns (s or d) per atom
   int rows_pad;            // padded rho rows per channel block of X
   int chunk_steps;         // k-steps per exactly accumulated chunk of leading products
@@ -306,39 +309,50 @@ __device__ __forceinline__ void issue_lead(uint32_t t0r, uint32_t t0i, uint32_t 
   umma(t0i, xi1, yr1, id_pos, 1u);
 }
 
-template <int EPI, int FMT>
+template <int EPI, int FMT, bool PAIR>
 __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlParams p) {
   using C = Cfg<FMT>;
-  constexpr int STAGES = C::STAGES;
-  constexpr int X_BYTES = x_bytes<FMT>(), STAGE_BYTES = stage_bytes<FMT>(), STEP_EL = sl_step_el(FMT);
+  constexpr int STAGES = PAIR ? C::STAGES_PAIR : C::STAGES;
+  constexpr int X_BYTES = x_bytes<FMT>(), Y_BYTES = PAIR ? X_BYTES / 2 : X_BYTES, STAGE_BYTES = X_BYTES + Y_BYTES;
+  constexpr int STEP_EL = sl_step_el(FMT);
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + STAGES * STAGE_BYTES);
-  uint64_t* full = bars;                 // [STAGES]
-  uint64_t* empty = bars + STAGES;       // [STAGES]
-  uint64_t* c0_full = bars + 2 * STAGES;       // leading accumulators of a chunk complete
-  uint64_t* c0_empty = bars + 2 * STAGES + 1;  // ... drained by the epilogue warps
-  uint64_t* c12_full = bars + 2 * STAGES + 2;  // small-product accumulators of a (tile, channel) complete
-  uint64_t* c12_empty = bars + 2 * STAGES + 3;
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * STAGES + 4);
+  uint64_t* full = bars;                       // [STAGES] operands of this CTA have landed
+  uint64_t* empty = bars + STAGES;             // [STAGES] every MMA reading the stage has completed
+  uint64_t* peer_full = bars + 2 * STAGES;     // [STAGES] (pair leader only) the peer CTA's operands have landed
+  uint64_t* c0_full = bars + 3 * STAGES;       // leading accumulators of a chunk complete
+  uint64_t* c0_empty = bars + 3 * STAGES + 1;  // ... drained by the epilogue warps (of both CTAs of a pair)
+  uint64_t* c12_full = bars + 3 * STAGES + 2;  // small-product accumulators of a (tile, channel) complete
+  uint64_t* c12_empty = bars + 3 * STAGES + 3;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 3 * STAGES + 4);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int n_my_items = p.n_items > (int)blockIdx.x ? (p.n_items - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
+  // a worker is a CTA, or a pair of CTAs (cluster of 2 on one TPC) working on two row tiles of the same column tile
+  const uint32_t rank = PAIR ? cluster_ctarank() : 0;
+  const int worker = PAIR ? (int)(blockIdx.x >> 1) : (int)blockIdx.x, n_workers = PAIR ? (int)(gridDim.x >> 1) : (int)gridDim.x;
+  const int n_my_items = p.n_items > worker ? (p.n_items - 1 - worker) / n_workers + 1 : 0;
 
   if (warp == 0 && lane == 0) {
-    for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+    for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); mbar_init(&peer_full[s], 1); }
     mbar_init(c0_full, 1);
-    mbar_init(c0_empty, NUM_EPI_WARPS);
+    mbar_init(c0_empty, PAIR ? 2 * NUM_EPI_WARPS : NUM_EPI_WARPS);
     mbar_init(c12_full, 1);
-    mbar_init(c12_empty, NUM_EPI_WARPS);
+    mbar_init(c12_empty, PAIR ? 2 * NUM_EPI_WARPS : NUM_EPI_WARPS);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (warp == 1) {   // the whole tensor memory: 512 columns
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  if (warp == 1) {   // the whole tensor memory: 512 columns (of both CTAs of a pair)
+    if (PAIR) {
+      asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    } else {
+      asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();
+  if (PAIR) cluster_sync_all();          // the peer's barriers are initialised before anything arrives on them
   asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
   const uint32_t tmem_base = *tmem_slot;
 
@@ -346,26 +360,36 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
     // ================= bulk-copy producer =================
     if (lane == 0) {
       uint32_t it = 0;
-      for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
+      for (int item = worker; item < p.n_items; item += n_workers) {
         int atom, rt, ct;
         decode_item(p, item, atom, rt, ct);
-        const uint16_t* ysrc = p.Y + (int64_t)atom * p.y_batch_stride + (int64_t)ct * p.ksteps * STEP_EL;
+        if (PAIR) rt = 2 * rt + (int)rank;
+        // a CTA of a pair loads rows [64 rank, 64 rank + 64) of every part of the Y tile
+        const uint16_t* ysrc = p.Y + (int64_t)atom * p.y_batch_stride + (int64_t)ct * p.ksteps * STEP_EL + (PAIR ? rank * (SL_TILE_EL / 2) : 0);
         for (int n = 0; n < p.n_ch_loop; ++n) {
-          const uint16_t* xsrc = p.X + (int64_t)atom * p.x_batch_stride + ((int64_t)n * p.n_rt + rt) * p.ksteps * STEP_EL;
+          const uint16_t* xsrc = p.X + (int64_t)atom * p.x_batch_stride + ((int64_t)n * p.n_rt_x + rt) * p.ksteps * STEP_EL;
           for (int ks = 0; ks < p.ksteps; ++ks, ++it) {
             const int s = it % STAGES;
             mbar_wait(&empty[s], ((it / STAGES) & 1) ^ 1);
             uint8_t* st = smem + s * STAGE_BYTES;
             mbar_expect_tx(&full[s], STAGE_BYTES);
             bulk_load(st, xsrc + (int64_t)ks * STEP_EL, X_BYTES, &full[s]);
-            bulk_load(st + X_BYTES, ysrc + (int64_t)ks * STEP_EL, X_BYTES, &full[s]);
+            if (PAIR) {
+#pragma unroll
+              for (int part = 0; part < C::PARTS; ++part)
+                bulk_load(st + X_BYTES + part * (PART_BYTES / 2), ysrc + (int64_t)ks * STEP_EL + part * SL_TILE_EL, PART_BYTES / 2, &full[s]);
+            } else {
+              bulk_load(st + X_BYTES, ysrc + (int64_t)ks * STEP_EL, X_BYTES, &full[s]);
+            }
           }
         }
       }
+      // tail: every tcgen05.commit arrival on the stage barriers has landed before the CTA may exit
+      for (int j = 0; j < STAGES; ++j, ++it) mbar_wait(&empty[it % STAGES], ((it / STAGES) & 1) ^ 1);
     }
   } else if (warp == 1) {
     // ================= MMA issuer =================
-    // The k-steps of all (tile, channel) segments of this CTA form one sequence g = 0 .. total - 1.  The small
+    // The k-steps of all (tile, channel) segments of this worker form one sequence g = 0 .. total - 1.  The small
     // products of k-step g are issued first; the leading products follow through a second cursor (`pending` k-steps
     // behind).  When the leading cursor reaches a new chunk whose C0 the epilogue has not drained yet, the issuer
     // does not block: it keeps queueing small products (up to lag_max k-steps ahead), so the tensor pipe stays busy
@@ -374,25 +398,37 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
     // The whole warp runs the control flow (converged); one elected lane issues the tcgen05 instructions -- a
     // lane-divergent `if (lane == 0)` region makes ptxas wrap every uniform-datapath instruction in an ELECT loop,
     // and the issuing thread, not the tensor pipe, becomes the bottleneck (profiles/r01_fp16x4_issue_bound.md).
-    const uint32_t t0r = tmem_base, t0i = tmem_base + TN, t12r = tmem_base + 2 * TN, t12i = tmem_base + 3 * TN;
+    // In a pair only the leader CTA (rank 0) issues (tcgen05.mma.cta_group::2 drives both tensor cores); the peer's
+    // warp 1 forwards "my operands have landed" to the leader's peer_full barriers.
     const uint32_t total = (uint32_t)n_my_items * (uint32_t)p.n_ch_loop * (uint32_t)p.ksteps;
+    if (PAIR && rank != 0) {
+      uint32_t s = 0, ph = 0;
+      for (uint32_t g = 0; g < total; ++g) {
+        mbar_wait(&full[s], ph);
+        if (elect_one()) mbar_arrive_cluster(&peer_full[s], 0);
+        __syncwarp();
+        if (++s == STAGES) { s = 0; ph ^= 1; }
+      }
+    } else {
+    const uint32_t t0r = tmem_base, t0i = tmem_base + TN, t12r = tmem_base + 2 * TN, t12i = tmem_base + 3 * TN;
     const uint32_t ksteps = (uint32_t)p.ksteps, chunk = (uint32_t)p.chunk_steps, lag_max = (uint32_t)p.lag_max;
     const uint32_t smem_base = smem_u32(smem);
     uint32_t s_small = 0, ph_small = 0;            // stage and phase of the small-product cursor
     uint32_t ks_s = 0, seg_par = 0;                // its k-step inside the segment; segment parity
     uint32_t s_lead = 0, ks_l = 0, in_chunk = 0, chunk_par = 0, pending = 0;   // leading-product cursor
+    auto wait_epi = [&](uint64_t* bar, uint32_t parity) { if (PAIR) mbar_wait_cluster(bar, parity); else mbar_wait(bar, parity); };
     auto lead = [&]() {
       if (in_chunk == 0) {
-        mbar_wait(c0_empty, chunk_par ^ 1);                          // epilogue has drained the previous chunk's C0
+        wait_epi(c0_empty, chunk_par ^ 1);                           // epilogue has drained the previous chunk's C0
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
       }
       ++ks_l;
       const bool chunk_end = in_chunk + 1 == chunk || ks_l == ksteps;
       if (elect_one()) {
         const uint32_t a0 = smem_base + s_lead * STAGE_BYTES;
-        issue_lead<FMT, false>(t0r, t0i, a0, a0 + X_BYTES, in_chunk ? 1u : 0u);
-        umma_commit<false>(&empty[s_lead]);                          // stage reusable once every MMA so far has read it
-        if (chunk_end) umma_commit<false>(c0_full);
+        issue_lead<FMT, PAIR>(t0r, t0i, a0, a0 + X_BYTES, in_chunk ? 1u : 0u);
+        umma_commit<PAIR>(&empty[s_lead]);                           // stage reusable once every MMA so far has read it
+        if (chunk_end) umma_commit<PAIR>(c0_full);
       }
       __syncwarp();
       if (chunk_end) { in_chunk = 0; chunk_par ^= 1; } else ++in_chunk;
@@ -402,16 +438,17 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
     };
     for (uint32_t g = 0; g < total; ++g) {
       mbar_wait(&full[s_small], ph_small);
+      if (PAIR) mbar_wait_cluster(&peer_full[s_small], ph_small);
       if (ks_s == 0) {
         while (pending) lead();
-        mbar_wait(c12_empty, seg_par ^ 1);                           // epilogue has drained the previous segment's C12
+        wait_epi(c12_empty, seg_par ^ 1);                            // epilogue has drained the previous segment's C12
       }
       asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
       const bool seg_end = ks_s + 1 == ksteps;
       if (elect_one()) {
         const uint32_t a0 = smem_base + s_small * STAGE_BYTES;
-        issue_small<FMT, false>(t12r, t12i, a0, a0 + X_BYTES, ks_s ? 1u : 0u);
-        if (seg_end) umma_commit<false>(c12_full);
+        issue_small<FMT, PAIR>(t12r, t12i, a0, a0 + X_BYTES, ks_s ? 1u : 0u);
+        if (seg_end) umma_commit<PAIR>(c12_full);
       }
       __syncwarp();
       if (seg_end) { ks_s = 0; seg_par ^= 1; } else ++ks_s;
@@ -423,6 +460,7 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
       }
     }
     while (pending) lead();
+    }
   } else {
     // ================= epilogue warps =================
     const int quarter = warp & 3;                      // TMEM lanes [32 q, 32 q + 32) are visible to warps with warp % 4 == q
@@ -430,9 +468,10 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
     const uint32_t t_lane = tmem_base + ((uint32_t)(quarter * 32) << 16) + half * 64;
     const int n_chunks = (p.ksteps + p.chunk_steps - 1) / p.chunk_steps;
     uint32_t chunk_id = 0, seg = 0;
-    for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
+    for (int item = worker; item < p.n_items; item += n_workers) {
       int atom, rt, ct;
       decode_item(p, item, atom, rt, ct);
+      if (PAIR) rt = 2 * rt + (int)rank;               // the leader's TMEM holds the even row tile, the peer's the odd one
       const int row = rt * TM + quarter * 32 + lane;   // this thread's rho
       const bool row_ok = row < p.n_rows;
       const int col0 = ct * TN + half * 64;
@@ -462,7 +501,10 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
           }
           asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
           __syncwarp();
-          if (lane == 0) mbar_arrive(small ? c12_empty : c0_empty);
+          if (lane == 0) {                           // the accumulators may be overwritten: tell the issuing CTA
+            uint64_t* bar = small ? c12_empty : c0_empty;
+            if (PAIR && rank != 0) mbar_arrive_cluster(bar, 0); else mbar_arrive(bar);
+          }
           if (!small) ++chunk_id;
         }
         // ---- end of a (tile, channel): fused epilogue on the running sums ----
@@ -515,7 +557,12 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
 
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();
-  if (warp == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
+  if (PAIR) {
+    cluster_sync_all();                    // neither CTA frees tensor memory or exits while the other still uses its barriers
+    if (warp == 1) asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
+  } else {
+    if (warp == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
+  }
 }
 
 // a5: Phi_n[rho][s] = H_n[s] Psi[rho][s] as sliced rows (n, rho) with their power-of-two scales.
@@ -552,29 +599,45 @@ __global__ void __launch_bounds__(256) k_quantize_phi(const float2* __restrict__
   }
 }
 
-template <int EPI, int FMT>
+template <int EPI, int FMT, bool PAIR>
 int32_t launch_fmt(bip_ctx* ctx, const SlParams& p) {
   static bool attr_set = false;
   if (!attr_set) {
-    BIP_CUDA(ctx, cudaFuncSetAttribute(k_sliced_contract<EPI, FMT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<FMT>()));
+    BIP_CUDA(ctx, cudaFuncSetAttribute(k_sliced_contract<EPI, FMT, PAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<FMT, PAIR>()));
     attr_set = true;
   }
-  if (p.n_items <= 0) return BIP_OK;
   SlParams q = p;
+  q.n_rt_x = p.n_rt;
+  if (PAIR) {
+    if (p.n_rt % 2) return fail(ctx, BIP_ERR_INVALID, "pair kernel: the X operand must be padded to a multiple of 256 rows");
+    q.n_rt = p.n_rt / 2;
+  }
+  q.n_items = p.n_items / p.n_rt * q.n_rt;
+  if (q.n_items <= 0) return BIP_OK;
   q.chunk_steps = Cfg<FMT>::CHUNK_STEPS;
   q.lag_max = Cfg<FMT>::LAG_MAX;
   if (const char* e = std::getenv("BIP_TUNE_CHUNK")) q.chunk_steps = std::max(1, std::atoi(e));   // timing experiments only: breaks exactness
-  if (const char* e = std::getenv("BIP_TUNE_LAG")) q.lag_max = std::min(std::max(1, std::atoi(e)), Cfg<FMT>::STAGES - 1);
-  const int grid = std::max(1, std::min(p.n_items, ctx->sm_count));
-  k_sliced_contract<EPI, FMT><<<grid, NUM_THREADS, smem_bytes<FMT>(), ctx->stream>>>(q);
-  BIP_CUDA(ctx, cudaGetLastError());
+  if (const char* e = std::getenv("BIP_TUNE_LAG")) q.lag_max = std::min(std::max(1, std::atoi(e)), (PAIR ? Cfg<FMT>::STAGES_PAIR : Cfg<FMT>::STAGES) - 1);
+  const int workers = std::max(1, std::min(q.n_items, PAIR ? ctx->sm_count / 2 : ctx->sm_count));
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(PAIR ? 2 * workers : workers);
+  cfg.blockDim = dim3(NUM_THREADS);
+  cfg.dynamicSmemBytes = smem_bytes<FMT, PAIR>();
+  cfg.stream = ctx->stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = PAIR ? 2 : 1; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  BIP_CUDA(ctx, cudaLaunchKernelEx(&cfg, k_sliced_contract<EPI, FMT, PAIR>, q));
   ctx->timing.kernel_launches++;
   return BIP_OK;
 }
 
 template <int EPI>
 int32_t launch(bip_ctx* ctx, const SlParams& p, int fmt) {
-  return fmt == SL_FMT_FP16X4 ? launch_fmt<EPI, SL_FMT_FP16X4>(ctx, p) : launch_fmt<EPI, SL_FMT_BF16X6>(ctx, p);
+  static const bool pair = [] { const char* e = std::getenv("BIP_TUNE_PAIR"); return e ? std::atoi(e) != 0 : true; }();
+  if (pair) return fmt == SL_FMT_FP16X4 ? launch_fmt<EPI, SL_FMT_FP16X4, true>(ctx, p) : launch_fmt<EPI, SL_FMT_BF16X6, true>(ctx, p);
+  return fmt == SL_FMT_FP16X4 ? launch_fmt<EPI, SL_FMT_FP16X4, false>(ctx, p) : launch_fmt<EPI, SL_FMT_BF16X6, false>(ctx, p);
 }
 
 }  // namespace
