@@ -58,6 +58,11 @@ typedef enum { BIP_RECON_LINEAR = 0, BIP_RECON_MAGPHASE = 1 } bip_recon;
  *   product is the four-term sum x1 y1 + (x1 y2 + x2 y1 + x2 y2) -- 2/3 of the tensor time of 3xTF32.  The leading
  *   products x1 y1 are small integers and accumulate EXACTLY in TMEM over chunks of 128 k-elements; chunk sums are
  *   added in fp32 round-to-nearest.  Meets the 1e-6 summed-intensity bound.
+ * FP16X3: FP16X4 without the x2 y2 term (each at most 2^-18 of the leading product, zero-mean): three MMAs per real
+ *   product, 3/4 of the tensor time of FP16X4.  The analogue of the customary 3xTF32 scheme, which drops lo x lo.
+ *   Offered for the detector-reduced outputs (MAP, QEELS_X / _Y), where it is held to the same parity bounds by the
+ *   tests (1e-4 per pixel, 1e-6 summed); BIP_MODE_CUBE returns BIP_ERR_UNSUPPORTED (single cube pixels of tiny
+ *   windows exceed 1e-4 without the x2 y2 term).
  * BF16X6: the same construction with three bf16 slices per real number (8-bit leading slice, chunks of 256
  *   k-elements) and the six-term product x1 y1 + (x1 y2 + x2 y1) + (x1 y3 + x2 y2 + x3 y1): representation error
  *   2^-24 of the row maximum at the tensor time of 3xTF32.
@@ -66,7 +71,7 @@ typedef enum { BIP_RECON_LINEAR = 0, BIP_RECON_MAGPHASE = 1 } bip_recon;
  *   1e-4 but the summed intensity is biased by ~ -1.25e-8 per accumulating MMA (-2.6e-5 at configs[0]).  Kept as the
  *   measured A/B case for that finding.
  * FP32_SIMT: the same contractions on CUDA cores in fp32 -- the A/B reference for the tensor-core kernels. */
-typedef enum { BIP_PREC_TF32X3 = 0, BIP_PREC_FP32_SIMT = 1, BIP_PREC_BF16X6 = 2, BIP_PREC_FP16X4 = 3 } bip_precision;
+typedef enum { BIP_PREC_TF32X3 = 0, BIP_PREC_FP32_SIMT = 1, BIP_PREC_BF16X6 = 2, BIP_PREC_FP16X4 = 3, BIP_PREC_FP16X3 = 4 } bip_precision;
 
 typedef struct bip_ctx bip_ctx;
 

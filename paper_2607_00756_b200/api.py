@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libbip.so")
 
 MODE_MAP, MODE_QEELS_X, MODE_QEELS_Y, MODE_CUBE = 0, 1, 2, 3
 RECON_LINEAR, RECON_MAGPHASE = 0, 1
-PREC_TF32X3, PREC_FP32_SIMT, PREC_BF16X6, PREC_FP16X4 = 0, 1, 2, 3
+PREC_TF32X3, PREC_FP32_SIMT, PREC_BF16X6, PREC_FP16X4, PREC_FP16X3 = 0, 1, 2, 3, 4
 MAX_NN = 16
 _STATUS = {1: "BIP_ERR_INVALID", 2: "BIP_ERR_STATE", 3: "BIP_ERR_OOM", 4: "BIP_ERR_CUDA", 5: "BIP_ERR_UNSUPPORTED"}
 

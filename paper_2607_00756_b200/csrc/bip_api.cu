@@ -86,7 +86,7 @@ static int32_t sliced_in(bip_ctx* ctx, DevBuf& buf, Sliced& S, int fmt, int64_t 
 
 // a3, built on first use in the format the requested arithmetic reads.
 static void free_illumination(bip_ctx* ctx);
-static inline int sliced_fmt_of(int precision) { return precision == BIP_PREC_FP16X4 ? SL_FMT_FP16X4 : precision == BIP_PREC_BF16X6 ? SL_FMT_BF16X6 : -1; }
+static inline int sliced_fmt_of(int precision) { return precision == BIP_PREC_FP16X4 || precision == BIP_PREC_FP16X3 ? SL_FMT_FP16X4 : precision == BIP_PREC_BF16X6 ? SL_FMT_BF16X6 : -1; }
 
 static int32_t ensure_illumination(bip_ctx* ctx, int precision) {
   const int fmt = sliced_fmt_of(precision);
@@ -210,7 +210,7 @@ static size_t scratch_budget() {
 }
 
 // Steps a1-a8 on the sliced 16-bit operands (BIP_PREC_FP16X4 / BIP_PREC_BF16X6).
-static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, int32_t nb, int mode, int recon, int fmt, void* out) {
+static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, int32_t nb, int mode, int recon, int fmt, bool drop_tiny, void* out) {
   auto& sp = spans()[ctx];
   const int w2 = e.w * e.w;
   const int64_t rho_pad = round_up(ctx->n_rho, 2 * SL_ROWS);    // X operands are padded to pairs of row tiles (CTA-pair kernel)
@@ -235,7 +235,7 @@ static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, 
   // a3-a4: probe at the atom
   Gemm1SlArgs g1;
   g1.A = ctx->A_sl; g1.R1t = R1t; g1.Psi = (float2*)ctx->Psi.p; g1.psi_ld = psi_ld; g1.psi_batch_stride = (int64_t)ctx->n_rho * psi_ld;
-  g1.n_rho = ctx->n_rho; g1.w2 = w2; g1.n_atoms = nb;
+  g1.n_rho = ctx->n_rho; g1.w2 = w2; g1.n_atoms = nb; g1.drop_tiny = drop_tiny;
   BIP_TRY(launch_gemm1_sliced(ctx, g1));
   // a5: times H_n, split into slices
   BIP_TRY(launch_quantize_phi(ctx, g1.Psi, psi_ld, g1.psi_batch_stride, e.H_dev, Phi, ctx->n_rho, (int32_t)rho_pad, w2, e.n_ch, nb));
@@ -251,7 +251,7 @@ static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, 
   g2.mode = mode;
   g2.bin_of_det = mode == BIP_MODE_QEELS_X ? e.bin_of_det_x_dev : e.bin_of_det_y_dev;
   g2.n_bins = mode == BIP_MODE_QEELS_X ? (int)e.binx.size() : (int)e.biny.size();
-  g2.out = out;
+  g2.out = out; g2.drop_tiny = drop_tiny;
   {
     Span s(ctx, sp.pool_map, sp.gemm2);
     BIP_TRY(launch_gemm2_sliced(ctx, g2));
@@ -268,7 +268,7 @@ static int32_t contract_batch(bip_ctx* ctx, Edge& e, const int32_t* origin_dev, 
   auto& sp = spans()[ctx];
   const int w2 = e.w * e.w;
   const int32_t* org = origin_dev + 2 * (int64_t)a0;
-  if (sliced_fmt_of(precision) >= 0) return contract_batch_sliced(ctx, e, org, nb, mode, recon, sliced_fmt_of(precision), out);
+  if (sliced_fmt_of(precision) >= 0) return contract_batch_sliced(ctx, e, org, nb, mode, recon, sliced_fmt_of(precision), precision == BIP_PREC_FP16X3, out);
   Planes R1t, R2, Phi;
   BIP_TRY(ensure(ctx, ctx->D1, (size_t)nb * ctx->n_p1 * w2 * sizeof(float2), "D1 (de-tilted S1 windows)"));
   BIP_TRY(ensure(ctx, ctx->D2, (size_t)nb * ctx->n_p2 * w2 * sizeof(float2), "D2 (de-tilted S2 windows)"));
@@ -330,7 +330,9 @@ static int32_t run_edges(bip_ctx* ctx, const std::vector<int32_t>& ids, int mode
   if (ctx->n_rho <= 0) return fail(ctx, BIP_ERR_STATE, "bip_map: call bip_set_scan first");
   if (mode < BIP_MODE_MAP || mode > BIP_MODE_CUBE) return fail(ctx, BIP_ERR_INVALID, "bip_map: unknown mode %d", mode);
   if (recon != BIP_RECON_LINEAR && recon != BIP_RECON_MAGPHASE) return fail(ctx, BIP_ERR_INVALID, "bip_map: unknown recon %d", recon);
-  if (precision != BIP_PREC_TF32X3 && precision != BIP_PREC_FP32_SIMT && precision != BIP_PREC_BF16X6 && precision != BIP_PREC_FP16X4) return fail(ctx, BIP_ERR_INVALID, "bip_map: unknown precision %d", precision);
+  if (precision != BIP_PREC_TF32X3 && precision != BIP_PREC_FP32_SIMT && precision != BIP_PREC_BF16X6 && precision != BIP_PREC_FP16X4 && precision != BIP_PREC_FP16X3) return fail(ctx, BIP_ERR_INVALID, "bip_map: unknown precision %d", precision);
+  if (precision == BIP_PREC_FP16X3 && mode == BIP_MODE_CUBE)
+    return fail(ctx, BIP_ERR_UNSUPPORTED, "bip_map: FP16X3 drops the x2 y2 products and is offered for the reduced outputs (MAP, QEELS) only; use FP16X4 for the cube");
   if (precision != BIP_PREC_FP32_SIMT && !tc_available()) return fail(ctx, BIP_ERR_UNSUPPORTED, "bip_map: the tensor-core path is not built");
   for (size_t k = 0; k < ids.size(); ++k) {
     if (ids[k] < 0 || ids[k] >= (int)ctx->edges.size()) return fail(ctx, BIP_ERR_INVALID, "bip_map: edge %d does not exist", ids[k]);
@@ -361,7 +363,7 @@ static int32_t run_edges(bip_ctx* ctx, const std::vector<int32_t>& ids, int mode
       auto hi = std::upper_bound(e.slice.begin(), e.slice.end(), plane) - e.slice.begin();
       if (lo == hi) continue;
       const int64_t w2 = (int64_t)e.w * e.w;
-      const int64_t el = precision == BIP_PREC_FP16X4 ? 8 : precision == BIP_PREC_BF16X6 ? 12 : 16;      // operand bytes per complex element
+      const int64_t el = sliced_fmt_of(precision) == SL_FMT_FP16X4 ? 8 : precision == BIP_PREC_BF16X6 ? 12 : 16;      // operand bytes per complex element
       const size_t per_atom = (size_t)((ctx->n_p1 + ctx->n_p2) * w2 * 8 + (int64_t)ctx->n_rho * w2 * 8 +
                                        el * (round_up(w2, 128) * round_up(ctx->n_ap, 32) + round_up(e.n_det, 128) * round_up(w2, 32) +
                                              round_up(ctx->n_rho, 256) * e.n_ch * round_up(w2, 32)));
@@ -478,7 +480,7 @@ int32_t bip_destroy(bip_ctx* ctx) {
   if (ctx->T_owned) cudaFree((void*)ctx->T_dev);
   void* ptrs[] = {ctx->ap_h_dev, ctx->p1_h_dev, ctx->p2_h_dev, ctx->ap_c_dev, ctx->w1_idx_dev, ctx->w1_w_dev, ctx->rooty_dev,
                   ctx->rootx_dev, ctx->P_dev, ctx->ms_work, ctx->S1, ctx->S2, ctx->D1.p, ctx->D2.p, ctx->R1.p, ctx->R2.p, ctx->Psi.p,
-                  ctx->Phi.p, ctx->R1s.p, ctx->R2s.p, ctx->Phis.p, ctx->Scl.p, ctx->rho_dev};
+                  ctx->Phi.p, ctx->R1s.p, ctx->R2s.p, ctx->Phis.p, ctx->Scl.p, ctx->Sync.p, ctx->rho_dev};
   free_illumination(ctx);
   for (void* p : ptrs) if (p) cudaFree(p);
   cudaGetLastError();

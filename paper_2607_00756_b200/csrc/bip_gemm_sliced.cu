@@ -35,7 +35,7 @@ constexpr int TM = 128, TN = 128;
 constexpr int PART_BYTES = SL_TILE_EL * 2;       // 4 KB
 constexpr int NUM_EPI_WARPS = 8;
 constexpr int NUM_THREADS = 64 + 32 * NUM_EPI_WARPS;
-constexpr int DGROUP = 4;                        // column tiles per raster group (concurrent CTAs share operand tiles in L2)
+constexpr int DGROUP_DEFAULT = 16;               // column tiles per raster group (concurrent CTAs share operand tiles in L2)
 
 template <int FMT> struct Cfg;
 template <> struct Cfg<SL_FMT_FP16X4> {
@@ -67,6 +67,10 @@ struct SlParams {
   int rows_pad;            // padded rho rows per channel block of X
   int chunk_steps;         // k-steps per exactly accumulated chunk of leading products
   int lag_max;             // the leading products may trail the small ones by up to this many k-steps (< STAGES)
+  int dgroup;              // column tiles per raster group
+  int drop_tiny;           // FP16X3: the x2 y2 products (<= 2^-18 of the leading ones) are not issued
+  unsigned int* sync_counter;   // lockstep of the workers (below); NULL = free-running
+  int sync_steps;               // ... every this many k-steps of a segment
   // GEMM1 epilogue
   float2* Psi; int64_t psi_ld, psi_batch_stride;
   // GEMM2 epilogue
@@ -113,6 +117,19 @@ __device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {
 __device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+// Lockstep of the persistent workers.  Workers that share an operand stream (same row tile, neighbouring column
+// tiles) only hit in L2 while they read the same k range at about the same time; free-running they drift apart and
+// every worker ends up streaming its operands from HBM (profiles/r01_gemm2_l2_lockstep.md).  The producers of all
+// workers therefore meet at a global counter at the start of every (item, channel) segment: one relaxed
+// red + acquire-poll per ~150 us, all workers co-resident (persistent grid <= SM count).
+__device__ __forceinline__ void lockstep_arrive_wait(unsigned int* counter, unsigned int target) {
+  asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(counter) : "memory");
+  unsigned int v;
+  do {
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(counter) : "memory");
+  } while ((int)(v - target) < 0);
 }
 
 // K-major, no-swizzle shared-memory matrix descriptor (cute::UMMA::SmemDescriptor, LayoutType::INTERLEAVE):
@@ -224,8 +241,9 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
       : "r"(taddr));
 }
 
-// item -> (atom, row tile, column tile); column tiles rasterised in groups of DGROUP.
+// item -> (atom, row tile, column tile); column tiles rasterised in groups of p.dgroup.
 __device__ __forceinline__ void decode_item(const SlParams& p, int item, int& atom, int& rt, int& ct) {
+  const int DGROUP = p.dgroup;
   const int per_atom = p.n_rt * p.n_ct;
   atom = item / per_atom;
   int idx = item - atom * per_atom;
@@ -245,23 +263,30 @@ __device__ __forceinline__ void decode_item(const SlParams& p, int item, int& at
 
 // The small products of one k-step (accumulators C12r, C12i): everything except x1 y1.
 template <int FMT, bool PAIR>
-__device__ __forceinline__ void issue_small(uint32_t t12r, uint32_t t12i, uint32_t a0, uint32_t b0, uint32_t acc) {
+__device__ __forceinline__ void issue_small(uint32_t t12r, uint32_t t12i, uint32_t a0, uint32_t b0, uint32_t acc, bool drop_tiny) {
   constexpr uint32_t id_pos = umma_idesc(Cfg<FMT>::AB_FORMAT, false, PAIR), id_neg = umma_idesc(Cfg<FMT>::AB_FORMAT, true, PAIR);
   constexpr int YP = PAIR ? PART_BYTES / 2 : PART_BYTES;      // a CTA of a pair holds 64 of the 128 Y rows of every part
   auto umma = [](uint32_t d, uint64_t da, uint64_t db, uint32_t id, uint32_t ac) { umma_f16<PAIR>(d, da, db, id, ac); };
   if (FMT == SL_FMT_FP16X4) {
     const uint64_t xr1 = umma_desc(a0), xr2 = umma_desc(a0 + PART_BYTES), xi1 = umma_desc(a0 + 2 * PART_BYTES), xi2 = umma_desc(a0 + 3 * PART_BYTES);
     const uint64_t yr1 = umma_desc(b0), yr2 = umma_desc(b0 + YP), yi1 = umma_desc(b0 + 2 * YP), yi2 = umma_desc(b0 + 3 * YP);
-    // tiniest first: x2 y2, then x1 y2 + x2 y1
-    umma(t12r, xr2, yr2, id_pos, acc);
-    umma(t12r, xi2, yi2, id_neg, 1u);
-    umma(t12r, xr1, yr2, id_pos, 1u);
+    // tiniest first: x2 y2 (FP16X3 leaves them out), then x1 y2 + x2 y1
+    uint32_t acc_r = acc, acc_i = acc;
+    if (!drop_tiny) {
+      umma(t12r, xr2, yr2, id_pos, acc);
+      umma(t12r, xi2, yi2, id_neg, 1u);
+      acc_r = 1u;
+    }
+    umma(t12r, xr1, yr2, id_pos, acc_r);
     umma(t12r, xr2, yr1, id_pos, 1u);
     umma(t12r, xi1, yi2, id_neg, 1u);
     umma(t12r, xi2, yi1, id_neg, 1u);
-    umma(t12i, xr2, yi2, id_pos, acc);
-    umma(t12i, xi2, yr2, id_pos, 1u);
-    umma(t12i, xr1, yi2, id_pos, 1u);
+    if (!drop_tiny) {
+      umma(t12i, xr2, yi2, id_pos, acc);
+      umma(t12i, xi2, yr2, id_pos, 1u);
+      acc_i = 1u;
+    }
+    umma(t12i, xr1, yi2, id_pos, acc_i);
     umma(t12i, xr2, yi1, id_pos, 1u);
     umma(t12i, xi1, yr2, id_pos, 1u);
     umma(t12i, xi2, yr1, id_pos, 1u);
@@ -360,15 +385,22 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
     // ================= bulk-copy producer =================
     if (lane == 0) {
       uint32_t it = 0;
+      unsigned int sync_target = 0;
       for (int item = worker; item < p.n_items; item += n_workers) {
         int atom, rt, ct;
         decode_item(p, item, atom, rt, ct);
+        const unsigned int active = (unsigned int)min(n_workers, p.n_items - (item - worker));   // workers with an item in this wave
         if (PAIR) rt = 2 * rt + (int)rank;
         // a CTA of a pair loads rows [64 rank, 64 rank + 64) of every part of the Y tile
         const uint16_t* ysrc = p.Y + (int64_t)atom * p.y_batch_stride + (int64_t)ct * p.ksteps * STEP_EL + (PAIR ? rank * (SL_TILE_EL / 2) : 0);
         for (int n = 0; n < p.n_ch_loop; ++n) {
           const uint16_t* xsrc = p.X + (int64_t)atom * p.x_batch_stride + ((int64_t)n * p.n_rt_x + rt) * p.ksteps * STEP_EL;
-          for (int ks = 0; ks < p.ksteps; ++ks, ++it) {
+          for (int ks = 0, next_sync = 0; ks < p.ksteps; ++ks, ++it) {
+            if (p.sync_counter && ks == next_sync) {
+              next_sync += p.sync_steps;
+              sync_target += active;
+              if (rank == 0) lockstep_arrive_wait(p.sync_counter, sync_target);
+            }
             const int s = it % STAGES;
             mbar_wait(&empty[s], ((it / STAGES) & 1) ^ 1);
             uint8_t* st = smem + s * STAGE_BYTES;
@@ -413,6 +445,7 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
     const uint32_t t0r = tmem_base, t0i = tmem_base + TN, t12r = tmem_base + 2 * TN, t12i = tmem_base + 3 * TN;
     const uint32_t ksteps = (uint32_t)p.ksteps, chunk = (uint32_t)p.chunk_steps, lag_max = (uint32_t)p.lag_max;
     const uint32_t smem_base = smem_u32(smem);
+    const bool drop_tiny = FMT == SL_FMT_FP16X4 && p.drop_tiny != 0;
     uint32_t s_small = 0, ph_small = 0;            // stage and phase of the small-product cursor
     uint32_t ks_s = 0, seg_par = 0;                // its k-step inside the segment; segment parity
     uint32_t s_lead = 0, ks_l = 0, in_chunk = 0, chunk_par = 0, pending = 0;   // leading-product cursor
@@ -447,7 +480,7 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
       const bool seg_end = ks_s + 1 == ksteps;
       if (elect_one()) {
         const uint32_t a0 = smem_base + s_small * STAGE_BYTES;
-        issue_small<FMT, PAIR>(t12r, t12i, a0, a0 + X_BYTES, ks_s ? 1u : 0u);
+        issue_small<FMT, PAIR>(t12r, t12i, a0, a0 + X_BYTES, ks_s ? 1u : 0u, drop_tiny);
         if (seg_end) umma_commit<PAIR>(c12_full);
       }
       __syncwarp();
@@ -616,9 +649,21 @@ int32_t launch_fmt(bip_ctx* ctx, const SlParams& p) {
   if (q.n_items <= 0) return BIP_OK;
   q.chunk_steps = Cfg<FMT>::CHUNK_STEPS;
   q.lag_max = Cfg<FMT>::LAG_MAX;
+  q.dgroup = DGROUP_DEFAULT;
+  if (const char* e = std::getenv("BIP_TUNE_DGROUP")) q.dgroup = std::max(1, std::atoi(e));
   if (const char* e = std::getenv("BIP_TUNE_CHUNK")) q.chunk_steps = std::max(1, std::atoi(e));   // timing experiments only: breaks exactness
   if (const char* e = std::getenv("BIP_TUNE_LAG")) q.lag_max = std::min(std::max(1, std::atoi(e)), (PAIR ? Cfg<FMT>::STAGES_PAIR : Cfg<FMT>::STAGES) - 1);
-  const int workers = std::max(1, std::min(q.n_items, PAIR ? ctx->sm_count / 2 : ctx->sm_count));
+  static const bool lockstep = [] { const char* e = std::getenv("BIP_TUNE_LOCKSTEP"); return e ? std::atoi(e) != 0 : true; }();
+  q.sync_counter = nullptr;
+  q.sync_steps = 1 << 30;                // once per (item, channel) segment
+  if (const char* e = std::getenv("BIP_TUNE_SYNCSTEPS")) q.sync_steps = std::max(1, std::atoi(e));
+  if (lockstep) {      // a fresh zeroed counter per launch (64 slots, cleared on the stream before the kernel)
+    BIP_TRY(ensure(ctx, ctx->Sync, 64 * sizeof(unsigned int), "lockstep counters"));
+    q.sync_counter = reinterpret_cast<unsigned int*>(ctx->Sync.p) + (ctx->sync_slot++ & 63);
+    BIP_CUDA(ctx, cudaMemsetAsync(q.sync_counter, 0, sizeof(unsigned int), ctx->stream));
+  }
+  int workers = std::max(1, std::min(q.n_items, PAIR ? ctx->sm_count / 2 : ctx->sm_count));
+  if (const char* e = std::getenv("BIP_TUNE_WORKERS")) workers = std::max(1, std::min(workers, std::atoi(e)));   // timing experiments only
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = dim3(PAIR ? 2 * workers : workers);
   cfg.blockDim = dim3(NUM_THREADS);
@@ -652,6 +697,7 @@ int32_t launch_gemm1_sliced(bip_ctx* ctx, const Gemm1SlArgs& a) {
   p.n_ct = (int)(a.R1t.rows_pad / TN);
   p.n_items = a.n_atoms * p.n_rt * p.n_ct;
   p.n_ch_loop = 1;
+  p.drop_tiny = a.drop_tiny;
   p.n_rows = a.n_rho; p.n_cols = a.w2; p.rows_pad = (int)a.A.rows_pad;
   p.Psi = a.Psi; p.psi_ld = a.psi_ld; p.psi_batch_stride = a.psi_batch_stride;
   return launch<EPI_GEMM1>(ctx, p, a.A.fmt);
@@ -677,6 +723,7 @@ int32_t launch_gemm2_sliced(bip_ctx* ctx, const Gemm2SlArgs& a) {
   p.n_ct = (int)(a.R2.rows_pad / TN);
   p.n_items = a.n_atoms * p.n_rt * p.n_ct;
   p.n_ch_loop = a.n_ch;
+  p.drop_tiny = a.drop_tiny;
   p.n_rows = a.n_rho; p.n_cols = a.n_det;
   p.mode = a.mode; p.inv_G = a.inv_G; p.bin_of_det = a.bin_of_det; p.n_bins = a.n_bins; p.out = a.out;
   return launch<EPI_GEMM2>(ctx, p, a.Phi.fmt);

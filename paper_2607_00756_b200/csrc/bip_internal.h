@@ -98,6 +98,8 @@ struct bip_ctx {
   // scratch, grown on demand
   bip::DevBuf D1, D2, R1, R2, Psi, Phi;
   bip::DevBuf R1s, R2s, Phis, Scl;  // sliced operands of the tensor-core path and their row scales
+  bip::DevBuf Sync;                 // lockstep counters of the persistent contraction kernel (one per launch slot)
+  int sync_slot = 0;
 
   bip_timing timing{};
   cudaEvent_t ev[8] = {};
@@ -179,6 +181,7 @@ struct Gemm1SlArgs {     // a4: Psi = A . R1   (c64 [atom][rho][s])
   float2* Psi;
   int64_t psi_ld, psi_batch_stride;
   int32_t n_rho, w2, n_atoms;
+  int32_t drop_tiny = 0; // BIP_PREC_FP16X3
 };
 struct Gemm2SlArgs {     // a7 + a8
   Sliced Phi;            // rows (n, rho) = n * rows_pad + rho, k = window pixels, batch = atoms
@@ -190,6 +193,7 @@ struct Gemm2SlArgs {     // a7 + a8
   const int32_t* bin_of_det;
   int32_t n_bins;
   void* out;
+  int32_t drop_tiny = 0; // BIP_PREC_FP16X3
 };
 int32_t launch_gemm1_sliced(bip_ctx* ctx, const Gemm1SlArgs& a);
 int32_t launch_gemm2_sliced(bip_ctx* ctx, const Gemm2SlArgs& a);

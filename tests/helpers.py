@@ -68,3 +68,51 @@ def rel_err_map(got, want, floor=0.0):
     """max |got - want| / max(want, floor * max(want)); floor = 0 is the plain per-pixel form."""
     den = np.maximum(np.abs(want), floor * np.abs(want).max()) if floor > 0 else np.abs(want)
     return float(np.max(np.abs(got - want) / den))
+
+
+class OracleSample:
+    """A bounded sample of a full-size workload for the oracle (SURVEY 8(d) "Parity protocol"): the first ``n_atoms``
+    sites of the edge, a regular subset of ``n_scan`` scan positions, every channel and every detector beam.  The
+    slab is truncated to ``nz`` slices so that the fp64 parent columns are cheap to build; parents are processed in
+    chunks and only their W x W windows at the sampled sites are kept.  Contraction shapes per (scan, channel,
+    beam) are those of the full workload.  Used by the full-size parity test and by bench.py's oracle legs."""
+
+    def __init__(self, workload="cfg2", scale=1, nz=2, n_atoms=1, n_scan=256, n_jobs=None, edge=0):
+        import os
+        from bip_inputs.specimen import make_workload
+        self.wl = wl = make_workload(workload, scale=scale, nz=nz)
+        self.e = e = wl.edges[edge].take(np.arange(n_atoms))
+        self.orc = orc = OracleSetup(wl, e, n_jobs=n_jobs or os.cpu_count())
+        T = wl.T.astype(np.complex128)
+        planes = sorted(set(int(s) for s in e.slice))
+        self.crops = [[None, None] for _ in range(n_atoms)]
+        for which, par_h in ((0, orc.ap[orc.p1_pos]), (1, orc.det[orc.p2_pos])):
+            parts = [[] for _ in range(n_atoms)]
+            for c0 in range(0, len(par_h), 256):          # parents in chunks: only the windows are kept
+                hs = par_h[c0:c0 + 256]
+                for plane in planes:
+                    if which == 0:
+                        S = oms.build_S1(hs, wl.ny, wl.nx)
+                        for i in range(plane):
+                            S = oms.advance_S1(S, T[i], orc.P)
+                    else:
+                        S = oms.build_S2_at(hs, T, orc.P, plane)
+                    for a in np.nonzero(e.slice == plane)[0]:
+                        parts[a].append(obip.crop_window(S, e.centre[a], e.W, wl.ny, wl.nx))
+            for a in range(n_atoms):
+                self.crops[a][which] = np.concatenate(parts[a])
+        sy, sx = wl.scan_shape
+        side = max(1, int(round(np.sqrt(n_scan))))
+        sub = [iy * sx + ix for iy in range(0, sy, max(1, sy // side)) for ix in range(0, sx, max(1, sx // side))]
+        self.scan_idx = np.array(sub[:n_scan])
+        self.A = obip.illumination(orc.c, orc.ap, wl.scan[self.scan_idx], wl.ny, wl.nx)
+
+    def run(self, recon, atoms=None):
+        """Steps a1-a8 of the oracle on the sample: dict of reduce_modes() summed over the sampled atoms."""
+        o, e, wl, acc = self.orc, self.e, self.wl, None
+        for a in (range(e.n_atoms) if atoms is None else atoms):
+            amp, _ = obip.atom_amplitudes(None, None, o.ap[o.p1_pos], o.det[o.p2_pos], o.ap, o.det, o.w1, o.w2, self.A,
+                                          e.H.astype(np.complex128), e.centre[a], wl.ny, wl.nx, recon, crops=tuple(self.crops[a]))
+            r = obip.reduce_modes(amp, o.det)
+            acc = r if acc is None else {k: acc[k] + r[k] for k in acc}
+        return acc

@@ -1,0 +1,50 @@
+"""The N > 1 path of bench.py on CPU: two gloo ranks shard the sites of an edge (no data-path collective) and agree on
+the max-over-ranks time; the reference arm runs on rank 0 only."""
+import os
+import sys
+
+import numpy as np
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+sys.path.insert(0, ROOT)
+
+
+def _worker(rank, world, port, q):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    import bench
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    idx = bench.shard_atoms(rank, 3, 8)
+    t = bench.max_over_ranks(10.0 + 5.0 * rank, world, device="cpu")
+    # the partial maps of the shards add up to the map of the union (sites are independent: eq. 14) -- checked with a
+    # stand-in per-site contribution, since the contraction itself needs the GPU
+    contrib = torch.zeros(8, dtype=torch.float64)
+    contrib[idx] = torch.arange(8, dtype=torch.float64)[idx] + 1.0
+    dist.all_reduce(contrib)
+    q.put((rank, idx.tolist(), t, contrib.tolist()))
+    dist.destroy_process_group()
+
+
+def test_two_ranks_shard_sites_and_take_the_max_time():
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29500 + os.getpid() % 2000
+    ps = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in ps:
+        p.start()
+    got = sorted(q.get(timeout=120) for _ in ps)
+    for p in ps:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert got[0][1] == [0, 1, 2] and got[1][1] == [3, 4, 5]                 # disjoint contiguous blocks
+    assert got[0][2] == got[1][2] == 15.0                                    # max over ranks on both
+    assert got[0][3] == got[1][3] == [1.0, 2.0, 3.0, 4.0, 5.0, 6.0, 0.0, 0.0]
+
+
+def test_shard_clamps_at_the_end_of_the_edge():
+    import bench
+    assert bench.shard_atoms(2, 3, 8).tolist() == [6, 7]
+    assert bench.shard_atoms(3, 3, 8).tolist() == []
+    assert bench.max_over_ranks(3.5, 1) == 3.5
