@@ -37,6 +37,7 @@ sys.path.insert(0, ROOT)
 sys.path.insert(0, os.path.join(ROOT, "tests"))
 
 METRIC = "scan-pos x atom x channel x detector-beam amplitudes/s"
+CONFIG_INDEX = {"cfg1": 0, "cfg2": 1, "cfg3": 2, "cfg5": 4}
 UNIT = "amplitudes/s"
 SM_COUNT, FMA_LANES, = 148, 128
 
@@ -116,9 +117,10 @@ def max_over_ranks(x, world, device="cuda"):
 def build_problem(args, rank):
     """Synthetic configs[1] cell; the edge is sampled down to --atoms sites of the first ionisation plane(s)."""
     from bip_inputs.specimen import make_workload
-    wl = make_workload(args.workload, scale=args.scale)
-    e = wl.edges[0]
-    return wl, e.take(shard_atoms(rank, args.atoms, e.n_atoms))
+    pf = (args.parent_factor, args.parent_factor) if args.parent_factor else None
+    wl = make_workload(args.workload, scale=args.scale, parent_factor=pf)
+    src = wl.edges if args.edges == "all" else wl.edges[:1]
+    return wl, [e.take(shard_atoms(rank, args.atoms, e.n_atoms)) for e in src]
 
 
 def run_ours(args):
@@ -137,7 +139,9 @@ def run_ours(args):
     prec = {"fp16x4": B.PREC_FP16X4, "fp16x3": B.PREC_FP16X3, "bf16x6": B.PREC_BF16X6, "tf32x3": B.PREC_TF32X3, "fp32_simt": B.PREC_FP32_SIMT}[args.precision]
     recon = {"linear": B.RECON_LINEAR, "magphase": B.RECON_MAGPHASE}[args.recon]
 
-    wl, edge = build_problem(args, rank)
+    mode = {"map": B.MODE_MAP, "qeels_x": B.MODE_QEELS_X, "cube": B.MODE_CUBE}[args.mode]
+    wl, edges = build_problem(args, rank)
+    edge = edges[0]
     g = B.Grid(wl.ny, wl.nx, wl.ly, wl.lx, wl.nz, wl.dz, wl.lam)
     geo = B.plan_geometry(g, wl.alpha_mrad, edge.det_mrad, wl.defocus, wl.parent_factor)
     T_dev = torch.from_numpy(wl.T).cuda()
@@ -145,15 +149,16 @@ def run_ours(args):
     ctx.build_S1()
     ctx.build_S2()
     ctx.set_scan(wl.scan)
-    eid = ctx.add_edge(edge.slice, edge.centre, edge.H, geo.det_h, geo.w2)
+    eids = [ctx.add_edge(e.slice, e.centre, e.H, geo.det_h, geo.w2) for e in edges]
     torch.cuda.synchronize()
     t_build = ctx.get_timing()
-    out = torch.empty(ctx.n_rho, dtype=torch.float64, device="cuda")
-    first_plane = int(edge.slice.min())
+    first_plane = min(int(e.slice.min()) for e in edges)
+    K = geo.det_h.shape[0]
+    outs = [None]
 
     def step():
         ctx.seek_plane(max(first_plane - 1, 0))      # every step moves the plane cursor (ADVANCETO / PEELTO) again
-        ctx.map(eid, B.MODE_MAP, recon, prec, out=out)
+        outs[0] = ctx.map_all(mode, recon, prec)     # one plane loop shared by all registered edges
 
     def barrier():
         if world > 1:
@@ -182,21 +187,28 @@ def run_ours(args):
     clocks = sampler.stop() if rank == 0 else None
     ms_total = ev0.elapsed_time(ev1)
     ms_total = max_over_ranks(ms_total, world)
-    amps_step = float(ctx.n_rho) * edge.n_atoms * edge.n_ch * geo.det_h.shape[0]
+    amps_step = float(ctx.n_rho) * K * sum(e.n_atoms * e.n_ch for e in edges)
     value = amps_step * world * args.steps / (ms_total * 1e-3)
-    map_dev = out.cpu().numpy()
+    map_dev = outs[0][0].cpu().numpy()
+    out_bytes = sum(o.numel() * o.element_size() for o in outs[0])
 
     # ---- end to end through the host-buffer API: pinned inputs in, map out, every step ----
-    h_slice, h_centre, h_H = pinned(edge.slice), pinned(edge.centre), pinned(edge.H)
+    h_edges = [(pinned(e.slice), pinned(e.centre), pinned(e.H)) for e in edges]
     h_det, h_idx, h_w = pinned(geo.det_h), pinned(geo.w2[0]), pinned(geo.w2[1])
-    h2d = sum(a.nbytes for a in (h_slice, h_centre, h_H, h_det, h_idx, h_w)) + 2 * 4 * edge.n_atoms + 2 * 4 * geo.det_h.shape[0]
-    d2h = ctx.n_rho * 8
+    h2d = sum(sum(a.nbytes for a in he) + 2 * 4 * he[0].shape[0] + sum(a.nbytes for a in (h_det, h_idx, h_w)) + 2 * 4 * K for he in h_edges)
+    d2h = out_bytes
 
     def step_e2e():
         ctx.clear_edges()
-        e2 = ctx.add_edge(h_slice, h_centre, h_H, h_det, (h_idx, h_w))
-        ctx.seek_plane(max(first_plane - 1, 0))
-        return ctx.map_host(e2, B.MODE_MAP, recon, prec)
+        ids = [ctx.add_edge(hs, hc, hH, h_det, (h_idx, h_w)) for hs, hc, hH in h_edges]
+        if len(ids) == 1:
+            ctx.seek_plane(max(first_plane - 1, 0))
+            return ctx.map_host(ids[0], mode, recon, prec)
+        res = []
+        for i in ids:                                # the host-buffer entry point serves one edge per call
+            ctx.seek_plane(max(first_plane - 1, 0))
+            res.append(ctx.map_host(i, mode, recon, prec))
+        return res[0]
 
     step_e2e()
     barrier()
@@ -208,11 +220,10 @@ def run_ours(args):
     e2e_s = time.perf_counter() - t0
     e2e_s = max_over_ranks(e2e_s, world)
     e2e_value = amps_step * world * e2e_steps / e2e_s
-    assert np.allclose(m_host, map_dev, rtol=1e-5, atol=0), "host-buffer path disagrees with the device path"
+    assert np.allclose(m_host, map_dev, rtol=1e-5, atol=1e-6 * float(np.abs(map_dev).max())), "host-buffer path disagrees with the device path"
 
     # ---- roofline of the dominant kernel (a7-a8) ----
-    w2 = edge.W * edge.W
-    flops_gemm2_step = 8.0 * ctx.n_rho * w2 * edge.n_atoms * edge.n_ch * geo.det_h.shape[0]
+    flops_gemm2_step = 8.0 * ctx.n_rho * K * sum(e.W * e.W * e.n_atoms * e.n_ch for e in edges)
     achieved = flops_gemm2_step * args.steps / (gemm2_ms * 1e-3) / 1e12 if gemm2_ms > 0 else 0.0
     if args.precision in ("fp16x4", "fp16x3", "bf16x6"):
         bf16_peak = peaks["bf16_tflops"]           # burst figure: the larger, hence the conservative denominator
@@ -236,9 +247,15 @@ def run_ours(args):
                 "traffic": None, "kernel": "k_gemm2_simt",
                 "note": "fp32 FMA peak = 148 SMs x 128 lanes x 2 x max SM clock (reference CUDA-core path)",
                 "avg_launch_ms": gemm2_ms / max(gemm2_launches, 1), "launches": gemm2_launches}
-    traffic_file = os.path.join(ROOT, "profiles", "gemm2_traffic.json")
-    if os.path.exists(traffic_file):
-        roof["traffic"] = json.load(open(traffic_file)).get(roof["kernel"])
+    # DRAM bytes per launch of the same kernel from the committed ncu --set full capture (profiles/r01_gemm2_ncu_full.md)
+    traffic_file = os.path.join(ROOT, "profiles", "r01_gemm2_traffic.txt")
+    if os.path.exists(traffic_file) and args.precision == "fp16x4" and args.workload == "cfg2" and args.mode == "map":
+        tok = open(traffic_file).read().split()
+        kv = dict(zip(tok[0::2], tok[1::2]))
+        atoms_launch = sum(e.n_atoms for e in edges) * args.steps / max(gemm2_launches, 1)
+        roof["traffic"] = (float(kv["dram_bytes_read"]) + float(kv["dram_bytes_write"])) * atoms_launch / float(kv["atoms_per_launch"])
+        roof["traffic_unit"] = "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum)"
+        roof["algorithmic_bytes"] = atoms_launch * 8.0 * edge.W * edge.W * (ctx.n_rho * edge.n_ch + K)
 
     line = None
     if rank == 0:
@@ -247,12 +264,12 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": {"fp16x4": "fp16x4(c64)", "fp16x3": "fp16x3(c64)", "bf16x6": "bf16x6(c64)", "tf32x3": "tf32x3(c64)", "fp32_simt": "f32(c64)"}[args.precision], "data": "synthetic",
-            "config": {"workload": f"BASELINE configs[1] ({wl.name}): {wl.ny}x{wl.nx} grid, {wl.nz} slices, B={geo.ap_h.shape[0]}, "
-                                   f"K={geo.det_h.shape[0]}, parents=({ctx.n_p1},{ctx.n_p2}), W={edge.W}, N_ch={edge.n_ch}, "
-                                   f"N_rho={ctx.n_rho}, map output, recon={args.recon}",
-                       "atoms_per_step_per_gpu": edge.n_atoms, "sampled": "first sites of the first B plane; the full edge has "
-                       f"{wl.edges[0].n_atoms} sites", "precision": args.precision,
-                       "l2": "per-step working set (operand planes > 5 GB per atom) far exceeds the 126 MB L2: no flush needed",
+            "config": {"workload": f"BASELINE configs[{CONFIG_INDEX.get(args.workload, '?')}] ({wl.name}): {wl.ny}x{wl.nx} grid, {wl.nz} slices, "
+                                   f"B={geo.ap_h.shape[0]}, K={K}, parents=({ctx.n_p1},{ctx.n_p2}), parent factor {wl.parent_factor[0]:g}, "
+                                   f"W={edge.W}, N_ch={[e.n_ch for e in edges]}, N_rho={ctx.n_rho}, {args.mode} output, recon={args.recon}",
+                       "atoms_per_step_per_gpu": [e.n_atoms for e in edges], "sampled": "first sites of each edge's first plane(s); the "
+                       f"full edges have {[e.n_atoms for e in (wl.edges if args.edges == 'all' else wl.edges[:1])]} sites", "precision": args.precision,
+                       "l2": "per-step working set (sliced operands, > 0.5 GB per atom, rewritten every step) exceeds the 126 MB L2: no flush needed",
                        "parallelism": f"atoms sharded over {world} GPU(s), no data-path collective"},
             "clocks": clocks, "gpu_launches": launches,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
@@ -343,6 +360,9 @@ def main():
     ap.add_argument("--atoms", type=int, default=8, help="ionised atoms per step per GPU")
     ap.add_argument("--precision", default=os.environ.get("BIP_BENCH_PRECISION", "fp16x4"), choices=["fp16x4", "fp16x3", "bf16x6", "tf32x3", "fp32_simt"])
     ap.add_argument("--recon", default="magphase", choices=["linear", "magphase"])
+    ap.add_argument("--mode", default="map", choices=["map", "qeels_x", "cube"])
+    ap.add_argument("--edges", default="first", choices=["first", "all"], help="all: every edge of the workload shares one plane loop (configs[2])")
+    ap.add_argument("--parent-factor", type=float, default=0.0, help="override the workload's parent factor (configs[4] sweeps 1/2/4/8)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -171,6 +171,19 @@ BIP_API int32_t bip_build_S2(bip_ctx* ctx);
  * c_b(rho) = c_b exp(-2 pi i h_b.rho/N) on the device. */
 BIP_API int32_t bip_set_scan(bip_ctx* ctx, int32_t n_rho, const double* rho_px);
 
+/* PRISM beam subsampling (Alg. 2 line 1): positions (ascending) of the beams of h [n][2]
+ * with h_y = 0 (mod fy) and h_x = 0 (mod fx) into keep_out [cap]; *n_keep = their number (BIP_ERR_INVALID if cap is too
+ * small).  The retained probe coefficients are to be multiplied by fy * fx, "the DFT decimation factor".
+ * Host only. */
+BIP_API int32_t bip_prism_subsample(int32_t n, const int32_t* h, int32_t fy, int32_t fx, int32_t* keep_out, int32_t cap,
+                                    int32_t* n_keep);
+
+/* PRISM crop mask: from now on a site contributes only to the scan positions inside its 1/f window,
+ * |rho - tau| < N / (2 f) on both axes (periodic distance from the atom's pixel; reading c19).  fy = fx = 1
+ * switches the mask off (the default).  The contraction then runs, per site, over that site's scan rows only: the
+ * cost per site falls by fy * fx.  Tensor-core precisions only (BIP_PREC_FP16X4 / FP16X3 / BF16X6). */
+BIP_API int32_t bip_set_crop(bip_ctx* ctx, int32_t fy, int32_t fx);
+
 /* Register an ionisation edge: its sites, transition-potential windows and detector.
  *   slice [n_atoms]        slice index i(tau) of each site, 0 <= slice < nz
  *   centre_px [n_atoms][2] pixel the atom sits on; the window covers centre - w/2 .. centre + w/2 - 1 (periodic)

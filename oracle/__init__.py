@@ -8,7 +8,8 @@ the other.  The only module both use is ``bip_inputs`` (seeded synthetic problem
 Everything here is a plain, slow, NumPy complex128 restatement of PAPER.md written to be checked
 against the paper by eye, one function per equation / algorithm step, each citing its passage:
 
-  beams.py       beam sets (eq. 5 / Alg. 4 l.1), probe coefficients (eq. 1), hex-ring parents
+  beams.py       beam sets (eq. 5 / Alg. 4 l.1), probe coefficients (eq. 1), hex-ring parents,
+                 PRISM beam subsampling, coefficient rescale and crop mask
   sibson.py      natural-neighbour weights (eq. 8) by half-plane clipping
   multislice.py  Fresnel step (eq. 2, 6), S1 build/advance, S2 build/peel (eq. 12), Alg. 1, Alg. 3
   bip.py         windowed reconstruction (eq. 15, eq. 11), amplitudes (eq. 13-14), output modes (§2.2.6), Alg. 5
@@ -24,6 +25,8 @@ Pins (tests/test_oracle_*.py, all ``-m "not gpu"``):
   reducers             : sum over q_par of qEELS == map == sum over d of cube
   weights              : w >= 0, rows sum to 1, delta at parents, linear precision inside the hull, identity limit
   hex-ring             : n_radial = 4 gives 61 parents from 365 beams (tests/golden/hexring_counts.txt)
+  PRISM f              : subsampled probe == exact probe replicated with period N/f (aliasing identity); crop mask
+                         == per-site maps masked and summed
   MAGPHASE             : equals LINEAR for in-phase rows; exact at parents; |R|_MAGPHASE >= |R|_LINEAR
 PARITY UNPINNED: the Sibson weights for beams outside the parents' convex hull (c8) and the
 numerical value of BiP maps at parent factor f > 1 have no printed value in the paper to compare against; they are

@@ -30,6 +30,28 @@ def beams_in_disc(ny, nx, ly, lx, qmax):
     return np.asarray(out, dtype=np.int64).reshape(-1, 2)
 
 
+def prism_subsample(beams, fy, fx):
+    """PRISM beam subsampling (Alg. 2 line 1): keep h with h_y = 0 (mod f_y) and
+    h_x = 0 (mod f_x).  Returns the positions into ``beams`` (ascending, so the flat-index order is kept)."""
+    keep = (beams[:, 0] % fy == 0) & (beams[:, 1] % fx == 0)
+    return np.nonzero(keep)[0]
+
+
+def prism_coefficients(c_full, keep, fy, fx):
+    """Coefficients of the retained beams, rescaled by f_y f_x, "the DFT decimation factor": the
+    synthesised probe is then the exact probe replicated with period (N_y / f_y, N_x / f_x)."""
+    return c_full[keep] * float(fy * fx)
+
+
+def crop_mask(scan, centre, ny, nx, fy, fx):
+    """PRISM crop mask: the scans inside the atom's 1/f window, i.e. whose periodic distance from the
+    atom's pixel is below half the alias-free period, |rho - tau| < N / (2 f) on both axes (reading c19).
+    scan [n_rho, 2] in pixels; returns bool [n_rho]."""
+    dy = (scan[:, 0] - centre[0] + ny / 2.0) % ny - ny / 2.0
+    dx = (scan[:, 1] - centre[1] + nx / 2.0) % nx - nx / 2.0
+    return (np.abs(dy) < ny / (2.0 * fy)) & (np.abs(dx) < nx / (2.0 * fx))
+
+
 def aperture_coefficients(beams, ny, nx, ly, lx, lam, defocus):
     """c_b = Psi(h_b) = exp(-i pi lam df |q_b|^2) / sqrt(G B): pure-defocus lens phase inside the aperture,
     probe normalised to sum_r |psi_0|^2 = 1 (eq. 1)."""

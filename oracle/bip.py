@@ -101,12 +101,14 @@ def reduce_modes(a, det_beams):
 
 
 def bip_run(T, P, ap_beams, c, p1_h, w1, det_beams, p2_h, w2, scan, sites_slice, sites_centre, H,
-            recon="linear", want_psi=False):
+            recon="linear", want_psi=False, crop_f=None):
     """Algorithm 5: build S1 / S2 on the parents, then for every ionisation plane with >= 1
     site ADVANCETO / PEELTO and run the on-atom contraction for every site and channel, accumulating the outputs.
     T complex [nz, ny, nx]; weights w1 [B, Bp1], w2 [K, Bp2] (dense or scipy.sparse).  Returns the dict of
-    reduce_modes() summed over sites (eq. 14)."""
+    reduce_modes() summed over sites (eq. 14).  ``crop_f`` = (f_y, f_x) applies the PRISM crop mask:
+    a site contributes only to the scans of beams.crop_mask()."""
     from . import multislice as ms
+    from . import beams as ob
     nz, ny, nx = T.shape
     T = T.astype(np.complex128)
     w1 = sp.csr_matrix(w1)
@@ -122,6 +124,9 @@ def bip_run(T, P, ap_beams, c, p1_h, w1, det_beams, p2_h, w2, scan, sites_slice,
             a, Psi = atom_amplitudes(S1, S2, p1_h, p2_h, ap_beams, det_beams, w1, w2, A,
                                      H.astype(np.complex128), sites_centre[a_idx], ny, nx, recon)
             r = reduce_modes(a, det_beams)
+            if crop_f is not None:
+                inside = ob.crop_mask(scan, sites_centre[a_idx], ny, nx, crop_f[0], crop_f[1])
+                r = {k: v * (inside[:, None] if v.ndim == 2 else inside) for k, v in r.items()}
             acc = r if acc is None else {k: acc[k] + r[k] for k in acc}
             if want_psi:
                 psis.append(Psi)

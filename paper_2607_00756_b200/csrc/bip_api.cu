@@ -210,10 +210,60 @@ static size_t scratch_budget() {
 }
 
 // Steps a1-a8 on the sliced 16-bit operands (BIP_PREC_FP16X4 / BIP_PREC_BF16X6).
-static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, int32_t nb, int mode, int recon, int fmt, bool drop_tiny, void* out) {
+// PRISM crop mask (reading c19): the scan rows of each site of the batch, [nb][stride] with -1 padding.
+// The arithmetic is the oracle's, in the same order, in fp64: d = ((rho - c + N/2) mod N) - N/2, |d| < N / (2 f).
+static void crop_row_lists(const bip_ctx* ctx, const Edge& e, int32_t a0, int32_t nb, std::vector<int32_t>& rows, int32_t& n_rows_max,
+                           int64_t& stride, double& n_rows_total) {
+  const int ny = ctx->g.ny, nx = ctx->g.nx;
+  std::vector<std::vector<int32_t>> lists(nb);
+  n_rows_max = 0; n_rows_total = 0;
+  for (int32_t a = 0; a < nb; ++a) {
+    const double cy = (e.origin[2 * (size_t)(a0 + a)] + e.w / 2) % ny, cx = (e.origin[2 * (size_t)(a0 + a) + 1] + e.w / 2) % nx;
+    for (int32_t r = 0; r < ctx->n_rho; ++r) {
+      double dy = std::fmod(ctx->rho_host[2 * (size_t)r] - cy + ny / 2.0, (double)ny);
+      double dx = std::fmod(ctx->rho_host[2 * (size_t)r + 1] - cx + nx / 2.0, (double)nx);
+      if (dy < 0) dy += ny;
+      if (dx < 0) dx += nx;
+      dy -= ny / 2.0; dx -= nx / 2.0;
+      if (std::fabs(dy) < ny / (2.0 * ctx->crop_fy) && std::fabs(dx) < nx / (2.0 * ctx->crop_fx)) lists[a].push_back(r);
+    }
+    n_rows_max = std::max<int32_t>(n_rows_max, (int32_t)lists[a].size());
+    n_rows_total += (double)lists[a].size();
+  }
+  n_rows_max = std::max(n_rows_max, 1);
+  stride = round_up(n_rows_max, 2 * SL_ROWS);
+  rows.assign((size_t)nb * stride, -1);
+  for (int32_t a = 0; a < nb; ++a) std::copy(lists[a].begin(), lists[a].end(), rows.begin() + (size_t)a * stride);
+}
+
+static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, int32_t a0, int32_t nb, int mode, int recon, int fmt, bool drop_tiny, void* out) {
   auto& sp = spans()[ctx];
   const int w2 = e.w * e.w;
-  const int64_t rho_pad = round_up(ctx->n_rho, 2 * SL_ROWS);    // X operands are padded to pairs of row tiles (CTA-pair kernel)
+  // scan rows of the contraction: all of them, or (crop mask) each site's own list, gathered into a per-site A operand
+  const bool crop = ctx->crop_fy > 1 || ctx->crop_fx > 1;
+  int32_t n_rows = ctx->n_rho;
+  double n_rows_total = (double)ctx->n_rho * nb;
+  const int32_t* row_idx_dev = nullptr;
+  int64_t rho_pad = round_up(ctx->n_rho, 2 * SL_ROWS);    // X operands are padded to pairs of row tiles (CTA-pair kernel)
+  Sliced Ax = ctx->A_sl;
+  if (crop) {
+    std::vector<int32_t> rows;
+    crop_row_lists(ctx, e, a0, nb, rows, n_rows, rho_pad, n_rows_total);
+    BIP_TRY(ensure(ctx, ctx->RowIdx, rows.size() * sizeof(int32_t), "crop-mask row lists"));
+    BIP_CUDA(ctx, cudaMemcpyAsync(ctx->RowIdx.p, rows.data(), rows.size() * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream));
+    BIP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));          // `rows` goes out of scope
+    row_idx_dev = reinterpret_cast<const int32_t*>(ctx->RowIdx.p);
+    Sliced Ac = ctx->A_sl;
+    Ac.rows = n_rows; Ac.rows_pad = rho_pad;
+    Ac.batch_stride = rho_pad / SL_ROWS * Ac.ksteps * sl_step_el(fmt);
+    Ac.scale_batch_stride = rho_pad;
+    const size_t op_bytes = (size_t)(Ac.batch_stride * nb) * sizeof(uint16_t), sc_bytes = (size_t)nb * rho_pad * sizeof(float);
+    BIP_TRY(ensure(ctx, ctx->Acrop, op_bytes + sc_bytes, "illumination rows of the cropped scans"));
+    Ac.base = reinterpret_cast<uint16_t*>(ctx->Acrop.p);
+    Ac.scale = reinterpret_cast<float*>(reinterpret_cast<char*>(ctx->Acrop.p) + op_bytes);
+    BIP_TRY(launch_gather_rows_sliced(ctx, ctx->A_sl, row_idx_dev, rho_pad, Ac, nb));
+    Ax = Ac;
+  }
   Sliced R1t, R2, Phi;
   BIP_TRY(ensure(ctx, ctx->D1, (size_t)nb * ctx->n_p1 * w2 * sizeof(float2), "D1 (de-tilted S1 windows)"));
   BIP_TRY(ensure(ctx, ctx->D2, (size_t)nb * ctx->n_p2 * w2 * sizeof(float2), "D2 (de-tilted S2 windows)"));
@@ -221,7 +271,7 @@ static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, 
   BIP_TRY(sliced_in(ctx, ctx->R2s, R2, fmt, e.n_det, w2, nb, "R2 (reconstructed S2 windows, sliced)"));
   BIP_TRY(sliced_in(ctx, ctx->Phis, Phi, fmt, rho_pad * e.n_ch, w2, nb, "Phi (H_n psi, sliced)"));
   const int64_t psi_ld = w2;
-  BIP_TRY(ensure(ctx, ctx->Psi, (size_t)nb * ctx->n_rho * psi_ld * sizeof(float2), "Psi (probe at the atom)"));
+  BIP_TRY(ensure(ctx, ctx->Psi, (size_t)nb * n_rows * psi_ld * sizeof(float2), "Psi (probe at the atom)"));
   const int64_t n_scale = (int64_t)nb * (R1t.rows_pad + R2.rows_pad + Phi.rows_pad);
   BIP_TRY(ensure(ctx, ctx->Scl, (size_t)n_scale * sizeof(float), "row scales"));
   R1t.scale = reinterpret_cast<float*>(ctx->Scl.p);           R1t.scale_batch_stride = R1t.rows_pad;
@@ -234,11 +284,11 @@ static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, 
                                 ctx->nn1, +1, recon, org, nb, e.w, R1t));
   // a3-a4: probe at the atom
   Gemm1SlArgs g1;
-  g1.A = ctx->A_sl; g1.R1t = R1t; g1.Psi = (float2*)ctx->Psi.p; g1.psi_ld = psi_ld; g1.psi_batch_stride = (int64_t)ctx->n_rho * psi_ld;
-  g1.n_rho = ctx->n_rho; g1.w2 = w2; g1.n_atoms = nb; g1.drop_tiny = drop_tiny;
+  g1.A = Ax; g1.R1t = R1t; g1.Psi = (float2*)ctx->Psi.p; g1.psi_ld = psi_ld; g1.psi_batch_stride = (int64_t)n_rows * psi_ld;
+  g1.n_rho = n_rows; g1.w2 = w2; g1.n_atoms = nb; g1.drop_tiny = drop_tiny;
   BIP_TRY(launch_gemm1_sliced(ctx, g1));
   // a5: times H_n, split into slices
-  BIP_TRY(launch_quantize_phi(ctx, g1.Psi, psi_ld, g1.psi_batch_stride, e.H_dev, Phi, ctx->n_rho, (int32_t)rho_pad, w2, e.n_ch, nb));
+  BIP_TRY(launch_quantize_phi(ctx, g1.Psi, psi_ld, g1.psi_batch_stride, e.H_dev, Phi, n_rows, (int32_t)rho_pad, w2, e.n_ch, nb));
   // a6: S2 windows -> R2[d][s]
   BIP_TRY(launch_crop_detilt(ctx, ctx->S2, ctx->p2_h_dev, ctx->n_p2, -1, org, nb, e.w, (float2*)ctx->D2.p));
   BIP_TRY(launch_recon_rows_sliced(ctx, (const float2*)ctx->D2.p, ctx->n_p2, e.det_h_dev, e.n_det, e.nn_idx_dev, e.nn_w_dev, e.max_nn,
@@ -246,7 +296,8 @@ static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, 
   // a7-a8: detector projection and reduction
   Gemm2SlArgs g2;
   g2.Phi = Phi; g2.R2 = R2; g2.rows_pad = (int32_t)rho_pad;
-  g2.n_rho = ctx->n_rho; g2.n_det = e.n_det; g2.n_ch = e.n_ch; g2.n_atoms = nb;
+  g2.n_rho = n_rows; g2.n_det = e.n_det; g2.n_ch = e.n_ch; g2.n_atoms = nb;
+  g2.row_idx = row_idx_dev; g2.row_idx_stride = rho_pad;
   g2.inv_G = (float)(1.0 / ((double)ctx->g.ny * ctx->g.nx));
   g2.mode = mode;
   g2.bin_of_det = mode == BIP_MODE_QEELS_X ? e.bin_of_det_x_dev : e.bin_of_det_y_dev;
@@ -257,8 +308,8 @@ static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, 
     BIP_TRY(launch_gemm2_sliced(ctx, g2));
   }
   ctx->timing.gemm2_launches++;
-  ctx->timing.amplitudes += (double)ctx->n_rho * nb * e.n_ch * e.n_det;
-  ctx->timing.flops += 8.0 * ctx->n_rho * w2 * ((double)nb * ctx->n_ap + (double)nb * e.n_ch * e.n_det);
+  ctx->timing.amplitudes += n_rows_total * e.n_ch * e.n_det;
+  ctx->timing.flops += 8.0 * n_rows_total * w2 * ((double)ctx->n_ap + (double)e.n_ch * e.n_det);
   return BIP_OK;
 }
 
@@ -268,7 +319,8 @@ static int32_t contract_batch(bip_ctx* ctx, Edge& e, const int32_t* origin_dev, 
   auto& sp = spans()[ctx];
   const int w2 = e.w * e.w;
   const int32_t* org = origin_dev + 2 * (int64_t)a0;
-  if (sliced_fmt_of(precision) >= 0) return contract_batch_sliced(ctx, e, org, nb, mode, recon, sliced_fmt_of(precision), precision == BIP_PREC_FP16X3, out);
+  if (sliced_fmt_of(precision) >= 0) return contract_batch_sliced(ctx, e, org, a0, nb, mode, recon, sliced_fmt_of(precision), precision == BIP_PREC_FP16X3, out);
+  if (ctx->crop_fy > 1 || ctx->crop_fx > 1) return fail(ctx, BIP_ERR_UNSUPPORTED, "bip_map: the crop mask needs a tensor-core precision (FP16X4, FP16X3, BF16X6)");
   Planes R1t, R2, Phi;
   BIP_TRY(ensure(ctx, ctx->D1, (size_t)nb * ctx->n_p1 * w2 * sizeof(float2), "D1 (de-tilted S1 windows)"));
   BIP_TRY(ensure(ctx, ctx->D2, (size_t)nb * ctx->n_p2 * w2 * sizeof(float2), "D2 (de-tilted S2 windows)"));
@@ -480,7 +532,7 @@ int32_t bip_destroy(bip_ctx* ctx) {
   if (ctx->T_owned) cudaFree((void*)ctx->T_dev);
   void* ptrs[] = {ctx->ap_h_dev, ctx->p1_h_dev, ctx->p2_h_dev, ctx->ap_c_dev, ctx->w1_idx_dev, ctx->w1_w_dev, ctx->rooty_dev,
                   ctx->rootx_dev, ctx->P_dev, ctx->ms_work, ctx->S1, ctx->S2, ctx->D1.p, ctx->D2.p, ctx->R1.p, ctx->R2.p, ctx->Psi.p,
-                  ctx->Phi.p, ctx->R1s.p, ctx->R2s.p, ctx->Phis.p, ctx->Scl.p, ctx->Sync.p, ctx->rho_dev};
+                  ctx->Phi.p, ctx->R1s.p, ctx->R2s.p, ctx->Phis.p, ctx->Scl.p, ctx->Sync.p, ctx->RowIdx.p, ctx->Acrop.p, ctx->rho_dev};
   free_illumination(ctx);
   for (void* p : ptrs) if (p) cudaFree(p);
   cudaGetLastError();
@@ -524,7 +576,28 @@ int32_t bip_set_scan(bip_ctx* ctx, int32_t n_rho, const double* rho_px) {
   BIP_CUDA(ctx, cudaMemcpyAsync(ctx->rho_dev, rho_px, sizeof(double) * 2 * n_rho, cudaMemcpyHostToDevice, ctx->stream));
   BIP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));      // the host array may go away after return
   ctx->n_rho = n_rho;
+  ctx->rho_host.assign(rho_px, rho_px + 2 * (size_t)n_rho);
   return BIP_OK;                                           // the illumination matrix (a3) is built on first use
+}
+
+int32_t bip_prism_subsample(int32_t n, const int32_t* h, int32_t fy, int32_t fx, int32_t* keep_out, int32_t cap, int32_t* n_keep) {
+  if (n < 0 || (n > 0 && !h) || fy < 1 || fx < 1 || !n_keep) return fail(nullptr, BIP_ERR_INVALID, "bip_prism_subsample: bad argument");
+  int32_t m = 0;
+  for (int32_t b = 0; b < n; ++b)
+    if (h[2 * b] % fy == 0 && h[2 * b + 1] % fx == 0) {
+      if (keep_out && m < cap) keep_out[m] = b;
+      ++m;
+    }
+  *n_keep = m;
+  if (keep_out && m > cap) return fail(nullptr, BIP_ERR_INVALID, "bip_prism_subsample: %d beams retained, capacity %d", m, cap);
+  return BIP_OK;
+}
+
+int32_t bip_set_crop(bip_ctx* ctx, int32_t fy, int32_t fx) {
+  if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
+  if (fy < 1 || fx < 1 || fy > ctx->g.ny / 2 || fx > ctx->g.nx / 2) return fail(ctx, BIP_ERR_INVALID, "bip_set_crop: factors (%d, %d) outside 1..N/2", fy, fx);
+  ctx->crop_fy = fy; ctx->crop_fx = fx;
+  return BIP_OK;
 }
 
 int32_t bip_add_edge(bip_ctx* ctx, int32_t n_atoms, const int32_t* slice, const int32_t* centre_px, int32_t n_ch, int32_t w,

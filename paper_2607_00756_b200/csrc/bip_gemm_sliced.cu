@@ -75,6 +75,7 @@ struct SlParams {
   float2* Psi; int64_t psi_ld, psi_batch_stride;
   // GEMM2 epilogue
   int mode; float inv_G; const int32_t* bin_of_det; int n_bins; void* out;
+  const int32_t* row_idx; int64_t row_idx_stride;   // crop mask: output scan index of every (site, local row), -1 = none
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -505,8 +506,13 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
       int atom, rt, ct;
       decode_item(p, item, atom, rt, ct);
       if (PAIR) rt = 2 * rt + (int)rank;               // the leader's TMEM holds the even row tile, the peer's the odd one
-      const int row = rt * TM + quarter * 32 + lane;   // this thread's rho
-      const bool row_ok = row < p.n_rows;
+      const int row = rt * TM + quarter * 32 + lane;   // this thread's rho (local row of the site under a crop mask)
+      bool row_ok = row < p.n_rows;
+      int out_row = row;
+      if (EPI == EPI_GEMM2 && p.row_idx) {
+        out_row = row_ok ? __ldg(p.row_idx + (int64_t)atom * p.row_idx_stride + row) : -1;
+        row_ok = out_row >= 0;
+      }
       const int col0 = ct * TN + half * 64;
       const float* sy = p.sy + (int64_t)atom * p.sy_batch_stride;
       float rowsum = 0.f;
@@ -562,8 +568,8 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
               if (d < p.n_cols) {
                 const float s = __ldg(sy + d);
                 const float v = fmaf(rr[j], rr[j], ri[j] * ri[j]) * (s * s) * f;
-                if (p.mode == BIP_MODE_CUBE) atomicAdd(out + (int64_t)row * p.n_cols + d, v);
-                else atomicAdd(out + (int64_t)row * p.n_bins + __ldg(p.bin_of_det + d), v);
+                if (p.mode == BIP_MODE_CUBE) atomicAdd(out + (int64_t)out_row * p.n_cols + d, v);
+                else atomicAdd(out + (int64_t)out_row * p.n_bins + __ldg(p.bin_of_det + d), v);
               }
             }
           }
@@ -584,7 +590,7 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
         }
       }
       if (EPI == EPI_GEMM2 && p.mode == BIP_MODE_MAP && row_ok)
-        atomicAdd(reinterpret_cast<double*>(p.out) + row, (double)rowsum * (double)p.inv_G);
+        atomicAdd(reinterpret_cast<double*>(p.out) + out_row, (double)rowsum * (double)p.inv_G);
     }
   }
 
@@ -630,6 +636,22 @@ __global__ void __launch_bounds__(256) k_quantize_phi(const float2* __restrict__
     }
     sl_store_group(Phi, atom, row, g, re, im, inv);
   }
+}
+
+// Crop mask: the illumination rows of every site's own scan positions, gathered from the shared
+// matrix A into a per-site X operand.  One thread per (site, local row, group of 8 beams); rows without a scan are zero.
+__global__ void __launch_bounds__(256) k_gather_rows_sliced(Sliced src, const int32_t* __restrict__ row_idx, int64_t idx_stride,
+                                                            Sliced dst, int n_groups) {
+  const int g = blockIdx.x * blockDim.x + threadIdx.x;
+  const int row = blockIdx.y, atom = blockIdx.z;
+  if (g >= n_groups) return;
+  const int s = row_idx[(int64_t)atom * idx_stride + row];
+  const int parts = sl_parts(src.fmt);
+  uint16_t* d = dst.base + (int64_t)atom * dst.batch_stride + sl_group_offset(dst, row, g);
+  const uint16_t* q = s >= 0 ? src.base + sl_group_offset(src, s, g) : nullptr;
+  for (int part = 0; part < parts; ++part)
+    *reinterpret_cast<uint4*>(d + part * SL_TILE_EL) = q ? *reinterpret_cast<const uint4*>(q + part * SL_TILE_EL) : make_uint4(0, 0, 0, 0);
+  if (g == 0) dst.scale[(int64_t)atom * dst.scale_batch_stride + row] = s >= 0 ? src.scale[s] : 1.f;
 }
 
 template <int EPI, int FMT, bool PAIR>
@@ -690,7 +712,7 @@ int32_t launch(bip_ctx* ctx, const SlParams& p, int fmt) {
 int32_t launch_gemm1_sliced(bip_ctx* ctx, const Gemm1SlArgs& a) {
   if (a.A.fmt != a.R1t.fmt) return fail(ctx, BIP_ERR_INVALID, "gemm1: operand formats differ");
   SlParams p{};
-  p.X = a.A.base; p.sx = a.A.scale; p.x_batch_stride = 0; p.sx_batch_stride = 0;
+  p.X = a.A.base; p.sx = a.A.scale; p.x_batch_stride = a.A.batch_stride; p.sx_batch_stride = a.A.scale_batch_stride;
   p.Y = a.R1t.base; p.sy = a.R1t.scale; p.y_batch_stride = a.R1t.batch_stride; p.sy_batch_stride = a.R1t.scale_batch_stride;
   p.ksteps = (int)a.A.ksteps;
   p.n_rt = (int)(a.A.rows_pad / TM);
@@ -701,6 +723,15 @@ int32_t launch_gemm1_sliced(bip_ctx* ctx, const Gemm1SlArgs& a) {
   p.n_rows = a.n_rho; p.n_cols = a.w2; p.rows_pad = (int)a.A.rows_pad;
   p.Psi = a.Psi; p.psi_ld = a.psi_ld; p.psi_batch_stride = a.psi_batch_stride;
   return launch<EPI_GEMM1>(ctx, p, a.A.fmt);
+}
+
+int32_t launch_gather_rows_sliced(bip_ctx* ctx, const Sliced& src, const int32_t* row_idx, int64_t idx_stride, const Sliced& dst, int32_t n_atoms) {
+  const int n_groups = 2 * (int)src.ksteps;
+  dim3 grid((unsigned)((n_groups + 255) / 256), (unsigned)dst.rows_pad, (unsigned)n_atoms);
+  k_gather_rows_sliced<<<grid, 256, 0, ctx->stream>>>(src, row_idx, idx_stride, dst, n_groups);
+  BIP_CUDA(ctx, cudaGetLastError());
+  ctx->timing.kernel_launches++;
+  return BIP_OK;
 }
 
 int32_t launch_quantize_phi(bip_ctx* ctx, const float2* Psi, int64_t psi_ld, int64_t psi_batch_stride, const float2* H,
@@ -726,6 +757,7 @@ int32_t launch_gemm2_sliced(bip_ctx* ctx, const Gemm2SlArgs& a) {
   p.drop_tiny = a.drop_tiny;
   p.n_rows = a.n_rho; p.n_cols = a.n_det;
   p.mode = a.mode; p.inv_G = a.inv_G; p.bin_of_det = a.bin_of_det; p.n_bins = a.n_bins; p.out = a.out;
+  p.row_idx = a.row_idx; p.row_idx_stride = a.row_idx_stride;
   return launch<EPI_GEMM2>(ctx, p, a.Phi.fmt);
 }
 

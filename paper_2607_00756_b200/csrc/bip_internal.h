@@ -90,6 +90,9 @@ struct bip_ctx {
   // scan
   int32_t n_rho = 0;
   double* rho_dev = nullptr;       // [n_rho][2] scan positions in pixels
+  std::vector<double> rho_host;    // the same on the host (crop-mask row lists)
+  int32_t crop_fy = 1, crop_fx = 1;  // PRISM crop mask (bip_set_crop); 1 = off
+  bip::DevBuf RowIdx, Acrop;       // per-site scan-row lists and gathered illumination rows (crop mask)
   bip::Planes A;                   // illumination [n_rho][n_ap] split planes (K-major over b); built on first use
   bip::Sliced A_sl;                // the same as a sliced 16-bit operand (format A_sl.fmt); built on first use
 
@@ -194,7 +197,10 @@ struct Gemm2SlArgs {     // a7 + a8
   int32_t n_bins;
   void* out;
   int32_t drop_tiny = 0; // BIP_PREC_FP16X3
+  const int32_t* row_idx = nullptr;   // crop mask: [atom][row_idx_stride] output scan index of each local row, -1 = none
+  int64_t row_idx_stride = 0;
 };
+int32_t launch_gather_rows_sliced(bip_ctx* ctx, const Sliced& src, const int32_t* row_idx, int64_t idx_stride, const Sliced& dst, int32_t n_atoms);
 int32_t launch_gemm1_sliced(bip_ctx* ctx, const Gemm1SlArgs& a);
 int32_t launch_gemm2_sliced(bip_ctx* ctx, const Gemm2SlArgs& a);
 int32_t launch_quantize_phi(bip_ctx* ctx, const float2* Psi, int64_t psi_ld, int64_t psi_batch_stride, const float2* H,
