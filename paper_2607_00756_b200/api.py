@@ -62,7 +62,8 @@ ABI_SYMBOLS = (
     "bip_beams_in_disc", "bip_aperture_coeffs", "bip_hexring", "bip_n_radial_from_factor", "bip_sibson", "bip_create",
     "bip_destroy", "bip_last_error", "bip_build_S1", "bip_build_S2", "bip_set_scan", "bip_add_edge", "bip_clear_edges",
     "bip_output_size", "bip_map", "bip_map_host", "bip_map_all", "bip_get_windows", "bip_get_qeels_bins",
-    "bip_seek_plane", "bip_copy_S", "bip_debug_reconstruct", "bip_get_timing", "bip_version",
+    "bip_seek_plane", "bip_copy_S", "bip_debug_reconstruct", "bip_get_timing", "bip_version", "bip_prism_subsample",
+    "bip_set_crop",
 )
 
 _lib: Optional[C.CDLL] = None
@@ -134,6 +135,15 @@ def bip_hexring(g: Grid, h: np.ndarray, qmax: float, n_radial: int, n_angular: i
     return pos[: n.value].copy()
 
 
+def bip_prism_subsample(h: np.ndarray, fy: int, fx: int) -> np.ndarray:
+    """Positions of the beams kept by PRISM subsampling (h_y = 0 mod fy, h_x = 0 mod fx)."""
+    h = _i32(h)
+    keep = np.empty(h.shape[0], dtype=np.int32)
+    n = C.c_int32(0)
+    _check(load_library().bip_prism_subsample(h.shape[0], _p(h, C.c_int32), int(fy), int(fx), _p(keep, C.c_int32), keep.shape[0], C.byref(n)))
+    return keep[: n.value].copy()
+
+
 def bip_sibson(g: Grid, h: np.ndarray, parent_h: np.ndarray, qmax: float, max_nn: int = 8) -> Tuple[np.ndarray, np.ndarray]:
     h, parent_h = _i32(h), _i32(parent_h)
     idx = np.empty((h.shape[0], max_nn), dtype=np.int32)
@@ -174,13 +184,19 @@ class Geometry:
 
 
 def plan_geometry(g: Grid, alpha_mrad: float, det_mrad: float, defocus: float, parent_factor: Sequence[float],
-                  max_nn: int = 8) -> Geometry:
+                  max_nn: int = 8, prism: Sequence[int] = (1, 1)) -> Geometry:
     """Aperture / detector beams (eq. 5), hex-ring parents and Sibson tables (eq. 8) through the
-    library's own helpers.  parent_factor f = 1 is the exactness limit: parents = all beams, w = I."""
+    library's own helpers.  parent_factor f = 1 is the exactness limit: parents = all beams, w = I.
+    ``prism`` = (f_y, f_x) keeps every f-th beam of both sets and rescales the probe coefficients by f_y f_x
+    (PAPER.md:129); parents and weights are then chosen among the retained beams."""
     qa, qd = alpha_mrad * 1e-3 / g.lam, det_mrad * 1e-3 / g.lam
     ap_h = bip_beams_in_disc(g, qa)
     det_h = bip_beams_in_disc(g, qd)
     ap_c = bip_aperture_coeffs(g, ap_h, defocus)
+    if tuple(prism) != (1, 1):
+        keep = bip_prism_subsample(ap_h, prism[0], prism[1])
+        ap_h, ap_c = ap_h[keep], (ap_c[keep] * np.float32(prism[0] * prism[1])).astype(np.float32)
+        det_h = det_h[bip_prism_subsample(det_h, prism[0], prism[1])]
 
     def part(h, q, f):
         if f == 1:
@@ -249,6 +265,10 @@ class Context:
         rho = np.ascontiguousarray(rho_px, dtype=np.float64)
         self._ck(self._lib.bip_set_scan(self._ctx, rho.shape[0], _p(rho, C.c_double)))
         self.n_rho = rho.shape[0]
+
+    def set_crop(self, fy: int, fx: int):
+        """PRISM crop mask: sites contribute only to the scans within N / (2 f) of them; (1, 1) = off."""
+        self._ck(self._lib.bip_set_crop(self._ctx, int(fy), int(fx)))
 
     def add_edge(self, slice_, centre_px, H, det_h, w2) -> int:
         slice_, centre_px, det_h = _i32(slice_), _i32(centre_px), _i32(det_h)

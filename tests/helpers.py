@@ -10,7 +10,7 @@ from oracle import sibson as osb
 class OracleSetup:
     """Everything the oracle derives from a workload edge: beams, parents, weights, coefficients, propagator."""
 
-    def __init__(self, wl, edge, parent_factor=None, n_jobs=1):
+    def __init__(self, wl, edge, parent_factor=None, n_jobs=1, prism=(1, 1)):
         f1, f2 = parent_factor if parent_factor is not None else wl.parent_factor
         ny, nx, ly, lx = wl.ny, wl.nx, wl.ly, wl.lx
         self.qa = wl.alpha_mrad * 1e-3 / wl.lam
@@ -19,6 +19,10 @@ class OracleSetup:
         self.det = ob.beams_in_disc(ny, nx, ly, lx, self.qd)
         self.c = ob.aperture_coefficients(self.ap, ny, nx, ly, lx, wl.lam, wl.defocus)
         self.P = oms.fresnel_propagator(ny, nx, ly, lx, wl.lam, wl.dz)
+        if tuple(prism) != (1, 1):                    # PRISM beam subsampling of both sets
+            keep = ob.prism_subsample(self.ap, *prism)
+            self.ap, self.c = self.ap[keep], ob.prism_coefficients(self.c, keep, *prism)
+            self.det = self.det[ob.prism_subsample(self.det, *prism)]
 
         def part(beams, q, f):
             if f == 1:
@@ -41,25 +45,26 @@ class OracleSetup:
         self.p1_pos, self.w1 = part(self.ap, self.qa, f1)
         self.p2_pos, self.w2 = part(self.det, self.qd, f2)
 
-    def run(self, wl, edge, recon="linear", scan=None):
+    def run(self, wl, edge, recon="linear", scan=None, crop_f=None):
         return obip.bip_run(wl.T.astype(np.complex128), self.P, self.ap, self.c, self.ap[self.p1_pos], self.w1, self.det,
                             self.det[self.p2_pos], self.w2, wl.scan if scan is None else scan, edge.slice, edge.centre,
-                            edge.H, recon=recon)
+                            edge.H, recon=recon, crop_f=crop_f)
 
 
-def gpu_context(wl, edges, parent_factor=None, max_nn=8, T_on_device=True):
+def gpu_context(wl, edges, parent_factor=None, max_nn=8, T_on_device=True, prism=(1, 1), crop=(1, 1)):
     """Create a library context for a workload; geometry comes from the library's own helpers.
     All edges must share the detector angle of edges[0] for the S2 parent set (as in every config here)."""
     import torch
     import paper_2607_00756_b200 as B
     g = B.Grid(wl.ny, wl.nx, wl.ly, wl.lx, wl.nz, wl.dz, wl.lam)
     pf = parent_factor if parent_factor is not None else wl.parent_factor
-    geo = B.plan_geometry(g, wl.alpha_mrad, edges[0].det_mrad, wl.defocus, pf, max_nn)
+    geo = B.plan_geometry(g, wl.alpha_mrad, edges[0].det_mrad, wl.defocus, pf, max_nn, prism=prism)
     T = torch.from_numpy(wl.T).cuda() if T_on_device else wl.T
     ctx = B.Context(g, T, geo.ap_h, geo.ap_c, geo.p1_h, geo.w1, geo.p2_h)
     ctx.build_S1()
     ctx.build_S2()
     ctx.set_scan(wl.scan)
+    ctx.set_crop(*crop)
     ids = [ctx.add_edge(e.slice, e.centre, e.H, geo.det_h, geo.w2) for e in edges]
     return ctx, geo, ids
 

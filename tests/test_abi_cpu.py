@@ -118,3 +118,12 @@ def test_argument_validation_and_no_cpu_fallback():
         with pytest.raises(B.BipError) as ei:
             B.Context(g, T, geo.ap_h, geo.ap_c, geo.p1_h, geo.w1, geo.p2_h, stream=0)
         assert ei.value.status == 4 and "no CPU path" in str(ei.value)           # fails loudly: no fallback
+
+
+def test_prism_subsample_matches_oracle():
+    """bip_prism_subsample against the oracle's rule, bit-exact, incl. negative indices."""
+    import paper_2607_00756_b200 as B
+    from oracle import beams as ob
+    beams = ob.beams_in_disc(64, 48, 20.0, 15.0, 0.9)
+    for fy, fx in ((1, 1), (2, 2), (4, 3), (5, 1)):
+        assert np.array_equal(B.bip_prism_subsample(beams, fy, fx), ob.prism_subsample(beams, fy, fx))

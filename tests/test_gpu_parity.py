@@ -248,3 +248,45 @@ def test_full_size_cfg2_sampled_pixels(prec_name):
     t = ctx.get_timing()
     assert t["amplitudes"] == 4096 * 2 * 9 * 79105
     ctx.close()
+
+
+@pytest.mark.parametrize("prec_name", ["fp16x4", "bf16x6"])
+def test_prism_subsampling_and_crop_mask(prec_name):
+    """NEXT-1: configs[0] geometry with PRISM f = 2 beam lists (coefficients x 4) and the crop
+    mask at f = 4 -- every site contributes to the scans within N/8 of it only, its contraction runs over those rows alone.
+    Ragged on purpose: 25 x 25 scan with sub-pixel positions, so the sites see different numbers of scan rows."""
+    import torch
+    import paper_2607_00756_b200 as B
+    wl = make_workload("cfg1", nz=4, scan=(25, 25))
+    wl.scan = wl.scan + np.array([0.37, 0.21])
+    e = wl.edges[0].take(np.array([0, 1, 2, 17, 30]))
+    orc = OracleSetup(wl, e, prism=(2, 2))
+    want = orc.run(wl, e, "magphase", crop_f=(4, 4))
+    ctx, geo, ids = gpu_context(wl, [e], prism=(2, 2), crop=(4, 4))
+    assert np.array_equal(geo.ap_h, orc.ap) and np.array_equal(geo.det_h, orc.det)                    # bit-exact beam lists
+    assert np.array_equal(geo.p1_h, orc.ap[orc.p1_pos]) and np.array_equal(geo.p2_h, orc.det[orc.p2_pos])
+    assert np.abs(geo.ap_c.view(np.complex64).ravel() - orc.c).max() <= 1e-6 * np.abs(orc.c).max()
+    prec = _prec(prec_name)
+    m = _first(lambda: ctx.map(0, B.MODE_MAP, B.RECON_MAGPHASE, prec))
+    qx = ctx.map(0, B.MODE_QEELS_X, B.RECON_MAGPHASE, prec)
+    cube = ctx.map(0, B.MODE_CUBE, B.RECON_MAGPHASE, prec)
+    torch.cuda.synchronize()
+    m, qx, cube = m.cpu().numpy(), qx.cpu().numpy(), cube.cpu().numpy()
+    lit = want["map"] > 0
+    assert lit.any() and (~lit).any() and np.all(m[~lit] == 0.0)              # scans outside every window: exactly zero
+    assert rel_err_map(m, want["map"], 1e-3) <= TOL_PIXEL
+    assert abs(m.sum() - want["map"].sum()) <= TOL_SUM * want["map"].sum()
+    assert rel_err_map(qx, want["qeels_x"], 1e-3) <= TOL_PIXEL and rel_err_map(cube, want["cube"], 1e-3) <= TOL_PIXEL
+    # the mask cut the work: amplitudes counted = sum over sites of their own scan rows
+    from oracle import beams as ob
+    rows = sum(int(ob.crop_mask(wl.scan, c, wl.ny, wl.nx, 4, 4).sum()) for c in e.centre)
+    assert ctx.get_timing()["amplitudes"] == rows * e.n_ch * geo.det_h.shape[0] and rows < 5 * 625
+    with pytest.raises(B.BipError) as ei:
+        ctx.map(0, B.MODE_MAP, B.RECON_MAGPHASE, B.PREC_FP32_SIMT)                # crop mask: tensor-core precisions only
+    assert ei.value.status == 5
+    ctx.set_crop(1, 1)                                                            # mask off again: the unmasked map
+    full = orc.run(wl, e, "magphase")["map"]
+    m2 = ctx.map(0, B.MODE_MAP, B.RECON_MAGPHASE, prec)
+    torch.cuda.synchronize()
+    assert rel_err_map(m2.cpu().numpy(), full) <= TOL_PIXEL
+    ctx.close()
