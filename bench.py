@@ -37,7 +37,7 @@ sys.path.insert(0, ROOT)
 sys.path.insert(0, os.path.join(ROOT, "tests"))
 
 METRIC = "scan-pos x atom x channel x detector-beam amplitudes/s"
-CONFIG_INDEX = {"cfg1": 0, "cfg2": 1, "cfg3": 2, "cfg5": 4}
+CONFIG_INDEX = {"cfg1": 0, "cfg2": 1, "cfg3": 2, "cfg4": 3, "cfg5": 4}
 UNIT = "amplitudes/s"
 SM_COUNT, FMA_LANES, = 148, 128
 
@@ -143,12 +143,13 @@ def run_ours(args):
     wl, edges = build_problem(args, rank)
     edge = edges[0]
     g = B.Grid(wl.ny, wl.nx, wl.ly, wl.lx, wl.nz, wl.dz, wl.lam)
-    geo = B.plan_geometry(g, wl.alpha_mrad, edge.det_mrad, wl.defocus, wl.parent_factor)
+    geo = B.plan_geometry(g, wl.alpha_mrad, edge.det_mrad, wl.defocus, wl.parent_factor, prism=wl.prism)
     T_dev = torch.from_numpy(wl.T).cuda()
     ctx = B.Context(g, T_dev, geo.ap_h, geo.ap_c, geo.p1_h, geo.w1, geo.p2_h)
     ctx.build_S1()
     ctx.build_S2()
     ctx.set_scan(wl.scan)
+    ctx.set_crop(*wl.crop)                           # PRISM crop mask of the workload ((1, 1) = none)
     eids = [ctx.add_edge(e.slice, e.centre, e.H, geo.det_h, geo.w2) for e in edges]
     torch.cuda.synchronize()
     t_build = ctx.get_timing()
@@ -187,7 +188,7 @@ def run_ours(args):
     clocks = sampler.stop() if rank == 0 else None
     ms_total = ev0.elapsed_time(ev1)
     ms_total = max_over_ranks(ms_total, world)
-    amps_step = float(ctx.n_rho) * K * sum(e.n_atoms * e.n_ch for e in edges)
+    amps_step = float(ctx.get_timing()["amplitudes"])          # scan rows actually contracted (crop mask) x channels x beams
     value = amps_step * world * args.steps / (ms_total * 1e-3)
     map_dev = outs[0][0].cpu().numpy()
     out_bytes = sum(o.numel() * o.element_size() for o in outs[0])
@@ -223,7 +224,7 @@ def run_ours(args):
     assert np.allclose(m_host, map_dev, rtol=1e-5, atol=1e-6 * float(np.abs(map_dev).max())), "host-buffer path disagrees with the device path"
 
     # ---- roofline of the dominant kernel (a7-a8) ----
-    flops_gemm2_step = 8.0 * ctx.n_rho * K * sum(e.W * e.W * e.n_atoms * e.n_ch for e in edges)
+    flops_gemm2_step = 8.0 * edge.W * edge.W * amps_step          # a7: 8 W^2 real flops per amplitude (every edge here has the same W)
     achieved = flops_gemm2_step * args.steps / (gemm2_ms * 1e-3) / 1e12 if gemm2_ms > 0 else 0.0
     if args.precision in ("fp16x4", "fp16x3", "bf16x6"):
         bf16_peak = peaks["bf16_tflops"]           # burst figure: the larger, hence the conservative denominator

@@ -76,6 +76,8 @@ class Workload:
     scan: np.ndarray       # float64 [n_rho, 2] (py, px) in pixels
     scan_shape: Tuple[int, int]
     edges: List[Edge]
+    prism: Tuple[int, int] = (1, 1)      # PRISM beam subsampling (f_y, f_x) of aperture and detector sets
+    crop: Tuple[int, int] = (1, 1)       # PRISM crop mask factors; (1, 1) = no mask
 
     @property
     def n_rho(self) -> int:
@@ -152,6 +154,62 @@ def _perovskite(cells_y, cells_x, cells_z, a, ZA_of_col, ZB_of_col, ZO):
     return f(Z, np.float64), f(Y, np.float64), f(X, np.float64), f(S, np.int32), f(TAG, np.int32), f(COL, np.int32)
 
 
+def _fept_sphere(cell_y, cell_x, cell_z, radius, a, c):
+    """FePt L1_0 (Fe at (0,0,0), (1/2,1/2,0); Pt at (1/2,0,1/2), (0,1/2,1/2); a = b, c along the beam), the lattice
+    sites within ``radius`` of the cell centre.  The lattice is placed so that no atomic plane sits on a slice
+    boundary: planes are c/2 = 1.855 A apart against 2 A slices, and with the centre plane 1.505 A above the cell's
+    mid-height every plane within the sphere stays >= 0.04 A away from a boundary (c11 then assigns slices safely).
+    Returns Z, y, x, z (Angstrom) and tag (0 = Fe, 1 = Pt)."""
+    cy, cx, cz = 0.5 * cell_y, 0.5 * cell_x, 0.5 * cell_z + 1.505
+    n = int(math.ceil(radius / min(a, c))) + 1
+    Z, Y, X, Zc, TAG = [], [], [], [], []
+    basis = ((26, 0.0, 0.0, 0.0, 0), (26, 0.5, 0.5, 0.0, 0), (78, 0.5, 0.0, 0.5, 1), (78, 0.0, 0.5, 0.5, 1))
+    for kz in range(-n, n + 1):
+        for ky in range(-n, n + 1):
+            for kx in range(-n, n + 1):
+                for z_, fy, fx, fz, tag in basis:
+                    dy, dx, dz_ = (ky + fy) * a, (kx + fx) * a, (kz + fz) * c
+                    if dy * dy + dx * dx + dz_ * dz_ <= radius * radius:
+                        Z.append(z_); Y.append(cy + dy); X.append(cx + dx); Zc.append(cz + dz_); TAG.append(tag)
+    f = lambda v, t: np.asarray(v, dtype=t)
+    return f(Z, np.float64), f(Y, np.float64), f(X, np.float64), f(Zc, np.float64), f(TAG, np.int32)
+
+
+def _make_fept(name, rc, scale, nz, scan, parent_factor, h_kind, window) -> Workload:
+    """BASELINE.json configs[3] in the paper's own regime (PRISM f, crop mask: "4-prism" of SURVEY 8(d))."""
+    gy, gx = rc["grid"]
+    if gy % scale or gx % scale:
+        raise ValueError("scale must divide the grid")
+    gy, gx = gy // scale, gx // scale
+    ly, lx, lz = rc["cell"][0] / scale, rc["cell"][1] / scale, rc["cell"][2]
+    dz = rc["dz"]
+    nz_full = int(round(lz / dz))
+    nz_use = nz_full if nz is None else int(nz)
+    if not 1 <= nz_use <= nz_full:
+        raise ValueError("nz out of range")
+    kv = rc["kv"]
+    lam, sigma = electron_wavelength(kv), interaction_constant(kv)
+    rng = np.random.default_rng(rc["seed"])
+    Z, Y, X, Zc, TAG = _fept_sphere(ly, lx, lz, rc["radius"] / scale, rc["a"], rc["c"])
+    S = np.minimum(nz_full - 1, np.floor(Zc / dz).astype(np.int64)).astype(np.int32)     # c11
+    keep = S < nz_use
+    Z, Y, X, Zc, TAG, S = Z[keep], Y[keep], X[keep], Zc[keep], TAG[keep], S[keep]
+    T = transmission_functions(gy, gx, ly, lx, nz_use, sigma, Z, Y, X, S)
+    edges = []
+    for e in rc["edges"]:
+        idx = np.nonzero(TAG == e["tag"])[0]
+        sl, centre = snap_sites(Y[idx], X[idx], Zc[idx], gy, gx, ly, lx, nz_use, dz)
+        W = int(window) if window is not None else e["W"]
+        H = transition_windows(rng, e["n_ch"], W, h_kind)
+        order = np.argsort(sl, kind="stable")
+        edges.append(Edge(e["name"], sl[order], centre[order], H, e["det"]))
+    sy, sx = scan if scan is not None else (max(1, rc["scan"][0] // scale), max(1, rc["scan"][1] // scale))
+    pf = tuple(parent_factor) if parent_factor is not None else tuple(rc["parent_factor"])
+    return Workload(name=f"{name}/s{scale}", ny=gy, nx=gx, ly=ly, lx=lx, nz=nz_use, dz=dz, kv=kv, lam=lam, sigma=sigma,
+                    alpha_mrad=rc["alpha"], defocus=rc["defocus"], parent_factor=pf, T=T, scan=_scan_grid(gy, gx, sy, sx),
+                    scan_shape=(sy, sx), edges=edges, prism=tuple(rc["prism"]), crop=tuple(rc["crop"]))
+
+
 def _scan_grid(ny, nx, sy, sx):
     """rho_ij = (i N_y / S_y, j N_x / S_x) px, row-major."""
     iy, ix = np.meshgrid(np.arange(sy), np.arange(sx), indexing="ij")
@@ -178,6 +236,11 @@ CONFIGS: Dict[str, dict] = {
                         dict(name="B_right", tag=1, side=1, n_ch=9, W=48, det=40.0),
                         dict(name="A_left", tag=0, side=0, n_ch=9, W=48, det=40.0),
                         dict(name="A_right", tag=0, side=1, n_ch=9, W=48, det=40.0)]),
+    # BASELINE.json configs[3]: FePt L1_0 nanoparticle in vacuum, in the regime the paper ran it (PRISM f = 8 beam lists,
+    # n_radial = 8 -> 217 + 217 parents, crop mask f = 8 -> 32 x 32 scans per atom; SURVEY §8(d) "4-prism")
+    "cfg4": dict(seed=75604, kind="fept", cell=(120.0, 120.0, 90.0), dz=2.0, radius=42.0, a=3.85, c=3.71, grid=(2048, 2048),
+                 kv=300.0, alpha=25.0, defocus=0.0, parent_factor=(2.4, 2.4), prism=(8, 8), crop=(8, 8), scan=(256, 256),
+                 edges=[dict(name="Fe", tag=0, n_ch=9, W=64, det=25.0)]),
     # BASELINE.json configs[4]: config-2 pixel size on 10x10x20 cells (SURVEY §8(d) cfg 5)
     "cfg5": dict(seed=75605, kind="perovskite", cells=(10, 10, 20), a=3.905, grid=(256, 256), kv=300.0, alpha=25.0,
                  defocus=-50.0, jitter=0.0, ZA=(38, 38), ZB=(22, 22), ZO=8, parent_factor=(4.0, 4.0),
@@ -191,6 +254,8 @@ def make_workload(name: str, scale: int = 1, nz: Optional[int] = None, scan: Opt
     """Instantiate a config.  ``scale`` shrinks cells and grid together (pixel size kept), ``nz`` truncates
     the slab to its first ``nz`` slices, ``scan`` overrides the scan raster, ``window`` overrides W."""
     rc = CONFIGS[name]
+    if rc["kind"] == "fept":
+        return _make_fept(name, rc, scale, nz, scan, parent_factor, h_kind, window)
     cy, cx, cz = rc["cells"]
     gy, gx = rc["grid"]
     if cy % scale or cx % scale or gy % scale or gx % scale:

@@ -210,32 +210,6 @@ static size_t scratch_budget() {
 }
 
 // Steps a1-a8 on the sliced 16-bit operands (BIP_PREC_FP16X4 / BIP_PREC_BF16X6).
-// PRISM crop mask (reading c19): the scan rows of each site of the batch, [nb][stride] with -1 padding.
-// The arithmetic is the oracle's, in the same order, in fp64: d = ((rho - c + N/2) mod N) - N/2, |d| < N / (2 f).
-static void crop_row_lists(const bip_ctx* ctx, const Edge& e, int32_t a0, int32_t nb, std::vector<int32_t>& rows, int32_t& n_rows_max,
-                           int64_t& stride, double& n_rows_total) {
-  const int ny = ctx->g.ny, nx = ctx->g.nx;
-  std::vector<std::vector<int32_t>> lists(nb);
-  n_rows_max = 0; n_rows_total = 0;
-  for (int32_t a = 0; a < nb; ++a) {
-    const double cy = (e.origin[2 * (size_t)(a0 + a)] + e.w / 2) % ny, cx = (e.origin[2 * (size_t)(a0 + a) + 1] + e.w / 2) % nx;
-    for (int32_t r = 0; r < ctx->n_rho; ++r) {
-      double dy = std::fmod(ctx->rho_host[2 * (size_t)r] - cy + ny / 2.0, (double)ny);
-      double dx = std::fmod(ctx->rho_host[2 * (size_t)r + 1] - cx + nx / 2.0, (double)nx);
-      if (dy < 0) dy += ny;
-      if (dx < 0) dx += nx;
-      dy -= ny / 2.0; dx -= nx / 2.0;
-      if (std::fabs(dy) < ny / (2.0 * ctx->crop_fy) && std::fabs(dx) < nx / (2.0 * ctx->crop_fx)) lists[a].push_back(r);
-    }
-    n_rows_max = std::max<int32_t>(n_rows_max, (int32_t)lists[a].size());
-    n_rows_total += (double)lists[a].size();
-  }
-  n_rows_max = std::max(n_rows_max, 1);
-  stride = round_up(n_rows_max, 2 * SL_ROWS);
-  rows.assign((size_t)nb * stride, -1);
-  for (int32_t a = 0; a < nb; ++a) std::copy(lists[a].begin(), lists[a].end(), rows.begin() + (size_t)a * stride);
-}
-
 static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, int32_t a0, int32_t nb, int mode, int recon, int fmt, bool drop_tiny, void* out) {
   auto& sp = spans()[ctx];
   const int w2 = e.w * e.w;
@@ -244,15 +218,24 @@ static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, 
   int32_t n_rows = ctx->n_rho;
   double n_rows_total = (double)ctx->n_rho * nb;
   const int32_t* row_idx_dev = nullptr;
+  int64_t row_idx_stride = 0;
   int64_t rho_pad = round_up(ctx->n_rho, 2 * SL_ROWS);    // X operands are padded to pairs of row tiles (CTA-pair kernel)
   Sliced Ax = ctx->A_sl;
   if (crop) {
-    std::vector<int32_t> rows;
-    crop_row_lists(ctx, e, a0, nb, rows, n_rows, rho_pad, n_rows_total);
-    BIP_TRY(ensure(ctx, ctx->RowIdx, rows.size() * sizeof(int32_t), "crop-mask row lists"));
-    BIP_CUDA(ctx, cudaMemcpyAsync(ctx->RowIdx.p, rows.data(), rows.size() * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream));
-    BIP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));          // `rows` goes out of scope
-    row_idx_dev = reinterpret_cast<const int32_t*>(ctx->RowIdx.p);
+    // per-site scan-row lists on the device (k_crop_rows), their lengths back on the host
+    const int64_t idx_stride = round_up(ctx->n_rho, 2 * SL_ROWS);
+    BIP_TRY(ensure(ctx, ctx->RowIdx, ((size_t)nb * idx_stride + nb) * sizeof(int32_t), "crop-mask row lists"));
+    int32_t* rows_dev = reinterpret_cast<int32_t*>(ctx->RowIdx.p);
+    int32_t* counts_dev = rows_dev + (size_t)nb * idx_stride;
+    BIP_TRY(launch_crop_rows(ctx, org, nb, e.w, rows_dev, idx_stride, counts_dev));
+    std::vector<int32_t> counts(nb);
+    BIP_CUDA(ctx, cudaMemcpyAsync(counts.data(), counts_dev, nb * sizeof(int32_t), cudaMemcpyDeviceToHost, ctx->stream));
+    BIP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    n_rows = 1; n_rows_total = 0;
+    for (int32_t c : counts) { n_rows = std::max(n_rows, c); n_rows_total += c; }
+    rho_pad = round_up(n_rows, 2 * SL_ROWS);
+    row_idx_dev = rows_dev;
+    row_idx_stride = idx_stride;
     Sliced Ac = ctx->A_sl;
     Ac.rows = n_rows; Ac.rows_pad = rho_pad;
     Ac.batch_stride = rho_pad / SL_ROWS * Ac.ksteps * sl_step_el(fmt);
@@ -261,7 +244,7 @@ static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, 
     BIP_TRY(ensure(ctx, ctx->Acrop, op_bytes + sc_bytes, "illumination rows of the cropped scans"));
     Ac.base = reinterpret_cast<uint16_t*>(ctx->Acrop.p);
     Ac.scale = reinterpret_cast<float*>(reinterpret_cast<char*>(ctx->Acrop.p) + op_bytes);
-    BIP_TRY(launch_gather_rows_sliced(ctx, ctx->A_sl, row_idx_dev, rho_pad, Ac, nb));
+    BIP_TRY(launch_gather_rows_sliced(ctx, ctx->A_sl, row_idx_dev, row_idx_stride, Ac, nb));
     Ax = Ac;
   }
   Sliced R1t, R2, Phi;
@@ -297,7 +280,7 @@ static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, 
   Gemm2SlArgs g2;
   g2.Phi = Phi; g2.R2 = R2; g2.rows_pad = (int32_t)rho_pad;
   g2.n_rho = n_rows; g2.n_det = e.n_det; g2.n_ch = e.n_ch; g2.n_atoms = nb;
-  g2.row_idx = row_idx_dev; g2.row_idx_stride = rho_pad;
+  g2.row_idx = row_idx_dev; g2.row_idx_stride = row_idx_stride;
   g2.inv_G = (float)(1.0 / ((double)ctx->g.ny * ctx->g.nx));
   g2.mode = mode;
   g2.bin_of_det = mode == BIP_MODE_QEELS_X ? e.bin_of_det_x_dev : e.bin_of_det_y_dev;
@@ -416,9 +399,13 @@ static int32_t run_edges(bip_ctx* ctx, const std::vector<int32_t>& ids, int mode
       if (lo == hi) continue;
       const int64_t w2 = (int64_t)e.w * e.w;
       const int64_t el = sliced_fmt_of(precision) == SL_FMT_FP16X4 ? 8 : precision == BIP_PREC_BF16X6 ? 12 : 16;      // operand bytes per complex element
-      const size_t per_atom = (size_t)((ctx->n_p1 + ctx->n_p2) * w2 * 8 + (int64_t)ctx->n_rho * w2 * 8 +
+      // scan rows per site: all of them, or (crop mask) about n_rho / (f_y f_x) -- an estimate for the batch size only
+      const int64_t rows_est = ctx->crop_fy * ctx->crop_fx > 1
+                                   ? std::min<int64_t>(ctx->n_rho, (int64_t)(1.5 * ctx->n_rho / (ctx->crop_fy * ctx->crop_fx)) + 2 * SL_ROWS) : ctx->n_rho;
+      const size_t per_atom = (size_t)((ctx->n_p1 + ctx->n_p2) * w2 * 8 + rows_est * w2 * 8 +
                                        el * (round_up(w2, 128) * round_up(ctx->n_ap, 32) + round_up(e.n_det, 128) * round_up(w2, 32) +
-                                             round_up(ctx->n_rho, 256) * e.n_ch * round_up(w2, 32)));
+                                             round_up(rows_est, 256) * (e.n_ch * round_up(w2, 32) + round_up(ctx->n_ap, 32))) +
+                                       (ctx->crop_fy * ctx->crop_fx > 1 ? round_up(ctx->n_rho, 256) * 4 : 0));
       const int32_t nb_max = (int32_t)std::max<size_t>(1, std::min<size_t>(budget / std::max<size_t>(per_atom, 1), 4096));
       Span s(ctx, sp.pool_map, sp.contract);
       for (int32_t a0 = (int32_t)lo; a0 < (int32_t)hi; a0 += nb_max)     // lines 5-8

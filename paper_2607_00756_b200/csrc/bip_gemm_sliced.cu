@@ -654,6 +654,46 @@ __global__ void __launch_bounds__(256) k_gather_rows_sliced(Sliced src, const in
   if (g == 0) dst.scale[(int64_t)atom * dst.scale_batch_stride + row] = s >= 0 ? src.scale[s] : 1.f;
 }
 
+// Crop mask (reading c19): the scan rows of every site, in ascending scan order.  One block per site walks
+// the scan list in chunks of 256 with an ordered block compaction.  fp64, the oracle's expression order:
+// d = ((rho - c + N/2) mod N) - N/2, inside iff |d_y| < N_y / (2 f_y) and |d_x| < N_x / (2 f_x).
+__global__ void __launch_bounds__(256) k_crop_rows(const double* __restrict__ rho, int n_rho, const int32_t* __restrict__ origin, int w,
+                                                   int ny, int nx, int fy, int fx, int32_t* __restrict__ row_idx, int64_t idx_stride,
+                                                   int32_t* __restrict__ counts) {
+  __shared__ int warp_sum[8];
+  __shared__ int base;
+  const int atom = blockIdx.x, lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const double cy = (double)((origin[2 * atom] + w / 2) % ny), cx = (double)((origin[2 * atom + 1] + w / 2) % nx);
+  const double hy = ny / (2.0 * fy), hx = nx / (2.0 * fx);
+  int32_t* out = row_idx + (int64_t)atom * idx_stride;
+  if (threadIdx.x == 0) base = 0;
+  __syncthreads();
+  for (int r0 = 0; r0 < n_rho; r0 += 256) {
+    const int r = r0 + threadIdx.x;
+    bool in = false;
+    if (r < n_rho) {
+      double dy = fmod(rho[2 * (int64_t)r] - cy + ny / 2.0, (double)ny);
+      double dx = fmod(rho[2 * (int64_t)r + 1] - cx + nx / 2.0, (double)nx);
+      if (dy < 0) dy += ny;
+      if (dx < 0) dx += nx;
+      dy -= ny / 2.0; dx -= nx / 2.0;
+      in = fabs(dy) < hy && fabs(dx) < hx;
+    }
+    const unsigned m = __ballot_sync(0xffffffffu, in);
+    if (lane == 0) warp_sum[wid] = __popc(m);
+    __syncthreads();
+    int off = base;
+    for (int k = 0; k < wid; ++k) off += warp_sum[k];
+    if (in) out[off + __popc(m & ((1u << lane) - 1u))] = r;
+    __syncthreads();
+    if (threadIdx.x == 0) { int t = 0; for (int k = 0; k < 8; ++k) t += warp_sum[k]; base += t; }
+    __syncthreads();
+  }
+  const int n = base;
+  for (int64_t i = n + threadIdx.x; i < idx_stride; i += 256) out[i] = -1;
+  if (threadIdx.x == 0) counts[atom] = n;
+}
+
 template <int EPI, int FMT, bool PAIR>
 int32_t launch_fmt(bip_ctx* ctx, const SlParams& p) {
   static bool attr_set = false;
@@ -723,6 +763,14 @@ int32_t launch_gemm1_sliced(bip_ctx* ctx, const Gemm1SlArgs& a) {
   p.n_rows = a.n_rho; p.n_cols = a.w2; p.rows_pad = (int)a.A.rows_pad;
   p.Psi = a.Psi; p.psi_ld = a.psi_ld; p.psi_batch_stride = a.psi_batch_stride;
   return launch<EPI_GEMM1>(ctx, p, a.A.fmt);
+}
+
+int32_t launch_crop_rows(bip_ctx* ctx, const int32_t* origin_dev, int32_t n_atoms, int32_t w, int32_t* row_idx, int64_t idx_stride, int32_t* counts) {
+  k_crop_rows<<<(unsigned)n_atoms, 256, 0, ctx->stream>>>(ctx->rho_dev, ctx->n_rho, origin_dev, w, ctx->g.ny, ctx->g.nx, ctx->crop_fy,
+                                                          ctx->crop_fx, row_idx, idx_stride, counts);
+  BIP_CUDA(ctx, cudaGetLastError());
+  ctx->timing.kernel_launches++;
+  return BIP_OK;
 }
 
 int32_t launch_gather_rows_sliced(bip_ctx* ctx, const Sliced& src, const int32_t* row_idx, int64_t idx_stride, const Sliced& dst, int32_t n_atoms) {

@@ -200,6 +200,7 @@ struct Gemm2SlArgs {     // a7 + a8
   const int32_t* row_idx = nullptr;   // crop mask: [atom][row_idx_stride] output scan index of each local row, -1 = none
   int64_t row_idx_stride = 0;
 };
+int32_t launch_crop_rows(bip_ctx* ctx, const int32_t* origin_dev, int32_t n_atoms, int32_t w, int32_t* row_idx, int64_t idx_stride, int32_t* counts);
 int32_t launch_gather_rows_sliced(bip_ctx* ctx, const Sliced& src, const int32_t* row_idx, int64_t idx_stride, const Sliced& dst, int32_t n_atoms);
 int32_t launch_gemm1_sliced(bip_ctx* ctx, const Gemm1SlArgs& a);
 int32_t launch_gemm2_sliced(bip_ctx* ctx, const Gemm2SlArgs& a);

@@ -10,7 +10,7 @@ from oracle import sibson as osb
 class OracleSetup:
     """Everything the oracle derives from a workload edge: beams, parents, weights, coefficients, propagator."""
 
-    def __init__(self, wl, edge, parent_factor=None, n_jobs=1, prism=(1, 1)):
+    def __init__(self, wl, edge, parent_factor=None, n_jobs=1, prism=None):
         f1, f2 = parent_factor if parent_factor is not None else wl.parent_factor
         ny, nx, ly, lx = wl.ny, wl.nx, wl.ly, wl.lx
         self.qa = wl.alpha_mrad * 1e-3 / wl.lam
@@ -19,7 +19,8 @@ class OracleSetup:
         self.det = ob.beams_in_disc(ny, nx, ly, lx, self.qd)
         self.c = ob.aperture_coefficients(self.ap, ny, nx, ly, lx, wl.lam, wl.defocus)
         self.P = oms.fresnel_propagator(ny, nx, ly, lx, wl.lam, wl.dz)
-        if tuple(prism) != (1, 1):                    # PRISM beam subsampling of both sets
+        prism = tuple(prism) if prism is not None else tuple(getattr(wl, 'prism', (1, 1)))
+        if prism != (1, 1):                           # PRISM beam subsampling of both sets
             keep = ob.prism_subsample(self.ap, *prism)
             self.ap, self.c = self.ap[keep], ob.prism_coefficients(self.c, keep, *prism)
             self.det = self.det[ob.prism_subsample(self.det, *prism)]
@@ -51,13 +52,15 @@ class OracleSetup:
                             edge.H, recon=recon, crop_f=crop_f)
 
 
-def gpu_context(wl, edges, parent_factor=None, max_nn=8, T_on_device=True, prism=(1, 1), crop=(1, 1)):
+def gpu_context(wl, edges, parent_factor=None, max_nn=8, T_on_device=True, prism=None, crop=None):
     """Create a library context for a workload; geometry comes from the library's own helpers.
     All edges must share the detector angle of edges[0] for the S2 parent set (as in every config here)."""
     import torch
     import paper_2607_00756_b200 as B
     g = B.Grid(wl.ny, wl.nx, wl.ly, wl.lx, wl.nz, wl.dz, wl.lam)
     pf = parent_factor if parent_factor is not None else wl.parent_factor
+    prism = tuple(prism) if prism is not None else tuple(getattr(wl, 'prism', (1, 1)))
+    crop = tuple(crop) if crop is not None else tuple(getattr(wl, 'crop', (1, 1)))
     geo = B.plan_geometry(g, wl.alpha_mrad, edges[0].det_mrad, wl.defocus, pf, max_nn, prism=prism)
     T = torch.from_numpy(wl.T).cuda() if T_on_device else wl.T
     ctx = B.Context(g, T, geo.ap_h, geo.ap_c, geo.p1_h, geo.w1, geo.p2_h)

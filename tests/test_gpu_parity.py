@@ -290,3 +290,26 @@ def test_prism_subsampling_and_crop_mask(prec_name):
     torch.cuda.synchronize()
     assert rel_err_map(m2.cpu().numpy(), full) <= TOL_PIXEL
     ctx.close()
+
+
+def test_cfg4_fept_quarter_clone_prism_regime():
+    """BASELINE.json configs[3] (FePt L1_0 nanoparticle in vacuum) as a quarter-size clone in the paper's regime: 512^2
+    grid over 30 A, PRISM f = 8 beam lists, hex-ring parents, crop mask f = 8 (8 x 8 of the 64 x 64 scans per Fe site),
+    9 channels on 64 x 64 windows; first 20 slices, which hold the lower part of the particle."""
+    import torch
+    import paper_2607_00756_b200 as B
+    wl = make_workload("cfg4", scale=4, nz=20)
+    e = wl.edges[0].take(np.arange(8))
+    orc = OracleSetup(wl, e)
+    want = orc.run(wl, e, "magphase", crop_f=wl.crop)
+    ctx, geo, ids = gpu_context(wl, [e])
+    assert np.array_equal(geo.ap_h, orc.ap) and np.array_equal(geo.p1_h, orc.ap[orc.p1_pos]) and np.array_equal(geo.p2_h, orc.det[orc.p2_pos])
+    m = _first(lambda: ctx.map(0, B.MODE_MAP, B.RECON_MAGPHASE, B.PREC_FP16X4))
+    cube = ctx.map(0, B.MODE_CUBE, B.RECON_MAGPHASE, B.PREC_FP16X4)
+    torch.cuda.synchronize()
+    m, cube = m.cpu().numpy(), cube.cpu().numpy()
+    assert np.all(m[want["map"] == 0] == 0.0) and (want["map"] > 0).sum() > 0
+    assert rel_err_map(m, want["map"], 1e-3) <= TOL_PIXEL
+    assert abs(m.sum() - want["map"].sum()) <= TOL_SUM * want["map"].sum()
+    assert rel_err_map(cube, want["cube"], 1e-3) <= TOL_PIXEL
+    ctx.close()
