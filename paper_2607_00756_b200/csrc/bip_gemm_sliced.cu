@@ -605,36 +605,71 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
 }
 
 // a5: Phi_n[rho][s] = H_n[s] Psi[rho][s] as sliced rows (n, rho) with their power-of-two scales.
-// One warp per (rho, n, atom); lanes stride over the groups of 8 window pixels; two passes (row maximum, then split).
+// One block per (8 consecutive rho, chunk of QCH channels, atom).  Pass 1: warp w takes row w and finds the row maxima of
+// all channels of the chunk in one sweep over Psi.  Pass 2: thread = (row = t & 7, k-group lane = t >> 3) keeps 8 Psi
+// values in registers and loops over the channels, so Psi is read twice in all (not twice per channel) and the 16-byte
+// slice groups of the 8 rows of one k-group land in one contiguous 128-byte line (the blocked layout puts rows r .. r+7
+// of a k-group side by side): every store instruction writes whole lines.
+constexpr int QCH = 9;
 __global__ void __launch_bounds__(256) k_quantize_phi(const float2* __restrict__ Psi, int64_t psi_ld, int64_t psi_batch_stride,
-                                                      const float2* __restrict__ H, Sliced Phi, int n_rho, int rows_pad, int w2) {
-  const int rho = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
-  const int n = blockIdx.y, atom = blockIdx.z;
-  if (rho >= n_rho) return;
-  const float2* prow = Psi + (int64_t)atom * psi_batch_stride + (int64_t)rho * psi_ld;
-  const float2* hrow = H + (int64_t)n * w2;
-  const int n_groups = 2 * (int)Phi.ksteps;
-  float m = 0.f;
-  for (int s = lane; s < w2; s += 32) {
-    const float2 a = prow[s], h = __ldg(hrow + s);
-    m = fmaxf(m, fmaxf(fabsf(h.x * a.x - h.y * a.y), fabsf(h.x * a.y + h.y * a.x)));
-  }
+                                                      const float2* __restrict__ H, Sliced Phi, int n_rho, int rows_pad, int w2, int n_ch) {
+  __shared__ float inv_s[8][QCH];
+  const int rho0 = blockIdx.x * 8, n0 = blockIdx.y * QCH, atom = blockIdx.z;
+  const int nch = min(QCH, n_ch - n0);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const float2* pbase = Psi + (int64_t)atom * psi_batch_stride;
+  {
+    const int rho = rho0 + warp;
+    float m[QCH];
 #pragma unroll
-  for (int o = 16; o; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
-  const float scale = sl_pow2_scale(m), inv = 1.f / scale;
-  const int64_t row = (int64_t)n * rows_pad + rho;
-  if (lane == 0) Phi.scale[(int64_t)atom * Phi.scale_batch_stride + row] = scale;
-  for (int g = lane; g < n_groups; g += 32) {
-    float re[8], im[8];
+    for (int c = 0; c < QCH; ++c) m[c] = 0.f;
+    if (rho < n_rho) {
+      const float2* prow = pbase + (int64_t)rho * psi_ld;
+      for (int s = lane; s < w2; s += 32) {
+        const float2 a = prow[s];
+#pragma unroll
+        for (int c = 0; c < QCH; ++c)
+          if (c < nch) {
+            const float2 h = __ldg(H + (int64_t)(n0 + c) * w2 + s);
+            m[c] = fmaxf(m[c], fmaxf(fabsf(h.x * a.x - h.y * a.y), fabsf(h.x * a.y + h.y * a.x)));
+          }
+      }
+    }
+#pragma unroll
+    for (int c = 0; c < QCH; ++c) {
+#pragma unroll
+      for (int o = 16; o; o >>= 1) m[c] = fmaxf(m[c], __shfl_xor_sync(0xffffffffu, m[c], o));
+      if (lane == 0 && c < nch) {
+        const float scale = sl_pow2_scale(m[c]);
+        inv_s[warp][c] = 1.f / scale;
+        if (rho < n_rho) Phi.scale[(int64_t)atom * Phi.scale_batch_stride + (int64_t)(n0 + c) * rows_pad + rho] = scale;
+      }
+    }
+  }
+  __syncthreads();
+  const int r = threadIdx.x & 7, rho = rho0 + r;
+  if (rho >= n_rho) return;
+  const float2* prow = pbase + (int64_t)rho * psi_ld;
+  const int n_groups = 2 * (int)Phi.ksteps;
+  for (int g = threadIdx.x >> 3; g < n_groups; g += 32) {
+    float2 a[8];
 #pragma unroll
     for (int j = 0; j < 8; ++j) {
       const int s = g * 8 + j;
-      float2 a = make_float2(0.f, 0.f), h = a;
-      if (s < w2) { a = prow[s]; h = __ldg(hrow + s); }
-      re[j] = h.x * a.x - h.y * a.y;
-      im[j] = h.x * a.y + h.y * a.x;
+      a[j] = s < w2 ? prow[s] : make_float2(0.f, 0.f);
     }
-    sl_store_group(Phi, atom, row, g, re, im, inv);
+    for (int c = 0; c < nch; ++c) {
+      const float2* hrow = H + (int64_t)(n0 + c) * w2;
+      float re[8], im[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const int s = g * 8 + j;
+        const float2 h = s < w2 ? __ldg(hrow + s) : make_float2(0.f, 0.f);
+        re[j] = h.x * a[j].x - h.y * a[j].y;
+        im[j] = h.x * a[j].y + h.y * a[j].x;
+      }
+      sl_store_group(Phi, atom, (int64_t)(n0 + c) * rows_pad + rho, g, re, im, inv_s[r][c]);
+    }
   }
 }
 
@@ -715,15 +750,6 @@ int32_t launch_fmt(bip_ctx* ctx, const SlParams& p) {
   if (const char* e = std::getenv("BIP_TUNE_DGROUP")) q.dgroup = std::max(1, std::atoi(e));
   if (const char* e = std::getenv("BIP_TUNE_CHUNK")) q.chunk_steps = std::max(1, std::atoi(e));   // timing experiments only: breaks exactness
   if (const char* e = std::getenv("BIP_TUNE_LAG")) q.lag_max = std::min(std::max(1, std::atoi(e)), (PAIR ? Cfg<FMT>::STAGES_PAIR : Cfg<FMT>::STAGES) - 1);
-  static const bool lockstep = [] { const char* e = std::getenv("BIP_TUNE_LOCKSTEP"); return e ? std::atoi(e) != 0 : true; }();
-  q.sync_counter = nullptr;
-  q.sync_steps = 1 << 30;                // once per (item, channel) segment
-  if (const char* e = std::getenv("BIP_TUNE_SYNCSTEPS")) q.sync_steps = std::max(1, std::atoi(e));
-  if (lockstep) {      // a fresh zeroed counter per launch (64 slots, cleared on the stream before the kernel)
-    BIP_TRY(ensure(ctx, ctx->Sync, 64 * sizeof(unsigned int), "lockstep counters"));
-    q.sync_counter = reinterpret_cast<unsigned int*>(ctx->Sync.p) + (ctx->sync_slot++ & 63);
-    BIP_CUDA(ctx, cudaMemsetAsync(q.sync_counter, 0, sizeof(unsigned int), ctx->stream));
-  }
   int workers = std::max(1, std::min(q.n_items, PAIR ? ctx->sm_count / 2 : ctx->sm_count));
   if (const char* e = std::getenv("BIP_TUNE_WORKERS")) workers = std::max(1, std::min(workers, std::atoi(e)));   // timing experiments only
   cudaLaunchConfig_t cfg{};
@@ -735,6 +761,23 @@ int32_t launch_fmt(bip_ctx* ctx, const SlParams& p) {
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = PAIR ? 2 : 1; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr; cfg.numAttrs = 1;
+  // Lockstep needs every worker resident at once (they wait for one another): checked against the occupancy the
+  // driver reports for this launch configuration, once per kernel variant; otherwise the workers run free.
+  static const bool lockstep_wanted = [] { const char* e = std::getenv("BIP_TUNE_LOCKSTEP"); return e ? std::atoi(e) != 0 : true; }();
+  static int max_clusters = -1;
+  if (max_clusters < 0) {
+    int n = 0;
+    if (cudaOccupancyMaxActiveClusters(&n, k_sliced_contract<EPI, FMT, PAIR>, &cfg) != cudaSuccess) { cudaGetLastError(); n = 0; }
+    max_clusters = n;
+  }
+  q.sync_counter = nullptr;
+  q.sync_steps = 1 << 30;                // once per (item, channel) segment
+  if (const char* e = std::getenv("BIP_TUNE_SYNCSTEPS")) q.sync_steps = std::max(1, std::atoi(e));
+  if (lockstep_wanted && workers <= max_clusters) {      // a fresh zeroed counter per launch (64 slots, cleared on the stream)
+    BIP_TRY(ensure(ctx, ctx->Sync, 64 * sizeof(unsigned int), "lockstep counters"));
+    q.sync_counter = reinterpret_cast<unsigned int*>(ctx->Sync.p) + (ctx->sync_slot++ & 63);
+    BIP_CUDA(ctx, cudaMemsetAsync(q.sync_counter, 0, sizeof(unsigned int), ctx->stream));
+  }
   BIP_CUDA(ctx, cudaLaunchKernelEx(&cfg, k_sliced_contract<EPI, FMT, PAIR>, q));
   ctx->timing.kernel_launches++;
   return BIP_OK;
@@ -784,8 +827,8 @@ int32_t launch_gather_rows_sliced(bip_ctx* ctx, const Sliced& src, const int32_t
 
 int32_t launch_quantize_phi(bip_ctx* ctx, const float2* Psi, int64_t psi_ld, int64_t psi_batch_stride, const float2* H,
                             const Sliced& Phi, int32_t n_rho, int32_t rows_pad, int32_t w2, int32_t n_ch, int32_t n_atoms) {
-  dim3 grid((unsigned)((n_rho + 7) / 8), (unsigned)n_ch, (unsigned)n_atoms);
-  k_quantize_phi<<<grid, 256, 0, ctx->stream>>>(Psi, psi_ld, psi_batch_stride, H, Phi, n_rho, rows_pad, w2);
+  dim3 grid((unsigned)((n_rho + 7) / 8), (unsigned)((n_ch + QCH - 1) / QCH), (unsigned)n_atoms);
+  k_quantize_phi<<<grid, 256, 0, ctx->stream>>>(Psi, psi_ld, psi_batch_stride, H, Phi, n_rho, rows_pad, w2, n_ch);
   BIP_CUDA(ctx, cudaGetLastError());
   ctx->timing.kernel_launches++;
   return BIP_OK;
