@@ -50,11 +50,20 @@ template <> struct Cfg<SL_FMT_BF16X6> {
 };
 template <int FMT> __host__ __device__ constexpr int x_bytes() { return Cfg<FMT>::PARTS * PART_BYTES; }
 template <int FMT> __host__ __device__ constexpr int stage_bytes() { return 2 * x_bytes<FMT>(); }
-template <int FMT, bool PAIR> __host__ __device__ constexpr int smem_bytes() {
-  return (PAIR ? Cfg<FMT>::STAGES_PAIR * (x_bytes<FMT>() * 3 / 2) : Cfg<FMT>::STAGES * stage_bytes<FMT>()) + 1024 /*align*/ + 512 /*barriers*/;
+// EPI_GEMM2_TILE (CTA pairs, QEELS / CUBE outputs): |a|^2 of the channels of an item is summed in a shared-memory tile
+// [column][row] (129-float pitch: conflict-free both when a thread walks its own row and when a warp flushes 32
+// consecutive columns of one row), and the tile goes to global memory once per item with coalesced fp32 REDs --
+// N_ch times fewer global atomics than reducing per channel.  The tile takes the room of three pipeline stages.
+enum { EPI_GEMM1 = 1, EPI_GEMM2 = 2, EPI_GEMM2_TILE = 3 };
+constexpr int ACC_LD = TM + 1;
+constexpr int ACC_BYTES = TN * ACC_LD * 4;       // 66 048
+template <int EPI, int FMT, bool PAIR> __host__ __device__ constexpr int n_stages() {
+  return EPI == EPI_GEMM2_TILE ? (FMT == SL_FMT_FP16X4 ? 6 : 4) : PAIR ? Cfg<FMT>::STAGES_PAIR : Cfg<FMT>::STAGES;
 }
-
-enum { EPI_GEMM1 = 1, EPI_GEMM2 = 2 };
+template <int EPI, int FMT, bool PAIR> __host__ __device__ constexpr int smem_bytes() {
+  return n_stages<EPI, FMT, PAIR>() * (PAIR ? x_bytes<FMT>() * 3 / 2 : stage_bytes<FMT>()) + 1024 /*align*/ + 512 /*barriers*/ +
+         (EPI == EPI_GEMM2_TILE ? ACC_BYTES : 0);
+}
 
 struct SlParams {
   const uint16_t* X; const uint16_t* Y;
@@ -338,7 +347,8 @@ __device__ __forceinline__ void issue_lead(uint32_t t0r, uint32_t t0i, uint32_t 
 template <int EPI, int FMT, bool PAIR>
 __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlParams p) {
   using C = Cfg<FMT>;
-  constexpr int STAGES = PAIR ? C::STAGES_PAIR : C::STAGES;
+  constexpr int STAGES = n_stages<EPI, FMT, PAIR>();
+  constexpr bool IS_G2 = EPI == EPI_GEMM2 || EPI == EPI_GEMM2_TILE, TILE = EPI == EPI_GEMM2_TILE;
   constexpr int X_BYTES = x_bytes<FMT>(), Y_BYTES = PAIR ? X_BYTES / 2 : X_BYTES, STAGE_BYTES = X_BYTES + Y_BYTES;
   constexpr int STEP_EL = sl_step_el(FMT);
   extern __shared__ uint8_t smem_raw[];
@@ -352,6 +362,7 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
   uint64_t* c12_full = bars + 3 * STAGES + 2;  // small-product accumulators of a (tile, channel) complete
   uint64_t* c12_empty = bars + 3 * STAGES + 3;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 3 * STAGES + 4);
+  float* acc_tile = reinterpret_cast<float*>(smem + STAGES * STAGE_BYTES + 512);   // EPI_GEMM2_TILE only
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   // a worker is a CTA, or a pair of CTAs (cluster of 2 on one TPC) working on two row tiles of the same column tile
@@ -509,13 +520,18 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
       const int row = rt * TM + quarter * 32 + lane;   // this thread's rho (local row of the site under a crop mask)
       bool row_ok = row < p.n_rows;
       int out_row = row;
-      if (EPI == EPI_GEMM2 && p.row_idx) {
+      if (IS_G2 && p.row_idx) {
         out_row = row_ok ? __ldg(p.row_idx + (int64_t)atom * p.row_idx_stride + row) : -1;
         row_ok = out_row >= 0;
       }
       const int col0 = ct * TN + half * 64;
       const float* sy = p.sy + (int64_t)atom * p.sy_batch_stride;
       float rowsum = 0.f;
+      float* acc_row = acc_tile + (half * 64) * ACC_LD + quarter * 32 + lane;      // this thread's cells: acc_row[j * ACC_LD]
+      if (TILE) {
+#pragma unroll
+        for (int j = 0; j < 64; ++j) acc_row[j * ACC_LD] = 0.f;
+      }
       for (int n = 0; n < p.n_ch_loop; ++n, ++seg) {
         float rr[64], ri[64];
 #pragma unroll
@@ -548,7 +564,15 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
         }
         // ---- end of a (tile, channel): fused epilogue on the running sums ----
         const float sxr = row_ok ? p.sx[(int64_t)atom * p.sx_batch_stride + (int64_t)n * p.rows_pad + row] : 0.f;
-        if (EPI == EPI_GEMM2) {
+        if (TILE) {
+          const float sx2 = sxr * sxr;
+#pragma unroll
+          for (int j = 0; j < 64; ++j) {
+            const int d = col0 + j;
+            const float s = d < p.n_cols ? __ldg(sy + d) : 0.f;
+            acc_row[j * ACC_LD] += fmaf(rr[j], rr[j], ri[j] * ri[j]) * (s * s) * sx2;
+          }
+        } else if (EPI == EPI_GEMM2) {
           const float sx2 = sxr * sxr;
           if (p.mode == BIP_MODE_MAP) {
             float acc = 0.f;
@@ -591,6 +615,28 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
       }
       if (EPI == EPI_GEMM2 && p.mode == BIP_MODE_MAP && row_ok)
         atomicAdd(reinterpret_cast<double*>(p.out) + out_row, (double)rowsum * (double)p.inv_G);
+      if (TILE) {
+        // flush: the eight epilogue warps take 16 rows each; a warp writes 32 consecutive detector columns per RED
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        float* out = reinterpret_cast<float*>(p.out);
+        const int ew = warp - 2;
+        for (int i = 0; i < 16; ++i) {
+          const int rl = ew * 16 + i, grow = rt * TM + rl;
+          int orow = grow < p.n_rows ? grow : -1;
+          if (orow >= 0 && p.row_idx) orow = __ldg(p.row_idx + (int64_t)atom * p.row_idx_stride + grow);
+          if (orow < 0) continue;
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            const int c = lane + 32 * k, d = ct * TN + c;
+            if (d < p.n_cols) {
+              const float v = acc_tile[c * ACC_LD + rl] * p.inv_G;
+              if (p.mode == BIP_MODE_CUBE) atomicAdd(out + (int64_t)orow * p.n_cols + d, v);
+              else atomicAdd(out + (int64_t)orow * p.n_bins + __ldg(p.bin_of_det + d), v);
+            }
+          }
+        }
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+      }
     }
   }
 
@@ -733,7 +779,7 @@ template <int EPI, int FMT, bool PAIR>
 int32_t launch_fmt(bip_ctx* ctx, const SlParams& p) {
   static bool attr_set = false;
   if (!attr_set) {
-    BIP_CUDA(ctx, cudaFuncSetAttribute(k_sliced_contract<EPI, FMT, PAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<FMT, PAIR>()));
+    BIP_CUDA(ctx, cudaFuncSetAttribute(k_sliced_contract<EPI, FMT, PAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<EPI, FMT, PAIR>()));
     attr_set = true;
   }
   SlParams q = p;
@@ -749,13 +795,14 @@ int32_t launch_fmt(bip_ctx* ctx, const SlParams& p) {
   q.dgroup = DGROUP_DEFAULT;
   if (const char* e = std::getenv("BIP_TUNE_DGROUP")) q.dgroup = std::max(1, std::atoi(e));
   if (const char* e = std::getenv("BIP_TUNE_CHUNK")) q.chunk_steps = std::max(1, std::atoi(e));   // timing experiments only: breaks exactness
-  if (const char* e = std::getenv("BIP_TUNE_LAG")) q.lag_max = std::min(std::max(1, std::atoi(e)), (PAIR ? Cfg<FMT>::STAGES_PAIR : Cfg<FMT>::STAGES) - 1);
+  if (const char* e = std::getenv("BIP_TUNE_LAG")) q.lag_max = std::min(std::max(1, std::atoi(e)), n_stages<EPI, FMT, PAIR>() - 1);
   int workers = std::max(1, std::min(q.n_items, PAIR ? ctx->sm_count / 2 : ctx->sm_count));
   if (const char* e = std::getenv("BIP_TUNE_WORKERS")) workers = std::max(1, std::min(workers, std::atoi(e)));   // timing experiments only
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = dim3(PAIR ? 2 * workers : workers);
   cfg.blockDim = dim3(NUM_THREADS);
-  cfg.dynamicSmemBytes = smem_bytes<FMT, PAIR>();
+  q.lag_max = std::min(q.lag_max, n_stages<EPI, FMT, PAIR>() - 1);
+  cfg.dynamicSmemBytes = smem_bytes<EPI, FMT, PAIR>();
   cfg.stream = ctx->stream;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeClusterDimension;
@@ -786,6 +833,9 @@ int32_t launch_fmt(bip_ctx* ctx, const SlParams& p) {
 template <int EPI>
 int32_t launch(bip_ctx* ctx, const SlParams& p, int fmt) {
   static const bool pair = [] { const char* e = std::getenv("BIP_TUNE_PAIR"); return e ? std::atoi(e) != 0 : true; }();
+  static const bool tile = [] { const char* e = std::getenv("BIP_TUNE_TILEACC"); return e ? std::atoi(e) != 0 : true; }();
+  if (pair && tile && EPI == EPI_GEMM2 && p.mode != BIP_MODE_MAP)
+    return fmt == SL_FMT_FP16X4 ? launch_fmt<EPI_GEMM2_TILE, SL_FMT_FP16X4, true>(ctx, p) : launch_fmt<EPI_GEMM2_TILE, SL_FMT_BF16X6, true>(ctx, p);
   if (pair) return fmt == SL_FMT_FP16X4 ? launch_fmt<EPI, SL_FMT_FP16X4, true>(ctx, p) : launch_fmt<EPI, SL_FMT_BF16X6, true>(ctx, p);
   return fmt == SL_FMT_FP16X4 ? launch_fmt<EPI, SL_FMT_FP16X4, false>(ctx, p) : launch_fmt<EPI, SL_FMT_BF16X6, false>(ctx, p);
 }
