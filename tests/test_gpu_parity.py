@@ -313,3 +313,33 @@ def test_cfg4_fept_quarter_clone_prism_regime():
     assert abs(m.sum() - want["map"].sum()) <= TOL_SUM * want["map"].sum()
     assert rel_err_map(cube, want["cube"], 1e-3) <= TOL_PIXEL
     ctx.close()
+
+
+def test_cfg5_factor_one_against_conventional_multislice_at_scale():
+    """BASELINE.json configs[4] at parent factor 1 (parents = all 7721 aperture and 19 797 detector beams, w = I): the
+    GPU path against Algorithm 1 itself -- conventional transition-potential multislice per scan position, the ground
+    truth -- at the full 256^2 size, on 4 sampled scan positions: full cube rows and map
+    pixels.  No BiP oracle code in between.  Slab truncated to 3 slices (site in slice 1: one slice above, two through
+    the exit) so that the 27 518 parent columns build quickly."""
+    import torch
+    import paper_2607_00756_b200 as B
+    from oracle import beams as ob
+    wl = make_workload("cfg5", nz=3, parent_factor=(1.0, 1.0))
+    e = wl.edges[0].take(np.arange(2))
+    assert set(e.slice.tolist()) == {1}
+    qa, qd = wl.alpha_mrad * 1e-3 / wl.lam, e.det_mrad * 1e-3 / wl.lam
+    ap, det = ob.beams_in_disc(wl.ny, wl.nx, wl.ly, wl.lx, qa), ob.beams_in_disc(wl.ny, wl.nx, wl.ly, wl.lx, qd)
+    c = ob.aperture_coefficients(ap, wl.ny, wl.nx, wl.ly, wl.lx, wl.lam, wl.defocus)
+    P = oms.fresnel_propagator(wl.ny, wl.nx, wl.ly, wl.lx, wl.lam, wl.dz)
+    sub = np.array([0, 1000, 2079, 4095])
+    I1 = oms.conventional_cube(c, ap, wl.T.astype(np.complex128), P, wl.scan[sub], e.slice, e.centre, e.H.astype(complex), det)
+    ctx, geo, ids = gpu_context(wl, [e])
+    assert (ctx.n_p1, ctx.n_p2) == (7721, 19797) and geo.det_h.shape[0] == 19797
+    cube = _first(lambda: ctx.map(0, B.MODE_CUBE, B.RECON_LINEAR, B.PREC_FP16X4))
+    m = ctx.map(0, B.MODE_MAP, B.RECON_MAGPHASE, B.PREC_FP16X4)
+    torch.cuda.synchronize()
+    cube, m = cube.cpu().numpy(), m.cpu().numpy()
+    assert rel_err_map(cube[sub], I1, 1e-3) <= TOL_PIXEL
+    assert rel_err_map(m[sub], I1.sum(1)) <= TOL_PIXEL
+    assert abs(m[sub].sum() - I1.sum()) <= 2 * TOL_SUM * I1.sum()
+    ctx.close()
