@@ -404,7 +404,7 @@ static int32_t run_edges(bip_ctx* ctx, const std::vector<int32_t>& ids, int mode
                                    ? std::min<int64_t>(ctx->n_rho, (int64_t)(1.5 * ctx->n_rho / (ctx->crop_fy * ctx->crop_fx)) + 2 * SL_ROWS) : ctx->n_rho;
       const size_t per_atom = (size_t)((ctx->n_p1 + ctx->n_p2) * w2 * 8 + rows_est * w2 * 8 +
                                        el * (round_up(w2, 128) * round_up(ctx->n_ap, 32) + round_up(e.n_det, 128) * round_up(w2, 32) +
-                                             round_up(rows_est, 256) * (e.n_ch * round_up(w2, 32) + round_up(ctx->n_ap, 32))) +
+                                             round_up(rows_est, 256) * (e.n_ch * round_up(w2, 32) + (ctx->crop_fy * ctx->crop_fx > 1 ? round_up(ctx->n_ap, 32) : 0))) +
                                        (ctx->crop_fy * ctx->crop_fx > 1 ? round_up(ctx->n_rho, 256) * 4 : 0));
       const int32_t nb_max = (int32_t)std::max<size_t>(1, std::min<size_t>(budget / std::max<size_t>(per_atom, 1), 4096));
       Span s(ctx, sp.pool_map, sp.contract);
@@ -519,7 +519,7 @@ int32_t bip_destroy(bip_ctx* ctx) {
   if (ctx->T_owned) cudaFree((void*)ctx->T_dev);
   void* ptrs[] = {ctx->ap_h_dev, ctx->p1_h_dev, ctx->p2_h_dev, ctx->ap_c_dev, ctx->w1_idx_dev, ctx->w1_w_dev, ctx->rooty_dev,
                   ctx->rootx_dev, ctx->P_dev, ctx->ms_work, ctx->S1, ctx->S2, ctx->D1.p, ctx->D2.p, ctx->R1.p, ctx->R2.p, ctx->Psi.p,
-                  ctx->Phi.p, ctx->R1s.p, ctx->R2s.p, ctx->Phis.p, ctx->Scl.p, ctx->Sync.p, ctx->RowIdx.p, ctx->Acrop.p, ctx->rho_dev};
+                  ctx->Phi.p, ctx->R1s.p, ctx->R2s.p, ctx->Phis.p, ctx->Scl.p, ctx->Sync.p, ctx->RowIdx.p, ctx->Acrop.p, ctx->Pmax.p, ctx->rho_dev};
   free_illumination(ctx);
   for (void* p : ptrs) if (p) cudaFree(p);
   cudaGetLastError();

@@ -92,6 +92,7 @@ struct bip_ctx {
   double* rho_dev = nullptr;       // [n_rho][2] scan positions in pixels
   std::vector<double> rho_host;    // the same on the host (crop-mask row lists)
   int32_t crop_fy = 1, crop_fx = 1;  // PRISM crop mask (bip_set_crop); 1 = off
+  bip::DevBuf Pmax;                // max_s |D2[p][s]| per (site, parent): row-scale bound of R2
   bip::DevBuf RowIdx, Acrop;       // per-site scan-row lists and gathered illumination rows (crop mask)
   bip::Planes A;                   // illumination [n_rho][n_ap] split planes (K-major over b); built on first use
   bip::Sliced A_sl;                // the same as a sliced 16-bit operand (format A_sl.fmt); built on first use

@@ -227,57 +227,66 @@ __global__ void __launch_bounds__(256) k_recon_t_sliced(const float2* __restrict
 
 // a6 as the K-major operand of the detector GEMM: rows = detector beams d, k = window pixels s.
 // One block per (beam, atom): pass 1 finds the row maximum, pass 2 splits and stores.
+// max_s |D[a][p][s]| of every parent window: one warp per (parent, atom).  Feeds the row scales of R2 below.
+__global__ void __launch_bounds__(256) k_parent_rowmax(const float2* __restrict__ D, int n_par, int w2, float* __restrict__ pmax) {
+  const int p = blockIdx.x * 8 + (threadIdx.x >> 5), a = blockIdx.y, lane = threadIdx.x & 31;
+  if (p >= n_par) return;
+  const float2* row = D + ((int64_t)a * n_par + p) * w2;
+  float m = 0.f;
+  for (int s = lane; s < w2; s += 32) { const float2 d = row[s]; m = fmaxf(m, d.x * d.x + d.y * d.y); }
+#pragma unroll
+  for (int o = 16; o; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if (lane == 0) pmax[(int64_t)a * n_par + p] = sqrtf(m);
+}
+
 __global__ void __launch_bounds__(256) k_recon_rows_sliced(const float2* __restrict__ D, int n_par, const int32_t* __restrict__ bh, int n_beams,
                                     const int32_t* __restrict__ nn_idx, const float* __restrict__ nn_w, int max_nn, int carrier,
                                     int recon, const int32_t* __restrict__ origin, int w, int ny, int nx,
-                                    const float2* __restrict__ rooty, const float2* __restrict__ rootx, Sliced out) {
+                                    const float2* __restrict__ rooty, const float2* __restrict__ rootx,
+                                    const float* __restrict__ pmax, Sliced out) {
   // One block per (8 consecutive beams, atom); thread = (row = t & 7, k-group lane = t >> 3).  The blocked slice layout
   // keeps the 16-byte groups of rows r .. r+7 of one k-group side by side, so the 8 row-lanes of a store instruction
-  // fill one 128-byte line (a block per single row wrote 16 bytes of every line it touched).
+  // fill one 128-byte line.  Single pass: the row scale is the power of two above sum_p w_p max_s |D_p[s]|, a bound on
+  // |R2[d][s]| for both reconstructions (the weights are a convex combination, eq. 8; eq. 11 has magnitude
+  // sum_p w_p |D_p|), so no element has to be evaluated twice to find the exact row maximum.
   const int a = blockIdx.y, r = threadIdx.x & 7, gl = threadIdx.x >> 3, b = blockIdx.x * 8 + r;
   const bool row_ok = b < n_beams;
   const int w2 = w * w;
   __shared__ int32_t s_idx[8][BIP_MAX_NN];
   __shared__ float s_w[8][BIP_MAX_NN];
-  __shared__ int s_max[8];
-  if (threadIdx.x < 8) s_max[threadIdx.x] = 0;
   for (int i = threadIdx.x; i < 8 * max_nn; i += blockDim.x) {
     const int rr = i / max_nn, j = i - rr * max_nn, bb = blockIdx.x * 8 + rr;
     s_idx[rr][j] = bb < n_beams ? nn_idx[(int64_t)bb * max_nn + j] : -1;
     s_w[rr][j] = bb < n_beams ? nn_w[(int64_t)bb * max_nn + j] : 0.f;
   }
   __syncthreads();
-  const int oy = origin[2 * a], ox = origin[2 * a + 1];
-  const int hyp = row_ok ? ((bh[2 * b] % ny) + ny) % ny : 0, hxp = row_ok ? ((bh[2 * b + 1] % nx) + nx) % nx : 0;
-  const float2* Da = D + (int64_t)a * n_par * w2;
-  auto value = [&](int s) {
-    const int sy = s / w, sx = s - sy * w;
-    int ry = oy + sy; if (ry >= ny) ry -= ny;
-    int rx = ox + sx; if (rx >= nx) rx -= nx;
-    float2 t = tilt(rooty, rootx, hyp, hxp, ry, rx, ny, nx);
-    if (carrier < 0) t.y = -t.y;
-    return recon_elem(Da, s_idx[r], s_w[r], max_nn, w2, s, recon, t);
-  };
-  const int n_groups = 2 * (int)out.ksteps;
-  float m = 0.f;
-  if (row_ok)
-    for (int g = gl; g < n_groups; g += 32)
-#pragma unroll
-      for (int j = 0; j < 8; ++j) {
-        const int s = g * 8 + j;
-        if (s < w2) { const float2 v = value(s); m = fmaxf(m, fmaxf(fabsf(v.x), fabsf(v.y))); }
-      }
-  atomicMax(&s_max[r], __float_as_int(m));          // non-negative floats order like their bit patterns
-  __syncthreads();
   if (!row_ok) return;
-  const float scale = sl_pow2_scale(__int_as_float(s_max[r])), inv = 1.f / scale;
+  float bound = 0.f;
+  for (int j = 0; j < max_nn; ++j) {
+    const int p = s_idx[r][j];
+    if (p < 0) break;
+    bound = fmaf(s_w[r][j], __ldg(pmax + (int64_t)a * n_par + p), bound);
+  }
+  const float scale = sl_pow2_scale(1.001f * bound), inv = 1.f / scale;
   if (gl == 0) out.scale[(int64_t)a * out.scale_batch_stride + b] = scale;
+  const int oy = origin[2 * a], ox = origin[2 * a + 1];
+  const int hyp = ((bh[2 * b] % ny) + ny) % ny, hxp = ((bh[2 * b + 1] % nx) + nx) % nx;
+  const float2* Da = D + (int64_t)a * n_par * w2;
+  const int n_groups = 2 * (int)out.ksteps;
   for (int g = gl; g < n_groups; g += 32) {
     float re[8], im[8];
 #pragma unroll
     for (int j = 0; j < 8; ++j) {
       const int s = g * 8 + j;
-      const float2 v = s < w2 ? value(s) : make_float2(0.f, 0.f);
+      float2 v = make_float2(0.f, 0.f);
+      if (s < w2) {
+        const int sy = s / w, sx = s - sy * w;
+        int ry = oy + sy; if (ry >= ny) ry -= ny;
+        int rx = ox + sx; if (rx >= nx) rx -= nx;
+        float2 t = tilt(rooty, rootx, hyp, hxp, ry, rx, ny, nx);
+        if (carrier < 0) t.y = -t.y;
+        v = recon_elem(Da, s_idx[r], s_w[r], max_nn, w2, s, recon, t);
+      }
       re[j] = v.x; im[j] = v.y;
     }
     sl_store_group(out, a, b, g, re, im, inv);
@@ -396,15 +405,21 @@ int32_t launch_recon_t_sliced(bip_ctx* ctx, const float2* D, int32_t n_par, cons
 int32_t launch_recon_rows_sliced(bip_ctx* ctx, const float2* D, int32_t n_par, const int32_t* bh_dev, int32_t n_beams,
                                  const int32_t* nn_idx, const float* nn_w, int32_t max_nn, int carrier, int recon,
                                  const int32_t* origin_dev, int32_t n_atoms, int32_t w, Sliced out) {
+  BIP_TRY(ensure(ctx, ctx->Pmax, (size_t)n_atoms * n_par * sizeof(float), "parent window maxima"));
+  float* pmax = reinterpret_cast<float*>(ctx->Pmax.p);
   for (int a0 = 0; a0 < n_atoms; a0 += 65535) {          // gridDim.y limit
     const int na = std::min(65535, n_atoms - a0);
+    k_parent_rowmax<<<dim3((unsigned)((n_par + 7) / 8), (unsigned)na), 256, 0, ctx->stream>>>(D + (int64_t)a0 * n_par * w * w, n_par, w * w,
+                                                                                              pmax + (int64_t)a0 * n_par);
+    BIP_CUDA(ctx, cudaGetLastError());
+    ctx->timing.kernel_launches++;
     Sliced o = out;
     o.base += (int64_t)a0 * out.batch_stride;
     o.scale += (int64_t)a0 * out.scale_batch_stride;
     dim3 grid((unsigned)((n_beams + 7) / 8), (unsigned)na);
     k_recon_rows_sliced<<<grid, 256, 0, ctx->stream>>>(D + (int64_t)a0 * n_par * w * w, n_par, bh_dev, n_beams, nn_idx, nn_w, max_nn, carrier,
                                                       recon, origin_dev + 2 * (int64_t)a0, w, ctx->g.ny, ctx->g.nx, ctx->rooty_dev,
-                                                      ctx->rootx_dev, o);
+                                                      ctx->rootx_dev, pmax + (int64_t)a0 * n_par, o);
     BIP_CUDA(ctx, cudaGetLastError());
     ctx->timing.kernel_launches++;
   }
