@@ -343,3 +343,24 @@ def test_cfg5_factor_one_against_conventional_multislice_at_scale():
     assert rel_err_map(m[sub], I1.sum(1)) <= TOL_PIXEL
     assert abs(m[sub].sum() - I1.sum()) <= 2 * TOL_SUM * I1.sum()
     ctx.close()
+
+
+@pytest.mark.parametrize("prec_name", ["fp16x4", "bf16x6"])
+def test_many_channels_and_window_as_large_as_the_grid(prec_name):
+    """Degenerate / maximum cases of the window and channel loops: 11 channels (more than one channel chunk of
+    k_quantize_phi; the paper's La-M edge has 75) and a window as large as the short grid axis
+    (W = 12 on a 16 x 12 grid: every window wraps), against Alg. 1 brute force with parents = all beams."""
+    import torch
+    import paper_2607_00756_b200 as B
+    wl = tiny_random_workload(77, W=12, n_ch=11, n_atoms=3, n_scan=4)
+    e = wl.edges[0]
+    orc = OracleSetup(wl, e, parent_factor=(1, 1))
+    I1 = oms.conventional_cube(orc.c, orc.ap, wl.T.astype(np.complex128), orc.P, wl.scan, e.slice, e.centre,
+                               e.H.astype(complex), orc.det)
+    ctx, geo, ids = gpu_context(wl, [e], parent_factor=(1, 1))
+    cube = _first(lambda: ctx.map(0, B.MODE_CUBE, B.RECON_LINEAR, _prec(prec_name)))
+    m = ctx.map(0, B.MODE_MAP, B.RECON_MAGPHASE, _prec(prec_name))
+    torch.cuda.synchronize()
+    assert rel_err_map(cube.cpu().numpy(), I1, 1e-3) <= TOL_PIXEL
+    assert rel_err_map(m.cpu().numpy(), I1.sum(1)) <= TOL_PIXEL
+    ctx.close()
