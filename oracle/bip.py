@@ -81,6 +81,24 @@ def atom_amplitudes(S1, S2, p1_h, p2_h, ap_beams, det_beams, w1, w2, A, H, centr
     return a, Psi
 
 
+def atom_amplitudes_coupling(S1, S2, p1_h, p2_h, ap_beams, det_beams, w1, w2, A, H, centre, ny, nx, recon, crops=None):
+    """The other association of the same triple product (eq. 13; Alg. 4 lines 6-8):
+    first the scan-independent transition coupling matrix of the site and channel,
+
+        M^{(n,tau)}_{d,b} = sum_{r in Omega_tau} S2^d(r) H_n(r - tau) S1^b(r)        [K, B]
+
+    then a_d(rho) = G^-1/2 sum_b M_{d,b} c_b(rho) for all scan positions at once.  Returns a[n, rho, d]."""
+    W = H.shape[1]
+    c1, c2 = crops if crops is not None else (None, None)
+    R1 = reconstruct_window(S1, p1_h, ap_beams, w1, centre, W, ny, nx, +1, recon, c1)     # S1^b | Omega   [B, W^2]
+    R2 = reconstruct_window(S2, p2_h, det_beams, w2, centre, W, ny, nx, -1, recon, c2)    # S2^d | Omega   [K, W^2]
+    a = np.empty((H.shape[0], A.shape[0], det_beams.shape[0]), dtype=np.complex128)
+    for n in range(H.shape[0]):
+        M = (R2 * H[n].reshape(1, -1)) @ R1.T                                             # [K, B]
+        a[n] = (A @ M.T) / np.sqrt(float(ny * nx))
+    return a
+
+
 def qeels_bins(det_beams, axis):
     """Distinct signed beam indices along the resolved axis, ascending. axis 1 = x, 0 = y."""
     return np.unique(det_beams[:, axis])
@@ -101,7 +119,7 @@ def reduce_modes(a, det_beams):
 
 
 def bip_run(T, P, ap_beams, c, p1_h, w1, det_beams, p2_h, w2, scan, sites_slice, sites_centre, H,
-            recon="linear", want_psi=False, crop_f=None):
+            recon="linear", want_psi=False, crop_f=None, association="probe"):
     """Algorithm 5: build S1 / S2 on the parents, then for every ionisation plane with >= 1
     site ADVANCETO / PEELTO and run the on-atom contraction for every site and channel, accumulating the outputs.
     T complex [nz, ny, nx]; weights w1 [B, Bp1], w2 [K, Bp2] (dense or scipy.sparse).  Returns the dict of
@@ -121,8 +139,12 @@ def bip_run(T, P, ap_beams, c, p1_h, w1, det_beams, p2_h, w2, scan, sites_slice,
     psis = []
     for i in range(nz):
         for a_idx in np.nonzero(sites_slice == i)[0]:
-            a, Psi = atom_amplitudes(S1, S2, p1_h, p2_h, ap_beams, det_beams, w1, w2, A,
-                                     H.astype(np.complex128), sites_centre[a_idx], ny, nx, recon)
+            if association == "coupling":                # eq. 13 as printed: M first, then all scans (NEXT-2)
+                a, Psi = atom_amplitudes_coupling(S1, S2, p1_h, p2_h, ap_beams, det_beams, w1, w2, A,
+                                                  H.astype(np.complex128), sites_centre[a_idx], ny, nx, recon), None
+            else:
+                a, Psi = atom_amplitudes(S1, S2, p1_h, p2_h, ap_beams, det_beams, w1, w2, A,
+                                         H.astype(np.complex128), sites_centre[a_idx], ny, nx, recon)
             r = reduce_modes(a, det_beams)
             if crop_f is not None:
                 inside = ob.crop_mask(scan, sites_centre[a_idx], ny, nx, crop_f[0], crop_f[1])

@@ -46,10 +46,10 @@ class OracleSetup:
         self.p1_pos, self.w1 = part(self.ap, self.qa, f1)
         self.p2_pos, self.w2 = part(self.det, self.qd, f2)
 
-    def run(self, wl, edge, recon="linear", scan=None, crop_f=None):
+    def run(self, wl, edge, recon="linear", scan=None, crop_f=None, association="probe"):
         return obip.bip_run(wl.T.astype(np.complex128), self.P, self.ap, self.c, self.ap[self.p1_pos], self.w1, self.det,
                             self.det[self.p2_pos], self.w2, wl.scan if scan is None else scan, edge.slice, edge.centre,
-                            edge.H, recon=recon, crop_f=crop_f)
+                            edge.H, recon=recon, crop_f=crop_f, association=association)
 
 
 def gpu_context(wl, edges, parent_factor=None, max_nn=8, T_on_device=True, prism=None, crop=None):

@@ -191,3 +191,21 @@ def test_translation_covariance():
     cen2 = (e.centre + np.array([dy, dx])) % np.array([wl.ny, wl.nx])
     r2 = bip.bip_run(T2, *args, wl.scan + np.array([dy, dx]), e.slice, cen2.astype(np.int32), e.H)
     assert np.abs(r["cube"] - r2["cube"]).max() <= 1e-12 * r["cube"].max()
+
+
+def test_coupling_matrix_association_equals_conventional():
+    """Eq. 13 as printed (coupling matrix M first, then all scans; Alg. 4 lines 6-8) with parents = all beams against
+    Alg. 1 brute force, and against the probe-first association of the same triple product (BiP, f > 1)."""
+    from bip_inputs.specimen import make_workload
+    from helpers import OracleSetup
+    wl, e, ap, det, c, P, T = _setup(5, W=8, n_atoms=3, n_scan=4)
+    I1 = ms.conventional_cube(c, ap, T, P, wl.scan, e.slice, e.centre, e.H.astype(complex), det)
+    r = bip.bip_run(T, P, ap, c, ap, np.eye(len(ap)), det, det, np.eye(len(det)), wl.scan, e.slice, e.centre, e.H,
+                    association="coupling")
+    assert np.abs(r["cube"] - I1).max() <= 1e-12 * I1.max()
+    wl2 = make_workload("cfg1", scale=2, nz=3, scan=(3, 3))
+    e2 = wl2.edges[0].take([0, 1])
+    orc2 = OracleSetup(wl2, e2)
+    for recon in ("linear", "magphase"):
+        a, b = orc2.run(wl2, e2, recon), orc2.run(wl2, e2, recon, association="coupling")
+        assert np.abs(a["cube"] - b["cube"]).max() <= 1e-12 * a["cube"].max()
