@@ -52,6 +52,14 @@ typedef enum {
 
 typedef enum { BIP_MODE_MAP = 0, BIP_MODE_QEELS_X = 1, BIP_MODE_QEELS_Y = 2, BIP_MODE_CUBE = 3 } bip_mode;
 typedef enum { BIP_RECON_LINEAR = 0, BIP_RECON_MAGPHASE = 1 } bip_recon;
+/* Association of the triple product sum_s sum_b S2^d(s) H_n(s) S1^b(s) c_b(rho) (eq. 13):
+ * PROBE     probe first: Psi[rho, s] = sum_b c_b(rho) S1^b(s), then a = sum_s S2^d H_n Psi (the paper's contract="probe",
+ *           PAPER.md:519); cost per site ~ N_rho W^2 (B + N_ch K).  The default.
+ * COUPLING  eq. 13 as printed / Alg. 4 lines 6-8: the scan-independent coupling matrix M^(n,tau)[d, b] = sum_s S2^d H_n S1^b
+ *           first, then a = M c(rho) for all scans; cost per site ~ N_ch K B (W^2 + N_rho).  Pays when a site sees few scan
+ *           positions (crop mask, small rasters).  Needs N_ch K W^2 operand elements of scratch per site.
+ * AUTO      per edge, whichever of the two has the lower cost by these formulas (and fits the scratch budget). */
+typedef enum { BIP_ASSOC_PROBE = 0, BIP_ASSOC_COUPLING = 1, BIP_ASSOC_AUTO = 2 } bip_assoc;
 /* Arithmetic of the two contractions (all fp32-equivalent).
  * FP16X4 (the one to use): tcgen05 tensor cores on operands split, against a power-of-two row scale, into a 9-bit
  *   fixed-point leading slice and an fp16 residual slice (representation error 2^-21 of the row maximum); a real
@@ -183,6 +191,10 @@ BIP_API int32_t bip_prism_subsample(int32_t n, const int32_t* h, int32_t fy, int
  * switches the mask off (the default).  The contraction then runs, per site, over that site's scan rows only: the
  * cost per site falls by fy * fx.  Tensor-core precisions only (BIP_PREC_FP16X4 / FP16X3 / BF16X6). */
 BIP_API int32_t bip_set_crop(bip_ctx* ctx, int32_t fy, int32_t fx);
+
+/* Choose the association of the on-atom contraction (bip_assoc above) for the following bip_map calls.  Tensor-core
+ * precisions only for COUPLING; AUTO falls back to PROBE otherwise. */
+BIP_API int32_t bip_set_association(bip_ctx* ctx, int32_t assoc);
 
 /* Register an ionisation edge: its sites, transition-potential windows and detector.
  *   slice [n_atoms]        slice index i(tau) of each site, 0 <= slice < nz

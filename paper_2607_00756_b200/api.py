@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libbip.so")
 
 MODE_MAP, MODE_QEELS_X, MODE_QEELS_Y, MODE_CUBE = 0, 1, 2, 3
 RECON_LINEAR, RECON_MAGPHASE = 0, 1
+ASSOC_PROBE, ASSOC_COUPLING, ASSOC_AUTO = 0, 1, 2
 PREC_TF32X3, PREC_FP32_SIMT, PREC_BF16X6, PREC_FP16X4, PREC_FP16X3 = 0, 1, 2, 3, 4
 MAX_NN = 16
 _STATUS = {1: "BIP_ERR_INVALID", 2: "BIP_ERR_STATE", 3: "BIP_ERR_OOM", 4: "BIP_ERR_CUDA", 5: "BIP_ERR_UNSUPPORTED"}
@@ -63,7 +64,7 @@ ABI_SYMBOLS = (
     "bip_destroy", "bip_last_error", "bip_build_S1", "bip_build_S2", "bip_set_scan", "bip_add_edge", "bip_clear_edges",
     "bip_output_size", "bip_map", "bip_map_host", "bip_map_all", "bip_get_windows", "bip_get_qeels_bins",
     "bip_seek_plane", "bip_copy_S", "bip_debug_reconstruct", "bip_get_timing", "bip_version", "bip_prism_subsample",
-    "bip_set_crop",
+    "bip_set_crop", "bip_set_association",
 )
 
 _lib: Optional[C.CDLL] = None
@@ -265,6 +266,10 @@ class Context:
         rho = np.ascontiguousarray(rho_px, dtype=np.float64)
         self._ck(self._lib.bip_set_scan(self._ctx, rho.shape[0], _p(rho, C.c_double)))
         self.n_rho = rho.shape[0]
+
+    def set_association(self, assoc: int):
+        """Probe-first (default), coupling-matrix (eq. 13 as printed) or automatic association of the contraction."""
+        self._ck(self._lib.bip_set_association(self._ctx, int(assoc)))
 
     def set_crop(self, fy: int, fx: int):
         """PRISM crop mask: sites contribute only to the scans within N / (2 f) of them; (1, 1) = off."""

@@ -210,6 +210,74 @@ static size_t scratch_budget() {
 }
 
 // Steps a1-a8 on the sliced 16-bit operands (BIP_PREC_FP16X4 / BIP_PREC_BF16X6).
+// NEXT-2: the coupling-matrix association (eq. 13 as printed; Alg. 4 lines 6-8) on the same kernels:
+//   X1 = H_n R2 rows (n, d) [k = s],  Y1 = R1 rows b [k = s]   ->  M[(n, d)][b]  (GEMM, c64 out)       n_ch K B W^2
+//   X2 = A rows rho [k = b],          Y2 = M rows (n, d) [k = b] ->  |a|^2 reduced per mode (GEMM2 epilogue; the
+//   channels run as extra columns c = n K + d)                                                          N_rho n_ch K B
+static int32_t contract_coupling(bip_ctx* ctx, Edge& e, const int32_t* org, int32_t nb, int mode, int recon, int fmt, bool drop_tiny,
+                                 void* out, const Sliced& Ax, int32_t n_rows, int64_t rho_pad, const int32_t* row_idx_dev,
+                                 int64_t row_idx_stride, double n_rows_total) {
+  auto& sp = spans()[ctx];
+  const int w2 = e.w * e.w;
+  const int64_t n_nd = (int64_t)e.n_ch * e.n_det;                 // rows (n, d) = n K + d
+  Sliced R1r, HR2, Ms;
+  BIP_TRY(ensure(ctx, ctx->D1, (size_t)nb * ctx->n_p1 * w2 * sizeof(float2), "D1 (de-tilted S1 windows)"));
+  BIP_TRY(ensure(ctx, ctx->D2, (size_t)nb * ctx->n_p2 * w2 * sizeof(float2), "D2 (de-tilted S2 windows)"));
+  BIP_TRY(sliced_in(ctx, ctx->R1r, R1r, fmt, ctx->n_ap, w2, nb, "R1 rows (coupling)"));
+  BIP_TRY(sliced_in(ctx, ctx->HR2, HR2, fmt, n_nd, w2, nb, "H_n R2 rows (coupling)", 2 * SL_ROWS));
+  BIP_TRY(sliced_in(ctx, ctx->Ms, Ms, fmt, n_nd, ctx->n_ap, nb, "coupling matrix (sliced)"));
+  const int64_t m_ld = round_up(ctx->n_ap, 2);                   // even pitch: the GEMM epilogue stores pairs of complex values
+  BIP_TRY(ensure(ctx, ctx->Mc, (size_t)nb * n_nd * m_ld * sizeof(float2), "coupling matrix"));
+  const int64_t n_scale = (int64_t)nb * (R1r.rows_pad + HR2.rows_pad + Ms.rows_pad);
+  BIP_TRY(ensure(ctx, ctx->Scl, (size_t)n_scale * sizeof(float), "row scales"));
+  R1r.scale = reinterpret_cast<float*>(ctx->Scl.p);           R1r.scale_batch_stride = R1r.rows_pad;
+  HR2.scale = R1r.scale + (int64_t)nb * R1r.rows_pad;         HR2.scale_batch_stride = HR2.rows_pad;
+  Ms.scale = HR2.scale + (int64_t)nb * HR2.rows_pad;          Ms.scale_batch_stride = Ms.rows_pad;
+  // a1-a2, a6: both reconstructions as rows over the window pixels; H_n folded into the S2 side
+  BIP_TRY(launch_crop_detilt(ctx, ctx->S1, ctx->p1_h_dev, ctx->n_p1, +1, org, nb, e.w, (float2*)ctx->D1.p));
+  BIP_TRY(launch_recon_rows_sliced(ctx, (const float2*)ctx->D1.p, ctx->n_p1, ctx->ap_h_dev, ctx->n_ap, ctx->w1_idx_dev, ctx->w1_w_dev,
+                                   ctx->nn1, +1, recon, org, nb, e.w, R1r));
+  BIP_TRY(launch_crop_detilt(ctx, ctx->S2, ctx->p2_h_dev, ctx->n_p2, -1, org, nb, e.w, (float2*)ctx->D2.p));
+  BIP_TRY(launch_recon_rows_sliced(ctx, (const float2*)ctx->D2.p, ctx->n_p2, e.det_h_dev, e.n_det, e.nn_idx_dev, e.nn_w_dev, e.max_nn,
+                                   -1, recon, org, nb, e.w, HR2, e.H_dev, e.n_ch, e.hmax_dev));
+  // M[(n, d)][b] = sum_s (H_n R2)[(n, d)][s] R1[b][s]
+  Gemm1SlArgs g1;
+  g1.A = HR2; g1.R1t = R1r; g1.Psi = (float2*)ctx->Mc.p; g1.psi_ld = m_ld; g1.psi_batch_stride = n_nd * m_ld;
+  g1.n_rho = (int32_t)n_nd; g1.w2 = ctx->n_ap; g1.n_atoms = nb; g1.drop_tiny = drop_tiny;
+  BIP_TRY(launch_gemm1_sliced(ctx, g1));
+  BIP_TRY(launch_quantize_phi(ctx, g1.Psi, g1.psi_ld, g1.psi_batch_stride, nullptr, Ms, (int32_t)n_nd, (int32_t)Ms.rows_pad, ctx->n_ap, 1, nb));
+  // a[rho][(n, d)] = G^-1/2 sum_b A[rho][b] M[(n, d)][b]; |a|^2 reduced in the epilogue
+  Gemm2SlArgs g2;
+  g2.Phi = Ax; g2.R2 = Ms; g2.rows_pad = (int32_t)rho_pad;
+  g2.n_rho = n_rows; g2.n_det = (int32_t)n_nd; g2.n_out_cols = e.n_det; g2.n_ch = 1; g2.n_atoms = nb;
+  g2.row_idx = row_idx_dev; g2.row_idx_stride = row_idx_stride;
+  g2.inv_G = (float)(1.0 / ((double)ctx->g.ny * ctx->g.nx));
+  g2.mode = mode;
+  g2.bin_of_det = mode == BIP_MODE_QEELS_X ? e.bin_of_det_x_dev : e.bin_of_det_y_dev;
+  g2.n_bins = mode == BIP_MODE_QEELS_X ? (int)e.binx.size() : (int)e.biny.size();
+  g2.out = out; g2.drop_tiny = drop_tiny;
+  {
+    Span s(ctx, sp.pool_map, sp.gemm2);
+    BIP_TRY(launch_gemm2_sliced(ctx, g2));
+  }
+  ctx->timing.gemm2_launches++;
+  ctx->timing.amplitudes += n_rows_total * e.n_ch * e.n_det;
+  ctx->timing.flops += 8.0 * (double)n_nd * ctx->n_ap * ((double)nb * w2 + n_rows_total);
+  return BIP_OK;
+}
+
+// Which association runs for this edge (bip_set_association): the cost model of include/bip.h.
+static bool use_coupling(const bip_ctx* ctx, const Edge& e, double rows_per_site, size_t budget) {
+  if (ctx->assoc == BIP_ASSOC_PROBE) return false;
+  const double w2 = (double)e.w * e.w, nd = (double)e.n_ch * e.n_det, B = ctx->n_ap;
+  if (ctx->assoc == BIP_ASSOC_AUTO) {
+    const double probe = rows_per_site * w2 * (B + nd), coup = nd * B * (w2 + rows_per_site);
+    const double bytes = 8.0 * (nd * w2 + B * w2 + 2.0 * nd * B);
+    return coup < probe && bytes < (double)budget;
+  }
+  return true;
+}
+
 static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, int32_t a0, int32_t nb, int mode, int recon, int fmt, bool drop_tiny, void* out) {
   auto& sp = spans()[ctx];
   const int w2 = e.w * e.w;
@@ -247,6 +315,8 @@ static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, 
     BIP_TRY(launch_gather_rows_sliced(ctx, ctx->A_sl, row_idx_dev, row_idx_stride, Ac, nb));
     Ax = Ac;
   }
+  if (use_coupling(ctx, e, n_rows_total / nb, scratch_budget()))
+    return contract_coupling(ctx, e, org, nb, mode, recon, fmt, drop_tiny, out, Ax, n_rows, rho_pad, row_idx_dev, row_idx_stride, n_rows_total);
   Sliced R1t, R2, Phi;
   BIP_TRY(ensure(ctx, ctx->D1, (size_t)nb * ctx->n_p1 * w2 * sizeof(float2), "D1 (de-tilted S1 windows)"));
   BIP_TRY(ensure(ctx, ctx->D2, (size_t)nb * ctx->n_p2 * w2 * sizeof(float2), "D2 (de-tilted S2 windows)"));
@@ -304,6 +374,7 @@ static int32_t contract_batch(bip_ctx* ctx, Edge& e, const int32_t* origin_dev, 
   const int32_t* org = origin_dev + 2 * (int64_t)a0;
   if (sliced_fmt_of(precision) >= 0) return contract_batch_sliced(ctx, e, org, a0, nb, mode, recon, sliced_fmt_of(precision), precision == BIP_PREC_FP16X3, out);
   if (ctx->crop_fy > 1 || ctx->crop_fx > 1) return fail(ctx, BIP_ERR_UNSUPPORTED, "bip_map: the crop mask needs a tensor-core precision (FP16X4, FP16X3, BF16X6)");
+  if (ctx->assoc == BIP_ASSOC_COUPLING) return fail(ctx, BIP_ERR_UNSUPPORTED, "bip_map: the coupling association needs a tensor-core precision (FP16X4, FP16X3, BF16X6)");
   Planes R1t, R2, Phi;
   BIP_TRY(ensure(ctx, ctx->D1, (size_t)nb * ctx->n_p1 * w2 * sizeof(float2), "D1 (de-tilted S1 windows)"));
   BIP_TRY(ensure(ctx, ctx->D2, (size_t)nb * ctx->n_p2 * w2 * sizeof(float2), "D2 (de-tilted S2 windows)"));
@@ -406,7 +477,13 @@ static int32_t run_edges(bip_ctx* ctx, const std::vector<int32_t>& ids, int mode
                                        el * (round_up(w2, 128) * round_up(ctx->n_ap, 32) + round_up(e.n_det, 128) * round_up(w2, 32) +
                                              round_up(rows_est, 256) * (e.n_ch * round_up(w2, 32) + (ctx->crop_fy * ctx->crop_fx > 1 ? round_up(ctx->n_ap, 32) : 0))) +
                                        (ctx->crop_fy * ctx->crop_fx > 1 ? round_up(ctx->n_rho, 256) * 4 : 0));
-      const int32_t nb_max = (int32_t)std::max<size_t>(1, std::min<size_t>(budget / std::max<size_t>(per_atom, 1), 4096));
+      size_t per_atom_use = per_atom;
+      if (sliced_fmt_of(precision) >= 0 && use_coupling(ctx, e, (double)rows_est, budget)) {
+        const int64_t nd = round_up((int64_t)e.n_ch * e.n_det, 256), Bp = round_up(ctx->n_ap, 128), w2p = round_up(w2, 32);
+        per_atom_use = (size_t)((ctx->n_p1 + ctx->n_p2) * w2 * 8 + el * (nd * w2p + Bp * w2p + nd * round_up(ctx->n_ap, 32)) + 8 * nd * Bp +
+                                (ctx->crop_fy * ctx->crop_fx > 1 ? el * round_up(rows_est, 256) * round_up(ctx->n_ap, 32) + round_up(ctx->n_rho, 256) * 4 : 0));
+      }
+      const int32_t nb_max = (int32_t)std::max<size_t>(1, std::min<size_t>(budget / std::max<size_t>(per_atom_use, 1), 4096));
       Span s(ctx, sp.pool_map, sp.contract);
       for (int32_t a0 = (int32_t)lo; a0 < (int32_t)hi; a0 += nb_max)     // lines 5-8
         BIP_TRY(contract_batch(ctx, e, origin_dev, a0, std::min<int32_t>(nb_max, (int32_t)hi - a0), mode, recon, precision, outs[k]));
@@ -499,7 +576,7 @@ int32_t bip_clear_edges(bip_ctx* ctx) {
   auto& ed = edge_dev()[ctx];
   for (size_t k = 0; k < ctx->edges.size(); ++k) {
     Edge& e = ctx->edges[k];
-    cudaFree(e.H_dev); cudaFree(e.det_h_dev); cudaFree(e.nn_idx_dev); cudaFree(e.nn_w_dev);
+    cudaFree(e.H_dev); cudaFree(e.hmax_dev); cudaFree(e.det_h_dev); cudaFree(e.nn_idx_dev); cudaFree(e.nn_w_dev);
     cudaFree(e.bin_of_det_x_dev); cudaFree(e.bin_of_det_y_dev);
     if (k < ed.size()) cudaFree(ed[k].origin_dev);
   }
@@ -519,7 +596,7 @@ int32_t bip_destroy(bip_ctx* ctx) {
   if (ctx->T_owned) cudaFree((void*)ctx->T_dev);
   void* ptrs[] = {ctx->ap_h_dev, ctx->p1_h_dev, ctx->p2_h_dev, ctx->ap_c_dev, ctx->w1_idx_dev, ctx->w1_w_dev, ctx->rooty_dev,
                   ctx->rootx_dev, ctx->P_dev, ctx->ms_work, ctx->S1, ctx->S2, ctx->D1.p, ctx->D2.p, ctx->R1.p, ctx->R2.p, ctx->Psi.p,
-                  ctx->Phi.p, ctx->R1s.p, ctx->R2s.p, ctx->Phis.p, ctx->Scl.p, ctx->Sync.p, ctx->RowIdx.p, ctx->Acrop.p, ctx->Pmax.p, ctx->rho_dev};
+                  ctx->Phi.p, ctx->R1s.p, ctx->R2s.p, ctx->Phis.p, ctx->Scl.p, ctx->Sync.p, ctx->RowIdx.p, ctx->Acrop.p, ctx->Pmax.p, ctx->R1r.p, ctx->HR2.p, ctx->Mc.p, ctx->Ms.p, ctx->rho_dev};
   free_illumination(ctx);
   for (void* p : ptrs) if (p) cudaFree(p);
   cudaGetLastError();
@@ -580,6 +657,13 @@ int32_t bip_prism_subsample(int32_t n, const int32_t* h, int32_t fy, int32_t fx,
   return BIP_OK;
 }
 
+int32_t bip_set_association(bip_ctx* ctx, int32_t assoc) {
+  if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
+  if (assoc < BIP_ASSOC_PROBE || assoc > BIP_ASSOC_AUTO) return fail(ctx, BIP_ERR_INVALID, "bip_set_association: unknown association %d", assoc);
+  ctx->assoc = assoc;
+  return BIP_OK;
+}
+
 int32_t bip_set_crop(bip_ctx* ctx, int32_t fy, int32_t fx) {
   if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
   if (fy < 1 || fx < 1 || fy > ctx->g.ny / 2 || fx > ctx->g.nx / 2) return fail(ctx, BIP_ERR_INVALID, "bip_set_crop: factors (%d, %d) outside 1..N/2", fy, fx);
@@ -625,6 +709,13 @@ int32_t bip_add_edge(bip_ctx* ctx, int32_t n_atoms, const int32_t* slice, const 
   }
   EdgeDev ed;
   BIP_TRY(upload(ctx, (float**)&e.H_dev, H, 2 * (size_t)n_ch * w * w, "H windows"));
+  std::vector<float> hmax(n_ch, 0.f);
+  for (int n = 0; n < n_ch; ++n)
+    for (size_t s = 0; s < (size_t)w * w; ++s) {
+      const float* h = H + 2 * ((size_t)n * w * w + s);
+      hmax[n] = std::max(hmax[n], 1.0001f * std::hypot(h[0], h[1]));
+    }
+  BIP_TRY(upload(ctx, &e.hmax_dev, hmax.data(), (size_t)n_ch, "H maxima"));
   BIP_TRY(upload(ctx, &e.det_h_dev, det_h, 2 * (size_t)n_det, "detector beams"));
   BIP_TRY(upload(ctx, &e.nn_idx_dev, w2->nn_idx, (size_t)n_det * w2->max_nn, "w2 indices"));
   BIP_TRY(upload(ctx, &e.nn_w_dev, w2->nn_w, (size_t)n_det * w2->max_nn, "w2 weights"));

@@ -84,6 +84,8 @@ struct SlParams {
   float2* Psi; int64_t psi_ld, psi_batch_stride;
   // GEMM2 epilogue
   int mode; float inv_G; const int32_t* bin_of_det; int n_bins; void* out;
+  int n_out_cols;          // detector beams K of the output: column c of the contraction is beam c % K (the coupling
+                           // association runs the channels as extra columns, c = n K + d)
   const int32_t* row_idx; int64_t row_idx_stride;   // crop mask: output scan index of every (site, local row), -1 = none
 };
 
@@ -592,8 +594,9 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
               if (d < p.n_cols) {
                 const float s = __ldg(sy + d);
                 const float v = fmaf(rr[j], rr[j], ri[j] * ri[j]) * (s * s) * f;
-                if (p.mode == BIP_MODE_CUBE) atomicAdd(out + (int64_t)out_row * p.n_cols + d, v);
-                else atomicAdd(out + (int64_t)out_row * p.n_bins + __ldg(p.bin_of_det + d), v);
+                const int dk = d % p.n_out_cols;
+                if (p.mode == BIP_MODE_CUBE) atomicAdd(out + (int64_t)out_row * p.n_out_cols + dk, v);
+                else atomicAdd(out + (int64_t)out_row * p.n_bins + __ldg(p.bin_of_det + dk), v);
               }
             }
           }
@@ -630,8 +633,9 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
             const int c = lane + 32 * k, d = ct * TN + c;
             if (d < p.n_cols) {
               const float v = acc_tile[c * ACC_LD + rl] * p.inv_G;
-              if (p.mode == BIP_MODE_CUBE) atomicAdd(out + (int64_t)orow * p.n_cols + d, v);
-              else atomicAdd(out + (int64_t)orow * p.n_bins + __ldg(p.bin_of_det + d), v);
+              const int dk = d % p.n_out_cols;
+              if (p.mode == BIP_MODE_CUBE) atomicAdd(out + (int64_t)orow * p.n_out_cols + dk, v);
+              else atomicAdd(out + (int64_t)orow * p.n_bins + __ldg(p.bin_of_det + dk), v);
             }
           }
         }
@@ -676,7 +680,7 @@ __global__ void __launch_bounds__(256) k_quantize_phi(const float2* __restrict__
 #pragma unroll
         for (int c = 0; c < QCH; ++c)
           if (c < nch) {
-            const float2 h = __ldg(H + (int64_t)(n0 + c) * w2 + s);
+            const float2 h = H ? __ldg(H + (int64_t)(n0 + c) * w2 + s) : make_float2(1.f, 0.f);
             m[c] = fmaxf(m[c], fmaxf(fabsf(h.x * a.x - h.y * a.y), fabsf(h.x * a.y + h.y * a.x)));
           }
       }
@@ -710,7 +714,7 @@ __global__ void __launch_bounds__(256) k_quantize_phi(const float2* __restrict__
 #pragma unroll
       for (int j = 0; j < 8; ++j) {
         const int s = g * 8 + j;
-        const float2 h = s < w2 ? __ldg(hrow + s) : make_float2(0.f, 0.f);
+        const float2 h = s < w2 ? (H ? __ldg(hrow + s) : make_float2(1.f, 0.f)) : make_float2(0.f, 0.f);
         re[j] = h.x * a[j].x - h.y * a[j].y;
         im[j] = h.x * a[j].y + h.y * a[j].x;
       }
@@ -897,6 +901,7 @@ int32_t launch_gemm2_sliced(bip_ctx* ctx, const Gemm2SlArgs& a) {
   p.n_ch_loop = a.n_ch;
   p.drop_tiny = a.drop_tiny;
   p.n_rows = a.n_rho; p.n_cols = a.n_det;
+  p.n_out_cols = a.n_out_cols > 0 ? a.n_out_cols : a.n_det;
   p.mode = a.mode; p.inv_G = a.inv_G; p.bin_of_det = a.bin_of_det; p.n_bins = a.n_bins; p.out = a.out;
   p.row_idx = a.row_idx; p.row_idx_stride = a.row_idx_stride;
   return launch<EPI_GEMM2>(ctx, p, a.Phi.fmt);

@@ -49,6 +49,7 @@ struct Edge {
   std::vector<int32_t> det_h;          // [n_det][2]
   std::vector<int32_t> binx, biny;     // distinct h_x / h_y ascending
   float2* H_dev = nullptr;             // [n_ch][w*w]
+  float* hmax_dev = nullptr;           // [n_ch] max_s |H_n[s]| (row-scale bound of the coupling operands)
   int32_t* det_h_dev = nullptr;        // [n_det][2]
   int32_t* nn_idx_dev = nullptr;       // [n_det][max_nn]
   float* nn_w_dev = nullptr;           // [n_det][max_nn]
@@ -92,6 +93,8 @@ struct bip_ctx {
   double* rho_dev = nullptr;       // [n_rho][2] scan positions in pixels
   std::vector<double> rho_host;    // the same on the host (crop-mask row lists)
   int32_t crop_fy = 1, crop_fx = 1;  // PRISM crop mask (bip_set_crop); 1 = off
+  int32_t assoc = 0;                 // bip_assoc (bip_set_association)
+  bip::DevBuf R1r, HR2, Mc, Ms;      // coupling association: R1 rows, H_n R2 rows, M (c64) and M sliced
   bip::DevBuf Pmax;                // max_s |D2[p][s]| per (site, parent): row-scale bound of R2
   bip::DevBuf RowIdx, Acrop;       // per-site scan-row lists and gathered illumination rows (crop mask)
   bip::Planes A;                   // illumination [n_rho][n_ap] split planes (K-major over b); built on first use
@@ -198,6 +201,7 @@ struct Gemm2SlArgs {     // a7 + a8
   int32_t n_bins;
   void* out;
   int32_t drop_tiny = 0; // BIP_PREC_FP16X3
+  int32_t n_out_cols = 0;             // 0: = n_det; else column c is detector beam c % n_out_cols (coupling association)
   const int32_t* row_idx = nullptr;   // crop mask: [atom][row_idx_stride] output scan index of each local row, -1 = none
   int64_t row_idx_stride = 0;
 };
@@ -212,7 +216,8 @@ int32_t launch_recon_t_sliced(bip_ctx* ctx, const float2* D, int32_t n_par, cons
                               const int32_t* origin_dev, int32_t n_atoms, int32_t w, Sliced out);
 int32_t launch_recon_rows_sliced(bip_ctx* ctx, const float2* D, int32_t n_par, const int32_t* bh_dev, int32_t n_beams,
                                  const int32_t* nn_idx, const float* nn_w, int32_t max_nn, int carrier, int recon,
-                                 const int32_t* origin_dev, int32_t n_atoms, int32_t w, Sliced out);
+                                 const int32_t* origin_dev, int32_t n_atoms, int32_t w, Sliced out, const float2* H = nullptr, int32_t n_ch = 1,
+                                 const float* hmax = nullptr);
 int32_t launch_illumination_sliced(bip_ctx* ctx, const double* rho_dev, int32_t n_rho, float scale, Sliced out);
 
 }  // namespace bip

@@ -243,7 +243,8 @@ __global__ void __launch_bounds__(256) k_recon_rows_sliced(const float2* __restr
                                     const int32_t* __restrict__ nn_idx, const float* __restrict__ nn_w, int max_nn, int carrier,
                                     int recon, const int32_t* __restrict__ origin, int w, int ny, int nx,
                                     const float2* __restrict__ rooty, const float2* __restrict__ rootx,
-                                    const float* __restrict__ pmax, Sliced out) {
+                                    const float* __restrict__ pmax, const float2* __restrict__ H, int n_ch,
+                                    const float* __restrict__ hmax, Sliced out) {
   // One block per (8 consecutive beams, atom); thread = (row = t & 7, k-group lane = t >> 3).  The blocked slice layout
   // keeps the 16-byte groups of rows r .. r+7 of one k-group side by side, so the 8 row-lanes of a store instruction
   // fill one 128-byte line.  Single pass: the row scale is the power of two above sum_p w_p max_s |D_p[s]|, a bound on
@@ -267,8 +268,11 @@ __global__ void __launch_bounds__(256) k_recon_rows_sliced(const float2* __restr
     if (p < 0) break;
     bound = fmaf(s_w[r][j], __ldg(pmax + (int64_t)a * n_par + p), bound);
   }
-  const float scale = sl_pow2_scale(1.001f * bound), inv = 1.f / scale;
-  if (gl == 0) out.scale[(int64_t)a * out.scale_batch_stride + b] = scale;
+  // H != NULL (coupling association, eq. 13): the rows written are H_n[s] R[b][s], row n * n_beams + b, n = 0 .. n_ch-1
+  const int n_rep = H ? n_ch : 1;
+  if (gl == 0)
+    for (int n = 0; n < n_rep; ++n)
+      out.scale[(int64_t)a * out.scale_batch_stride + (int64_t)n * n_beams + b] = sl_pow2_scale(1.001f * bound * (H ? hmax[n] : 1.f));
   const int oy = origin[2 * a], ox = origin[2 * a + 1];
   const int hyp = ((bh[2 * b] % ny) + ny) % ny, hxp = ((bh[2 * b + 1] % nx) + nx) % nx;
   const float2* Da = D + (int64_t)a * n_par * w2;
@@ -289,7 +293,21 @@ __global__ void __launch_bounds__(256) k_recon_rows_sliced(const float2* __restr
       }
       re[j] = v.x; im[j] = v.y;
     }
-    sl_store_group(out, a, b, g, re, im, inv);
+    if (!H) {
+      sl_store_group(out, a, b, g, re, im, 1.f / sl_pow2_scale(1.001f * bound));
+    } else {
+      for (int n = 0; n < n_ch; ++n) {
+        float hr[8], hi[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const int s = g * 8 + j;
+          const float2 h = s < w2 ? __ldg(H + (int64_t)n * w2 + s) : make_float2(0.f, 0.f);
+          hr[j] = h.x * re[j] - h.y * im[j];
+          hi[j] = h.x * im[j] + h.y * re[j];
+        }
+        sl_store_group(out, a, (int64_t)n * n_beams + b, g, hr, hi, 1.f / sl_pow2_scale(1.001f * bound * hmax[n]));
+      }
+    }
   }
 }
 
@@ -404,7 +422,8 @@ int32_t launch_recon_t_sliced(bip_ctx* ctx, const float2* D, int32_t n_par, cons
 
 int32_t launch_recon_rows_sliced(bip_ctx* ctx, const float2* D, int32_t n_par, const int32_t* bh_dev, int32_t n_beams,
                                  const int32_t* nn_idx, const float* nn_w, int32_t max_nn, int carrier, int recon,
-                                 const int32_t* origin_dev, int32_t n_atoms, int32_t w, Sliced out) {
+                                 const int32_t* origin_dev, int32_t n_atoms, int32_t w, Sliced out, const float2* H, int32_t n_ch,
+                                 const float* hmax) {
   BIP_TRY(ensure(ctx, ctx->Pmax, (size_t)n_atoms * n_par * sizeof(float), "parent window maxima"));
   float* pmax = reinterpret_cast<float*>(ctx->Pmax.p);
   for (int a0 = 0; a0 < n_atoms; a0 += 65535) {          // gridDim.y limit
@@ -419,7 +438,7 @@ int32_t launch_recon_rows_sliced(bip_ctx* ctx, const float2* D, int32_t n_par, c
     dim3 grid((unsigned)((n_beams + 7) / 8), (unsigned)na);
     k_recon_rows_sliced<<<grid, 256, 0, ctx->stream>>>(D + (int64_t)a0 * n_par * w * w, n_par, bh_dev, n_beams, nn_idx, nn_w, max_nn, carrier,
                                                       recon, origin_dev + 2 * (int64_t)a0, w, ctx->g.ny, ctx->g.nx, ctx->rooty_dev,
-                                                      ctx->rootx_dev, pmax + (int64_t)a0 * n_par, o);
+                                                      ctx->rootx_dev, pmax + (int64_t)a0 * n_par, H, n_ch, hmax, o);
     BIP_CUDA(ctx, cudaGetLastError());
     ctx->timing.kernel_launches++;
   }

@@ -364,3 +364,60 @@ def test_many_channels_and_window_as_large_as_the_grid(prec_name):
     assert rel_err_map(cube.cpu().numpy(), I1, 1e-3) <= TOL_PIXEL
     assert rel_err_map(m.cpu().numpy(), I1.sum(1)) <= TOL_PIXEL
     ctx.close()
+
+
+@pytest.mark.parametrize("prec_name", ["fp16x4", "bf16x6"])
+@pytest.mark.parametrize("recon", ["linear", "magphase"])
+def test_coupling_matrix_association(recon, prec_name):
+    """NEXT-2 (eq. 13 as printed, Alg. 4 lines 6-8): coupling matrix M^(n,tau)[d, b] first, then all scans, against the
+    oracle's coupling routine -- configs[0] geometry at half size, ragged everywhere (K = 1101-like odd counts, 5
+    channels run as extra columns, 13 sub-pixel scan positions); then the same with PRISM beams and the crop mask;
+    AUTO must pick the cheaper association by the cost model of include/bip.h."""
+    import torch
+    import paper_2607_00756_b200 as B
+    prec = _prec(prec_name)
+    rc = B.RECON_LINEAR if recon == "linear" else B.RECON_MAGPHASE
+    wl = make_workload("cfg1", scale=2, nz=4, scan=(4, 4))
+    wl.scan = wl.scan[:13] + np.array([0.25, 0.4])
+    e = wl.edges[0].take(np.arange(6))
+    orc = OracleSetup(wl, e)
+    want = orc.run(wl, e, recon, association="coupling")
+    ctx, geo, ids = gpu_context(wl, [e])
+    ctx.set_association(B.ASSOC_COUPLING)
+    m = _first(lambda: ctx.map(0, B.MODE_MAP, rc, prec))
+    qx = ctx.map(0, B.MODE_QEELS_X, rc, prec)
+    cube = ctx.map(0, B.MODE_CUBE, rc, prec)
+    torch.cuda.synchronize()
+    t = ctx.get_timing()
+    nd, Bn, w2 = e.n_ch * geo.det_h.shape[0], geo.ap_h.shape[0], e.W * e.W
+    assert t["flops"] == 8.0 * nd * Bn * (6 * w2 + 6 * 13) and t["amplitudes"] == 13 * 6 * nd   # the coupling path ran
+    assert rel_err_map(m.cpu().numpy(), want["map"]) <= TOL_PIXEL
+    assert abs(float(m.sum()) - want["map"].sum()) <= TOL_SUM * want["map"].sum()
+    assert rel_err_map(qx.cpu().numpy(), want["qeels_x"], 1e-3) <= TOL_PIXEL
+    assert rel_err_map(cube.cpu().numpy(), want["cube"], 1e-3) <= TOL_PIXEL
+    with pytest.raises(B.BipError) as ei:
+        ctx.map(0, B.MODE_MAP, rc, B.PREC_FP32_SIMT)
+    assert ei.value.status == 5
+    # AUTO: 13 scans per site against B = 121-ish beams -> coupling is cheaper; with the mask off and many scans it is not
+    ctx.set_association(B.ASSOC_AUTO)
+    m2 = ctx.map(0, B.MODE_MAP, rc, prec)
+    torch.cuda.synchronize()
+    probe_cost, coup_cost = 13.0 * w2 * (Bn + nd), nd * Bn * (w2 + 13.0)
+    assert (ctx.get_timing()["flops"] == t["flops"]) == (coup_cost < probe_cost)
+    assert rel_err_map(m2.cpu().numpy(), want["map"]) <= TOL_PIXEL
+    ctx.close()
+    # PRISM beam lists + crop mask + coupling
+    wl = make_workload("cfg1", nz=4, scan=(25, 25))
+    wl.scan = wl.scan + np.array([0.37, 0.21])
+    e = wl.edges[0].take(np.array([0, 1, 2, 17, 30]))
+    orc = OracleSetup(wl, e, prism=(2, 2))
+    want = orc.run(wl, e, recon, crop_f=(4, 4), association="coupling")
+    ctx, geo, ids = gpu_context(wl, [e], prism=(2, 2), crop=(4, 4))
+    ctx.set_association(B.ASSOC_COUPLING)
+    m = ctx.map(0, B.MODE_MAP, rc, prec)
+    cube = ctx.map(0, B.MODE_CUBE, rc, prec)
+    torch.cuda.synchronize()
+    assert rel_err_map(m.cpu().numpy(), want["map"], 1e-3) <= TOL_PIXEL
+    assert np.all(m.cpu().numpy()[want["map"] == 0] == 0.0)
+    assert rel_err_map(cube.cpu().numpy(), want["cube"], 1e-3) <= TOL_PIXEL
+    ctx.close()
