@@ -149,7 +149,9 @@ def run_ours(args):
     ctx.build_S1()
     ctx.build_S2()
     ctx.set_scan(wl.scan)
-    ctx.set_crop(*wl.crop)                           # PRISM crop mask of the workload ((1, 1) = none)
+    crop = (args.crop, args.crop) if args.crop else wl.crop
+    ctx.set_crop(*crop)                              # PRISM crop mask of the workload ((1, 1) = none)
+    ctx.set_association({"probe": B.ASSOC_PROBE, "coupling": B.ASSOC_COUPLING, "auto": B.ASSOC_AUTO}[args.assoc])
     eids = [ctx.add_edge(e.slice, e.centre, e.H, geo.det_h, geo.w2) for e in edges]
     torch.cuda.synchronize()
     t_build = ctx.get_timing()
@@ -225,6 +227,16 @@ def run_ours(args):
 
     # ---- roofline of the dominant kernel (a7-a8) ----
     flops_gemm2_step = 8.0 * edge.W * edge.W * amps_step          # a7: 8 W^2 real flops per amplitude (every edge here has the same W)
+    n_b = geo.ap_h.shape[0]
+    rows_total = amps_step / (K * sum(e.n_ch for e in edges) / len(edges)) if len(edges) == 1 else None
+    assoc_ran = "probe"
+    if args.assoc != "probe" and rows_total is not None:
+        # which association the library ran (AUTO decides per edge): its flop count tells -- probe-first counts
+        # 8 W^2 (rows B + amplitudes), the coupling association 8 N_ch K B (sites W^2 + rows)
+        probe_flops = 8.0 * edge.W * edge.W * (rows_total * n_b + amps_step)
+        if abs(float(ctx.get_timing()["flops"]) - probe_flops) > 1e-6 * probe_flops:
+            assoc_ran = "coupling"
+            flops_gemm2_step = 8.0 * n_b * amps_step               # the timed kernel is then a = A M^T: 8 B real flops per amplitude
     achieved = flops_gemm2_step * args.steps / (gemm2_ms * 1e-3) / 1e12 if gemm2_ms > 0 else 0.0
     if args.precision in ("fp16x4", "fp16x3", "bf16x6"):
         bf16_peak = peaks["bf16_tflops"]           # burst figure: the larger, hence the conservative denominator
@@ -268,6 +280,7 @@ def run_ours(args):
             "config": {"workload": f"BASELINE configs[{CONFIG_INDEX.get(args.workload, '?')}] ({wl.name}): {wl.ny}x{wl.nx} grid, {wl.nz} slices, "
                                    f"B={geo.ap_h.shape[0]}, K={K}, parents=({ctx.n_p1},{ctx.n_p2}), parent factor {wl.parent_factor[0]:g}, "
                                    f"W={edge.W}, N_ch={[e.n_ch for e in edges]}, N_rho={ctx.n_rho}, {args.mode} output, recon={args.recon}",
+                       "association": args.assoc, "association_ran": assoc_ran, "crop_mask": list(crop),
                        "atoms_per_step_per_gpu": [e.n_atoms for e in edges], "sampled": "first sites of each edge's first plane(s); the "
                        f"full edges have {[e.n_atoms for e in (wl.edges if args.edges == 'all' else wl.edges[:1])]} sites", "precision": args.precision,
                        "l2": "per-step working set (sliced operands, > 0.5 GB per atom, rewritten every step) exceeds the 126 MB L2: no flush needed",
@@ -364,6 +377,8 @@ def main():
     ap.add_argument("--mode", default="map", choices=["map", "qeels_x", "cube"])
     ap.add_argument("--edges", default="first", choices=["first", "all"], help="all: every edge of the workload shares one plane loop (configs[2])")
     ap.add_argument("--parent-factor", type=float, default=0.0, help="override the workload's parent factor (configs[4] sweeps 1/2/4/8)")
+    ap.add_argument("--assoc", default="probe", choices=["probe", "coupling", "auto"], help="association of the contraction (bip_set_association)")
+    ap.add_argument("--crop", type=int, default=0, help="override the workload's crop-mask factor (0 = the workload's own)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
