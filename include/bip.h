@@ -113,8 +113,9 @@ typedef struct {
   float gemm2_ms;          /* the detector projection kernel alone (dominant kernel)    */
   int32_t gemm2_launches;  /* launches of that kernel in the last bip_map               */
   int32_t kernel_launches; /* all of the library's own kernel launches in the last bip_map (cuFFT excluded) */
-  double amplitudes;       /* scan x atom x channel x detector-beam amplitudes formed   */
-  double flops;            /* algorithmic real flops of a4 + a7: 8 N_rho W^2 (atoms B + events K) */
+  double amplitudes;       /* scan x atom x channel x detector-beam amplitudes formed (scans inside the crop mask only) */
+  double flops;            /* algorithmic real flops of the association that ran: probe-first 8 rows W^2 (B + N_ch K),
+                              coupling 8 N_ch K B (sites W^2 + rows); rows = scan rows contracted (crop mask) */
 } bip_timing;
 
 /* ------------------------------------------------------------------------------------------------------------
