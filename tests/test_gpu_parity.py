@@ -421,3 +421,30 @@ def test_coupling_matrix_association(recon, prec_name):
     assert np.all(m.cpu().numpy()[want["map"] == 0] == 0.0)
     assert rel_err_map(cube.cpu().numpy(), want["cube"], 1e-3) <= TOL_PIXEL
     ctx.close()
+
+
+def test_auto_association_per_edge_in_one_plane_loop():
+    """bip_map_all under BIP_ASSOC_AUTO: two edges of different channel counts share one plane loop and the cost model
+    decides per edge; whatever it picks, each map equals the oracle's."""
+    import torch
+    import paper_2607_00756_b200 as B
+    wl = make_workload("cfg1", scale=2, nz=4, scan=(6, 6))
+    e = wl.edges[0]
+    ea, eb = e.take([0, 1, 2, 5]), e.take([3, 4, 6, 7])
+    eb.H = (eb.H * np.exp(0.7j)).astype(np.complex64)[:1]                        # a one-channel edge (like O-K in configs[2])
+    orc = OracleSetup(wl, e)
+    wa, wb = orc.run(wl, ea, "magphase"), orc.run(wl, eb, "magphase")
+    ctx, geo, ids = gpu_context(wl, [ea, eb])
+    ctx.set_association(B.ASSOC_AUTO)
+    outs = _first(lambda: ctx.map_all(B.MODE_MAP, B.RECON_MAGPHASE, B.PREC_FP16X4))
+    torch.cuda.synchronize()
+    ma, mb = (o.cpu().numpy() for o in outs)
+    assert rel_err_map(ma, wa["map"]) <= TOL_PIXEL and rel_err_map(mb, wb["map"]) <= TOL_PIXEL
+    nb_, w2, rows = geo.ap_h.shape[0], e.W * e.W, 36.0
+    want_flops = 0.0
+    for ed in (ea, eb):                                                         # the cost model of include/bip.h, per edge
+        nd = ed.n_ch * geo.det_h.shape[0]
+        probe, coup = rows * w2 * (nb_ + nd), nd * nb_ * (w2 + rows)
+        want_flops += 8.0 * 4 * min(probe, coup)
+    assert abs(ctx.get_timing()["flops"] - want_flops) <= 1e-9 * want_flops
+    ctx.close()
