@@ -664,43 +664,55 @@ constexpr int QCH = 9;
 __global__ void __launch_bounds__(256) k_quantize_phi(const float2* __restrict__ Psi, int64_t psi_ld, int64_t psi_batch_stride,
                                                       const float2* __restrict__ H, Sliced Phi, int n_rho, int rows_pad, int w2, int n_ch) {
   __shared__ float inv_s[8][QCH];
+  __shared__ int s_max[8][QCH];                      // row maxima as bit patterns (non-negative floats order like ints)
   const int rho0 = blockIdx.x * 8, n0 = blockIdx.y * QCH, atom = blockIdx.z;
   const int nch = min(QCH, n_ch - n0);
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const float2* pbase = Psi + (int64_t)atom * psi_batch_stride;
+  const int n_groups = 2 * (int)Phi.ksteps;
+  if (threadIdx.x < 8 * QCH) s_max[threadIdx.x / QCH][threadIdx.x % QCH] = 0;
+  __syncthreads();
   {
-    const int rho = rho0 + warp;
+    // sweep 1, same thread layout as the split below (row = t & 7, k-group lane = t >> 3): 64 contiguous bytes of Psi
+    // per thread and iteration, independent iterations, the 9 channel maxima in registers
+    const int r1 = threadIdx.x & 7, rho1 = rho0 + r1;
     float m[QCH];
 #pragma unroll
     for (int c = 0; c < QCH; ++c) m[c] = 0.f;
-    if (rho < n_rho) {
-      const float2* prow = pbase + (int64_t)rho * psi_ld;
-      for (int s = lane; s < w2; s += 32) {
-        const float2 a = prow[s];
+    if (rho1 < n_rho) {
+      const float2* prow1 = pbase + (int64_t)rho1 * psi_ld;
+      for (int g = threadIdx.x >> 3; g < n_groups; g += 32) {
 #pragma unroll
-        for (int c = 0; c < QCH; ++c)
-          if (c < nch) {
-            const float2 h = H ? __ldg(H + (int64_t)(n0 + c) * w2 + s) : make_float2(1.f, 0.f);
-            m[c] = fmaxf(m[c], fmaxf(fabsf(h.x * a.x - h.y * a.y), fabsf(h.x * a.y + h.y * a.x)));
+        for (int j = 0; j < 8; ++j) {
+          const int s = g * 8 + j;
+          if (s < w2) {
+            const float2 a = prow1[s];
+#pragma unroll
+            for (int c = 0; c < QCH; ++c)
+              if (c < nch) {
+                const float2 h = H ? __ldg(H + (int64_t)(n0 + c) * w2 + s) : make_float2(1.f, 0.f);
+                m[c] = fmaxf(m[c], fmaxf(fabsf(h.x * a.x - h.y * a.y), fabsf(h.x * a.y + h.y * a.x)));
+              }
           }
+        }
       }
+#pragma unroll
+      for (int c = 0; c < QCH; ++c)
+        if (c < nch) atomicMax(&s_max[r1][c], __float_as_int(m[c]));
     }
-#pragma unroll
-    for (int c = 0; c < QCH; ++c) {
-#pragma unroll
-      for (int o = 16; o; o >>= 1) m[c] = fmaxf(m[c], __shfl_xor_sync(0xffffffffu, m[c], o));
-      if (lane == 0 && c < nch) {
-        const float scale = sl_pow2_scale(m[c]);
-        inv_s[warp][c] = 1.f / scale;
-        if (rho < n_rho) Phi.scale[(int64_t)atom * Phi.scale_batch_stride + (int64_t)(n0 + c) * rows_pad + rho] = scale;
-      }
+  }
+  __syncthreads();
+  if (threadIdx.x < 8 * QCH) {
+    const int rr = threadIdx.x / QCH, c = threadIdx.x % QCH, rho_w = rho0 + rr;
+    if (c < nch) {
+      const float scale = sl_pow2_scale(__int_as_float(s_max[rr][c]));
+      inv_s[rr][c] = 1.f / scale;
+      if (rho_w < n_rho) Phi.scale[(int64_t)atom * Phi.scale_batch_stride + (int64_t)(n0 + c) * rows_pad + rho_w] = scale;
     }
   }
   __syncthreads();
   const int r = threadIdx.x & 7, rho = rho0 + r;
   if (rho >= n_rho) return;
   const float2* prow = pbase + (int64_t)rho * psi_ld;
-  const int n_groups = 2 * (int)Phi.ksteps;
   for (int g = threadIdx.x >> 3; g < n_groups; g += 32) {
     float2 a[8];
 #pragma unroll
