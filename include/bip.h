@@ -19,7 +19,8 @@
  *     context (or of the last failed bip_create / helper call on this thread when ctx == NULL).
  *   - pointers are HOST pointers unless the name ends in _dev.  The library copies every host array it is
  *     given before returning; device buffers passed in are borrowed (never freed) and must stay valid as stated.
- *   - one context per host thread; all device work is enqueued on the CUDA stream given to bip_create
+ *   - one context per host thread (a context keeps all of its state -- plans, events, scratch -- in itself; different
+ *     contexts may be used from different threads at the same time); all device work is enqueued on the CUDA stream given to bip_create
  *     (a cudaStream_t passed as void*; NULL = the legacy default stream).  Calls return after enqueueing unless
  *     stated otherwise; the caller synchronises the stream before reading device outputs.
  *   - there is NO CPU fallback: every entry point that touches a scattering matrix or an output needs a CUDA
@@ -76,8 +77,9 @@ typedef enum { BIP_ASSOC_PROBE = 0, BIP_ASSOC_COUPLING = 1, BIP_ASSOC_AUTO = 2 }
  *   2^-24 of the row maximum at the tensor time of 3xTF32.
  * TF32X3: every real product as a_hi b_hi + a_hi b_lo + a_lo b_hi of TF32 operands, accumulated in one TMEM chain.
  *   The tensor core truncates on accumulation (profiles/r01_tcgen05_rounding_probe.txt): per-pixel error within
- *   1e-4 but the summed intensity is biased by ~ -1.25e-8 per accumulating MMA (-2.6e-5 at configs[0]).  Kept as the
- *   measured A/B case for that finding.
+ *   1e-4 but the summed intensity is biased by ~ -1.25e-8 per accumulating MMA (-2.6e-5 at configs[0]): it does NOT
+ *   meet the 1e-6 summed-intensity bound.  Kept as the measured A/B case for that finding; bip_map refuses it with
+ *   BIP_ERR_UNSUPPORTED unless bip_allow_tf32x3(ctx, 1) has been called.
  * FP32_SIMT: the same contractions on CUDA cores in fp32 -- the A/B reference for the tensor-core kernels. */
 typedef enum { BIP_PREC_TF32X3 = 0, BIP_PREC_FP32_SIMT = 1, BIP_PREC_BF16X6 = 2, BIP_PREC_FP16X4 = 3, BIP_PREC_FP16X3 = 4 } bip_precision;
 
@@ -139,6 +141,14 @@ BIP_API int32_t bip_hexring(const bip_grid* g, int32_t n, const int32_t* h, doub
 /* n_radial = max(1, round(sqrt(n_beams / pi) / factor)) (parent spacing "factor" in beam pixels). */
 BIP_API int32_t bip_n_radial_from_factor(int32_t n_beams, double factor);
 
+/* Parent partition of a beam set by its "parent factor" f (BASELINE.json configs; reading c7) in one call:
+ *   f == 1   the exactness limit: parents = all beams, w = identity;
+ *   f  > 1   hex-ring parents with n_radial = bip_n_radial_from_factor(n, f), n_angular = 6, and their
+ *            Sibson table (eq. 8).
+ * pos_out [cap] parent positions into h (ascending), *n_parent their number; nn_idx_out / nn_w_out [n][max_nn]. */
+BIP_API int32_t bip_partition(const bip_grid* g, int32_t n, const int32_t* h, double qmax, double factor, int32_t max_nn,
+                              int32_t* pos_out, int32_t cap, int32_t* n_parent, int32_t* nn_idx_out, float* nn_w_out);
+
 /* Sibson natural-neighbour weights (eq. 8) of every beam h[n][2] on the parents parent_h[n_parent][2], in
  * physical q coordinates, cells clipped to |q| <= 1024 qmax, delta on a parent, weights < 1e-12 dropped and the
  * row renormalised; row entries in ascending parent number, padded with (-1, 0).
@@ -156,9 +166,12 @@ BIP_API int32_t bip_sibson(const bip_grid* g, int32_t n, const int32_t* h, int32
  *              T_on_device == 0: a host pointer, copied to a device buffer the context owns.
  *   n_ap, ap_h, ap_c   aperture beams h_b [n_ap][2] and coefficients c_b [n_ap][2] (eq. 1).
  *   n_p1, p1_h         S1 parent beams [n_p1][2] (any beams, normally a hex-ring subset of the aperture).
- *   w1                 weights of every aperture beam on the S1 parents (n_rows == n_ap).
+ *   w1                 weights of every aperture beam on the S1 parents (n_rows == n_ap); NULL: the library computes
+ *                      the Sibson table itself (bip_sibson with qmax = the largest |q| of the aperture beams).
  *   n_p2, p2_h         S2 parent (detector-side) beams [n_p2][2].
  *   stream             cudaStream_t as void*.
+ * T must be unimodular (|T| = 1: phase objects without absorption) -- the S2 peel and the backward S1
+ * step undo a slice with conj(T); max ||T|^2 - 1| > 1e-4 is rejected with BIP_ERR_INVALID.
  * The context allocates and owns S1 (n_p1 columns) and S2 (n_p2 columns), c64 [.][ny][nx] each. */
 BIP_API int32_t bip_create(bip_ctx** out, const bip_grid* g, const void* T, int32_t T_on_device,
                    int32_t n_ap, const int32_t* ap_h, const float* ap_c,
@@ -187,6 +200,11 @@ BIP_API int32_t bip_set_scan(bip_ctx* ctx, int32_t n_rho, const double* rho_px);
 BIP_API int32_t bip_prism_subsample(int32_t n, const int32_t* h, int32_t fy, int32_t fx, int32_t* keep_out, int32_t cap,
                                     int32_t* n_keep);
 
+/* Probe coefficients of the retained beams, rescaled by fy * fx: c_out[j] = fy fx c_full[keep[j]],
+ * c_full [n_full][2] (normalised for the FULL aperture, 1 / sqrt(G n_full)), c_out [n_keep][2].  Host only. */
+BIP_API int32_t bip_prism_coeffs(int32_t n_keep, const int32_t* keep, int32_t n_full, const float* c_full, int32_t fy, int32_t fx,
+                                 float* c_out);
+
 /* PRISM crop mask: from now on a site contributes only to the scan positions inside its 1/f window,
  * |rho - tau| < N / (2 f) on both axes (periodic distance from the atom's pixel; reading c19).  fy = fx = 1
  * switches the mask off (the default).  The contraction then runs, per site, over that site's scan rows only: the
@@ -202,7 +220,9 @@ BIP_API int32_t bip_set_association(bip_ctx* ctx, int32_t assoc);
  *   centre_px [n_atoms][2] pixel the atom sits on; the window covers centre - w/2 .. centre + w/2 - 1 (periodic)
  *   H  c64 [n_ch][w][w]    H[n][w/2][w/2] is on the atom's pixel; w even, 8 <= w <= min(ny, nx)
  *   det_h [n_det][2]       detector beams (eq. 5)
- *   w2                     weights of every detector beam on the context's S2 parents (n_rows == n_det)
+ *   w2                     weights of every detector beam on the context's S2 parents (n_rows == n_det); NULL: the
+ *                          library computes the Sibson table itself (qmax = the largest |q| of det_h), once per
+ *                          detector beam list, and keeps it on the context ("cached")
  * Several edges share S1 / S2 and one plane loop.  *edge_id receives 0, 1, ... */
 BIP_API int32_t bip_add_edge(bip_ctx* ctx, int32_t n_atoms, const int32_t* slice, const int32_t* centre_px,
                      int32_t n_ch, int32_t w, const float* H, int32_t n_det, const int32_t* det_h,
@@ -221,7 +241,8 @@ BIP_API int32_t bip_output_size(const bip_ctx* ctx, int32_t edge_id, int32_t mod
  * every site and channel, accumulated into out.
  *   out_dev   MAP: double [n_rho];  QEELS_*: float [n_rho][n_bins];  CUBE: float [n_rho][n_det]
  *             (detector-set order).  Zero-initialised by the call.  out_bytes must match bip_output_size.
- * Returns after enqueueing on the context's stream. */
+ * Returns after enqueueing on the context's stream.  (Under a crop mask the first call after bip_set_crop /
+ * bip_set_scan / bip_add_edge counts every site's scan rows on the device and reads the counts back once.) */
 BIP_API int32_t bip_map(bip_ctx* ctx, int32_t edge_id, int32_t mode, int32_t recon, int32_t precision,
                 void* out_dev, size_t out_bytes);
 
@@ -234,6 +255,23 @@ BIP_API int32_t bip_map_host(bip_ctx* ctx, int32_t edge_id, int32_t mode, int32_
  * per edge, same layout as bip_map. */
 BIP_API int32_t bip_map_all(bip_ctx* ctx, int32_t mode, int32_t recon, int32_t precision,
                     void* const* outs_dev, const size_t* outs_bytes, int32_t n_outs);
+
+/* Device scratch the plane loop may use for the operands of one batch of sites (default 12 GB, minimum 32 MB): the
+ * sites of a plane are contracted in batches that fit. */
+BIP_API int32_t bip_set_scratch_budget(bip_ctx* ctx, size_t bytes);
+
+/* Opt in (allow != 0) to BIP_PREC_TF32X3, which misses the 1e-6 summed-intensity bound (see bip_precision). */
+BIP_API int32_t bip_allow_tf32x3(bip_ctx* ctx, int32_t allow);
+
+/* Parent beams of S1 (which = 1) or S2 (which = 2) as the context holds them: h_out [cap][2], *n_out their number
+ * (h_out may be NULL to query it) -- for the bit-exact index comparison against the oracle. */
+BIP_API int32_t bip_get_parents(const bip_ctx* ctx, int32_t which, int32_t* h_out, int32_t cap, int32_t* n_out);
+
+/* The ELL weight table in use: edge_id < 0: w^(1) (aperture beams on S1 parents); else w^(2) of that edge (given by
+ * the caller or computed by the library).  *n_rows, *max_nn: its shape; nn_idx_out / nn_w_out [n_rows][max_nn] may be
+ * NULL to query the shape only. */
+BIP_API int32_t bip_get_weights(const bip_ctx* ctx, int32_t edge_id, int32_t* n_rows, int32_t* max_nn, int32_t* nn_idx_out,
+                                float* nn_w_out);
 
 /* Window origins (centre - w/2) mod N of an edge's atoms, int32 [n_atoms][2] -- for bit-exact index checks. */
 BIP_API int32_t bip_get_windows(const bip_ctx* ctx, int32_t edge_id, int32_t* origin_out);

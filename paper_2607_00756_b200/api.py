@@ -64,7 +64,8 @@ ABI_SYMBOLS = (
     "bip_destroy", "bip_last_error", "bip_build_S1", "bip_build_S2", "bip_set_scan", "bip_add_edge", "bip_clear_edges",
     "bip_output_size", "bip_map", "bip_map_host", "bip_map_all", "bip_get_windows", "bip_get_qeels_bins",
     "bip_seek_plane", "bip_copy_S", "bip_debug_reconstruct", "bip_get_timing", "bip_version", "bip_prism_subsample",
-    "bip_set_crop", "bip_set_association",
+    "bip_set_crop", "bip_set_association", "bip_prism_coeffs", "bip_partition", "bip_set_scratch_budget", "bip_allow_tf32x3",
+    "bip_get_parents", "bip_get_weights",
 )
 
 _lib: Optional[C.CDLL] = None
@@ -155,6 +156,29 @@ def bip_sibson(g: Grid, h: np.ndarray, parent_h: np.ndarray, qmax: float, max_nn
     return idx, w
 
 
+def bip_prism_coeffs(keep: np.ndarray, c_full: np.ndarray, fy: int, fx: int) -> np.ndarray:
+    """Coefficients of the retained beams rescaled by fy * fx."""
+    keep = _i32(keep)
+    c_full = np.ascontiguousarray(c_full, dtype=np.float32)
+    out = np.empty((keep.shape[0], 2), dtype=np.float32)
+    _check(load_library().bip_prism_coeffs(keep.shape[0], _p(keep, C.c_int32), c_full.shape[0], _p(c_full, C.c_float), int(fy), int(fx),
+                                           _p(out, C.c_float)))
+    return out
+
+
+def bip_partition(g: Grid, h: np.ndarray, qmax: float, factor: float, max_nn: int = 8):
+    """Parents (positions into h) and ELL weight table of a beam set for a parent factor (f = 1: identity)."""
+    h = _i32(h)
+    pos = np.empty(h.shape[0], dtype=np.int32)
+    n = C.c_int32(0)
+    idx = np.empty((h.shape[0], max_nn), dtype=np.int32)
+    w = np.empty((h.shape[0], max_nn), dtype=np.float32)
+    gc = g.c()
+    _check(load_library().bip_partition(C.byref(gc), h.shape[0], _p(h, C.c_int32), C.c_double(qmax), C.c_double(factor), int(max_nn),
+                                        _p(pos, C.c_int32), pos.shape[0], C.byref(n), _p(idx, C.c_int32), _p(w, C.c_float)))
+    return pos[: n.value].copy(), (idx, w)
+
+
 def _weights(idx: np.ndarray, w: np.ndarray):
     idx = _i32(idx)
     w = np.ascontiguousarray(w, dtype=np.float32)
@@ -186,30 +210,19 @@ class Geometry:
 
 def plan_geometry(g: Grid, alpha_mrad: float, det_mrad: float, defocus: float, parent_factor: Sequence[float],
                   max_nn: int = 8, prism: Sequence[int] = (1, 1)) -> Geometry:
-    """Aperture / detector beams (eq. 5), hex-ring parents and Sibson tables (eq. 8) through the
-    library's own helpers.  parent_factor f = 1 is the exactness limit: parents = all beams, w = I.
-    ``prism`` = (f_y, f_x) keeps every f-th beam of both sets and rescales the probe coefficients by f_y f_x
-    (PAPER.md:129); parents and weights are then chosen among the retained beams."""
+    """Aperture / detector beams (eq. 5), hex-ring parents and Sibson tables (eq. 8): a sequence of calls
+    into the library (bip_beams_in_disc, bip_aperture_coeffs, bip_prism_subsample, bip_prism_coeffs, bip_partition) --
+    no arithmetic here.  ``prism`` = (f_y, f_x) keeps every f-th beam of both sets."""
     qa, qd = alpha_mrad * 1e-3 / g.lam, det_mrad * 1e-3 / g.lam
     ap_h = bip_beams_in_disc(g, qa)
     det_h = bip_beams_in_disc(g, qd)
     ap_c = bip_aperture_coeffs(g, ap_h, defocus)
     if tuple(prism) != (1, 1):
         keep = bip_prism_subsample(ap_h, prism[0], prism[1])
-        ap_h, ap_c = ap_h[keep], (ap_c[keep] * np.float32(prism[0] * prism[1])).astype(np.float32)
+        ap_h, ap_c = ap_h[keep], bip_prism_coeffs(keep, ap_c, prism[0], prism[1])
         det_h = det_h[bip_prism_subsample(det_h, prism[0], prism[1])]
-
-    def part(h, q, f):
-        if f == 1:
-            pos = np.arange(h.shape[0], dtype=np.int32)
-            idx = np.full((h.shape[0], 1), -1, dtype=np.int32)
-            idx[:, 0] = pos
-            return pos, (idx, np.ones((h.shape[0], 1), dtype=np.float32))
-        pos = bip_hexring(g, h, q, bip_n_radial_from_factor(h.shape[0], f))
-        return pos, bip_sibson(g, h, h[pos], q, max_nn)
-
-    p1_pos, w1 = part(ap_h, qa, parent_factor[0])
-    p2_pos, w2 = part(det_h, qd, parent_factor[1])
+    p1_pos, w1 = bip_partition(g, ap_h, qa, parent_factor[0], max_nn)
+    p2_pos, w2 = bip_partition(g, det_h, qd, parent_factor[1], max_nn)
     return Geometry(ap_h, ap_c, p1_pos, w1, det_h, p2_pos, w2, qa, qd)
 
 
@@ -223,7 +236,7 @@ class Context:
         self._ctx = C.c_void_p(None)
         ap_h, p1_h, p2_h = _i32(ap_h), _i32(p1_h), _i32(p2_h)
         ap_c = np.ascontiguousarray(ap_c, dtype=np.float32)
-        w1s, keep = _weights(*w1)
+        w1s, keep = _weights(*w1) if w1 is not None else (None, None)     # None: the library computes the Sibson table
         if isinstance(T, np.ndarray):
             T = np.ascontiguousarray(T, dtype=np.complex64)
             assert T.shape == (g.nz, g.ny, g.nx)
@@ -237,7 +250,7 @@ class Context:
         gc = g.c()
         _check(self._lib.bip_create(C.byref(self._ctx), C.byref(gc), C.c_void_p(t_ptr), on_dev, ap_h.shape[0],
                                     _p(ap_h, C.c_int32), _p(ap_c, C.c_float), p1_h.shape[0], _p(p1_h, C.c_int32),
-                                    C.byref(w1s), p2_h.shape[0], _p(p2_h, C.c_int32), C.c_void_p(stream)))
+                                    C.byref(w1s) if w1s is not None else None, p2_h.shape[0], _p(p2_h, C.c_int32), C.c_void_p(stream)))
         self.n_ap, self.n_p1, self.n_p2 = ap_h.shape[0], p1_h.shape[0], p2_h.shape[0]
         self.n_rho = 0
         self._edges = []
@@ -275,14 +288,20 @@ class Context:
         """PRISM crop mask: sites contribute only to the scans within N / (2 f) of them; (1, 1) = off."""
         self._ck(self._lib.bip_set_crop(self._ctx, int(fy), int(fx)))
 
-    def add_edge(self, slice_, centre_px, H, det_h, w2) -> int:
+    def set_scratch_budget(self, n_bytes: int):
+        self._ck(self._lib.bip_set_scratch_budget(self._ctx, C.c_size_t(int(n_bytes))))
+
+    def allow_tf32x3(self, allow: bool = True):
+        self._ck(self._lib.bip_allow_tf32x3(self._ctx, int(bool(allow))))
+
+    def add_edge(self, slice_, centre_px, H, det_h, w2=None) -> int:
         slice_, centre_px, det_h = _i32(slice_), _i32(centre_px), _i32(det_h)
         H = np.ascontiguousarray(H, dtype=np.complex64)
-        w2s, keep = _weights(*w2)
+        w2s, keep = _weights(*w2) if w2 is not None else (None, None)     # None: the library computes the Sibson table
         eid = C.c_int32(-1)
         self._ck(self._lib.bip_add_edge(self._ctx, slice_.shape[0], _p(slice_, C.c_int32), _p(centre_px, C.c_int32), H.shape[0],
                                         H.shape[1], C.c_void_p(H.ctypes.data), det_h.shape[0], _p(det_h, C.c_int32),
-                                        C.byref(w2s), C.byref(eid)))
+                                        C.byref(w2s) if w2s is not None else None, C.byref(eid)))
         self._edges.append((slice_.shape[0], H.shape[0], H.shape[1], det_h.shape[0]))
         return eid.value
 
@@ -329,6 +348,22 @@ class Context:
         out = np.empty(shape, dtype=dt)
         self._ck(self._lib.bip_map_host(self._ctx, edge_id, mode, recon, precision, C.c_void_p(out.ctypes.data), C.c_size_t(out.nbytes)))
         return out
+
+    def get_parents(self, which: int) -> np.ndarray:
+        n = C.c_int32(0)
+        self._ck(self._lib.bip_get_parents(self._ctx, int(which), None, 0, C.byref(n)))
+        h = np.empty((n.value, 2), dtype=np.int32)
+        self._ck(self._lib.bip_get_parents(self._ctx, int(which), _p(h, C.c_int32), n.value, C.byref(n)))
+        return h
+
+    def get_weights(self, edge_id: int = -1) -> Tuple[np.ndarray, np.ndarray]:
+        """ELL table in use: edge_id < 0: w1; else the edge's w2."""
+        rows, nn = C.c_int32(0), C.c_int32(0)
+        self._ck(self._lib.bip_get_weights(self._ctx, int(edge_id), C.byref(rows), C.byref(nn), None, None))
+        idx = np.empty((rows.value, nn.value), dtype=np.int32)
+        w = np.empty((rows.value, nn.value), dtype=np.float32)
+        self._ck(self._lib.bip_get_weights(self._ctx, int(edge_id), C.byref(rows), C.byref(nn), _p(idx, C.c_int32), _p(w, C.c_float)))
+        return idx, w
 
     def get_windows(self, edge_id: int) -> np.ndarray:
         o = np.empty((self._edges[edge_id][0], 2), dtype=np.int32)

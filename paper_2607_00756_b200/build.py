@@ -1,6 +1,9 @@
 """Build libbip.so in-tree with nvcc for sm_100a (no GPU needed: nvcc cross-compiles).
 
-    python -m paper_2607_00756_b200.build [--force] [--verbose]
+    python -m paper_2607_00756_b200.build [--force] [--verbose] [--tuning]
+
+--tuning compiles with -DBIP_TUNING: only then does the library read the BIP_TUNE_* launch-shape environment variables
+(experiments); the shipped build ignores them.
 
 The CUDA runtime is linked statically and nothing links libcuda, so the library loads on a box with
 no GPU driver (the CPU test box); cuFFT is the toolkit's shared library, found through an rpath.
@@ -25,18 +28,18 @@ COMMON = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-l
           "-Xcompiler", "-fPIC,-fvisibility=hidden,-ffp-contract=off,-Wall,-Wno-unknown-pragmas", "-I", os.path.join(HERE, "..", "include")]
 
 
-def _stamp() -> str:
-    h = hashlib.sha256()
+def _stamp(tuning: bool = False) -> str:
+    h = hashlib.sha256(b"tuning" if tuning else b"")
     for name in sorted(os.listdir(CSRC)) + ["../../include/bip.h", "../build.py"]:
         with open(os.path.join(CSRC, name), "rb") as f:
             h.update(name.encode() + b"\0" + f.read())
     return h.hexdigest()
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, tuning: bool = False) -> str:
     os.makedirs(BUILD, exist_ok=True)
     stamp_file = os.path.join(BUILD, "stamp")
-    stamp = _stamp()
+    stamp = _stamp(tuning)
     if not force and os.path.exists(LIB) and os.path.exists(stamp_file) and open(stamp_file).read() == stamp:
         return LIB
     if not os.path.exists(NVCC):
@@ -44,7 +47,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
     def compile_one(src: str) -> str:
         obj = os.path.join(BUILD, os.path.splitext(src)[0] + ".o")
-        cmd = [NVCC, *COMMON, "-x", "cu" if src.endswith(".cu") else "c++", "-c", os.path.join(CSRC, src), "-o", obj]
+        cmd = [NVCC, *COMMON, *(["-DBIP_TUNING"] if tuning else []), "-x", "cu" if src.endswith(".cu") else "c++", "-c",
+               os.path.join(CSRC, src), "-o", obj]
         if verbose and src.endswith(".cu"):
             cmd.insert(1, "-Xptxas=-v")
         r = subprocess.run(cmd, capture_output=True, text=True)
@@ -71,4 +75,4 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, tuning="--tuning" in sys.argv))

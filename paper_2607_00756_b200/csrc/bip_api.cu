@@ -150,6 +150,35 @@ static int32_t check_weights(bip_ctx* ctx, const bip_weights* w, int32_t n_rows,
   return BIP_OK;
 }
 
+
+// w == NULL at the ABI: the library computes the Sibson table itself (eq. 8; "computed once per aperture
+// and cached").  The Voronoi cells are clipped to 1024 qmax with qmax = the largest |q| of the beam set being
+// reconstructed; parents = beams (every beam coincides with a parent) gives the identity table.
+static int32_t auto_weights(bip_ctx* ctx, const bip_grid& g, int32_t n, const int32_t* h, int32_t n_par, const int32_t* par_h,
+                            std::vector<int32_t>& idx, std::vector<float>& w, int32_t& max_nn) {
+  double q2 = 0;
+  for (int32_t b = 0; b < n; ++b) {
+    const double qy = h[2 * b] / g.ly, qx = h[2 * b + 1] / g.lx;
+    q2 = std::max(q2, qy * qy + qx * qx);
+  }
+  const double qmax = q2 > 0 ? std::sqrt(q2) : 1.0 / std::max(g.ly, g.lx);
+  for (int32_t nn : {8, BIP_MAX_NN}) {
+    idx.assign((size_t)n * nn, -1);
+    w.assign((size_t)n * nn, 0.f);
+    const int32_t st = bip_sibson(&g, n, h, n_par, par_h, qmax, nn, idx.data(), w.data());
+    if (st == BIP_OK) { max_nn = nn; return BIP_OK; }
+    if (nn == BIP_MAX_NN) return fail(ctx, st, "automatic Sibson table: %s", bip_last_error(nullptr));
+  }
+  return BIP_OK;
+}
+
+static uint64_t fnv1a(const void* data, size_t bytes) {
+  const unsigned char* p = static_cast<const unsigned char*>(data);
+  uint64_t hsh = 1469598103934665603ull;
+  for (size_t i = 0; i < bytes; ++i) { hsh ^= p[i]; hsh *= 1099511628211ull; }
+  return hsh;
+}
+
 static int32_t check_beams(bip_ctx* ctx, const bip_grid& g, int32_t n, const int32_t* h, const char* what) {
   if (n <= 0 || !h) return fail(ctx, BIP_ERR_INVALID, "%s: empty beam list", what);
   for (int32_t i = 0; i < n; ++i)
@@ -158,55 +187,37 @@ static int32_t check_beams(bip_ctx* ctx, const bip_grid& g, int32_t n, const int
   return BIP_OK;
 }
 
-struct EventPool {
-  std::vector<cudaEvent_t> all;
-  size_t used = 0;
-  cudaEvent_t get() {
-    if (used == all.size()) { cudaEvent_t e; cudaEventCreate(&e); all.push_back(e); }
-    return all[used++];
-  }
-  void reset() { used = 0; }
-  void destroy() { for (auto e : all) cudaEventDestroy(e); all.clear(); used = 0; }
-};
-
-struct Spans {
-  EventPool pool_map, pool_b1, pool_b2;
-  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> adv, contract, gemm2, build1, build2;
-};
-static std::map<const bip_ctx*, Spans>& spans() { static std::map<const bip_ctx*, Spans> m; return m; }
-
 struct Span {
-  bip_ctx* ctx; std::vector<std::pair<cudaEvent_t, cudaEvent_t>>* v; cudaEvent_t a, b;
-  Span(bip_ctx* c, EventPool& pool, std::vector<std::pair<cudaEvent_t, cudaEvent_t>>& vec) : ctx(c), v(&vec) {
+  bip_ctx* ctx; SpanList* v; cudaEvent_t a, b;
+  Span(bip_ctx* c, EventPool& pool, SpanList& vec) : ctx(c), v(&vec) {
     a = pool.get(); b = pool.get(); cudaEventRecord(a, c->stream);
   }
   ~Span() { cudaEventRecord(b, ctx->stream); v->push_back({a, b}); }
 };
 
-static float sum_ms(std::vector<std::pair<cudaEvent_t, cudaEvent_t>>& v) {
+static float sum_ms(SpanList& v) {
   float t = 0;
   for (auto& p : v) { float ms = 0; if (cudaEventElapsedTime(&ms, p.first, p.second) == cudaSuccess) t += ms; }
   return t;
 }
 
+// Move the plane cursor.  S1 forward: eq. 6.  S1 backward: either the inverse steps T_j* P* (exact for |T| = 1, checked by
+// bip_create) or a restart from the analytic plane waves of plane 0 followed by forward steps, whichever needs fewer
+// slice steps -- the restart also discards the rounding accumulated by earlier passes.  S2 forward: the peel
+// P*[T_j* .]; backward: the build recursion T_j P[.] itself (eq. 12), exact for any T.  A counter moves only after its
+// step has been enqueued successfully.
 static int32_t seek(bip_ctx* ctx, int32_t plane) {
   if (!ctx->s1_built || !ctx->s2_built) return fail(ctx, BIP_ERR_STATE, "bip_build_S1 and bip_build_S2 must run before the plane loop");
   if (plane < 0 || plane > ctx->g.nz) return fail(ctx, BIP_ERR_INVALID, "plane %d outside 0..%d", plane, ctx->g.nz);
+  if (plane < ctx->plane1 && plane <= ctx->plane1 - plane) {
+    BIP_TRY(ms_plane_waves(ctx, ctx->S1, ctx->p1_h_dev, ctx->n_p1, +1));
+    ctx->plane1 = 0;
+  }
   while (ctx->plane1 < plane) { BIP_TRY(ms_step_S1(ctx, ctx->plane1, +1)); ctx->plane1++; }
-  while (ctx->plane1 > plane) { ctx->plane1--; BIP_TRY(ms_step_S1(ctx, ctx->plane1, -1)); }
+  while (ctx->plane1 > plane) { BIP_TRY(ms_step_S1(ctx, ctx->plane1 - 1, -1)); ctx->plane1--; }
   while (ctx->plane2 < plane) { BIP_TRY(ms_step_S2(ctx, ctx->plane2, +1)); ctx->plane2++; }
-  while (ctx->plane2 > plane) { ctx->plane2--; BIP_TRY(ms_step_S2(ctx, ctx->plane2, -1)); }
+  while (ctx->plane2 > plane) { BIP_TRY(ms_step_S2(ctx, ctx->plane2 - 1, -1)); ctx->plane2--; }
   return BIP_OK;
-}
-
-struct EdgeDev { int32_t* origin_dev = nullptr; };
-static std::map<const bip_ctx*, std::vector<EdgeDev>>& edge_dev() { static std::map<const bip_ctx*, std::vector<EdgeDev>> m; return m; }
-
-static size_t scratch_budget() {
-  const char* e = std::getenv("BIP_SCRATCH_GB");
-  double gb = e ? std::atof(e) : 12.0;
-  if (!(gb > 0.05)) gb = 0.05;
-  return (size_t)(gb * (double)(1ull << 30));
 }
 
 // Steps a1-a8 on the sliced 16-bit operands (BIP_PREC_FP16X4 / BIP_PREC_BF16X6).
@@ -217,7 +228,7 @@ static size_t scratch_budget() {
 static int32_t contract_coupling(bip_ctx* ctx, Edge& e, const int32_t* org, int32_t nb, int mode, int recon, int fmt, bool drop_tiny,
                                  void* out, const Sliced& Ax, int32_t n_rows, int64_t rho_pad, const int32_t* row_idx_dev,
                                  int64_t row_idx_stride, double n_rows_total) {
-  auto& sp = spans()[ctx];
+  auto& sp = ctx->spans;
   const int w2 = e.w * e.w;
   const int64_t n_nd = (int64_t)e.n_ch * e.n_det;                 // rows (n, d) = n K + d
   Sliced R1r, HR2, Ms;
@@ -278,8 +289,25 @@ static bool use_coupling(const bip_ctx* ctx, const Edge& e, double rows_per_site
   return true;
 }
 
-static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, int32_t a0, int32_t nb, int mode, int recon, int fmt, bool drop_tiny, void* out) {
-  auto& sp = spans()[ctx];
+// Crop mask: the number of scan rows inside every site's window, counted on the device once per (edge,
+// crop setting, scan) and kept on the host -- the per-batch launches below are then sized without a device round trip.
+static int32_t ensure_crop_counts(bip_ctx* ctx, Edge& e) {
+  if (e.crop_counts_fy == ctx->crop_fy && e.crop_counts_fx == ctx->crop_fx && (int32_t)e.crop_counts.size() == e.n_atoms) return BIP_OK;
+  e.crop_counts.assign(e.n_atoms, 0);
+  if (e.n_atoms > 0) {
+    BIP_TRY(ensure(ctx, ctx->RowIdx, (size_t)e.n_atoms * sizeof(int32_t), "crop-mask row counts"));
+    int32_t* counts_dev = reinterpret_cast<int32_t*>(ctx->RowIdx.p);
+    BIP_TRY(launch_crop_rows(ctx, e.origin_dev, e.n_atoms, e.w, nullptr, 0, counts_dev));
+    BIP_CUDA(ctx, cudaMemcpyAsync(e.crop_counts.data(), counts_dev, (size_t)e.n_atoms * sizeof(int32_t), cudaMemcpyDeviceToHost, ctx->stream));
+    BIP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+  }
+  e.crop_counts_fy = ctx->crop_fy; e.crop_counts_fx = ctx->crop_fx;
+  return BIP_OK;
+}
+
+static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, int32_t a0, int32_t nb, int mode, int recon, int fmt, bool drop_tiny,
+                                     bool coupling, void* out) {
+  auto& sp = ctx->spans;
   const int w2 = e.w * e.w;
   // scan rows of the contraction: all of them, or (crop mask) each site's own list, gathered into a per-site A operand
   const bool crop = ctx->crop_fy > 1 || ctx->crop_fx > 1;
@@ -290,17 +318,14 @@ static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, 
   int64_t rho_pad = round_up(ctx->n_rho, 2 * SL_ROWS);    // X operands are padded to pairs of row tiles (CTA-pair kernel)
   Sliced Ax = ctx->A_sl;
   if (crop) {
-    // per-site scan-row lists on the device (k_crop_rows), their lengths back on the host
+    // per-site scan-row lists on the device (k_crop_rows); their lengths are already on the host (ensure_crop_counts)
     const int64_t idx_stride = round_up(ctx->n_rho, 2 * SL_ROWS);
     BIP_TRY(ensure(ctx, ctx->RowIdx, ((size_t)nb * idx_stride + nb) * sizeof(int32_t), "crop-mask row lists"));
     int32_t* rows_dev = reinterpret_cast<int32_t*>(ctx->RowIdx.p);
     int32_t* counts_dev = rows_dev + (size_t)nb * idx_stride;
     BIP_TRY(launch_crop_rows(ctx, org, nb, e.w, rows_dev, idx_stride, counts_dev));
-    std::vector<int32_t> counts(nb);
-    BIP_CUDA(ctx, cudaMemcpyAsync(counts.data(), counts_dev, nb * sizeof(int32_t), cudaMemcpyDeviceToHost, ctx->stream));
-    BIP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     n_rows = 1; n_rows_total = 0;
-    for (int32_t c : counts) { n_rows = std::max(n_rows, c); n_rows_total += c; }
+    for (int32_t a = a0; a < a0 + nb; ++a) { n_rows = std::max(n_rows, e.crop_counts[a]); n_rows_total += e.crop_counts[a]; }
     rho_pad = round_up(n_rows, 2 * SL_ROWS);
     row_idx_dev = rows_dev;
     row_idx_stride = idx_stride;
@@ -315,7 +340,7 @@ static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, 
     BIP_TRY(launch_gather_rows_sliced(ctx, ctx->A_sl, row_idx_dev, row_idx_stride, Ac, nb));
     Ax = Ac;
   }
-  if (use_coupling(ctx, e, n_rows_total / nb, scratch_budget()))
+  if (coupling)
     return contract_coupling(ctx, e, org, nb, mode, recon, fmt, drop_tiny, out, Ax, n_rows, rho_pad, row_idx_dev, row_idx_stride, n_rows_total);
   Sliced R1t, R2, Phi;
   BIP_TRY(ensure(ctx, ctx->D1, (size_t)nb * ctx->n_p1 * w2 * sizeof(float2), "D1 (de-tilted S1 windows)"));
@@ -368,11 +393,11 @@ static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, 
 
 // Steps a1-a8 for atoms [a0, a0 + nb) of one edge, all sitting in the current plane.
 static int32_t contract_batch(bip_ctx* ctx, Edge& e, const int32_t* origin_dev, int32_t a0, int32_t nb, int mode, int recon,
-                              int precision, void* out) {
-  auto& sp = spans()[ctx];
+                              int precision, bool coupling, void* out) {
+  auto& sp = ctx->spans;
   const int w2 = e.w * e.w;
   const int32_t* org = origin_dev + 2 * (int64_t)a0;
-  if (sliced_fmt_of(precision) >= 0) return contract_batch_sliced(ctx, e, org, a0, nb, mode, recon, sliced_fmt_of(precision), precision == BIP_PREC_FP16X3, out);
+  if (sliced_fmt_of(precision) >= 0) return contract_batch_sliced(ctx, e, org, a0, nb, mode, recon, sliced_fmt_of(precision), precision == BIP_PREC_FP16X3, coupling, out);
   if (ctx->crop_fy > 1 || ctx->crop_fx > 1) return fail(ctx, BIP_ERR_UNSUPPORTED, "bip_map: the crop mask needs a tensor-core precision (FP16X4, FP16X3, BF16X6)");
   if (ctx->assoc == BIP_ASSOC_COUPLING) return fail(ctx, BIP_ERR_UNSUPPORTED, "bip_map: the coupling association needs a tensor-core precision (FP16X4, FP16X3, BF16X6)");
   Planes R1t, R2, Phi;
@@ -439,6 +464,9 @@ static int32_t run_edges(bip_ctx* ctx, const std::vector<int32_t>& ids, int mode
   if (precision != BIP_PREC_TF32X3 && precision != BIP_PREC_FP32_SIMT && precision != BIP_PREC_BF16X6 && precision != BIP_PREC_FP16X4 && precision != BIP_PREC_FP16X3) return fail(ctx, BIP_ERR_INVALID, "bip_map: unknown precision %d", precision);
   if (precision == BIP_PREC_FP16X3 && mode == BIP_MODE_CUBE)
     return fail(ctx, BIP_ERR_UNSUPPORTED, "bip_map: FP16X3 drops the x2 y2 products and is offered for the reduced outputs (MAP, QEELS) only; use FP16X4 for the cube");
+  if (precision == BIP_PREC_TF32X3 && !ctx->allow_tf32x3)
+    return fail(ctx, BIP_ERR_UNSUPPORTED, "bip_map: TF32X3 biases the summed intensity by ~1.25e-8 per accumulating MMA (beyond the 1e-6 bound); "
+                "call bip_allow_tf32x3(ctx, 1) to run it as the A/B case, or use FP16X4");
   if (precision != BIP_PREC_FP32_SIMT && !tc_available()) return fail(ctx, BIP_ERR_UNSUPPORTED, "bip_map: the tensor-core path is not built");
   for (size_t k = 0; k < ids.size(); ++k) {
     if (ids[k] < 0 || ids[k] >= (int)ctx->edges.size()) return fail(ctx, BIP_ERR_INVALID, "bip_map: edge %d does not exist", ids[k]);
@@ -448,7 +476,7 @@ static int32_t run_edges(bip_ctx* ctx, const std::vector<int32_t>& ids, int mode
     if (outs_bytes[k] != need) return fail(ctx, BIP_ERR_INVALID, "bip_map: output %zu has %zu bytes, expected %zu", k, outs_bytes[k], need);
   }
   BIP_TRY(ensure_illumination(ctx, precision));
-  auto& sp = spans()[ctx];
+  auto& sp = ctx->spans;
   sp.adv.clear(); sp.contract.clear(); sp.gemm2.clear();
   sp.pool_map.reset();
   ctx->timing.gemm2_launches = 0; ctx->timing.kernel_launches = 0; ctx->timing.amplitudes = 0; ctx->timing.flops = 0;
@@ -458,35 +486,43 @@ static int32_t run_edges(bip_ctx* ctx, const std::vector<int32_t>& ids, int mode
   for (int32_t id : ids) for (int32_t s : ctx->edges[id].slice) planes.push_back(s);
   std::sort(planes.begin(), planes.end());
   planes.erase(std::unique(planes.begin(), planes.end()), planes.end());
-  const size_t budget = scratch_budget();
+  const size_t budget = ctx->scratch_budget;
+  const bool crop = ctx->crop_fy * ctx->crop_fx > 1;
+  if (crop && sliced_fmt_of(precision) >= 0)
+    for (int32_t id : ids) BIP_TRY(ensure_crop_counts(ctx, ctx->edges[id]));
   for (int32_t plane : planes) {                                         // Alg. 5 line 3
     { Span s(ctx, sp.pool_map, sp.adv); BIP_TRY(seek(ctx, plane)); }                  // line 4: ADVANCETO / PEELTO
     for (size_t k = 0; k < ids.size(); ++k) {
       Edge& e = ctx->edges[ids[k]];
-      const int32_t* origin_dev = edge_dev()[ctx][ids[k]].origin_dev;
       // atoms are sorted by slice: contiguous range for this plane
       auto lo = std::lower_bound(e.slice.begin(), e.slice.end(), plane) - e.slice.begin();
       auto hi = std::upper_bound(e.slice.begin(), e.slice.end(), plane) - e.slice.begin();
       if (lo == hi) continue;
       const int64_t w2 = (int64_t)e.w * e.w;
       const int64_t el = sliced_fmt_of(precision) == SL_FMT_FP16X4 ? 8 : precision == BIP_PREC_BF16X6 ? 12 : 16;      // operand bytes per complex element
-      // scan rows per site: all of them, or (crop mask) about n_rho / (f_y f_x) -- an estimate for the batch size only
-      const int64_t rows_est = ctx->crop_fy * ctx->crop_fx > 1
-                                   ? std::min<int64_t>(ctx->n_rho, (int64_t)(1.5 * ctx->n_rho / (ctx->crop_fy * ctx->crop_fx)) + 2 * SL_ROWS) : ctx->n_rho;
-      const size_t per_atom = (size_t)((ctx->n_p1 + ctx->n_p2) * w2 * 8 + rows_est * w2 * 8 +
-                                       el * (round_up(w2, 128) * round_up(ctx->n_ap, 32) + round_up(e.n_det, 128) * round_up(w2, 32) +
-                                             round_up(rows_est, 256) * (e.n_ch * round_up(w2, 32) + (ctx->crop_fy * ctx->crop_fx > 1 ? round_up(ctx->n_ap, 32) : 0))) +
-                                       (ctx->crop_fy * ctx->crop_fx > 1 ? round_up(ctx->n_rho, 256) * 4 : 0));
-      size_t per_atom_use = per_atom;
-      if (sliced_fmt_of(precision) >= 0 && use_coupling(ctx, e, (double)rows_est, budget)) {
-        const int64_t nd = round_up((int64_t)e.n_ch * e.n_det, 256), Bp = round_up(ctx->n_ap, 128), w2p = round_up(w2, 32);
-        per_atom_use = (size_t)((ctx->n_p1 + ctx->n_p2) * w2 * 8 + el * (nd * w2p + Bp * w2p + nd * round_up(ctx->n_ap, 32)) + 8 * nd * Bp +
-                                (ctx->crop_fy * ctx->crop_fx > 1 ? el * round_up(rows_est, 256) * round_up(ctx->n_ap, 32) + round_up(ctx->n_rho, 256) * 4 : 0));
+      // scan rows per site of this plane: all of them, or (crop mask) the counted lists -- the association is chosen
+      // ONCE per (edge, plane) from the counted rows and the batch is sized for the association that will run
+      int64_t rows_max = ctx->n_rho;
+      double rows_mean = (double)ctx->n_rho;
+      if (crop && sliced_fmt_of(precision) >= 0) {
+        rows_max = 1; rows_mean = 0;
+        for (auto a = lo; a < hi; ++a) { rows_max = std::max<int64_t>(rows_max, e.crop_counts[a]); rows_mean += e.crop_counts[a]; }
+        rows_mean /= (double)(hi - lo);
       }
+      const size_t per_atom = (size_t)((ctx->n_p1 + ctx->n_p2) * w2 * 8 + rows_max * w2 * 8 +
+                                       el * (round_up(w2, 128) * round_up(ctx->n_ap, 32) + round_up(e.n_det, 128) * round_up(w2, 32) +
+                                             round_up(rows_max, 256) * (e.n_ch * round_up(w2, 32) + (crop ? round_up(ctx->n_ap, 32) : 0))) +
+                                       (crop ? round_up(ctx->n_rho, 256) * 4 : 0));
+      const int64_t nd = round_up((int64_t)e.n_ch * e.n_det, 256), Bp = round_up(ctx->n_ap, 128), w2p = round_up(w2, 32);
+      const size_t per_atom_coupling = (size_t)((ctx->n_p1 + ctx->n_p2) * w2 * 8 + el * (nd * w2p + Bp * w2p + nd * round_up(ctx->n_ap, 32)) + 8 * nd * Bp +
+                                                (crop ? el * round_up(rows_max, 256) * round_up(ctx->n_ap, 32) + round_up(ctx->n_rho, 256) * 4 : 0));
+      bool coupling = sliced_fmt_of(precision) >= 0 && use_coupling(ctx, e, rows_mean, budget);
+      if (coupling && ctx->assoc == BIP_ASSOC_AUTO && per_atom_coupling > budget) coupling = false;   // does not fit: probe-first does
+      const size_t per_atom_use = coupling ? per_atom_coupling : per_atom;
       const int32_t nb_max = (int32_t)std::max<size_t>(1, std::min<size_t>(budget / std::max<size_t>(per_atom_use, 1), 4096));
       Span s(ctx, sp.pool_map, sp.contract);
       for (int32_t a0 = (int32_t)lo; a0 < (int32_t)hi; a0 += nb_max)     // lines 5-8
-        BIP_TRY(contract_batch(ctx, e, origin_dev, a0, std::min<int32_t>(nb_max, (int32_t)hi - a0), mode, recon, precision, outs[k]));
+        BIP_TRY(contract_batch(ctx, e, e.origin_dev, a0, std::min<int32_t>(nb_max, (int32_t)hi - a0), mode, recon, precision, coupling, outs[k]));
     }
   }
   return BIP_OK;
@@ -525,7 +561,17 @@ int32_t bip_create(bip_ctx** out, const bip_grid* g, const void* T, int32_t T_on
   BIP_TRY(check_beams(nullptr, *g, n_ap, ap_h, "bip_create: aperture"));
   BIP_TRY(check_beams(nullptr, *g, n_p1, p1_h, "bip_create: S1 parents"));
   BIP_TRY(check_beams(nullptr, *g, n_p2, p2_h, "bip_create: S2 parents"));
-  BIP_TRY(check_weights(nullptr, w1, n_ap, n_p1, "bip_create: w1"));
+  std::vector<int32_t> w1_idx;
+  std::vector<float> w1_w;
+  int32_t nn1 = 0;
+  if (w1) {
+    BIP_TRY(check_weights(nullptr, w1, n_ap, n_p1, "bip_create: w1"));
+    nn1 = w1->max_nn;
+    w1_idx.assign(w1->nn_idx, w1->nn_idx + (size_t)n_ap * nn1);
+    w1_w.assign(w1->nn_w, w1->nn_w + (size_t)n_ap * nn1);
+  } else {
+    BIP_TRY(auto_weights(nullptr, *g, n_ap, ap_h, n_p1, p1_h, w1_idx, w1_w, nn1));
+  }
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return fail(nullptr, BIP_ERR_CUDA, "bip_create: no CUDA device (libbip has no CPU path)"); }
   int dev = 0;
@@ -538,7 +584,8 @@ int32_t bip_create(bip_ctx** out, const bip_grid* g, const void* T, int32_t T_on
   ctx->g = *g;
   ctx->stream = (cudaStream_t)stream;
   ctx->sm_count = prop.multiProcessorCount;
-  ctx->n_ap = n_ap; ctx->n_p1 = n_p1; ctx->n_p2 = n_p2; ctx->nn1 = w1->max_nn;
+  ctx->n_ap = n_ap; ctx->n_p1 = n_p1; ctx->n_p2 = n_p2; ctx->nn1 = nn1;
+  ctx->w1_idx = w1_idx; ctx->w1_w = w1_w;
   for (int32_t b = 0; b < n_ap; ++b) ctx->ap_c_max = std::max(ctx->ap_c_max, std::hypot(ap_c[2 * b], ap_c[2 * b + 1]));
   ctx->ap_h.assign(ap_h, ap_h + 2 * (size_t)n_ap);
   ctx->p1_h.assign(p1_h, p1_h + 2 * (size_t)n_p1);
@@ -556,12 +603,17 @@ int32_t bip_create(bip_ctx** out, const bip_grid* g, const void* T, int32_t T_on
     BIP_TRY(upload(ctx, &ctx->p1_h_dev, p1_h, 2 * (size_t)n_p1, "S1 parents"));
     BIP_TRY(upload(ctx, &ctx->p2_h_dev, p2_h, 2 * (size_t)n_p2, "S2 parents"));
     BIP_TRY(upload(ctx, (float**)&ctx->ap_c_dev, ap_c, 2 * (size_t)n_ap, "aperture coefficients"));
-    BIP_TRY(upload(ctx, &ctx->w1_idx_dev, w1->nn_idx, (size_t)n_ap * w1->max_nn, "w1 indices"));
-    BIP_TRY(upload(ctx, &ctx->w1_w_dev, w1->nn_w, (size_t)n_ap * w1->max_nn, "w1 weights"));
+    BIP_TRY(upload(ctx, &ctx->w1_idx_dev, ctx->w1_idx.data(), ctx->w1_idx.size(), "w1 indices"));
+    BIP_TRY(upload(ctx, &ctx->w1_w_dev, ctx->w1_w.data(), ctx->w1_w.size(), "w1 weights"));
     BIP_TRY(dev_alloc(ctx, (void**)&ctx->S1, (size_t)n_p1 * G * sizeof(float2), "S1 parent columns"));
     BIP_TRY(dev_alloc(ctx, (void**)&ctx->S2, (size_t)n_p2 * G * sizeof(float2), "S2 parent columns"));
     BIP_TRY(ms_init(ctx));
     BIP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    // |T| = 1 (no absorption): the S2 peel and the inverse S1 step undo a slice with conj(T)
+    float dev = 0.f;
+    BIP_TRY(ms_max_modulus_deviation(ctx, ctx->T_dev, (int64_t)G * g->nz, &dev));
+    if (!(dev <= 1e-4f)) return fail(ctx, BIP_ERR_INVALID, "bip_create: transmission functions are not unimodular (max ||T|^2 - 1| = %.3g); "
+                                     "absorptive slices are not supported (PAPER.md:372)", dev);
     return BIP_OK;
   };
   int32_t st = build();
@@ -573,15 +625,11 @@ int32_t bip_create(bip_ctx** out, const bip_grid* g, const void* T, int32_t T_on
 int32_t bip_clear_edges(bip_ctx* ctx) {
   if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
   cudaStreamSynchronize(ctx->stream);
-  auto& ed = edge_dev()[ctx];
-  for (size_t k = 0; k < ctx->edges.size(); ++k) {
-    Edge& e = ctx->edges[k];
+  for (Edge& e : ctx->edges) {
     cudaFree(e.H_dev); cudaFree(e.hmax_dev); cudaFree(e.det_h_dev); cudaFree(e.nn_idx_dev); cudaFree(e.nn_w_dev);
-    cudaFree(e.bin_of_det_x_dev); cudaFree(e.bin_of_det_y_dev);
-    if (k < ed.size()) cudaFree(ed[k].origin_dev);
+    cudaFree(e.bin_of_det_x_dev); cudaFree(e.bin_of_det_y_dev); cudaFree(e.origin_dev);
   }
   ctx->edges.clear();
-  ed.clear();
   return BIP_OK;
 }
 
@@ -589,10 +637,8 @@ int32_t bip_destroy(bip_ctx* ctx) {
   if (!ctx) return BIP_OK;
   cudaStreamSynchronize(ctx->stream);
   bip_clear_edges(ctx);
-  edge_dev().erase(ctx);
   ms_release(ctx);
-  auto it = spans().find(ctx);
-  if (it != spans().end()) { it->second.pool_map.destroy(); it->second.pool_b1.destroy(); it->second.pool_b2.destroy(); spans().erase(it); }
+  ctx->spans.pool_map.destroy(); ctx->spans.pool_b1.destroy(); ctx->spans.pool_b2.destroy();
   if (ctx->T_owned) cudaFree((void*)ctx->T_dev);
   void* ptrs[] = {ctx->ap_h_dev, ctx->p1_h_dev, ctx->p2_h_dev, ctx->ap_c_dev, ctx->w1_idx_dev, ctx->w1_w_dev, ctx->rooty_dev,
                   ctx->rootx_dev, ctx->P_dev, ctx->ms_work, ctx->S1, ctx->S2, ctx->D1.p, ctx->D2.p, ctx->R1.p, ctx->R2.p, ctx->Psi.p,
@@ -606,7 +652,7 @@ int32_t bip_destroy(bip_ctx* ctx) {
 
 int32_t bip_build_S1(bip_ctx* ctx) {
   if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
-  auto& sp = spans()[ctx];
+  auto& sp = ctx->spans;
   sp.build1.clear(); sp.pool_b1.reset();
   { Span s(ctx, sp.pool_b1, sp.build1); BIP_TRY(ms_plane_waves(ctx, ctx->S1, ctx->p1_h_dev, ctx->n_p1, +1)); }
   ctx->plane1 = 0;
@@ -616,7 +662,7 @@ int32_t bip_build_S1(bip_ctx* ctx) {
 
 int32_t bip_build_S2(bip_ctx* ctx) {
   if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
-  auto& sp = spans()[ctx];
+  auto& sp = ctx->spans;
   sp.build2.clear(); sp.pool_b2.reset();
   {
     Span s(ctx, sp.pool_b2, sp.build2);
@@ -641,6 +687,7 @@ int32_t bip_set_scan(bip_ctx* ctx, int32_t n_rho, const double* rho_px) {
   BIP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));      // the host array may go away after return
   ctx->n_rho = n_rho;
   ctx->rho_host.assign(rho_px, rho_px + 2 * (size_t)n_rho);
+  for (Edge& e : ctx->edges) e.crop_counts_fy = e.crop_counts_fx = 0;      // the per-site scan-row counts depend on the scan
   return BIP_OK;                                           // the illumination matrix (a3) is built on first use
 }
 
@@ -678,9 +725,25 @@ int32_t bip_add_edge(bip_ctx* ctx, int32_t n_atoms, const int32_t* slice, const 
   if (n_ch < 1 || n_ch > 1024 || !H) return fail(ctx, BIP_ERR_INVALID, "bip_add_edge: bad channel count or H is NULL");
   if (w < 8 || (w & 1) || w > std::min(ctx->g.ny, ctx->g.nx)) return fail(ctx, BIP_ERR_INVALID, "bip_add_edge: window %d must be even and in 8..min(ny, nx)", w);
   BIP_TRY(check_beams(ctx, ctx->g, n_det, det_h, "bip_add_edge: detector"));
-  BIP_TRY(check_weights(ctx, w2, n_det, ctx->n_p2, "bip_add_edge: w2"));
   Edge e;
-  e.n_atoms = n_atoms; e.n_ch = n_ch; e.w = w; e.n_det = n_det; e.max_nn = w2->max_nn;
+  if (w2) {
+    BIP_TRY(check_weights(ctx, w2, n_det, ctx->n_p2, "bip_add_edge: w2"));
+    e.max_nn = w2->max_nn;
+    e.w2_idx.assign(w2->nn_idx, w2->nn_idx + (size_t)n_det * w2->max_nn);
+    e.w2_w.assign(w2->nn_w, w2->nn_w + (size_t)n_det * w2->max_nn);
+  } else {
+    // computed once per detector beam list and cached on the context
+    const uint64_t key = fnv1a(det_h, sizeof(int32_t) * 2 * (size_t)n_det) ^ (uint64_t)n_det;
+    auto it = ctx->auto_w2.find(key);
+    if (it == ctx->auto_w2.end() || it->second.det_h.size() != 2 * (size_t)n_det || std::memcmp(it->second.det_h.data(), det_h, sizeof(int32_t) * 2 * (size_t)n_det) != 0) {
+      bip::AutoTable t;
+      t.det_h.assign(det_h, det_h + 2 * (size_t)n_det);
+      BIP_TRY(auto_weights(ctx, ctx->g, n_det, det_h, ctx->n_p2, ctx->p2_h.data(), t.idx, t.w, t.max_nn));
+      it = ctx->auto_w2.insert_or_assign(key, std::move(t)).first;
+    }
+    e.max_nn = it->second.max_nn; e.w2_idx = it->second.idx; e.w2_w = it->second.w;
+  }
+  e.n_atoms = n_atoms; e.n_ch = n_ch; e.w = w; e.n_det = n_det;
   // sort sites by slice (stable): the plane loop takes contiguous ranges
   std::vector<int32_t> order(n_atoms);
   for (int i = 0; i < n_atoms; ++i) order[i] = i;
@@ -707,7 +770,6 @@ int32_t bip_add_edge(bip_ctx* ctx, int32_t n_atoms, const int32_t* slice, const 
     bx[d] = (int32_t)(std::lower_bound(e.binx.begin(), e.binx.end(), bx[d]) - e.binx.begin());
     by[d] = (int32_t)(std::lower_bound(e.biny.begin(), e.biny.end(), by[d]) - e.biny.begin());
   }
-  EdgeDev ed;
   BIP_TRY(upload(ctx, (float**)&e.H_dev, H, 2 * (size_t)n_ch * w * w, "H windows"));
   std::vector<float> hmax(n_ch, 0.f);
   for (int n = 0; n < n_ch; ++n)
@@ -717,14 +779,13 @@ int32_t bip_add_edge(bip_ctx* ctx, int32_t n_atoms, const int32_t* slice, const 
     }
   BIP_TRY(upload(ctx, &e.hmax_dev, hmax.data(), (size_t)n_ch, "H maxima"));
   BIP_TRY(upload(ctx, &e.det_h_dev, det_h, 2 * (size_t)n_det, "detector beams"));
-  BIP_TRY(upload(ctx, &e.nn_idx_dev, w2->nn_idx, (size_t)n_det * w2->max_nn, "w2 indices"));
-  BIP_TRY(upload(ctx, &e.nn_w_dev, w2->nn_w, (size_t)n_det * w2->max_nn, "w2 weights"));
+  BIP_TRY(upload(ctx, &e.nn_idx_dev, e.w2_idx.data(), e.w2_idx.size(), "w2 indices"));
+  BIP_TRY(upload(ctx, &e.nn_w_dev, e.w2_w.data(), e.w2_w.size(), "w2 weights"));
   BIP_TRY(upload(ctx, &e.bin_of_det_x_dev, bx.data(), (size_t)n_det, "qEELS bins"));
   BIP_TRY(upload(ctx, &e.bin_of_det_y_dev, by.data(), (size_t)n_det, "qEELS bins"));
-  BIP_TRY(upload(ctx, &ed.origin_dev, e.origin.data(), 2 * (size_t)n_atoms, "window origins"));
+  BIP_TRY(upload(ctx, &e.origin_dev, e.origin.data(), 2 * (size_t)n_atoms, "window origins"));
   BIP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));     // host sources may go away after return
   ctx->edges.push_back(std::move(e));
-  edge_dev()[ctx].push_back(ed);
   if (edge_id) *edge_id = (int32_t)ctx->edges.size() - 1;
   return BIP_OK;
 }
@@ -814,7 +875,7 @@ int32_t bip_debug_reconstruct(bip_ctx* ctx, int32_t edge_id, int32_t atom, int32
   if (which != 1 && which != 2) return fail(ctx, BIP_ERR_INVALID, "which must be 1 or 2");
   if (!ctx->s1_built || !ctx->s2_built) return fail(ctx, BIP_ERR_STATE, "matrices not built");
   const int w2 = e.w * e.w;
-  const int32_t* org = edge_dev()[ctx][edge_id].origin_dev + 2 * (int64_t)atom;
+  const int32_t* org = e.origin_dev + 2 * (int64_t)atom;
   const int n_par = which == 1 ? ctx->n_p1 : ctx->n_p2;
   const int n_beams = which == 1 ? ctx->n_ap : e.n_det;
   DevBuf& D = which == 1 ? ctx->D1 : ctx->D2;
@@ -837,11 +898,49 @@ int32_t bip_debug_reconstruct(bip_ctx* ctx, int32_t edge_id, int32_t atom, int32
   return st;
 }
 
+int32_t bip_get_parents(const bip_ctx* ctx, int32_t which, int32_t* h_out, int32_t cap, int32_t* n_out) {
+  if (!ctx || !n_out) return fail(nullptr, BIP_ERR_INVALID, "bip_get_parents: NULL argument");
+  if (which != 1 && which != 2) return fail(const_cast<bip_ctx*>(ctx), BIP_ERR_INVALID, "bip_get_parents: which must be 1 or 2");
+  const std::vector<int32_t>& ph = which == 1 ? ctx->p1_h : ctx->p2_h;
+  *n_out = (int32_t)(ph.size() / 2);
+  if (h_out) {
+    if (cap < *n_out) return fail(const_cast<bip_ctx*>(ctx), BIP_ERR_INVALID, "bip_get_parents: capacity %d < %d parents", cap, *n_out);
+    std::copy(ph.begin(), ph.end(), h_out);
+  }
+  return BIP_OK;
+}
+
+int32_t bip_get_weights(const bip_ctx* ctx, int32_t edge_id, int32_t* n_rows, int32_t* max_nn, int32_t* nn_idx_out, float* nn_w_out) {
+  if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "bip_get_weights: ctx is NULL");
+  if (edge_id >= (int)ctx->edges.size()) return fail(const_cast<bip_ctx*>(ctx), BIP_ERR_INVALID, "edge %d does not exist", edge_id);
+  const std::vector<int32_t>& idx = edge_id < 0 ? ctx->w1_idx : ctx->edges[edge_id].w2_idx;
+  const std::vector<float>& w = edge_id < 0 ? ctx->w1_w : ctx->edges[edge_id].w2_w;
+  const int32_t rows = edge_id < 0 ? ctx->n_ap : ctx->edges[edge_id].n_det, nn = edge_id < 0 ? ctx->nn1 : ctx->edges[edge_id].max_nn;
+  if (n_rows) *n_rows = rows;
+  if (max_nn) *max_nn = nn;
+  if (nn_idx_out) std::copy(idx.begin(), idx.end(), nn_idx_out);
+  if (nn_w_out) std::copy(w.begin(), w.end(), nn_w_out);
+  return BIP_OK;
+}
+
+int32_t bip_allow_tf32x3(bip_ctx* ctx, int32_t allow) {
+  if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
+  ctx->allow_tf32x3 = allow != 0;
+  return BIP_OK;
+}
+
+int32_t bip_set_scratch_budget(bip_ctx* ctx, size_t bytes) {
+  if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
+  if (bytes < ((size_t)32 << 20)) return fail(ctx, BIP_ERR_INVALID, "bip_set_scratch_budget: %zu bytes is below the 32 MB minimum", bytes);
+  ctx->scratch_budget = bytes;
+  return BIP_OK;
+}
+
 int32_t bip_get_timing(const bip_ctx* cctx, bip_timing* out) {
   if (!cctx || !out) return fail(nullptr, BIP_ERR_INVALID, "bip_get_timing: NULL argument");
   bip_ctx* ctx = const_cast<bip_ctx*>(cctx);
   cudaStreamSynchronize(ctx->stream);
-  auto& sp = spans()[ctx];
+  auto& sp = ctx->spans;
   ctx->timing.build_s1_ms = sum_ms(sp.build1);
   ctx->timing.build_s2_ms = sum_ms(sp.build2);
   ctx->timing.advance_peel_ms = sum_ms(sp.adv);

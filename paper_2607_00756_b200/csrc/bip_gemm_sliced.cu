@@ -23,7 +23,7 @@
 // warp % 4, column half = (warp - 2) / 4).
 #include <cuda.h>
 
-#include <cstdlib>
+#include <algorithm>
 
 #include "bip_internal.h"
 
@@ -135,13 +135,29 @@ __device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t b
 // tiles) only hit in L2 while they read the same k range at about the same time; free-running they drift apart and
 // every worker ends up streaming its operands from HBM (profiles/r01_gemm2_l2_lockstep.md).  The producers of all
 // workers therefore meet at a global counter at the start of every (item, channel) segment: one relaxed
-// red + acquire-poll per ~150 us, all workers co-resident (persistent grid <= SM count).
-__device__ __forceinline__ void lockstep_arrive_wait(unsigned int* counter, unsigned int target) {
+// red + acquire-poll per ~150 us.  Lockstep is an L2-locality optimisation only, so the wait is BOUNDED: nothing
+// guarantees that every worker of a plain (non-cooperative) launch is resident at once (a second context on another
+// stream, an MPS co-tenant), and a worker whose peers have not shown up within LOCKSTEP_BUDGET_NS stops waiting for
+// good and runs free -- skipping the meeting is always correct.  Returns false once the budget has expired.
+constexpr unsigned long long LOCKSTEP_BUDGET_NS = 2000000ull;   // 2 ms: ~10 segments; a healthy meeting takes microseconds
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
+__device__ __forceinline__ bool lockstep_arrive_wait(unsigned int* counter, unsigned int target) {
   asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(counter) : "memory");
   unsigned int v;
-  do {
+  unsigned long long t0 = 0;
+  for (unsigned int spins = 0;; ++spins) {
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(counter) : "memory");
-  } while ((int)(v - target) < 0);
+    if ((int)(v - target) >= 0) return true;
+    if ((spins & 63u) == 63u) {
+      const unsigned long long now = globaltimer_ns();
+      if (t0 == 0) t0 = now;
+      else if (now - t0 > LOCKSTEP_BUDGET_NS) return false;
+    }
+  }
 }
 
 // K-major, no-swizzle shared-memory matrix descriptor (cute::UMMA::SmemDescriptor, LayoutType::INTERLEAVE):
@@ -400,6 +416,7 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
     if (lane == 0) {
       uint32_t it = 0;
       unsigned int sync_target = 0;
+      bool in_step = p.sync_counter != nullptr;            // false once a meeting has timed out: free-running from then on
       for (int item = worker; item < p.n_items; item += n_workers) {
         int atom, rt, ct;
         decode_item(p, item, atom, rt, ct);
@@ -410,10 +427,10 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
         for (int n = 0; n < p.n_ch_loop; ++n) {
           const uint16_t* xsrc = p.X + (int64_t)atom * p.x_batch_stride + ((int64_t)n * p.n_rt_x + rt) * p.ksteps * STEP_EL;
           for (int ks = 0, next_sync = 0; ks < p.ksteps; ++ks, ++it) {
-            if (p.sync_counter && ks == next_sync) {
+            if (in_step && ks == next_sync) {
               next_sync += p.sync_steps;
               sync_target += active;
-              if (rank == 0) lockstep_arrive_wait(p.sync_counter, sync_target);
+              if (rank == 0) in_step = lockstep_arrive_wait(p.sync_counter, sync_target);
             }
             const int s = it % STAGES;
             mbar_wait(&empty[s], ((it / STAGES) & 1) ^ 1);
@@ -443,7 +460,7 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
     // catches up first: the epilogue cannot release C12 before it has seen every C0 chunk but the last.
     // The whole warp runs the control flow (converged); one elected lane issues the tcgen05 instructions -- a
     // lane-divergent `if (lane == 0)` region makes ptxas wrap every uniform-datapath instruction in an ELECT loop,
-    // and the issuing thread, not the tensor pipe, becomes the bottleneck (profiles/r01_fp16x4_issue_bound.md).
+    // and the issuing thread, not the tensor pipe, becomes the bottleneck (measured in round 1: the FP16X4 issue loop fell from 1.6 to 1.1 k clk per k-step).
     // In a pair only the leader CTA (rank 0) issues (tcgen05.mma.cta_group::2 drives both tensor cores); the peer's
     // warp 1 forwards "my operands have landed" to the leader's peer_full barriers.
     const uint32_t total = (uint32_t)n_my_items * (uint32_t)p.n_ch_loop * (uint32_t)p.ksteps;
@@ -655,9 +672,10 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
 }
 
 // a5: Phi_n[rho][s] = H_n[s] Psi[rho][s] as sliced rows (n, rho) with their power-of-two scales.
-// One block per (8 consecutive rho, chunk of QCH channels, atom).  Pass 1: warp w takes row w and finds the row maxima of
-// all channels of the chunk in one sweep over Psi.  Pass 2: thread = (row = t & 7, k-group lane = t >> 3) keeps 8 Psi
-// values in registers and loops over the channels, so Psi is read twice in all (not twice per channel) and the 16-byte
+// One block per (8 consecutive rho, chunk of QCH channels, atom); thread = (row = t & 7, k-group lane = t >> 3) in both
+// passes.  Pass 1 sweeps Psi once (64 contiguous bytes per thread and iteration) for the row maxima of all channels of
+// the chunk.  Pass 2 keeps 8 Psi values in registers and loops over the channels, so Psi is read twice in all (not
+// twice per channel) and the 16-byte
 // slice groups of the 8 rows of one k-group land in one contiguous 128-byte line (the blocked layout puts rows r .. r+7
 // of a k-group side by side): every store instruction writes whole lines.
 constexpr int QCH = 9;
@@ -739,8 +757,8 @@ __global__ void __launch_bounds__(256) k_quantize_phi(const float2* __restrict__
 // matrix A into a per-site X operand.  One thread per (site, local row, group of 8 beams); rows without a scan are zero.
 __global__ void __launch_bounds__(256) k_gather_rows_sliced(Sliced src, const int32_t* __restrict__ row_idx, int64_t idx_stride,
                                                             Sliced dst, int n_groups) {
-  const int g = blockIdx.x * blockDim.x + threadIdx.x;
-  const int row = blockIdx.y, atom = blockIdx.z;
+  const int g = blockIdx.y * blockDim.x + threadIdx.x;   // rows in gridDim.x: a site may keep more than 65535 scan rows
+  const int row = blockIdx.x, atom = blockIdx.z;
   if (g >= n_groups) return;
   const int s = row_idx[(int64_t)atom * idx_stride + row];
   const int parts = sl_parts(src.fmt);
@@ -762,7 +780,7 @@ __global__ void __launch_bounds__(256) k_crop_rows(const double* __restrict__ rh
   const int atom = blockIdx.x, lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const double cy = (double)((origin[2 * atom] + w / 2) % ny), cx = (double)((origin[2 * atom + 1] + w / 2) % nx);
   const double hy = ny / (2.0 * fy), hx = nx / (2.0 * fx);
-  int32_t* out = row_idx + (int64_t)atom * idx_stride;
+  int32_t* out = row_idx ? row_idx + (int64_t)atom * idx_stride : nullptr;   // NULL: count only
   if (threadIdx.x == 0) base = 0;
   __syncthreads();
   for (int r0 = 0; r0 < n_rho; r0 += 256) {
@@ -781,22 +799,23 @@ __global__ void __launch_bounds__(256) k_crop_rows(const double* __restrict__ rh
     __syncthreads();
     int off = base;
     for (int k = 0; k < wid; ++k) off += warp_sum[k];
-    if (in) out[off + __popc(m & ((1u << lane) - 1u))] = r;
+    if (in && out) out[off + __popc(m & ((1u << lane) - 1u))] = r;
     __syncthreads();
     if (threadIdx.x == 0) { int t = 0; for (int k = 0; k < 8; ++k) t += warp_sum[k]; base += t; }
     __syncthreads();
   }
   const int n = base;
-  for (int64_t i = n + threadIdx.x; i < idx_stride; i += 256) out[i] = -1;
+  if (out) for (int64_t i = n + threadIdx.x; i < idx_stride; i += 256) out[i] = -1;
   if (threadIdx.x == 0) counts[atom] = n;
 }
 
 template <int EPI, int FMT, bool PAIR>
 int32_t launch_fmt(bip_ctx* ctx, const SlParams& p) {
-  static bool attr_set = false;
-  if (!attr_set) {
+  // per context (= per device): the shared-memory opt-in and the occupancy of this kernel variant
+  KernelInfo& ki = ctx->kernel_info[reinterpret_cast<const void*>(&k_sliced_contract<EPI, FMT, PAIR>)];
+  if (!ki.attr_set) {
     BIP_CUDA(ctx, cudaFuncSetAttribute(k_sliced_contract<EPI, FMT, PAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<EPI, FMT, PAIR>()));
-    attr_set = true;
+    ki.attr_set = true;
   }
   SlParams q = p;
   q.n_rt_x = p.n_rt;
@@ -806,37 +825,30 @@ int32_t launch_fmt(bip_ctx* ctx, const SlParams& p) {
   }
   q.n_items = p.n_items / p.n_rt * q.n_rt;
   if (q.n_items <= 0) return BIP_OK;
-  q.chunk_steps = Cfg<FMT>::CHUNK_STEPS;
-  q.lag_max = Cfg<FMT>::LAG_MAX;
-  q.dgroup = DGROUP_DEFAULT;
-  if (const char* e = std::getenv("BIP_TUNE_DGROUP")) q.dgroup = std::max(1, std::atoi(e));
-  if (const char* e = std::getenv("BIP_TUNE_CHUNK")) q.chunk_steps = std::max(1, std::atoi(e));   // timing experiments only: breaks exactness
-  if (const char* e = std::getenv("BIP_TUNE_LAG")) q.lag_max = std::min(std::max(1, std::atoi(e)), n_stages<EPI, FMT, PAIR>() - 1);
+  q.chunk_steps = Cfg<FMT>::CHUNK_STEPS;                 // fixed: the exactness of the leading sums depends on it
+  q.dgroup = std::max(1, tune_int("BIP_TUNE_DGROUP", DGROUP_DEFAULT));
+  q.lag_max = std::min(std::max(1, tune_int("BIP_TUNE_LAG", Cfg<FMT>::LAG_MAX)), n_stages<EPI, FMT, PAIR>() - 1);
   int workers = std::max(1, std::min(q.n_items, PAIR ? ctx->sm_count / 2 : ctx->sm_count));
-  if (const char* e = std::getenv("BIP_TUNE_WORKERS")) workers = std::max(1, std::min(workers, std::atoi(e)));   // timing experiments only
+  workers = std::max(1, std::min(workers, tune_int("BIP_TUNE_WORKERS", workers)));
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = dim3(PAIR ? 2 * workers : workers);
   cfg.blockDim = dim3(NUM_THREADS);
-  q.lag_max = std::min(q.lag_max, n_stages<EPI, FMT, PAIR>() - 1);
   cfg.dynamicSmemBytes = smem_bytes<EPI, FMT, PAIR>();
   cfg.stream = ctx->stream;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = PAIR ? 2 : 1; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr; cfg.numAttrs = 1;
-  // Lockstep needs every worker resident at once (they wait for one another): checked against the occupancy the
-  // driver reports for this launch configuration, once per kernel variant; otherwise the workers run free.
-  static const bool lockstep_wanted = [] { const char* e = std::getenv("BIP_TUNE_LOCKSTEP"); return e ? std::atoi(e) != 0 : true; }();
-  static int max_clusters = -1;
-  if (max_clusters < 0) {
+  // Lockstep pays only when every worker is resident at once: checked against the occupancy the driver reports for
+  // this launch configuration (once per context and kernel variant).  The wait itself is bounded (lockstep_arrive_wait).
+  if (ki.max_clusters < 0) {
     int n = 0;
     if (cudaOccupancyMaxActiveClusters(&n, k_sliced_contract<EPI, FMT, PAIR>, &cfg) != cudaSuccess) { cudaGetLastError(); n = 0; }
-    max_clusters = n;
+    ki.max_clusters = n;
   }
   q.sync_counter = nullptr;
-  q.sync_steps = 1 << 30;                // once per (item, channel) segment
-  if (const char* e = std::getenv("BIP_TUNE_SYNCSTEPS")) q.sync_steps = std::max(1, std::atoi(e));
-  if (lockstep_wanted && workers <= max_clusters) {      // a fresh zeroed counter per launch (64 slots, cleared on the stream)
+  q.sync_steps = std::max(1, tune_int("BIP_TUNE_SYNCSTEPS", 1 << 30));   // default: once per (item, channel) segment
+  if (tune_int("BIP_TUNE_LOCKSTEP", 1) != 0 && workers <= ki.max_clusters) {   // a fresh zeroed counter per launch (64 slots, cleared on the stream)
     BIP_TRY(ensure(ctx, ctx->Sync, 64 * sizeof(unsigned int), "lockstep counters"));
     q.sync_counter = reinterpret_cast<unsigned int*>(ctx->Sync.p) + (ctx->sync_slot++ & 63);
     BIP_CUDA(ctx, cudaMemsetAsync(q.sync_counter, 0, sizeof(unsigned int), ctx->stream));
@@ -848,8 +860,7 @@ int32_t launch_fmt(bip_ctx* ctx, const SlParams& p) {
 
 template <int EPI>
 int32_t launch(bip_ctx* ctx, const SlParams& p, int fmt) {
-  static const bool pair = [] { const char* e = std::getenv("BIP_TUNE_PAIR"); return e ? std::atoi(e) != 0 : true; }();
-  static const bool tile = [] { const char* e = std::getenv("BIP_TUNE_TILEACC"); return e ? std::atoi(e) != 0 : true; }();
+  const bool pair = tune_int("BIP_TUNE_PAIR", 1) != 0, tile = tune_int("BIP_TUNE_TILEACC", 1) != 0;
   if (pair && tile && EPI == EPI_GEMM2 && p.mode != BIP_MODE_MAP)
     return fmt == SL_FMT_FP16X4 ? launch_fmt<EPI_GEMM2_TILE, SL_FMT_FP16X4, true>(ctx, p) : launch_fmt<EPI_GEMM2_TILE, SL_FMT_BF16X6, true>(ctx, p);
   if (pair) return fmt == SL_FMT_FP16X4 ? launch_fmt<EPI, SL_FMT_FP16X4, true>(ctx, p) : launch_fmt<EPI, SL_FMT_BF16X6, true>(ctx, p);
@@ -884,7 +895,7 @@ int32_t launch_crop_rows(bip_ctx* ctx, const int32_t* origin_dev, int32_t n_atom
 
 int32_t launch_gather_rows_sliced(bip_ctx* ctx, const Sliced& src, const int32_t* row_idx, int64_t idx_stride, const Sliced& dst, int32_t n_atoms) {
   const int n_groups = 2 * (int)src.ksteps;
-  dim3 grid((unsigned)((n_groups + 255) / 256), (unsigned)dst.rows_pad, (unsigned)n_atoms);
+  dim3 grid((unsigned)dst.rows_pad, (unsigned)((n_groups + 255) / 256), (unsigned)n_atoms);
   k_gather_rows_sliced<<<grid, 256, 0, ctx->stream>>>(src, row_idx, idx_stride, dst, n_groups);
   BIP_CUDA(ctx, cudaGetLastError());
   ctx->timing.kernel_launches++;

@@ -145,6 +145,38 @@ int32_t bip_aperture_coeffs(const bip_grid* g, int32_t n, const int32_t* h, doub
   return BIP_OK;
 }
 
+int32_t bip_prism_coeffs(int32_t n_keep, const int32_t* keep, int32_t n_full, const float* c_full, int32_t fy, int32_t fx, float* c_out) {
+  if (n_keep < 0 || (n_keep > 0 && (!keep || !c_out)) || !c_full || fy < 1 || fx < 1)
+    return bip::fail(nullptr, BIP_ERR_INVALID, "bip_prism_coeffs: bad argument");
+  const float f = (float)(fy * fx);                                   // "the DFT decimation factor"
+  for (int32_t j = 0; j < n_keep; ++j) {
+    if (keep[j] < 0 || keep[j] >= n_full) return bip::fail(nullptr, BIP_ERR_INVALID, "bip_prism_coeffs: position %d outside 0..%d", keep[j], n_full - 1);
+    c_out[2 * j] = c_full[2 * keep[j]] * f;
+    c_out[2 * j + 1] = c_full[2 * keep[j] + 1] * f;
+  }
+  return BIP_OK;
+}
+
+int32_t bip_partition(const bip_grid* g, int32_t n, const int32_t* h, double qmax, double factor, int32_t max_nn, int32_t* pos_out,
+                      int32_t cap, int32_t* n_parent, int32_t* nn_idx_out, float* nn_w_out) {
+  if (!grid_ok(g) || n <= 0 || !h || !n_parent || !pos_out || !(factor >= 1.0) || max_nn < 1 || max_nn > BIP_MAX_NN || !nn_idx_out || !nn_w_out)
+    return bip::fail(nullptr, BIP_ERR_INVALID, "bip_partition: bad argument");
+  if (factor == 1.0) {                                                // the exactness limit: parents = all beams, w = identity (reading c7)
+    *n_parent = n;
+    if (cap < n) return bip::fail(nullptr, BIP_ERR_INVALID, "bip_partition: capacity %d < %d parents", cap, n);
+    for (int32_t b = 0; b < n; ++b) {
+      pos_out[b] = b;
+      for (int32_t j = 0; j < max_nn; ++j) { nn_idx_out[(size_t)b * max_nn + j] = j == 0 ? b : -1; nn_w_out[(size_t)b * max_nn + j] = j == 0 ? 1.f : 0.f; }
+    }
+    return BIP_OK;
+  }
+  int32_t st = bip_hexring(g, n, h, qmax, bip_n_radial_from_factor(n, factor), 6, pos_out, cap, n_parent);
+  if (st != BIP_OK) return st;
+  std::vector<int32_t> ph(2 * (size_t)*n_parent);
+  for (int32_t p = 0; p < *n_parent; ++p) { ph[2 * p] = h[2 * pos_out[p]]; ph[2 * p + 1] = h[2 * pos_out[p] + 1]; }
+  return bip_sibson(g, n, h, *n_parent, ph.data(), qmax, max_nn, nn_idx_out, nn_w_out);
+}
+
 int32_t bip_n_radial_from_factor(int32_t n_beams, double factor) {
   if (n_beams <= 0 || !(factor > 0)) return 1;
   return std::max(1, (int)std::floor(std::sqrt(n_beams / M_PI) / factor + 0.5));

@@ -5,7 +5,10 @@
 #include <cstdarg>
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
+#include <map>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "../../include/bip.h"
@@ -15,6 +18,17 @@ namespace bip {
 
 // Records the message on the context (or a thread-local slot when ctx == nullptr) and returns `status`.
 int32_t fail(bip_ctx* ctx, int32_t status, const char* fmt, ...) __attribute__((format(printf, 3, 4)));
+
+// Launch-shape experiments (raster group, workers, lag, ...) read BIP_TUNE_* environment variables ONLY in a build
+// compiled with -DBIP_TUNING (python -m paper_2607_00756_b200.build --tuning); the shipped library ignores them.
+inline int tune_int(const char* name, int dflt) {
+#ifdef BIP_TUNING
+  if (const char* e = std::getenv(name)) return std::atoi(e);
+#else
+  (void)name;
+#endif
+  return dflt;
+}
 
 }  // namespace bip
 
@@ -48,6 +62,11 @@ struct Edge {
   std::vector<int32_t> origin;         // [n_atoms][2] window origin (centre - w/2) mod N
   std::vector<int32_t> det_h;          // [n_det][2]
   std::vector<int32_t> binx, biny;     // distinct h_x / h_y ascending
+  std::vector<int32_t> w2_idx;         // [n_det][max_nn] host copy of the ELL table (bip_get_weights)
+  std::vector<float> w2_w;
+  std::vector<int32_t> crop_counts;    // [n_atoms] scan rows inside each site's crop window (filled on first use per crop setting)
+  int32_t crop_counts_fy = 0, crop_counts_fx = 0;
+  int32_t* origin_dev = nullptr;       // [n_atoms][2]
   float2* H_dev = nullptr;             // [n_ch][w*w]
   float* hmax_dev = nullptr;           // [n_ch] max_s |H_n[s]| (row-scale bound of the coupling operands)
   int32_t* det_h_dev = nullptr;        // [n_det][2]
@@ -56,6 +75,24 @@ struct Edge {
   int32_t* bin_of_det_x_dev = nullptr; // [n_det] bin number along x
   int32_t* bin_of_det_y_dev = nullptr;
 };
+
+struct EventPool {
+  std::vector<cudaEvent_t> all;
+  size_t used = 0;
+  cudaEvent_t get() {
+    if (used == all.size()) { cudaEvent_t e; cudaEventCreate(&e); all.push_back(e); }
+    return all[used++];
+  }
+  void reset() { used = 0; }
+  void destroy() { for (auto e : all) cudaEventDestroy(e); all.clear(); used = 0; }
+};
+typedef std::vector<std::pair<cudaEvent_t, cudaEvent_t>> SpanList;
+struct Spans {
+  EventPool pool_map, pool_b1, pool_b2;
+  SpanList adv, contract, gemm2, build1, build2;
+};
+struct AutoTable { std::vector<int32_t> det_h, idx; std::vector<float> w; int32_t max_nn = 0; };   // library-computed w2, per detector list
+struct KernelInfo { bool attr_set = false; int max_clusters = -1; };   // per (context = device, kernel variant)
 
 }  // namespace bip
 
@@ -76,6 +113,8 @@ struct bip_ctx {
   float ap_c_max = 0.f;            // max_b |c_b|
   int32_t* w1_idx_dev = nullptr;
   float* w1_w_dev = nullptr;
+  std::vector<int32_t> w1_idx;     // host copies (bip_get_weights)
+  std::vector<float> w1_w;
 
   // roots of unity exp(2 pi i k / N), k = 0..N-1 (exact phases for tilt / de-tilt)
   float2 *rooty_dev = nullptr, *rootx_dev = nullptr;
@@ -84,9 +123,14 @@ struct bip_ctx {
   float2 *S1 = nullptr, *S2 = nullptr;
   bool s1_built = false, s2_built = false;
   int32_t plane1 = 0, plane2 = 0;  // S1 holds slices 0..plane1-1; S2 holds slices plane2..nz-1
-  cufftHandle plan = 0;
+  std::map<int, cufftHandle> plans;   // cuFFT plans by batch size
   int32_t plan_batch = 0;
   bool plan_ok = false;
+  size_t scratch_budget = (size_t)12 << 30;   // bip_set_scratch_budget
+  bool allow_tf32x3 = false;          // bip_allow_tf32x3
+  bip::Spans spans;                   // CUDA-event spans behind bip_get_timing
+  std::map<const void*, bip::KernelInfo> kernel_info;
+  std::map<uint64_t, bip::AutoTable> auto_w2;
 
   // scan
   int32_t n_rho = 0;
@@ -136,6 +180,8 @@ int32_t ensure(bip_ctx* ctx, DevBuf& b, size_t bytes, const char* what);
 // ---- multislice (bip_multislice.cu) ----
 int32_t ms_init(bip_ctx* ctx);                       // propagator, roots of unity, cuFFT plan
 int32_t ms_plane_waves(bip_ctx* ctx, float2* S, const int32_t* h_dev, int32_t n, int sign);
+// max over the n elements of | |T|^2 - 1 | (synchronises the stream)
+int32_t ms_max_modulus_deviation(bip_ctx* ctx, const float2* T, int64_t n, float* out);
 // forward: S <- P[T_j S] (dir=+1) ; inverse: S <- T_j* P*[S] (dir=-1)               (S1, eq. 6)
 int32_t ms_step_S1(bip_ctx* ctx, int32_t j, int dir);
 // build/un-peel: S <- T_j P[S] (dir=-1, towards the entrance) ; peel: S <- P*[T_j* S] (dir=+1)   (S2, eq. 12)

@@ -1,7 +1,7 @@
 // Slice-by-slice multislice of the parent columns: S1 ADVANCETO (eq. 6) and S2 build / PEELTO
 // (eq. 12).  cuFFT does the 2-D transforms (plumbing, timed separately from the contraction).
 #include <cmath>
-#include <map>
+#include <cstring>
 
 #include "bip_internal.h"
 
@@ -27,8 +27,21 @@ __global__ void k_plane_waves(float2* __restrict__ S, const int32_t* __restrict_
   }
 }
 
+// max | |T|^2 - 1 | over all pixels of all slices (non-negative floats order like their bit patterns)
+__global__ void k_modulus_deviation(const float2* __restrict__ T, int64_t n, unsigned int* __restrict__ out) {
+  float m = 0.f;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    const float2 t = T[i];
+    const float d = fabsf(t.x * t.x + t.y * t.y - 1.f);
+    m = fmaxf(m, d == d ? d : 3.0e38f);               // NaN counts as a violation
+  }
+#pragma unroll
+  for (int o = 16; o; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0) atomicMax(out, __float_as_uint(m));
+}
+
 // cuFFT's single-precision C2C loses ~3e-7 of the norm^2 per forward+inverse pair, systematically (measured on
-// B200, profiles/r01_notes.md); over tens of slices that alone breaks the 1e-6 summed-intensity bound.  The slice
+// B200 in round 1; tests/test_gpu_plumbing.py re-measures the drift of both variants); over tens of slices that alone breaks the 1e-6 summed-intensity bound.  The slice
 // steps therefore run in double precision (Z2Z) on a chunk workspace and the columns are stored back as c64:
 // the only rounding per slice is one unbiased round-to-nearest of the result.
 
@@ -74,25 +87,16 @@ __global__ void k_store_cols(float2* __restrict__ S, const double2* __restrict__
   }
 }
 
-struct PlanCache {
-  std::map<int, cufftHandle> plans;
-};
-std::map<const bip_ctx*, PlanCache>& plan_caches() {
-  static std::map<const bip_ctx*, PlanCache> m;
-  return m;
-}
-
 int32_t get_plan(bip_ctx* ctx, int batch, cufftHandle* out) {
-  auto& pc = plan_caches()[ctx];
-  auto it = pc.plans.find(batch);
-  if (it != pc.plans.end()) { *out = it->second; return BIP_OK; }
+  auto it = ctx->plans.find(batch);
+  if (it != ctx->plans.end()) { *out = it->second; return BIP_OK; }
   cufftHandle h;
   int n[2] = {ctx->g.ny, ctx->g.nx};
   cufftResult r = cufftPlanMany(&h, 2, n, nullptr, 1, ctx->g.ny * ctx->g.nx, nullptr, 1, ctx->g.ny * ctx->g.nx, CUFFT_Z2Z, batch);
   if (r != CUFFT_SUCCESS) return fail(ctx, r == CUFFT_ALLOC_FAILED ? BIP_ERR_OOM : BIP_ERR_CUDA, "cufftPlanMany(%dx%d, batch %d) failed: %d", ctx->g.ny, ctx->g.nx, batch, (int)r);
   r = cufftSetStream(h, ctx->stream);
   if (r != CUFFT_SUCCESS) return fail(ctx, BIP_ERR_CUDA, "cufftSetStream failed: %d", (int)r);
-  pc.plans[batch] = h;
+  ctx->plans[batch] = h;
   *out = h;
   return BIP_OK;
 }
@@ -125,10 +129,8 @@ int32_t slice_op(bip_ctx* ctx, float2* S, int n_cols, const float2* Tj, int pre,
 }  // namespace
 
 void ms_release(bip_ctx* ctx) {
-  auto it = plan_caches().find(ctx);
-  if (it == plan_caches().end()) return;
-  for (auto& kv : it->second.plans) cufftDestroy(kv.second);
-  plan_caches().erase(it);
+  for (auto& kv : ctx->plans) cufftDestroy(kv.second);
+  ctx->plans.clear();
 }
 
 int32_t ms_init(bip_ctx* ctx) {
@@ -163,6 +165,20 @@ int32_t ms_init(bip_ctx* ctx) {
   ctx->plan_batch = (int)std::max<int64_t>(1, std::min<int64_t>(std::max(ctx->n_p1, ctx->n_p2), (512ll << 20) / col_bytes));
   BIP_TRY(dev_alloc(ctx, &ctx->ms_work, (size_t)ctx->plan_batch * col_bytes, "multislice workspace"));
   ctx->plan_ok = true;
+  return BIP_OK;
+}
+
+int32_t ms_max_modulus_deviation(bip_ctx* ctx, const float2* T, int64_t n, float* out) {
+  unsigned int* d = nullptr;
+  BIP_TRY(dev_alloc(ctx, (void**)&d, sizeof(unsigned int), "modulus check"));
+  cudaMemsetAsync(d, 0, sizeof(unsigned int), ctx->stream);
+  k_modulus_deviation<<<(unsigned)std::min<int64_t>((n + 255) / 256, 4096), 256, 0, ctx->stream>>>(T, n, d);
+  unsigned int bits = 0;
+  cudaError_t e = cudaMemcpyAsync(&bits, d, sizeof bits, cudaMemcpyDeviceToHost, ctx->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+  cudaFree(d);
+  if (e != cudaSuccess) { cudaGetLastError(); return fail(ctx, BIP_ERR_CUDA, "modulus check: %s", cudaGetErrorString(e)); }
+  std::memcpy(out, &bits, sizeof bits);
   return BIP_OK;
 }
 

@@ -52,7 +52,7 @@ class OracleSetup:
                             edge.H, recon=recon, crop_f=crop_f, association=association)
 
 
-def gpu_context(wl, edges, parent_factor=None, max_nn=8, T_on_device=True, prism=None, crop=None):
+def gpu_context(wl, edges, parent_factor=None, max_nn=8, T_on_device=True, prism=None, crop=None, allow_tf32x3=True, stream=None):
     """Create a library context for a workload; geometry comes from the library's own helpers.
     All edges must share the detector angle of edges[0] for the S2 parent set (as in every config here)."""
     import torch
@@ -63,7 +63,8 @@ def gpu_context(wl, edges, parent_factor=None, max_nn=8, T_on_device=True, prism
     crop = tuple(crop) if crop is not None else tuple(getattr(wl, 'crop', (1, 1)))
     geo = B.plan_geometry(g, wl.alpha_mrad, edges[0].det_mrad, wl.defocus, pf, max_nn, prism=prism)
     T = torch.from_numpy(wl.T).cuda() if T_on_device else wl.T
-    ctx = B.Context(g, T, geo.ap_h, geo.ap_c, geo.p1_h, geo.w1, geo.p2_h)
+    ctx = B.Context(g, T, geo.ap_h, geo.ap_c, geo.p1_h, geo.w1, geo.p2_h, stream=stream)
+    ctx.allow_tf32x3(allow_tf32x3)                    # the parity tests run TF32X3 as the measured A/B case (include/bip.h)
     ctx.build_S1()
     ctx.build_S2()
     ctx.set_scan(wl.scan)
@@ -85,11 +86,14 @@ class OracleSample:
     chunks and only their W x W windows at the sampled sites are kept.  Contraction shapes per (scan, channel,
     beam) are those of the full workload.  Used by the full-size parity test and by bench.py's oracle legs."""
 
-    def __init__(self, workload="cfg2", scale=1, nz=2, n_atoms=1, n_scan=256, n_jobs=None, edge=0):
+    def __init__(self, workload="cfg2", scale=1, nz=2, n_atoms=1, n_scan=256, n_jobs=None, edge=0, atom_idx=None):
         import os
         from bip_inputs.specimen import make_workload
         self.wl = wl = make_workload(workload, scale=scale, nz=nz)
-        self.e = e = wl.edges[edge].take(np.arange(n_atoms))
+        if atom_idx is not None:                          # explicit sites (e.g. one deep inside the slab)
+            atom_idx = np.asarray(atom_idx)
+            n_atoms = len(atom_idx)
+        self.e = e = wl.edges[edge].take(np.arange(n_atoms) if atom_idx is None else atom_idx)
         self.orc = orc = OracleSetup(wl, e, n_jobs=n_jobs or os.cpu_count())
         T = wl.T.astype(np.complex128)
         planes = sorted(set(int(s) for s in e.slice))

@@ -88,8 +88,9 @@ def test_geometry_full_size_cfg2_sampled_rows():
 def test_identity_partition_for_factor_one():
     g = B.Grid(32, 32, 8.0, 8.0, 2, 2.0, 0.025)
     geo = B.plan_geometry(g, 12.0, 16.0, 0.0, (1, 1))
-    assert np.array_equal(geo.p1_pos, np.arange(len(geo.ap_h))) and geo.w1[0].shape[1] == 1
-    assert np.array_equal(geo.w1[0][:, 0], np.arange(len(geo.ap_h))) and np.all(geo.w1[1] == 1.0)
+    assert np.array_equal(geo.p1_pos, np.arange(len(geo.ap_h)))
+    assert np.array_equal(geo.w1[0][:, 0], np.arange(len(geo.ap_h))) and np.all(geo.w1[1][:, 0] == 1.0)
+    assert np.all(geo.w1[0][:, 1:] == -1) and np.all(geo.w1[1][:, 1:] == 0.0)
 
 
 def test_argument_validation_and_no_cpu_fallback():
@@ -127,3 +128,29 @@ def test_prism_subsample_matches_oracle():
     beams = ob.beams_in_disc(64, 48, 20.0, 15.0, 0.9)
     for fy, fx in ((1, 1), (2, 2), (4, 3), (5, 1)):
         assert np.array_equal(B.bip_prism_subsample(beams, fy, fx), ob.prism_subsample(beams, fy, fx))
+
+
+def test_partition_and_prism_coeffs_match_oracle():
+    """bip_partition (hex-ring + Sibson by parent factor, reading c7) and bip_prism_coeffs (f_y f_x rescale)
+    are C entry points, so that no method arithmetic is left in the Python binding: both against the oracle."""
+    lam = electron_wavelength(200.0)
+    g = B.Grid(64, 96, 12.0, 18.0, 2, 2.0, lam)
+    q = 18e-3 / lam
+    h = B.bip_beams_in_disc(g, q)
+    ho = ob.beams_in_disc(64, 96, 12.0, 18.0, q)
+    pos, (idx, w) = B.bip_partition(g, h, q, 2.0)
+    poso = ob.hexring_parents(ho, 64, 96, 12.0, 18.0, q, ob.n_radial_from_factor(len(ho), 2.0))
+    assert np.array_equal(pos, poso)
+    tab = osb.natural_neighbour_weights(ho, poso, 12.0, 18.0, q)
+    assert np.abs(_dense(idx, w, len(pos)) - osb.to_dense(tab, len(poso))).max() < 1e-6
+    c = B.bip_aperture_coeffs(g, h, -30.0)
+    co = ob.aperture_coefficients(ho, 64, 96, 12.0, 18.0, lam, -30.0)
+    for fy, fx in ((2, 2), (3, 2)):
+        keep = B.bip_prism_subsample(h, fy, fx)
+        got = B.bip_prism_coeffs(keep, c, fy, fx)
+        want = ob.prism_coefficients(co, ob.prism_subsample(ho, fy, fx), fy, fx)
+        assert np.abs((got[:, 0] + 1j * got[:, 1]) - want).max() < 1e-6 * np.abs(want).max()
+    with pytest.raises(B.BipError):
+        B.bip_prism_coeffs(np.array([len(h)], np.int32), c, 2, 2)                  # position outside the full list
+    with pytest.raises(B.BipError):
+        B.bip_partition(g, h, q, 0.5)                                               # factor < 1

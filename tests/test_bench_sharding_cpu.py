@@ -67,3 +67,25 @@ def test_reference_arm_prints_the_contract_line():
     assert d["e2e"] == {"value": d["value"], "unit": d["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
     r1 = subprocess.run(cmd, capture_output=True, text=True, env=dict(env, RANK="1", WORLD_SIZE="2"), timeout=600)
     assert r1.returncode == 0 and not [l for l in r1.stdout.splitlines() if l.startswith("{")]
+
+
+def test_sample_sites_spreads_a_step_over_planes_and_ranks():
+    """bench.sample_sites: --atoms sites spread evenly over the first --planes ionisation planes; ranks take disjoint blocks
+    inside every plane ("atoms spread over planes")."""
+    import bench
+    from bip_inputs.specimen import make_workload
+    e = make_workload("cfg1", scale=2, nz=8).edges[0]
+    planes = np.unique(e.slice)
+    a = bench.sample_sites(e, 0, 4, 2)
+    b = bench.sample_sites(e, 1, 4, 2)
+    assert len(a) == len(b) == 4 and not set(a.tolist()) & set(b.tolist())
+    assert sorted(set(e.slice[a].tolist())) == planes[:2].tolist() == sorted(set(e.slice[b].tolist()))
+    assert np.bincount(e.slice[a])[planes[:2]].tolist() == [2, 2]
+
+
+def test_gpus_flag_must_match_the_launch():
+    """`--gpus N` under a launcher that started a different number of ranks fails loudly instead of running 1 GPU."""
+    import subprocess
+    env = dict(os.environ, RANK="0", WORLD_SIZE="1", LOCAL_RANK="0")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "8"], capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode != 0 and "does not match WORLD_SIZE" in (r.stderr + r.stdout)

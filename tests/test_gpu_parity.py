@@ -224,12 +224,12 @@ def test_call_order_and_argument_errors():
 def test_full_size_cfg2_sampled_pixels(prec_name):
     """BASELINE.json configs[1] at FULL contraction size, in the launch configuration bench.py times (512^2 grid,
     B = 30 909, K = 79 105, parents (1951, 4921), W = 48, 9 channels, all 4096 scan positions, MAGPHASE, map output,
-    two atoms per launch): the oracle computes 16 sampled map pixels one by one (every channel and detector beam);
+    two atoms per launch): the oracle computes 64 sampled map pixels one by one (every channel and detector beam);
     the slab is truncated to 2 slices so that the fp64 parent columns are affordable (SURVEY 8(d) parity protocol).
     Properties that hold at any size on the rest: non-negative, finite, window origins bit-exact."""
     import torch
     import paper_2607_00756_b200 as B
-    smp = OracleSample("cfg2", nz=2, n_atoms=2, n_scan=16)
+    smp = OracleSample("cfg2", nz=2, n_atoms=2, n_scan=64)
     wl, e = smp.wl, smp.e
     want = smp.run("magphase")["map"]
     ctx, geo, ids = gpu_context(wl, [e])
@@ -244,7 +244,7 @@ def test_full_size_cfg2_sampled_pixels(prec_name):
     assert m.shape == (4096,) and np.all(np.isfinite(m)) and np.all(m >= 0)
     got = m[smp.scan_idx]
     assert rel_err_map(got, want, 1e-3) <= TOL_PIXEL
-    assert abs(got.sum() - want.sum()) <= 2 * TOL_SUM * want.sum()      # 16 pixels only: rounding noise averages less
+    assert abs(got.sum() - want.sum()) <= TOL_SUM * want.sum()          # north_star bound on the sum of the 64 sampled pixels
     t = ctx.get_timing()
     assert t["amplitudes"] == 4096 * 2 * 9 * 79105
     ctx.close()
@@ -318,7 +318,7 @@ def test_cfg4_fept_quarter_clone_prism_regime():
 def test_cfg5_factor_one_against_conventional_multislice_at_scale():
     """BASELINE.json configs[4] at parent factor 1 (parents = all 7721 aperture and 19 797 detector beams, w = I): the
     GPU path against Algorithm 1 itself -- conventional transition-potential multislice per scan position, the ground
-    truth -- at the full 256^2 size, on 4 sampled scan positions: full cube rows and map
+    truth -- at the full 256^2 size, on 16 sampled scan positions: full cube rows and map
     pixels.  No BiP oracle code in between.  Slab truncated to 3 slices (site in slice 1: one slice above, two through
     the exit) so that the 27 518 parent columns build quickly."""
     import torch
@@ -331,7 +331,7 @@ def test_cfg5_factor_one_against_conventional_multislice_at_scale():
     ap, det = ob.beams_in_disc(wl.ny, wl.nx, wl.ly, wl.lx, qa), ob.beams_in_disc(wl.ny, wl.nx, wl.ly, wl.lx, qd)
     c = ob.aperture_coefficients(ap, wl.ny, wl.nx, wl.ly, wl.lx, wl.lam, wl.defocus)
     P = oms.fresnel_propagator(wl.ny, wl.nx, wl.ly, wl.lx, wl.lam, wl.dz)
-    sub = np.array([0, 1000, 2079, 4095])
+    sub = np.array([0, 273, 546, 819, 1000, 1365, 1638, 1911, 2079, 2457, 2730, 3003, 3276, 3549, 3822, 4095])
     I1 = oms.conventional_cube(c, ap, wl.T.astype(np.complex128), P, wl.scan[sub], e.slice, e.centre, e.H.astype(complex), det)
     ctx, geo, ids = gpu_context(wl, [e])
     assert (ctx.n_p1, ctx.n_p2) == (7721, 19797) and geo.det_h.shape[0] == 19797
@@ -341,7 +341,7 @@ def test_cfg5_factor_one_against_conventional_multislice_at_scale():
     cube, m = cube.cpu().numpy(), m.cpu().numpy()
     assert rel_err_map(cube[sub], I1, 1e-3) <= TOL_PIXEL
     assert rel_err_map(m[sub], I1.sum(1)) <= TOL_PIXEL
-    assert abs(m[sub].sum() - I1.sum()) <= 2 * TOL_SUM * I1.sum()
+    assert abs(m[sub].sum() - I1.sum()) <= TOL_SUM * I1.sum()
     ctx.close()
 
 
