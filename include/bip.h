@@ -256,9 +256,28 @@ BIP_API int32_t bip_map_host(bip_ctx* ctx, int32_t edge_id, int32_t mode, int32_
 BIP_API int32_t bip_map_all(bip_ctx* ctx, int32_t mode, int32_t recon, int32_t precision,
                     void* const* outs_dev, const size_t* outs_bytes, int32_t n_outs);
 
+/* Algorithm 3 of the paper (Table 1): the energy-filtered 4D cube on ALL exit beams with
+ * only S1 partitioned.  For every ionisation plane S1.ADVANCETO; for every site the partitioned probe on the window
+ * (eq. 15 / eq. 11 + eq. 7: steps a1-a4 of the map path), psi_n = H_n psi (eq. 3), carried to the exit surface by
+ * conventional multislice for every scan position and channel, |F psi_n|^2 accumulated (Alg. 1 lines 5-8).  S2 is not
+ * used (bip_build_S2 need not have run).
+ *   out_dev   float [n_rho][ny][nx], exit beam (ky, kx) on the corner-origin DFT grid, unitary F; zero-initialised by the
+ *             call; out_bytes = n_rho * ny * nx * 4.
+ *   precision BIP_PREC_FP16X4 or BIP_PREC_BF16X6 (arithmetic of the probe contraction a4).
+ * The wavefields of a chunk of scan positions live in half of the scratch budget.  Returns after enqueueing. */
+BIP_API int32_t bip_cube_alg3(bip_ctx* ctx, int32_t edge_id, int32_t recon, int32_t precision, float* out_dev, size_t out_bytes);
+
 /* Device scratch the plane loop may use for the operands of one batch of sites (default 12 GB, minimum 32 MB): the
  * sites of a plane are contracted in batches that fit. */
 BIP_API int32_t bip_set_scratch_budget(bip_ctx* ctx, size_t bytes);
+
+/* Route of the slice steps (bip_build_S2, ADVANCETO, PEELTO; plumbing, timed separately):
+ *   BIP_FFT_NATIVE     the library's own fused fp32 slice step, three passes over a column (power-of-two grids 8..4096;
+ *                      the default there);
+ *   BIP_FFT_CUFFT_F64  cuFFT Z2Z on a double-precision workspace, columns rounded to c64 once per slice (any grid; the
+ *                      default for grids that are not powers of two, and the A/B reference of the native route). */
+typedef enum { BIP_FFT_NATIVE = 0, BIP_FFT_CUFFT_F64 = 1 } bip_fft_backend;
+BIP_API int32_t bip_set_fft_backend(bip_ctx* ctx, int32_t backend);
 
 /* Opt in (allow != 0) to BIP_PREC_TF32X3, which misses the 1e-6 summed-intensity bound (see bip_precision). */
 BIP_API int32_t bip_allow_tf32x3(bip_ctx* ctx, int32_t allow);

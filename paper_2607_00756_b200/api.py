@@ -19,6 +19,7 @@ MODE_MAP, MODE_QEELS_X, MODE_QEELS_Y, MODE_CUBE = 0, 1, 2, 3
 RECON_LINEAR, RECON_MAGPHASE = 0, 1
 ASSOC_PROBE, ASSOC_COUPLING, ASSOC_AUTO = 0, 1, 2
 PREC_TF32X3, PREC_FP32_SIMT, PREC_BF16X6, PREC_FP16X4, PREC_FP16X3 = 0, 1, 2, 3, 4
+FFT_NATIVE, FFT_CUFFT_F64 = 0, 1
 MAX_NN = 16
 _STATUS = {1: "BIP_ERR_INVALID", 2: "BIP_ERR_STATE", 3: "BIP_ERR_OOM", 4: "BIP_ERR_CUDA", 5: "BIP_ERR_UNSUPPORTED"}
 
@@ -65,7 +66,7 @@ ABI_SYMBOLS = (
     "bip_output_size", "bip_map", "bip_map_host", "bip_map_all", "bip_get_windows", "bip_get_qeels_bins",
     "bip_seek_plane", "bip_copy_S", "bip_debug_reconstruct", "bip_get_timing", "bip_version", "bip_prism_subsample",
     "bip_set_crop", "bip_set_association", "bip_prism_coeffs", "bip_partition", "bip_set_scratch_budget", "bip_allow_tf32x3",
-    "bip_get_parents", "bip_get_weights",
+    "bip_get_parents", "bip_get_weights", "bip_set_fft_backend", "bip_cube_alg3",
 )
 
 _lib: Optional[C.CDLL] = None
@@ -291,6 +292,10 @@ class Context:
     def set_scratch_budget(self, n_bytes: int):
         self._ck(self._lib.bip_set_scratch_budget(self._ctx, C.c_size_t(int(n_bytes))))
 
+    def set_fft_backend(self, backend: int):
+        """Slice-step route: FFT_NATIVE (fused fp32 kernels, power-of-two grids) or FFT_CUFFT_F64."""
+        self._ck(self._lib.bip_set_fft_backend(self._ctx, int(backend)))
+
     def allow_tf32x3(self, allow: bool = True):
         self._ck(self._lib.bip_allow_tf32x3(self._ctx, int(bool(allow))))
 
@@ -330,6 +335,17 @@ class Context:
         assert out.is_cuda and out.is_contiguous() and out.dtype == tdt and tuple(out.shape) == shape
         self._ck(self._lib.bip_map(self._ctx, edge_id, mode, recon, precision, C.c_void_p(out.data_ptr()),
                                    C.c_size_t(out.numel() * out.element_size())))
+        return out
+
+    def cube_alg3(self, edge_id: int, recon: int = RECON_LINEAR, precision: int = PREC_FP16X4, out=None):
+        """bip_cube_alg3: the S1-partitioned 4D cube on all exit beams, float32 [n_rho, ny, nx] (torch CUDA tensor)."""
+        import torch
+        shape = (self.n_rho, self.g.ny, self.g.nx)
+        if out is None:
+            out = torch.empty(shape, dtype=torch.float32, device="cuda")
+        assert out.is_cuda and out.is_contiguous() and out.dtype == torch.float32 and tuple(out.shape) == shape
+        self._ck(self._lib.bip_cube_alg3(self._ctx, int(edge_id), int(recon), int(precision), C.c_void_p(out.data_ptr()),
+                                         C.c_size_t(out.numel() * 4)))
         return out
 
     def map_all(self, mode: int = MODE_MAP, recon: int = RECON_LINEAR, precision: int = PREC_FP16X4):

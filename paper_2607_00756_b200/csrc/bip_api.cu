@@ -206,8 +206,8 @@ static float sum_ms(SpanList& v) {
 // slice steps -- the restart also discards the rounding accumulated by earlier passes.  S2 forward: the peel
 // P*[T_j* .]; backward: the build recursion T_j P[.] itself (eq. 12), exact for any T.  A counter moves only after its
 // step has been enqueued successfully.
-static int32_t seek(bip_ctx* ctx, int32_t plane) {
-  if (!ctx->s1_built || !ctx->s2_built) return fail(ctx, BIP_ERR_STATE, "bip_build_S1 and bip_build_S2 must run before the plane loop");
+static int32_t seek_S1(bip_ctx* ctx, int32_t plane) {
+  if (!ctx->s1_built) return fail(ctx, BIP_ERR_STATE, "bip_build_S1 must run before the plane loop");
   if (plane < 0 || plane > ctx->g.nz) return fail(ctx, BIP_ERR_INVALID, "plane %d outside 0..%d", plane, ctx->g.nz);
   if (plane < ctx->plane1 && plane <= ctx->plane1 - plane) {
     BIP_TRY(ms_plane_waves(ctx, ctx->S1, ctx->p1_h_dev, ctx->n_p1, +1));
@@ -215,6 +215,12 @@ static int32_t seek(bip_ctx* ctx, int32_t plane) {
   }
   while (ctx->plane1 < plane) { BIP_TRY(ms_step_S1(ctx, ctx->plane1, +1)); ctx->plane1++; }
   while (ctx->plane1 > plane) { BIP_TRY(ms_step_S1(ctx, ctx->plane1 - 1, -1)); ctx->plane1--; }
+  return BIP_OK;
+}
+
+static int32_t seek(bip_ctx* ctx, int32_t plane) {
+  if (!ctx->s1_built || !ctx->s2_built) return fail(ctx, BIP_ERR_STATE, "bip_build_S1 and bip_build_S2 must run before the plane loop");
+  BIP_TRY(seek_S1(ctx, plane));
   while (ctx->plane2 < plane) { BIP_TRY(ms_step_S2(ctx, ctx->plane2, +1)); ctx->plane2++; }
   while (ctx->plane2 > plane) { BIP_TRY(ms_step_S2(ctx, ctx->plane2 - 1, -1)); ctx->plane2--; }
   return BIP_OK;
@@ -289,6 +295,24 @@ static bool use_coupling(const bip_ctx* ctx, const Edge& e, double rows_per_site
   return true;
 }
 
+// Steps a1-a4 for nb sites: S1 windows -> R1^T (sliced) -> probe at the atom Psi[site][rho][s] (c64, pitch w^2) in ctx->Psi.
+// R1t must have been carved (sliced_in) and given its scales by the caller.
+static int32_t probe_at_sites(bip_ctx* ctx, Edge& e, const int32_t* org, int32_t nb, int recon, bool drop_tiny, const Sliced& Ax,
+                              int32_t n_rows, const Sliced& R1t, Gemm1SlArgs* g1_out) {
+  const int w2 = e.w * e.w;
+  BIP_TRY(ensure(ctx, ctx->D1, (size_t)nb * ctx->n_p1 * w2 * sizeof(float2), "D1 (de-tilted S1 windows)"));
+  BIP_TRY(ensure(ctx, ctx->Psi, (size_t)nb * n_rows * w2 * sizeof(float2), "Psi (probe at the atom)"));
+  BIP_TRY(launch_crop_detilt(ctx, ctx->S1, ctx->p1_h_dev, ctx->n_p1, +1, org, nb, e.w, (float2*)ctx->D1.p));          // a1
+  BIP_TRY(launch_recon_t_sliced(ctx, (const float2*)ctx->D1.p, ctx->n_p1, ctx->ap_h_dev, ctx->n_ap, ctx->w1_idx_dev, ctx->w1_w_dev,
+                                ctx->nn1, +1, recon, org, nb, e.w, R1t));                                                   // a2
+  Gemm1SlArgs g1;                                                                                                            // a3-a4
+  g1.A = Ax; g1.R1t = R1t; g1.Psi = (float2*)ctx->Psi.p; g1.psi_ld = w2; g1.psi_batch_stride = (int64_t)n_rows * w2;
+  g1.n_rho = n_rows; g1.w2 = w2; g1.n_atoms = nb; g1.drop_tiny = drop_tiny;
+  BIP_TRY(launch_gemm1_sliced(ctx, g1));
+  if (g1_out) *g1_out = g1;
+  return BIP_OK;
+}
+
 // Crop mask: the number of scan rows inside every site's window, counted on the device once per (edge,
 // crop setting, scan) and kept on the host -- the per-batch launches below are then sized without a device round trip.
 static int32_t ensure_crop_counts(bip_ctx* ctx, Edge& e) {
@@ -343,28 +367,20 @@ static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, 
   if (coupling)
     return contract_coupling(ctx, e, org, nb, mode, recon, fmt, drop_tiny, out, Ax, n_rows, rho_pad, row_idx_dev, row_idx_stride, n_rows_total);
   Sliced R1t, R2, Phi;
-  BIP_TRY(ensure(ctx, ctx->D1, (size_t)nb * ctx->n_p1 * w2 * sizeof(float2), "D1 (de-tilted S1 windows)"));
   BIP_TRY(ensure(ctx, ctx->D2, (size_t)nb * ctx->n_p2 * w2 * sizeof(float2), "D2 (de-tilted S2 windows)"));
   BIP_TRY(sliced_in(ctx, ctx->R1s, R1t, fmt, w2, ctx->n_ap, nb, "R1 (reconstructed S1 windows, sliced)"));
   BIP_TRY(sliced_in(ctx, ctx->R2s, R2, fmt, e.n_det, w2, nb, "R2 (reconstructed S2 windows, sliced)"));
   BIP_TRY(sliced_in(ctx, ctx->Phis, Phi, fmt, rho_pad * e.n_ch, w2, nb, "Phi (H_n psi, sliced)"));
   const int64_t psi_ld = w2;
-  BIP_TRY(ensure(ctx, ctx->Psi, (size_t)nb * n_rows * psi_ld * sizeof(float2), "Psi (probe at the atom)"));
   const int64_t n_scale = (int64_t)nb * (R1t.rows_pad + R2.rows_pad + Phi.rows_pad);
   BIP_TRY(ensure(ctx, ctx->Scl, (size_t)n_scale * sizeof(float), "row scales"));
   R1t.scale = reinterpret_cast<float*>(ctx->Scl.p);           R1t.scale_batch_stride = R1t.rows_pad;
   R2.scale = R1t.scale + (int64_t)nb * R1t.rows_pad;          R2.scale_batch_stride = R2.rows_pad;
   Phi.scale = R2.scale + (int64_t)nb * R2.rows_pad;           Phi.scale_batch_stride = Phi.rows_pad;
 
-  // a1-a2: S1 windows -> R1^T[s][b]
-  BIP_TRY(launch_crop_detilt(ctx, ctx->S1, ctx->p1_h_dev, ctx->n_p1, +1, org, nb, e.w, (float2*)ctx->D1.p));
-  BIP_TRY(launch_recon_t_sliced(ctx, (const float2*)ctx->D1.p, ctx->n_p1, ctx->ap_h_dev, ctx->n_ap, ctx->w1_idx_dev, ctx->w1_w_dev,
-                                ctx->nn1, +1, recon, org, nb, e.w, R1t));
-  // a3-a4: probe at the atom
+  // a1-a4: S1 windows -> R1^T[s][b] -> probe at the atom
   Gemm1SlArgs g1;
-  g1.A = Ax; g1.R1t = R1t; g1.Psi = (float2*)ctx->Psi.p; g1.psi_ld = psi_ld; g1.psi_batch_stride = (int64_t)n_rows * psi_ld;
-  g1.n_rho = n_rows; g1.w2 = w2; g1.n_atoms = nb; g1.drop_tiny = drop_tiny;
-  BIP_TRY(launch_gemm1_sliced(ctx, g1));
+  BIP_TRY(probe_at_sites(ctx, e, org, nb, recon, drop_tiny, Ax, n_rows, R1t, &g1));
   // a5: times H_n, split into slices
   BIP_TRY(launch_quantize_phi(ctx, g1.Psi, psi_ld, g1.psi_batch_stride, e.H_dev, Phi, n_rows, (int32_t)rho_pad, w2, e.n_ch, nb));
   // a6: S2 windows -> R2[d][s]
@@ -528,6 +544,70 @@ static int32_t run_edges(bip_ctx* ctx, const std::vector<int32_t>& ids, int mode
   return BIP_OK;
 }
 
+// ---- NEXT-3: Algorithm 3 -- S1-partitioned probe, per-scan exit multislice, all G exit beams ----
+
+// fields[(rho, n)][r] = H_n[s] Psi[rho0 + rho][s] on the site's window (r = (origin + s) mod N), zero elsewhere (eq. 3)
+__global__ void k_embed_fields(const float2* __restrict__ Psi, int64_t psi_ld, const float2* __restrict__ H, int n_ch, int w, int oy, int ox, int ny,
+                               int nx, float2* __restrict__ F) {
+  const int rho = blockIdx.y, n = blockIdx.z, w2 = w * w;
+  float2* f = F + ((int64_t)rho * n_ch + n) * ny * nx;
+  for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < w2; s += gridDim.x * blockDim.x) {
+    const int sy = s / w, sx = s - sy * w;
+    int ry = oy + sy; if (ry >= ny) ry -= ny;
+    int rx = ox + sx; if (rx >= nx) rx -= nx;
+    const float2 h = __ldg(H + (int64_t)n * w2 + s), a = Psi[(int64_t)rho * psi_ld + s];
+    f[(int64_t)ry * nx + rx] = make_float2(h.x * a.x - h.y * a.y, h.x * a.y + h.y * a.x);
+  }
+}
+
+static int32_t run_alg3(bip_ctx* ctx, Edge& e, int recon, int precision, float* out) {
+  const int fmt = sliced_fmt_of(precision);
+  if (fmt < 0 || precision == BIP_PREC_FP16X3) return fail(ctx, BIP_ERR_UNSUPPORTED, "bip_cube_alg3: precision must be FP16X4 or BF16X6");
+  if (ctx->crop_fy * ctx->crop_fx > 1) return fail(ctx, BIP_ERR_UNSUPPORTED, "bip_cube_alg3: the crop mask is not applied to the full-grid cube; call bip_set_crop(ctx, 1, 1)");
+  BIP_TRY(ensure_illumination(ctx, precision));
+  auto& sp = ctx->spans;
+  sp.adv.clear(); sp.contract.clear(); sp.gemm2.clear(); sp.pool_map.reset();
+  ctx->timing.gemm2_launches = 0; ctx->timing.kernel_launches = 0; ctx->timing.amplitudes = 0; ctx->timing.flops = 0;
+  const int ny = ctx->g.ny, nx = ctx->g.nx, nz = ctx->g.nz, w2 = e.w * e.w;
+  const int64_t G = (int64_t)ny * nx;
+  BIP_CUDA(ctx, cudaMemsetAsync(out, 0, (size_t)ctx->n_rho * G * sizeof(float), ctx->stream));
+  // wavefields of one chunk of scan positions: (rho, channel) fields of the whole grid
+  const int64_t max_fields = std::max<int64_t>(e.n_ch, (int64_t)(ctx->scratch_budget / 2 / (G * sizeof(float2))));
+  const int32_t rho_chunk = (int32_t)std::max<int64_t>(1, std::min<int64_t>(ctx->n_rho, max_fields / e.n_ch));
+  BIP_TRY(ensure(ctx, ctx->Fields, (size_t)rho_chunk * e.n_ch * G * sizeof(float2), "exit wavefields (Algorithm 3)"));
+  float2* F = reinterpret_cast<float2*>(ctx->Fields.p);
+  Sliced R1t;
+  BIP_TRY(sliced_in(ctx, ctx->R1s, R1t, fmt, w2, ctx->n_ap, 1, "R1 (reconstructed S1 windows, sliced)"));
+  BIP_TRY(ensure(ctx, ctx->Scl, (size_t)R1t.rows_pad * sizeof(float), "row scales"));
+  R1t.scale = reinterpret_cast<float*>(ctx->Scl.p); R1t.scale_batch_stride = R1t.rows_pad;
+  int32_t a = 0;
+  while (a < e.n_atoms) {
+    const int32_t plane = e.slice[a];
+    { Span s(ctx, sp.pool_map, sp.adv); BIP_TRY(seek_S1(ctx, plane)); }                           // Alg. 3 line 4
+    Span sc(ctx, sp.pool_map, sp.contract);
+    for (; a < e.n_atoms && e.slice[a] == plane; ++a) {
+      Gemm1SlArgs g1;
+      BIP_TRY(probe_at_sites(ctx, e, e.origin_dev + 2 * (int64_t)a, 1, recon, false, ctx->A_sl, ctx->n_rho, R1t, &g1));   // lines 5-10 on the window
+      for (int32_t r0 = 0; r0 < ctx->n_rho; r0 += rho_chunk) {
+        const int32_t nr = std::min(rho_chunk, ctx->n_rho - r0), nf = nr * e.n_ch;
+        BIP_CUDA(ctx, cudaMemsetAsync(F, 0, (size_t)nf * G * sizeof(float2), ctx->stream));
+        for (int32_t q0 = 0; q0 < nr; q0 += 65535) {
+          const int32_t nq = std::min(65535, nr - q0);
+          k_embed_fields<<<dim3((unsigned)((w2 + 255) / 256), (unsigned)nq, (unsigned)e.n_ch), 256, 0, ctx->stream>>>(
+              g1.Psi + (int64_t)(r0 + q0) * g1.psi_ld, g1.psi_ld, e.H_dev, e.n_ch, e.w, e.origin[2 * a], e.origin[2 * a + 1], ny, nx, F + (int64_t)q0 * e.n_ch * G);
+        }
+        BIP_CUDA(ctx, cudaGetLastError());
+        ctx->timing.kernel_launches++;
+        for (int32_t j = plane; j < nz; ++j) BIP_TRY(ms_exit_step(ctx, F, nf, j));               // line 11: to the exit surface
+        BIP_TRY(ms_detect(ctx, F, nr, e.n_ch, out + (int64_t)r0 * G));                            // |F psi_n|^2, summed over n
+      }
+      ctx->timing.amplitudes += (double)ctx->n_rho * e.n_ch * (double)G;
+      ctx->timing.flops += 8.0 * ctx->n_rho * w2 * (double)ctx->n_ap;
+    }
+  }
+  return BIP_OK;
+}
+
 }  // namespace bip
 
 using namespace bip;
@@ -642,7 +722,7 @@ int32_t bip_destroy(bip_ctx* ctx) {
   if (ctx->T_owned) cudaFree((void*)ctx->T_dev);
   void* ptrs[] = {ctx->ap_h_dev, ctx->p1_h_dev, ctx->p2_h_dev, ctx->ap_c_dev, ctx->w1_idx_dev, ctx->w1_w_dev, ctx->rooty_dev,
                   ctx->rootx_dev, ctx->P_dev, ctx->ms_work, ctx->S1, ctx->S2, ctx->D1.p, ctx->D2.p, ctx->R1.p, ctx->R2.p, ctx->Psi.p,
-                  ctx->Phi.p, ctx->R1s.p, ctx->R2s.p, ctx->Phis.p, ctx->Scl.p, ctx->Sync.p, ctx->RowIdx.p, ctx->Acrop.p, ctx->Pmax.p, ctx->R1r.p, ctx->HR2.p, ctx->Mc.p, ctx->Ms.p, ctx->rho_dev};
+                  ctx->Phi.p, ctx->R1s.p, ctx->R2s.p, ctx->Phis.p, ctx->Scl.p, ctx->Sync.p, ctx->Fields.p, ctx->RowIdx.p, ctx->Acrop.p, ctx->Pmax.p, ctx->R1r.p, ctx->HR2.p, ctx->Mc.p, ctx->Ms.p, ctx->rho_dev};
   free_illumination(ctx);
   for (void* p : ptrs) if (p) cudaFree(p);
   cudaGetLastError();
@@ -831,6 +911,18 @@ int32_t bip_map_host(bip_ctx* ctx, int32_t edge_id, int32_t mode, int32_t recon,
   return st;
 }
 
+int32_t bip_cube_alg3(bip_ctx* ctx, int32_t edge_id, int32_t recon, int32_t precision, float* out_dev, size_t out_bytes) {
+  if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
+  if (edge_id < 0 || edge_id >= (int)ctx->edges.size()) return fail(ctx, BIP_ERR_INVALID, "bip_cube_alg3: edge %d does not exist", edge_id);
+  if (!ctx->s1_built) return fail(ctx, BIP_ERR_STATE, "bip_cube_alg3: call bip_build_S1 first (S2 is not used by Algorithm 3)");
+  if (ctx->n_rho <= 0) return fail(ctx, BIP_ERR_STATE, "bip_cube_alg3: call bip_set_scan first");
+  if (recon != BIP_RECON_LINEAR && recon != BIP_RECON_MAGPHASE) return fail(ctx, BIP_ERR_INVALID, "bip_cube_alg3: unknown recon %d", recon);
+  const size_t need = (size_t)ctx->n_rho * ctx->g.ny * ctx->g.nx * sizeof(float);
+  if (!out_dev || out_bytes != need) return fail(ctx, BIP_ERR_INVALID, "bip_cube_alg3: output has %zu bytes, expected %zu", out_bytes, need);
+  if (!tc_available()) return fail(ctx, BIP_ERR_UNSUPPORTED, "bip_cube_alg3: the tensor-core path is not built");
+  return run_alg3(ctx, ctx->edges[edge_id], recon, precision, out_dev);
+}
+
 int32_t bip_get_windows(const bip_ctx* ctx, int32_t edge_id, int32_t* origin_out) {
   if (!ctx || !origin_out) return fail(nullptr, BIP_ERR_INVALID, "bip_get_windows: NULL argument");
   if (edge_id < 0 || edge_id >= (int)ctx->edges.size()) return fail(const_cast<bip_ctx*>(ctx), BIP_ERR_INVALID, "edge %d does not exist", edge_id);
@@ -920,6 +1012,15 @@ int32_t bip_get_weights(const bip_ctx* ctx, int32_t edge_id, int32_t* n_rows, in
   if (max_nn) *max_nn = nn;
   if (nn_idx_out) std::copy(idx.begin(), idx.end(), nn_idx_out);
   if (nn_w_out) std::copy(w.begin(), w.end(), nn_w_out);
+  return BIP_OK;
+}
+
+int32_t bip_set_fft_backend(bip_ctx* ctx, int32_t backend) {
+  if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
+  if (backend != BIP_FFT_NATIVE && backend != BIP_FFT_CUFFT_F64) return fail(ctx, BIP_ERR_INVALID, "bip_set_fft_backend: unknown backend %d", backend);
+  if (backend == BIP_FFT_NATIVE && !fft_supported(ctx))
+    return fail(ctx, BIP_ERR_UNSUPPORTED, "bip_set_fft_backend: the native slice step needs a power-of-two grid (8..4096), this one is %d x %d", ctx->g.ny, ctx->g.nx);
+  ctx->fft_native = backend == BIP_FFT_NATIVE;
   return BIP_OK;
 }
 

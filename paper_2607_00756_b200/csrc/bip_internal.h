@@ -119,7 +119,12 @@ struct bip_ctx {
   // roots of unity exp(2 pi i k / N), k = 0..N-1 (exact phases for tilt / de-tilt)
   float2 *rooty_dev = nullptr, *rootx_dev = nullptr;
   void* P_dev = nullptr;           // Fresnel propagator / G as double2 [ny][nx]
-  void* ms_work = nullptr;         // double2 workspace of the slice steps [plan_batch][ny][nx]
+  void* ms_work = nullptr;         // double2 workspace of the cuFFT slice steps [plan_batch][ny][nx], allocated on first use
+  // native fused slice step for power-of-two grids (bip_fft.cu)
+  float2 *fft_rooty = nullptr, *fft_rootx = nullptr, *fft_P = nullptr;
+  int32_t *fft_permy = nullptr, *fft_permx = nullptr;   // true frequency index of every stored (digit-reversed) position
+  int fft_lines = 0, fft_cols = 0;
+  bool fft_native = false;         // route in use (bip_set_fft_backend)
   float2 *S1 = nullptr, *S2 = nullptr;
   bool s1_built = false, s2_built = false;
   int32_t plane1 = 0, plane2 = 0;  // S1 holds slices 0..plane1-1; S2 holds slices plane2..nz-1
@@ -149,6 +154,7 @@ struct bip_ctx {
   // scratch, grown on demand
   bip::DevBuf D1, D2, R1, R2, Psi, Phi;
   bip::DevBuf R1s, R2s, Phis, Scl;  // sliced operands of the tensor-core path and their row scales
+  bip::DevBuf Fields;               // wavefields of the per-scan exit multislice (Algorithm 3)
   bip::DevBuf Sync;                 // lockstep counters of the persistent contraction kernel (one per launch slot)
   int sync_slot = 0;
 
@@ -186,6 +192,17 @@ int32_t ms_max_modulus_deviation(bip_ctx* ctx, const float2* T, int64_t n, float
 int32_t ms_step_S1(bip_ctx* ctx, int32_t j, int dir);
 // build/un-peel: S <- T_j P[S] (dir=-1, towards the entrance) ; peel: S <- P*[T_j* S] (dir=+1)   (S2, eq. 12)
 int32_t ms_step_S2(bip_ctx* ctx, int32_t j, int dir);
+// exit multislice of Algorithm 3 on arbitrary wavefields: F <- P[T_j F] for n fields [n][ny][nx]
+int32_t ms_exit_step(bip_ctx* ctx, float2* fields, int n, int32_t j);
+// out[rho][ky][kx] += sum_n |F fields[rho][n]|^2 / G (unitary F, corner-origin order); fields are destroyed
+int32_t ms_detect(bip_ctx* ctx, float2* fields, int n_rho, int n_ch, float* out);
+
+// ---- native fused slice step for power-of-two grids (bip_fft.cu) ----
+bool fft_supported(const bip_ctx* ctx);
+int32_t fft_init(bip_ctx* ctx);
+int32_t fft_slice_op(bip_ctx* ctx, float2* S, int n_cols, const float2* Tj, int pre, int conj_p, int post);
+int32_t fft_detect(bip_ctx* ctx, float2* fields, int n_rho, int n_ch, float* out);
+void fft_release(bip_ctx* ctx);
 
 // ---- reconstruction (bip_recon.cu) ----
 // a1: D[a][p][s] = S_p(r) * exp(-carrier 2 pi i h_p.r/N) on the atoms' windows

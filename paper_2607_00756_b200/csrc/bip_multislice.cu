@@ -40,6 +40,7 @@ __global__ void k_modulus_deviation(const float2* __restrict__ T, int64_t n, uns
   if ((threadIdx.x & 31) == 0) atomicMax(out, __float_as_uint(m));
 }
 
+// The cuFFT route (grids that are not powers of two, and the A/B reference of the native slice step).
 // cuFFT's single-precision C2C loses ~3e-7 of the norm^2 per forward+inverse pair, systematically (measured on
 // B200 in round 1; tests/test_gpu_plumbing.py re-measures the drift of both variants); over tens of slices that alone breaks the 1e-6 summed-intensity bound.  The slice
 // steps therefore run in double precision (Z2Z) on a chunk workspace and the columns are stored back as c64:
@@ -104,8 +105,10 @@ int32_t get_plan(bip_ctx* ctx, int batch, cufftHandle* out) {
 // One unitary slice operation on all columns of S:  S <- post . F^-1[ Pspec . F[ pre . S ] ]
 //   pre / post: 0 = identity, 1 = T_j, 2 = conj T_j ;  conj_p: multiply the spectrum by conj(P) instead of P
 int32_t slice_op(bip_ctx* ctx, float2* S, int n_cols, const float2* Tj, int pre, int conj_p, int post) {
+  if (ctx->fft_native) return fft_slice_op(ctx, S, n_cols, Tj, pre, conj_p, post);
   const int64_t G = (int64_t)ctx->g.ny * ctx->g.nx;
   const int chunk = ctx->plan_batch;
+  if (!ctx->ms_work) BIP_TRY(dev_alloc(ctx, &ctx->ms_work, (size_t)ctx->plan_batch * G * sizeof(double2), "multislice workspace"));
   double2* W = reinterpret_cast<double2*>(ctx->ms_work);
   const double2* P = reinterpret_cast<const double2*>(ctx->P_dev);
   for (int c0 = 0; c0 < n_cols; c0 += chunk) {
@@ -126,9 +129,49 @@ int32_t slice_op(bip_ctx* ctx, float2* S, int n_cols, const float2* Tj, int pre,
   return BIP_OK;
 }
 
+// out[f / n_ch][i] += |W[f][i]|^2 / G summed over the n_ch fields of a scan position (cuFFT route of ms_detect)
+__global__ void k_detect_accum(const double2* __restrict__ W, int n_ch, float* __restrict__ out, double inv_G, int64_t G) {
+  const int64_t rho = blockIdx.y;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < G; i += (int64_t)gridDim.x * blockDim.x) {
+    double a = 0.0;
+    for (int n = 0; n < n_ch; ++n) {
+      const double2 v = W[(rho * n_ch + n) * G + i];
+      a += v.x * v.x + v.y * v.y;
+    }
+    out[rho * G + i] += (float)(a * inv_G);
+  }
+}
+
 }  // namespace
 
+int32_t ms_exit_step(bip_ctx* ctx, float2* fields, int n, int32_t j) {
+  const float2* Tj = ctx->T_dev + (int64_t)j * ctx->g.ny * ctx->g.nx;
+  return slice_op(ctx, fields, n, Tj, /*pre=*/1, /*conj_p=*/0, /*post=*/0);      // psi <- P[T_j psi] (eq. 6 on a wavefield)
+}
+
+int32_t ms_detect(bip_ctx* ctx, float2* fields, int n_rho, int n_ch, float* out) {
+  if (ctx->fft_native) return fft_detect(ctx, fields, n_rho, n_ch, out);
+  const int64_t G = (int64_t)ctx->g.ny * ctx->g.nx;
+  if (!ctx->ms_work) BIP_TRY(dev_alloc(ctx, &ctx->ms_work, (size_t)ctx->plan_batch * G * sizeof(double2), "multislice workspace"));
+  double2* W = reinterpret_cast<double2*>(ctx->ms_work);
+  const int rho_chunk = std::max(1, ctx->plan_batch / n_ch);
+  if (n_ch > ctx->plan_batch) return fail(ctx, BIP_ERR_UNSUPPORTED, "Algorithm 3 on the cuFFT route: %d channels exceed the transform batch %d", n_ch, ctx->plan_batch);
+  for (int r0 = 0; r0 < n_rho; r0 += rho_chunk) {
+    const int nr = std::min(rho_chunk, n_rho - r0), nf = nr * n_ch;
+    cufftHandle h;
+    BIP_TRY(get_plan(ctx, nf, &h));
+    dim3 grid((unsigned)std::min<int64_t>((G + 255) / 256, 2048), (unsigned)nf);
+    k_load_cols<<<grid, 256, 0, ctx->stream>>>(W, fields + (int64_t)r0 * n_ch * G, nullptr, G, 0);
+    cufftResult r = cufftExecZ2Z(h, reinterpret_cast<cufftDoubleComplex*>(W), reinterpret_cast<cufftDoubleComplex*>(W), CUFFT_FORWARD);
+    if (r != CUFFT_SUCCESS) return fail(ctx, BIP_ERR_CUDA, "cufftExecZ2Z failed: %d", (int)r);
+    k_detect_accum<<<dim3(grid.x, (unsigned)nr), 256, 0, ctx->stream>>>(W, n_ch, out + (int64_t)r0 * G, 1.0 / (double)G, G);
+    BIP_CUDA(ctx, cudaGetLastError());
+  }
+  return BIP_OK;
+}
+
 void ms_release(bip_ctx* ctx) {
+  fft_release(ctx);
   for (auto& kv : ctx->plans) cufftDestroy(kv.second);
   ctx->plans.clear();
 }
@@ -163,8 +206,9 @@ int32_t ms_init(bip_ctx* ctx) {
   // cuFFT batch: at most 512 MB of double-precision workspace per call
   const int64_t col_bytes = G * (int64_t)sizeof(double2);
   ctx->plan_batch = (int)std::max<int64_t>(1, std::min<int64_t>(std::max(ctx->n_p1, ctx->n_p2), (512ll << 20) / col_bytes));
-  BIP_TRY(dev_alloc(ctx, &ctx->ms_work, (size_t)ctx->plan_batch * col_bytes, "multislice workspace"));
   ctx->plan_ok = true;
+  // power-of-two grids take the native fused slice step (bip_fft.cu); any other grid the cuFFT route above
+  if (fft_supported(ctx)) { BIP_TRY(fft_init(ctx)); ctx->fft_native = true; }
   return BIP_OK;
 }
 
