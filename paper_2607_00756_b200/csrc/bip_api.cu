@@ -70,13 +70,14 @@ static int32_t planes_in(bip_ctx* ctx, DevBuf& buf, Planes& P, int64_t rows, int
 // the padding rows of the last row tile only have to be finite (they feed masked accumulator rows / columns), so the
 // buffer is cleared when it is (re)allocated and never again.
 static int32_t sliced_in(bip_ctx* ctx, DevBuf& buf, Sliced& S, int fmt, int64_t rows, int64_t k, int64_t batch, const char* what,
-                         int64_t row_align = SL_ROWS) {
+                         int64_t row_align = SL_ROWS, bool y_operand = false) {
   S.fmt = fmt;
+  S.neg_im = y_operand && sliced_wide(fmt) ? 1 : 0;       // Y operands of the N = 256 kernel carry the negated imaginary slices
   S.rows = rows;
   S.rows_pad = round_up(rows, row_align);
   S.k = k;
   S.ksteps = (k + SL_K - 1) / SL_K;
-  S.batch_stride = S.rows_pad / SL_ROWS * S.ksteps * sl_step_el(fmt);
+  S.batch_stride = S.rows_pad / SL_ROWS * S.ksteps * sl_step_el_of(S);
   const void* before = buf.p;
   BIP_TRY(ensure(ctx, buf, (size_t)(S.batch_stride * std::max<int64_t>(batch, 1)) * sizeof(uint16_t), what));
   if (buf.p != before) BIP_CUDA(ctx, cudaMemsetAsync(buf.p, 0, buf.bytes, ctx->stream));
@@ -240,9 +241,9 @@ static int32_t contract_coupling(bip_ctx* ctx, Edge& e, const int32_t* org, int3
   Sliced R1r, HR2, Ms;
   BIP_TRY(ensure(ctx, ctx->D1, (size_t)nb * ctx->n_p1 * w2 * sizeof(float2), "D1 (de-tilted S1 windows)"));
   BIP_TRY(ensure(ctx, ctx->D2, (size_t)nb * ctx->n_p2 * w2 * sizeof(float2), "D2 (de-tilted S2 windows)"));
-  BIP_TRY(sliced_in(ctx, ctx->R1r, R1r, fmt, ctx->n_ap, w2, nb, "R1 rows (coupling)"));
+  BIP_TRY(sliced_in(ctx, ctx->R1r, R1r, fmt, ctx->n_ap, w2, nb, "R1 rows (coupling)", SL_ROWS, true));
   BIP_TRY(sliced_in(ctx, ctx->HR2, HR2, fmt, n_nd, w2, nb, "H_n R2 rows (coupling)", 2 * SL_ROWS));
-  BIP_TRY(sliced_in(ctx, ctx->Ms, Ms, fmt, n_nd, ctx->n_ap, nb, "coupling matrix (sliced)"));
+  BIP_TRY(sliced_in(ctx, ctx->Ms, Ms, fmt, n_nd, ctx->n_ap, nb, "coupling matrix (sliced)", SL_ROWS, true));
   const int64_t m_ld = round_up(ctx->n_ap, 2);                   // even pitch: the GEMM epilogue stores pairs of complex values
   BIP_TRY(ensure(ctx, ctx->Mc, (size_t)nb * n_nd * m_ld * sizeof(float2), "coupling matrix"));
   const int64_t n_scale = (int64_t)nb * (R1r.rows_pad + HR2.rows_pad + Ms.rows_pad);
@@ -355,7 +356,7 @@ static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, 
     row_idx_stride = idx_stride;
     Sliced Ac = ctx->A_sl;
     Ac.rows = n_rows; Ac.rows_pad = rho_pad;
-    Ac.batch_stride = rho_pad / SL_ROWS * Ac.ksteps * sl_step_el(fmt);
+    Ac.batch_stride = rho_pad / SL_ROWS * Ac.ksteps * sl_step_el_of(Ac);
     Ac.scale_batch_stride = rho_pad;
     const size_t op_bytes = (size_t)(Ac.batch_stride * nb) * sizeof(uint16_t), sc_bytes = (size_t)nb * rho_pad * sizeof(float);
     BIP_TRY(ensure(ctx, ctx->Acrop, op_bytes + sc_bytes, "illumination rows of the cropped scans"));
@@ -368,8 +369,8 @@ static int32_t contract_batch_sliced(bip_ctx* ctx, Edge& e, const int32_t* org, 
     return contract_coupling(ctx, e, org, nb, mode, recon, fmt, drop_tiny, out, Ax, n_rows, rho_pad, row_idx_dev, row_idx_stride, n_rows_total);
   Sliced R1t, R2, Phi;
   BIP_TRY(ensure(ctx, ctx->D2, (size_t)nb * ctx->n_p2 * w2 * sizeof(float2), "D2 (de-tilted S2 windows)"));
-  BIP_TRY(sliced_in(ctx, ctx->R1s, R1t, fmt, w2, ctx->n_ap, nb, "R1 (reconstructed S1 windows, sliced)"));
-  BIP_TRY(sliced_in(ctx, ctx->R2s, R2, fmt, e.n_det, w2, nb, "R2 (reconstructed S2 windows, sliced)"));
+  BIP_TRY(sliced_in(ctx, ctx->R1s, R1t, fmt, w2, ctx->n_ap, nb, "R1 (reconstructed S1 windows, sliced)", SL_ROWS, true));
+  BIP_TRY(sliced_in(ctx, ctx->R2s, R2, fmt, e.n_det, w2, nb, "R2 (reconstructed S2 windows, sliced)", SL_ROWS, true));
   BIP_TRY(sliced_in(ctx, ctx->Phis, Phi, fmt, rho_pad * e.n_ch, w2, nb, "Phi (H_n psi, sliced)"));
   const int64_t psi_ld = w2;
   const int64_t n_scale = (int64_t)nb * (R1t.rows_pad + R2.rows_pad + Phi.rows_pad);
@@ -525,12 +526,14 @@ static int32_t run_edges(bip_ctx* ctx, const std::vector<int32_t>& ids, int mode
         for (auto a = lo; a < hi; ++a) { rows_max = std::max<int64_t>(rows_max, e.crop_counts[a]); rows_mean += e.crop_counts[a]; }
         rows_mean /= (double)(hi - lo);
       }
+      const int64_t ely = sliced_fmt_of(precision) >= 0 && sliced_wide(sliced_fmt_of(precision)) ? el * 3 / 2 : el;   // Y operands: + negated imaginary slices
       const size_t per_atom = (size_t)((ctx->n_p1 + ctx->n_p2) * w2 * 8 + rows_max * w2 * 8 +
-                                       el * (round_up(w2, 128) * round_up(ctx->n_ap, 32) + round_up(e.n_det, 128) * round_up(w2, 32) +
+                                       ely * (round_up(w2, 128) * round_up(ctx->n_ap, 32) + round_up(e.n_det, 128) * round_up(w2, 32)) +
+                                       el * (
                                              round_up(rows_max, 256) * (e.n_ch * round_up(w2, 32) + (crop ? round_up(ctx->n_ap, 32) : 0))) +
                                        (crop ? round_up(ctx->n_rho, 256) * 4 : 0));
       const int64_t nd = round_up((int64_t)e.n_ch * e.n_det, 256), Bp = round_up(ctx->n_ap, 128), w2p = round_up(w2, 32);
-      const size_t per_atom_coupling = (size_t)((ctx->n_p1 + ctx->n_p2) * w2 * 8 + el * (nd * w2p + Bp * w2p + nd * round_up(ctx->n_ap, 32)) + 8 * nd * Bp +
+      const size_t per_atom_coupling = (size_t)((ctx->n_p1 + ctx->n_p2) * w2 * 8 + el * nd * w2p + ely * (Bp * w2p + nd * round_up(ctx->n_ap, 32)) + 8 * nd * Bp +
                                                 (crop ? el * round_up(rows_max, 256) * round_up(ctx->n_ap, 32) + round_up(ctx->n_rho, 256) * 4 : 0));
       bool coupling = sliced_fmt_of(precision) >= 0 && use_coupling(ctx, e, rows_mean, budget);
       if (coupling && ctx->assoc == BIP_ASSOC_AUTO && per_atom_coupling > budget) coupling = false;   // does not fit: probe-first does
@@ -577,7 +580,7 @@ static int32_t run_alg3(bip_ctx* ctx, Edge& e, int recon, int precision, float* 
   BIP_TRY(ensure(ctx, ctx->Fields, (size_t)rho_chunk * e.n_ch * G * sizeof(float2), "exit wavefields (Algorithm 3)"));
   float2* F = reinterpret_cast<float2*>(ctx->Fields.p);
   Sliced R1t;
-  BIP_TRY(sliced_in(ctx, ctx->R1s, R1t, fmt, w2, ctx->n_ap, 1, "R1 (reconstructed S1 windows, sliced)"));
+  BIP_TRY(sliced_in(ctx, ctx->R1s, R1t, fmt, w2, ctx->n_ap, 1, "R1 (reconstructed S1 windows, sliced)", SL_ROWS, true));
   BIP_TRY(ensure(ctx, ctx->Scl, (size_t)R1t.rows_pad * sizeof(float), "row scales"));
   R1t.scale = reinterpret_cast<float*>(ctx->Scl.p); R1t.scale_batch_stride = R1t.rows_pad;
   int32_t a = 0;

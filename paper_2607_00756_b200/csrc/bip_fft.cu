@@ -12,9 +12,14 @@
 // i.e. 48 bytes of HBM traffic per pixel and slice step.  The forward transforms are decimation-in-frequency (natural
 // order in, digit-reversed order out), the inverse ones decimation-in-time (digit-reversed in, natural out), so no
 // reordering pass exists at all: the propagator table is stored once in the digit-reversed order of both axes.
-// Butterflies are radix-8 in registers (radix 4 / 2 for the last stage), fp32 with round-to-nearest throughout and
-// twiddles from a table of exact roots of unity computed in double -- every rounding is unbiased, so the column norms
-// do not drift systematically (tests/test_gpu_plumbing.py measures the drift against the fp64 cuFFT route).
+// Butterflies are radix-8 in registers (radix 4 / 2 for the last stage), fp32 with round-to-nearest throughout.
+// Every CONSTANT the data is multiplied by -- twiddles, sqrt(1/2), the propagator -- is held as a double-float pair
+// hi + lo (hi = fp32(c), lo = fp32(c - hi)) and applied with the small terms first inside one FMA chain.  A twiddle
+// rounded to fp32 alone has |w|^2 - 1 ~ +-6e-8, the same for every element that meets it, and those do NOT average out:
+// measured, a plain-fp32 version of these kernels lost 3.5e-7 of the column norm^2 per slice (the same systematic loss
+// cuFFT's C2C shows), i.e. 3.5e-6 of the summed intensity at 10 slices against a bound of 1e-6.  With double-float
+// constants only the data roundings remain, and those are unbiased (tests/test_gpu_plumbing.py measures the drift of
+// this route, of the fp64 cuFFT route and of plain cuFFT C2C).
 #include <cmath>
 
 #include "bip_internal.h"
@@ -24,7 +29,19 @@ namespace bip {
 namespace {
 
 __device__ __forceinline__ float2 cmulf(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
-__device__ __forceinline__ float2 cmulcf(float2 a, float2 b) { return make_float2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y); }   // a conj(b)
+// a * (hi + lo) with w = (hi.x, hi.y, lo.x, lo.y): the small products enter the FMA chain first, so they are part of the
+// exact sum that each final FMA rounds once
+__device__ __forceinline__ float2 cmul_dd(float2 a, float4 w) {
+  return make_float2(fmaf(a.x, w.x, fmaf(-a.y, w.y, fmaf(a.x, w.z, -a.y * w.w))),
+                     fmaf(a.x, w.y, fmaf(a.y, w.x, fmaf(a.x, w.w, a.y * w.z))));
+}
+__device__ __forceinline__ float2 cmulc_dd(float2 a, float4 w) {            // a * conj(hi + lo)
+  return make_float2(fmaf(a.x, w.x, fmaf(a.y, w.y, fmaf(a.x, w.z, a.y * w.w))),
+                     fmaf(a.y, w.x, fmaf(-a.x, w.y, fmaf(a.y, w.z, -a.x * w.w))));
+}
+__device__ __forceinline__ float mul_h(float v) {                            // v * sqrt(1/2), sqrt(1/2) = hi + lo
+  return fmaf(v, 0.70710676908493042f, v * 1.2101617485e-8f);
+}
 __device__ __forceinline__ float2 caddf(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ float2 csubf(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
 __device__ __forceinline__ float2 mul_mi(float2 a) { return make_float2(a.y, -a.x); }    // a * (-i)
@@ -42,14 +59,13 @@ __device__ __forceinline__ void dft_small(float2 (&x)[8]) {
     x[0] = caddf(s02, s13); x[2] = csubf(s02, s13);
     x[1] = caddf(d02, r);   x[3] = csubf(d02, r);
   } else {
-    const float h = 0.70710678118654752440f;
     float2 a[4], b[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k) { a[k] = caddf(x[k], x[k + 4]); b[k] = csubf(x[k], x[k + 4]); }
     // b_k *= w8^k, w8 = exp(-+ i pi / 4)
-    b[1] = INV ? make_float2((b[1].x - b[1].y) * h, (b[1].x + b[1].y) * h) : make_float2((b[1].x + b[1].y) * h, (b[1].y - b[1].x) * h);
+    b[1] = INV ? make_float2(mul_h(b[1].x - b[1].y), mul_h(b[1].x + b[1].y)) : make_float2(mul_h(b[1].x + b[1].y), mul_h(b[1].y - b[1].x));
     b[2] = INV ? mul_pi(b[2]) : mul_mi(b[2]);
-    b[3] = INV ? make_float2((-b[3].x - b[3].y) * h, (b[3].x - b[3].y) * h) : make_float2((b[3].y - b[3].x) * h, (-b[3].x - b[3].y) * h);
+    b[3] = INV ? make_float2(mul_h(-b[3].x - b[3].y), mul_h(b[3].x - b[3].y)) : make_float2(mul_h(b[3].y - b[3].x), mul_h(-b[3].x - b[3].y));
     {
       const float2 s02 = caddf(a[0], a[2]), d02 = csubf(a[0], a[2]), s13 = caddf(a[1], a[3]), d13 = csubf(a[1], a[3]);
       const float2 r = INV ? mul_pi(d13) : mul_mi(d13);
@@ -63,46 +79,54 @@ __device__ __forceinline__ void dft_small(float2 (&x)[8]) {
   }
 }
 
-// One stage on block length L with radix R over all lines of the block.  Forward (DIF): butterfly, then twiddle
-// w_L^(j m); inverse (DIT): conjugate twiddle, then inverse butterfly.  Element (line, i) lives at sm[line * pitch + i].
+// Shared-memory index of element i of a line: one float2 of padding after every 8, so that the stride-8 and stride-64
+// accesses of the later stages fall into different banks (a half-warp's 64-bit accesses then cover 16 distinct bank pairs).
+__device__ __forceinline__ int pad_idx(int i) { return i + (i >> 3); }
+__host__ __device__ constexpr int pad_len(int n) { return n + (n >> 3); }
+
+// One stage on block length L = 2^lL with radix R over all lines of the block.  Forward (DIF): butterfly, then twiddle
+// w_L^(j m); inverse (DIT): conjugate twiddle, then inverse butterfly.  Element (line, i) lives at sm[line * pitch + pad_idx(i)].
+// All sizes are powers of two: shifts and masks, no integer division.  A stage with L == R has j = 0 only: no twiddles.
 template <int R, bool INV>
-__device__ __forceinline__ void fft_stage(float2* sm, int N, int L, int n_lines, int pitch, const float2* __restrict__ root, int tid, int nthr) {
-  const int sub = L / R, per_line = N / R, tw_step = N / L;
-  for (int u = tid; u < n_lines * per_line; u += nthr) {
-    const int line = u / per_line, v = u - line * per_line;
-    const int blk = v / sub, j = v - blk * sub;
-    float2* p = sm + line * pitch + blk * L + j;
+__device__ __forceinline__ void fft_stage(float2* sm, int lN, int lL, int n_lines, int pitch, const float4* __restrict__ root, int tid, int nthr) {
+  constexpr int lR = R == 8 ? 3 : R == 4 ? 2 : 1;
+  const int lsub = lL - lR, sub = 1 << lsub, lper = lN - lR, N = 1 << lN, ltw = lN - lL;
+  const int total = n_lines << lper;
+  for (int u = tid; u < total; u += nthr) {
+    const int line = u >> lper, v = u & ((1 << lper) - 1);
+    const int blk = v >> lsub, j = v & (sub - 1);
+    float2* p = sm + line * pitch;
+    const int i0 = (blk << lL) + j;
     float2 x[8];
 #pragma unroll
-    for (int k = 0; k < R; ++k) x[k] = p[k * sub];
-    if (INV) {
+    for (int k = 0; k < R; ++k) x[k] = p[pad_idx(i0 + (k << lsub))];
+    if (INV && lsub > 0) {
 #pragma unroll
-      for (int m = 1; m < R; ++m) x[m] = cmulcf(x[m], __ldg(root + ((j * m * tw_step) & (N - 1))));
+      for (int m = 1; m < R; ++m) x[m] = cmulc_dd(x[m], __ldg(root + (((j * m) << ltw) & (N - 1))));
     }
     dft_small<R, INV>(x);
-    if (!INV) {
+    if (!INV && lsub > 0) {
 #pragma unroll
-      for (int m = 1; m < R; ++m) x[m] = cmulf(x[m], __ldg(root + ((j * m * tw_step) & (N - 1))));
+      for (int m = 1; m < R; ++m) x[m] = cmul_dd(x[m], __ldg(root + (((j * m) << ltw) & (N - 1))));
     }
 #pragma unroll
-    for (int k = 0; k < R; ++k) p[k * sub] = x[k];
+    for (int k = 0; k < R; ++k) p[pad_idx(i0 + (k << lsub))] = x[k];
   }
 }
 
 // Whole transform of every line: radix sequence 8, 8, ..., then 4 or 2 (forward); the inverse runs the same stages backwards.
 template <bool INV>
-__device__ __forceinline__ void fft_lines(float2* sm, int N, int n_lines, int pitch, const float2* __restrict__ root, int tid, int nthr) {
+__device__ __forceinline__ void fft_lines(float2* sm, int lN, int n_lines, int pitch, const float4* __restrict__ root, int tid, int nthr) {
   if (!INV) {
-    int L = N;
-    for (; L >= 8; L >>= 3) { fft_stage<8, false>(sm, N, L, n_lines, pitch, root, tid, nthr); __syncthreads(); }
-    if (L == 4) { fft_stage<4, false>(sm, N, 4, n_lines, pitch, root, tid, nthr); __syncthreads(); }
-    else if (L == 2) { fft_stage<2, false>(sm, N, 2, n_lines, pitch, root, tid, nthr); __syncthreads(); }
+    int lL = lN;
+    for (; lL >= 3; lL -= 3) { fft_stage<8, false>(sm, lN, lL, n_lines, pitch, root, tid, nthr); __syncthreads(); }
+    if (lL == 2) { fft_stage<4, false>(sm, lN, 2, n_lines, pitch, root, tid, nthr); __syncthreads(); }
+    else if (lL == 1) { fft_stage<2, false>(sm, lN, 1, n_lines, pitch, root, tid, nthr); __syncthreads(); }
   } else {
-    int L = N;
-    while (L >= 8) L >>= 3;                                  // length left for the last forward stage: 1, 2 or 4
-    if (L == 4) { fft_stage<4, true>(sm, N, 4, n_lines, pitch, root, tid, nthr); __syncthreads(); }
-    else if (L == 2) { fft_stage<2, true>(sm, N, 2, n_lines, pitch, root, tid, nthr); __syncthreads(); }
-    for (L = L * 8; L <= N; L <<= 3) { fft_stage<8, true>(sm, N, L, n_lines, pitch, root, tid, nthr); __syncthreads(); }
+    int lL = lN % 3;                                         // length left for the last forward stage: 2^0, 2^1 or 2^2
+    if (lL == 2) { fft_stage<4, true>(sm, lN, 2, n_lines, pitch, root, tid, nthr); __syncthreads(); }
+    else if (lL == 1) { fft_stage<2, true>(sm, lN, 1, n_lines, pitch, root, tid, nthr); __syncthreads(); }
+    for (lL += 3; lL <= lN; lL += 3) { fft_stage<8, true>(sm, lN, lL, n_lines, pitch, root, tid, nthr); __syncthreads(); }
   }
 }
 
@@ -116,25 +140,26 @@ __device__ __forceinline__ float2 apply_t(float2 v, const float2* __restrict__ T
 // Passes 1 and 3: LINES rows per block.  tmode: 0 none, 1 multiply by T, 2 by conj T (before the forward transform /
 // after the inverse one).
 template <bool INV>
-__global__ void __launch_bounds__(1024) k_ms_rows(float2* __restrict__ S, const float2* __restrict__ T, int tmode, int ny, int nx, int lines,
-                                                  const float2* __restrict__ rootx) {
+__global__ void __launch_bounds__(1024) k_ms_rows(float2* __restrict__ S, const float2* __restrict__ T, int tmode, int ny, int lnx, int lines,
+                                                  const float4* __restrict__ rootx) {
   extern __shared__ float2 sm_rows[];
+  const int nx = 1 << lnx, pitch = pad_len(nx);
   const int64_t G = (int64_t)ny * nx;
   float2* col = S + (int64_t)blockIdx.y * G;
   const int y0 = blockIdx.x * lines;
   const int n_lines = min(lines, ny - y0);
   const int tid = threadIdx.x, nthr = blockDim.x;
-  for (int i = tid; i < n_lines * nx; i += nthr) {
+  for (int i = tid; i < (n_lines << lnx); i += nthr) {
     const int64_t g = (int64_t)y0 * nx + i;
     float2 v = col[g];
     if (!INV) v = apply_t(v, T, g, tmode);
-    sm_rows[i] = v;
+    sm_rows[(i >> lnx) * pitch + pad_idx(i & (nx - 1))] = v;
   }
   __syncthreads();
-  fft_lines<INV>(sm_rows, nx, n_lines, nx, rootx, tid, nthr);
-  for (int i = tid; i < n_lines * nx; i += nthr) {
+  fft_lines<INV>(sm_rows, lnx, n_lines, pitch, rootx, tid, nthr);
+  for (int i = tid; i < (n_lines << lnx); i += nthr) {
     const int64_t g = (int64_t)y0 * nx + i;
-    float2 v = sm_rows[i];
+    float2 v = sm_rows[(i >> lnx) * pitch + pad_idx(i & (nx - 1))];
     if (INV) v = apply_t(v, T, g, tmode);
     col[g] = v;
   }
@@ -142,31 +167,32 @@ __global__ void __launch_bounds__(1024) k_ms_rows(float2* __restrict__ S, const 
 
 // Pass 2: a tile of `cols` columns (consecutive stored x positions) x ny rows per block; forward along y, spectrum
 // multiply with the digit-reversed propagator table (conjugated when conj_p), inverse along y.
-__global__ void __launch_bounds__(1024) k_ms_cols(float2* __restrict__ S, const float2* __restrict__ Pperm, int conj_p, int ny, int nx, int cols,
-                                                  const float2* __restrict__ rooty) {
+__global__ void __launch_bounds__(1024) k_ms_cols(float2* __restrict__ S, const float4* __restrict__ Pperm, int conj_p, int lny, int nx, int lcols,
+                                                  const float4* __restrict__ rooty) {
   extern __shared__ float2 sm_cols[];
+  const int ny = 1 << lny, cols = 1 << lcols;
   const int64_t G = (int64_t)ny * nx;
   float2* col = S + (int64_t)blockIdx.y * G;
-  const int x0 = blockIdx.x * cols;
-  const int pitch = ny + 1;
+  const int x0 = blockIdx.x << lcols;
+  const int pitch = pad_len(ny) + 1;
   const int tid = threadIdx.x, nthr = blockDim.x;
-  for (int i = tid; i < ny * cols; i += nthr) {
-    const int y = i / cols, c = i - y * cols;
-    sm_cols[c * pitch + y] = col[(int64_t)y * nx + x0 + c];
+  for (int i = tid; i < (ny << lcols); i += nthr) {
+    const int y = i >> lcols, c = i & (cols - 1);
+    sm_cols[c * pitch + pad_idx(y)] = col[(int64_t)y * nx + x0 + c];
   }
   __syncthreads();
-  fft_lines<false>(sm_cols, ny, cols, pitch, rooty, tid, nthr);
-  for (int i = tid; i < ny * cols; i += nthr) {
-    const int y = i / cols, c = i - y * cols;
-    float2 p = __ldg(Pperm + (int64_t)y * nx + x0 + c);
-    if (conj_p) p.y = -p.y;
-    sm_cols[c * pitch + y] = cmulf(sm_cols[c * pitch + y], p);
+  fft_lines<false>(sm_cols, lny, cols, pitch, rooty, tid, nthr);
+  for (int i = tid; i < (ny << lcols); i += nthr) {
+    const int y = i >> lcols, c = i & (cols - 1);
+    const float4 p = __ldg(Pperm + (int64_t)y * nx + x0 + c);
+    float2* e = sm_cols + c * pitch + pad_idx(y);
+    *e = conj_p ? cmulc_dd(*e, p) : cmul_dd(*e, p);
   }
   __syncthreads();
-  fft_lines<true>(sm_cols, ny, cols, pitch, rooty, tid, nthr);
-  for (int i = tid; i < ny * cols; i += nthr) {
-    const int y = i / cols, c = i - y * cols;
-    col[(int64_t)y * nx + x0 + c] = sm_cols[c * pitch + y];
+  fft_lines<true>(sm_cols, lny, cols, pitch, rooty, tid, nthr);
+  for (int i = tid; i < (ny << lcols); i += nthr) {
+    const int y = i >> lcols, c = i & (cols - 1);
+    col[(int64_t)y * nx + x0 + c] = sm_cols[c * pitch + pad_idx(y)];
   }
 }
 
@@ -175,40 +201,44 @@ __global__ void __launch_bounds__(1024) k_ms_cols(float2* __restrict__ S, const 
 //     out[rho][ky][kx] += sum_n |F psi_n|^2 / G
 // at the TRUE frequency (ky, kx) of the stored position (permy / permx undo the digit reversal).  A block owns the
 // (all y, its x tile) outputs of its scan position, so the read-modify-write needs no atomics.
-__global__ void __launch_bounds__(1024) k_ms_cols_detect(const float2* __restrict__ F, int n_ch, float* __restrict__ out, float inv_G, int ny, int nx,
-                                                         int cols, const float2* __restrict__ rooty, const int32_t* __restrict__ permy,
+__global__ void __launch_bounds__(1024) k_ms_cols_detect(const float2* __restrict__ F, int n_ch, float* __restrict__ out, float inv_G, int lny, int nx,
+                                                         int lcols, const float4* __restrict__ rooty, const int32_t* __restrict__ permy,
                                                          const int32_t* __restrict__ permx) {
   extern __shared__ float2 sm_det[];
+  const int ny = 1 << lny, cols = 1 << lcols;
   const int64_t G = (int64_t)ny * nx;
-  const int x0 = blockIdx.x * cols, rho = blockIdx.y;
-  const int pitch = ny + 1;
+  const int x0 = blockIdx.x << lcols, rho = blockIdx.y;
+  const int pitch = pad_len(ny) + 1;
   float* acc = reinterpret_cast<float*>(sm_det + (size_t)cols * pitch);       // [ny * cols], element i of the tile loop
   const int tid = threadIdx.x, nthr = blockDim.x;
-  for (int i = tid; i < ny * cols; i += nthr) acc[i] = 0.f;
+  for (int i = tid; i < (ny << lcols); i += nthr) acc[i] = 0.f;
   for (int n = 0; n < n_ch; ++n) {
     const float2* col = F + ((int64_t)rho * n_ch + n) * G;
     __syncthreads();
-    for (int i = tid; i < ny * cols; i += nthr) {
-      const int y = i / cols, c = i - y * cols;
-      sm_det[c * pitch + y] = col[(int64_t)y * nx + x0 + c];
+    for (int i = tid; i < (ny << lcols); i += nthr) {
+      const int y = i >> lcols, c = i & (cols - 1);
+      sm_det[c * pitch + pad_idx(y)] = col[(int64_t)y * nx + x0 + c];
     }
     __syncthreads();
-    fft_lines<false>(sm_det, ny, cols, pitch, rooty, tid, nthr);
-    for (int i = tid; i < ny * cols; i += nthr) {
-      const int y = i / cols, c = i - y * cols;
-      const float2 v = sm_det[c * pitch + y];
+    fft_lines<false>(sm_det, lny, cols, pitch, rooty, tid, nthr);
+    for (int i = tid; i < (ny << lcols); i += nthr) {
+      const int y = i >> lcols, c = i & (cols - 1);
+      const float2 v = sm_det[c * pitch + pad_idx(y)];
       acc[i] += v.x * v.x + v.y * v.y;
     }
   }
   float* o = out + (int64_t)rho * G;
-  for (int i = tid; i < ny * cols; i += nthr) {
-    const int y = i / cols, c = i - y * cols;
+  for (int i = tid; i < (ny << lcols); i += nthr) {
+    const int y = i >> lcols, c = i & (cols - 1);
     const int64_t k = (int64_t)__ldg(permy + y) * nx + __ldg(permx + x0 + c);
     o[k] += acc[i] * inv_G;
   }
 }
 
 bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+int ilog2(int n) { int l = 0; while ((1 << l) < n) ++l; return l; }
+size_t smem_rows_bytes(int lines, int nx) { return (size_t)lines * pad_len(nx) * sizeof(float2); }
+size_t smem_cols_bytes(int cols, int ny) { return (size_t)cols * (pad_len(ny) + 1) * sizeof(float2); }
 
 // frequency index held at stored position `pos` after the forward (DIF) transform of length N
 int dif_frequency(int pos, int N) {
@@ -227,9 +257,13 @@ bool fft_supported(const bip_ctx* ctx) {
 int32_t fft_init(bip_ctx* ctx) {
   const int ny = ctx->g.ny, nx = ctx->g.nx;
   const int64_t G = (int64_t)ny * nx;
-  std::vector<float2> ry(ny), rx(nx), P(G);
-  for (int t = 0; t < ny; ++t) ry[t] = make_float2((float)std::cos(-2.0 * M_PI * t / ny), (float)std::sin(-2.0 * M_PI * t / ny));
-  for (int t = 0; t < nx; ++t) rx[t] = make_float2((float)std::cos(-2.0 * M_PI * t / nx), (float)std::sin(-2.0 * M_PI * t / nx));
+  auto dd = [](double re, double im) {                       // double-float pair of a complex constant
+    const float hr = (float)re, hi = (float)im;
+    return make_float4(hr, hi, (float)(re - (double)hr), (float)(im - (double)hi));
+  };
+  std::vector<float4> ry(ny), rx(nx), P(G);
+  for (int t = 0; t < ny; ++t) ry[t] = dd(std::cos(-2.0 * M_PI * t / ny), std::sin(-2.0 * M_PI * t / ny));
+  for (int t = 0; t < nx; ++t) rx[t] = dd(std::cos(-2.0 * M_PI * t / nx), std::sin(-2.0 * M_PI * t / nx));
   // Fresnel propagator P(q) = exp(-i pi lambda dz |q|^2) / G (eq. 2; no band limit), in the stored (digit-reversed) order
   for (int py = 0; py < ny; ++py) {
     const int ky = dif_frequency(py, ny), hy = ky < (ny + 1) / 2 ? ky : ky - ny;
@@ -238,15 +272,15 @@ int32_t fft_init(bip_ctx* ctx) {
       const int kx = dif_frequency(px, nx), hx = kx < (nx + 1) / 2 ? kx : kx - nx;
       const double qx = hx / ctx->g.lx;
       const double ph = -M_PI * ctx->g.lambda * ctx->g.dz * (qy * qy + qx * qx);
-      P[(int64_t)py * nx + px] = make_float2((float)(std::cos(ph) / (double)G), (float)(std::sin(ph) / (double)G));
+      P[(int64_t)py * nx + px] = dd(std::cos(ph) / (double)G, std::sin(ph) / (double)G);
     }
   }
-  BIP_TRY(dev_alloc(ctx, (void**)&ctx->fft_rooty, sizeof(float2) * ny, "fft twiddles"));
-  BIP_TRY(dev_alloc(ctx, (void**)&ctx->fft_rootx, sizeof(float2) * nx, "fft twiddles"));
-  BIP_TRY(dev_alloc(ctx, (void**)&ctx->fft_P, sizeof(float2) * G, "propagator (digit-reversed order)"));
-  BIP_CUDA(ctx, cudaMemcpyAsync(ctx->fft_rooty, ry.data(), sizeof(float2) * ny, cudaMemcpyHostToDevice, ctx->stream));
-  BIP_CUDA(ctx, cudaMemcpyAsync(ctx->fft_rootx, rx.data(), sizeof(float2) * nx, cudaMemcpyHostToDevice, ctx->stream));
-  BIP_CUDA(ctx, cudaMemcpyAsync(ctx->fft_P, P.data(), sizeof(float2) * G, cudaMemcpyHostToDevice, ctx->stream));
+  BIP_TRY(dev_alloc(ctx, (void**)&ctx->fft_rooty, sizeof(float4) * ny, "fft twiddles"));
+  BIP_TRY(dev_alloc(ctx, (void**)&ctx->fft_rootx, sizeof(float4) * nx, "fft twiddles"));
+  BIP_TRY(dev_alloc(ctx, (void**)&ctx->fft_P, sizeof(float4) * G, "propagator (digit-reversed order)"));
+  BIP_CUDA(ctx, cudaMemcpyAsync(ctx->fft_rooty, ry.data(), sizeof(float4) * ny, cudaMemcpyHostToDevice, ctx->stream));
+  BIP_CUDA(ctx, cudaMemcpyAsync(ctx->fft_rootx, rx.data(), sizeof(float4) * nx, cudaMemcpyHostToDevice, ctx->stream));
+  BIP_CUDA(ctx, cudaMemcpyAsync(ctx->fft_P, P.data(), sizeof(float4) * G, cudaMemcpyHostToDevice, ctx->stream));
   std::vector<int32_t> py(ny), px(nx);
   for (int i = 0; i < ny; ++i) py[i] = dif_frequency(i, ny);
   for (int i = 0; i < nx; ++i) px[i] = dif_frequency(i, nx);
@@ -258,7 +292,7 @@ int32_t fft_init(bip_ctx* ctx) {
   // launch shapes: ~32 KB of rows per block, ~64 KB of columns per block (at least 4 columns: whole 32-byte sectors)
   ctx->fft_lines = std::max(1, std::min(ny, 4096 / nx));
   ctx->fft_cols = std::max(4, std::min(nx, 8192 / ny));
-  const size_t smem_cols = (size_t)ctx->fft_cols * (ny + 1) * sizeof(float2);
+  const size_t smem_cols = smem_cols_bytes(ctx->fft_cols, ny);
   BIP_CUDA(ctx, cudaFuncSetAttribute(k_ms_cols, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cols));
   BIP_CUDA(ctx, cudaFuncSetAttribute(k_ms_cols_detect, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(smem_cols + (size_t)ctx->fft_cols * ny * sizeof(float))));
   return BIP_OK;
@@ -269,13 +303,14 @@ int32_t fft_slice_op(bip_ctx* ctx, float2* S, int n_cols, const float2* Tj, int 
   const int ny = ctx->g.ny, nx = ctx->g.nx;
   const int lines = ctx->fft_lines, cols = ctx->fft_cols;
   const int thr_rows = std::max(32, std::min(1024, lines * nx / 8)), thr_cols = std::max(32, std::min(1024, cols * ny / 8));
-  const size_t smem_rows = (size_t)lines * nx * sizeof(float2), smem_cols = (size_t)cols * (ny + 1) * sizeof(float2);
+  const size_t smem_rows = smem_rows_bytes(lines, nx), smem_cols = smem_cols_bytes(cols, ny);
+  const int lnx = ilog2(nx), lny = ilog2(ny), lcols = ilog2(cols);
   for (int c0 = 0; c0 < n_cols; c0 += 65535) {                // gridDim.y limit
     const int nc = std::min(65535, n_cols - c0);
     float2* Sc = S + (int64_t)c0 * ny * nx;
-    k_ms_rows<false><<<dim3((unsigned)((ny + lines - 1) / lines), (unsigned)nc), thr_rows, smem_rows, ctx->stream>>>(Sc, Tj, pre, ny, nx, lines, ctx->fft_rootx);
-    k_ms_cols<<<dim3((unsigned)(nx / cols), (unsigned)nc), thr_cols, smem_cols, ctx->stream>>>(Sc, ctx->fft_P, conj_p, ny, nx, cols, ctx->fft_rooty);
-    k_ms_rows<true><<<dim3((unsigned)((ny + lines - 1) / lines), (unsigned)nc), thr_rows, smem_rows, ctx->stream>>>(Sc, Tj, post, ny, nx, lines, ctx->fft_rootx);
+    k_ms_rows<false><<<dim3((unsigned)((ny + lines - 1) / lines), (unsigned)nc), thr_rows, smem_rows, ctx->stream>>>(Sc, Tj, pre, ny, lnx, lines, ctx->fft_rootx);
+    k_ms_cols<<<dim3((unsigned)(nx / cols), (unsigned)nc), thr_cols, smem_cols, ctx->stream>>>(Sc, ctx->fft_P, conj_p, lny, nx, lcols, ctx->fft_rooty);
+    k_ms_rows<true><<<dim3((unsigned)((ny + lines - 1) / lines), (unsigned)nc), thr_rows, smem_rows, ctx->stream>>>(Sc, Tj, post, ny, lnx, lines, ctx->fft_rootx);
     BIP_CUDA(ctx, cudaGetLastError());
   }
   return BIP_OK;
@@ -286,17 +321,18 @@ int32_t fft_detect(bip_ctx* ctx, float2* fields, int n_rho, int n_ch, float* out
   const int ny = ctx->g.ny, nx = ctx->g.nx;
   const int lines = ctx->fft_lines, cols = ctx->fft_cols;
   const int thr_rows = std::max(32, std::min(1024, lines * nx / 8)), thr_cols = std::max(32, std::min(1024, cols * ny / 8));
-  const size_t smem_rows = (size_t)lines * nx * sizeof(float2);
-  const size_t smem_det = (size_t)cols * (ny + 1) * sizeof(float2) + (size_t)cols * ny * sizeof(float);
+  const size_t smem_rows = smem_rows_bytes(lines, nx);
+  const size_t smem_det = smem_cols_bytes(cols, ny) + (size_t)cols * ny * sizeof(float);
+  const int lnx = ilog2(nx), lny = ilog2(ny), lcols = ilog2(cols);
   const int64_t G = (int64_t)ny * nx;
   for (int r0 = 0; r0 < n_rho; r0 += 4096) {                  // gridDim.y limit (n_ch fields per scan position)
     const int nr = std::min(4096, n_rho - r0);
     float2* Fc = fields + (int64_t)r0 * n_ch * G;
     for (int f0 = 0; f0 < nr * n_ch; f0 += 65535) {
       const int nf = std::min(65535, nr * n_ch - f0);
-      k_ms_rows<false><<<dim3((unsigned)((ny + lines - 1) / lines), (unsigned)nf), thr_rows, smem_rows, ctx->stream>>>(Fc + (int64_t)f0 * G, nullptr, 0, ny, nx, lines, ctx->fft_rootx);
+      k_ms_rows<false><<<dim3((unsigned)((ny + lines - 1) / lines), (unsigned)nf), thr_rows, smem_rows, ctx->stream>>>(Fc + (int64_t)f0 * G, nullptr, 0, ny, lnx, lines, ctx->fft_rootx);
     }
-    k_ms_cols_detect<<<dim3((unsigned)(nx / cols), (unsigned)nr), thr_cols, smem_det, ctx->stream>>>(Fc, n_ch, out + (int64_t)r0 * G, (float)(1.0 / (double)G), ny, nx, cols,
+    k_ms_cols_detect<<<dim3((unsigned)(nx / cols), (unsigned)nr), thr_cols, smem_det, ctx->stream>>>(Fc, n_ch, out + (int64_t)r0 * G, (float)(1.0 / (double)G), lny, nx, lcols,
                                                                                                    ctx->fft_rooty, ctx->fft_permy, ctx->fft_permx);
     BIP_CUDA(ctx, cudaGetLastError());
   }

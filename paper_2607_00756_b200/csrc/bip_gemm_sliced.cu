@@ -19,6 +19,14 @@
 //   GEMM1 (a4):    Psi[rho][s] = sx[rho] sy[s] C           -> c64, quantised to Phi_n = H_n Psi by k_quantize_phi (a5)
 //   GEMM2 (a7-a8): |a_n[rho][d]|^2 / G summed over channels and reduced per output mode
 //
+// WIDE variant (FP16X4 on CTA pairs, the product path): the same arithmetic issued as N = 256 MMAs.  With the accumulator
+// columns laid out as [Cr | Ci] of the CTA's 64 detector columns, x_re . [y_re ; y_im] and x_im . [-y_im ; y_re] give both
+// components in one instruction each, so a k-step takes 8 MMAs of N = 256 instead of 16 of N = 128: every X slice is read
+// from shared memory half as often (64 KB instead of 96 KB of operand reads per k-step and CTA, against a shared-memory
+// bandwidth of 128 B / clk that the N = 128 form of FP16X3 saturated: profiles/r02_wide_mma.md).  The Y operand carries the
+// negated imaginary slices for it (bip_sliced.cuh); a stage holds, per slice, the 64-row blocks [-y_im][y_re][y_im], so
+// both 128-row B operands are contiguous.
+//
 // Warp roles: warp 0 bulk-copy producer, warp 1 TMEM owner + MMA issuer, warps 2-9 epilogue (TMEM lane quarter =
 // warp % 4, column half = (warp - 2) / 4).
 #include <cuda.h>
@@ -49,6 +57,11 @@ template <> struct Cfg<SL_FMT_BF16X6> {
   static constexpr uint32_t AB_FORMAT = 1;       // bf16
 };
 template <int FMT> __host__ __device__ constexpr int x_bytes() { return Cfg<FMT>::PARTS * PART_BYTES; }
+// bytes of the Y operand per stage and CTA: all of it (single CTA), this CTA's 64-row half of every part (pair), or the
+// half with the negated imaginary slices, 3 blocks of 64 rows per slice (WIDE)
+template <int FMT, bool PAIR, bool WIDE> __host__ __device__ constexpr int y_bytes() {
+  return WIDE ? 6 * (PART_BYTES / 2) : PAIR ? x_bytes<FMT>() / 2 : x_bytes<FMT>();
+}
 template <int FMT> __host__ __device__ constexpr int stage_bytes() { return 2 * x_bytes<FMT>(); }
 // EPI_GEMM2_TILE (CTA pairs, QEELS / CUBE outputs): |a|^2 of the channels of an item is summed in a shared-memory tile
 // [column][row] (129-float pitch: conflict-free both when a thread walks its own row and when a warp flushes 32
@@ -57,11 +70,12 @@ template <int FMT> __host__ __device__ constexpr int stage_bytes() { return 2 * 
 enum { EPI_GEMM1 = 1, EPI_GEMM2 = 2, EPI_GEMM2_TILE = 3 };
 constexpr int ACC_LD = TM + 1;
 constexpr int ACC_BYTES = TN * ACC_LD * 4;       // 66 048
-template <int EPI, int FMT, bool PAIR> __host__ __device__ constexpr int n_stages() {
-  return EPI == EPI_GEMM2_TILE ? (FMT == SL_FMT_FP16X4 ? 6 : 4) : PAIR ? Cfg<FMT>::STAGES_PAIR : Cfg<FMT>::STAGES;
+template <int EPI, int FMT, bool PAIR, bool WIDE> __host__ __device__ constexpr int n_stages() {
+  return WIDE ? (EPI == EPI_GEMM2_TILE ? 5 : 8)
+              : EPI == EPI_GEMM2_TILE ? (FMT == SL_FMT_FP16X4 ? 6 : 4) : PAIR ? Cfg<FMT>::STAGES_PAIR : Cfg<FMT>::STAGES;
 }
-template <int EPI, int FMT, bool PAIR> __host__ __device__ constexpr int smem_bytes() {
-  return n_stages<EPI, FMT, PAIR>() * (PAIR ? x_bytes<FMT>() * 3 / 2 : stage_bytes<FMT>()) + 1024 /*align*/ + 512 /*barriers*/ +
+template <int EPI, int FMT, bool PAIR, bool WIDE> __host__ __device__ constexpr int smem_bytes() {
+  return n_stages<EPI, FMT, PAIR, WIDE>() * (x_bytes<FMT>() + y_bytes<FMT, PAIR, WIDE>()) + 1024 /*align*/ + 512 /*barriers*/ +
          (EPI == EPI_GEMM2_TILE ? ACC_BYTES : 0);
 }
 
@@ -172,9 +186,9 @@ __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr) {
 }
 
 // cute::UMMA::InstrDescriptor for kind::f16 (fp16 or bf16 operands), fp32 accumulate, K-major A and B;
-// M = 128 (one CTA) or 256 (CTA pair, cta_group::2), N = 128
-__host__ __device__ constexpr uint32_t umma_idesc(uint32_t ab_format, bool neg_a, bool pair) {
-  return (1u << 4) | (ab_format << 7) | (ab_format << 10) | ((neg_a ? 1u : 0u) << 13) | ((uint32_t)(TN >> 3) << 17) |
+// M = 128 (one CTA) or 256 (CTA pair, cta_group::2), N = 128 or 256
+__host__ __device__ constexpr uint32_t umma_idesc(uint32_t ab_format, bool neg_a, bool pair, int n = TN) {
+  return (1u << 4) | (ab_format << 7) | (ab_format << 10) | ((neg_a ? 1u : 0u) << 13) | ((uint32_t)(n >> 3) << 17) |
          ((uint32_t)((pair ? 2 * TM : TM) >> 4) << 24);
 }
 
@@ -362,13 +376,39 @@ __device__ __forceinline__ void issue_lead(uint32_t t0r, uint32_t t0i, uint32_t 
   umma(t0i, xi1, yr1, id_pos, 1u);
 }
 
-template <int EPI, int FMT, bool PAIR>
+// WIDE (FP16X4, CTA pair): N = 256 MMAs on [Cr | Ci].  Stage layout of Y (64-row blocks of 2 KB):
+//   slice 1: [-yi1][yr1][yi1]   slice 2: [-yi2][yr2][yi2];  Fr(j) = [yr_j ; yi_j] starts at block 1, Fi(j) = [-yi_j ; yr_j] at block 0.
+constexpr int YB = PART_BYTES / 2;               // one 64-row block
+__device__ __forceinline__ void issue_small_wide(uint32_t t12, uint32_t a0, uint32_t b0, uint32_t acc, bool drop_tiny) {
+  constexpr uint32_t id = umma_idesc(Cfg<SL_FMT_FP16X4>::AB_FORMAT, false, true, 2 * TN);
+  const uint64_t xr1 = umma_desc(a0), xr2 = umma_desc(a0 + PART_BYTES), xi1 = umma_desc(a0 + 2 * PART_BYTES), xi2 = umma_desc(a0 + 3 * PART_BYTES);
+  const uint64_t fr1 = umma_desc(b0 + YB), fi1 = umma_desc(b0), fr2 = umma_desc(b0 + 4 * YB), fi2 = umma_desc(b0 + 3 * YB);
+  uint32_t a = acc;
+  if (!drop_tiny) {                              // tiniest first: x2 y2 (FP16X3 leaves them out)
+    umma_f16<true>(t12, xr2, fr2, id, a);
+    umma_f16<true>(t12, xi2, fi2, id, 1u);
+    a = 1u;
+  }
+  umma_f16<true>(t12, xr1, fr2, id, a);
+  umma_f16<true>(t12, xi1, fi2, id, 1u);
+  umma_f16<true>(t12, xr2, fr1, id, 1u);
+  umma_f16<true>(t12, xi2, fi1, id, 1u);
+}
+__device__ __forceinline__ void issue_lead_wide(uint32_t t0, uint32_t a0, uint32_t b0, uint32_t acc) {
+  constexpr uint32_t id = umma_idesc(Cfg<SL_FMT_FP16X4>::AB_FORMAT, false, true, 2 * TN);
+  umma_f16<true>(t0, umma_desc(a0), umma_desc(b0 + YB), id, acc);                      // xr1 . [yr1 ; yi1]
+  umma_f16<true>(t0, umma_desc(a0 + 2 * PART_BYTES), umma_desc(b0), id, 1u);           // xi1 . [-yi1 ; yr1]
+}
+
+template <int EPI, int FMT, bool PAIR, bool WIDE>
 __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlParams p) {
+  static_assert(!WIDE || (PAIR && FMT == SL_FMT_FP16X4), "the N = 256 formulation is built for FP16X4 on CTA pairs");
   using C = Cfg<FMT>;
-  constexpr int STAGES = n_stages<EPI, FMT, PAIR>();
+  constexpr int STAGES = n_stages<EPI, FMT, PAIR, WIDE>();
   constexpr bool IS_G2 = EPI == EPI_GEMM2 || EPI == EPI_GEMM2_TILE, TILE = EPI == EPI_GEMM2_TILE;
-  constexpr int X_BYTES = x_bytes<FMT>(), Y_BYTES = PAIR ? X_BYTES / 2 : X_BYTES, STAGE_BYTES = X_BYTES + Y_BYTES;
-  constexpr int STEP_EL = sl_step_el(FMT);
+  constexpr int X_BYTES = x_bytes<FMT>(), Y_BYTES = y_bytes<FMT, PAIR, WIDE>(), STAGE_BYTES = X_BYTES + Y_BYTES;
+  constexpr int STEP_EL = sl_step_el(FMT);                               // X operand: elements per (row tile, k-step)
+  constexpr int STEP_EL_Y = WIDE ? STEP_EL + 2 * SL_TILE_EL : STEP_EL;   // Y operand: + the negated imaginary slices
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + STAGES * STAGE_BYTES);
@@ -423,7 +463,7 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
         const unsigned int active = (unsigned int)min(n_workers, p.n_items - (item - worker));   // workers with an item in this wave
         if (PAIR) rt = 2 * rt + (int)rank;
         // a CTA of a pair loads rows [64 rank, 64 rank + 64) of every part of the Y tile
-        const uint16_t* ysrc = p.Y + (int64_t)atom * p.y_batch_stride + (int64_t)ct * p.ksteps * STEP_EL + (PAIR ? rank * (SL_TILE_EL / 2) : 0);
+        const uint16_t* ysrc = p.Y + (int64_t)atom * p.y_batch_stride + (int64_t)ct * p.ksteps * STEP_EL_Y + (PAIR ? rank * (SL_TILE_EL / 2) : 0);
         for (int n = 0; n < p.n_ch_loop; ++n) {
           const uint16_t* xsrc = p.X + (int64_t)atom * p.x_batch_stride + ((int64_t)n * p.n_rt_x + rt) * p.ksteps * STEP_EL;
           for (int ks = 0, next_sync = 0; ks < p.ksteps; ++ks, ++it) {
@@ -437,7 +477,13 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
             uint8_t* st = smem + s * STAGE_BYTES;
             mbar_expect_tx(&full[s], STAGE_BYTES);
             bulk_load(st, xsrc + (int64_t)ks * STEP_EL, X_BYTES, &full[s]);
-            if (PAIR) {
+            if (WIDE) {
+              // parts in memory: re1 re2 im1 im2 -im1 -im2; blocks in the stage: [-im1][re1][im1][-im2][re2][im2]
+              constexpr int dst_block[6] = {1, 4, 2, 5, 0, 3};
+#pragma unroll
+              for (int part = 0; part < 6; ++part)
+                bulk_load(st + X_BYTES + dst_block[part] * YB, ysrc + (int64_t)ks * STEP_EL_Y + part * SL_TILE_EL, YB, &full[s]);
+            } else if (PAIR) {
 #pragma unroll
               for (int part = 0; part < C::PARTS; ++part)
                 bulk_load(st + X_BYTES + part * (PART_BYTES / 2), ysrc + (int64_t)ks * STEP_EL + part * SL_TILE_EL, PART_BYTES / 2, &full[s]);
@@ -490,7 +536,8 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
       const bool chunk_end = in_chunk + 1 == chunk || ks_l == ksteps;
       if (elect_one()) {
         const uint32_t a0 = smem_base + s_lead * STAGE_BYTES;
-        issue_lead<FMT, PAIR>(t0r, t0i, a0, a0 + X_BYTES, in_chunk ? 1u : 0u);
+        if (WIDE) issue_lead_wide(t0r, a0, a0 + X_BYTES, in_chunk ? 1u : 0u);
+        else issue_lead<FMT, PAIR>(t0r, t0i, a0, a0 + X_BYTES, in_chunk ? 1u : 0u);
         umma_commit<PAIR>(&empty[s_lead]);                           // stage reusable once every MMA so far has read it
         if (chunk_end) umma_commit<PAIR>(c0_full);
       }
@@ -511,7 +558,8 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
       const bool seg_end = ks_s + 1 == ksteps;
       if (elect_one()) {
         const uint32_t a0 = smem_base + s_small * STAGE_BYTES;
-        issue_small<FMT, PAIR>(t12r, t12i, a0, a0 + X_BYTES, ks_s ? 1u : 0u, drop_tiny);
+        if (WIDE) issue_small_wide(t12r, a0, a0 + X_BYTES, ks_s ? 1u : 0u, drop_tiny);
+        else issue_small<FMT, PAIR>(t12r, t12i, a0, a0 + X_BYTES, ks_s ? 1u : 0u, drop_tiny);
         if (seg_end) umma_commit<PAIR>(c12_full);
       }
       __syncwarp();
@@ -529,7 +577,10 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
     // ================= epilogue warps =================
     const int quarter = warp & 3;                      // TMEM lanes [32 q, 32 q + 32) are visible to warps with warp % 4 == q
     const int half = (warp - 2) >> 2;                  // columns [64 half, 64 half + 64) of every accumulator
-    const uint32_t t_lane = tmem_base + ((uint32_t)(quarter * 32) << 16) + half * 64;
+    // accumulator columns: N = 128 form  C0r | C0i | C12r | C12i (128 each, this warp's half at + 64 half);
+    //                      WIDE          C0 = [Cr(d 0-63) | Ci(d 0-63) | Cr(d 64-127) | Ci(d 64-127)] | C12 likewise
+    constexpr int IM_OFF = WIDE ? 64 : TN;
+    const uint32_t t_lane = tmem_base + ((uint32_t)(quarter * 32) << 16) + half * (WIDE ? 128 : 64);
     const int n_chunks = (p.ksteps + p.chunk_steps - 1) / p.chunk_steps;
     uint32_t chunk_id = 0, seg = 0;
     for (int item = worker; item < p.n_items; item += n_workers) {
@@ -563,7 +614,7 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
           const bool small = c == n_chunks - 1;
           if (small) mbar_wait(c12_full, seg & 1); else mbar_wait(c0_full, chunk_id & 1);
           asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-          const uint32_t tr = t_lane + (small ? 2 * TN : 0), ti = tr + TN;
+          const uint32_t tr = t_lane + (small ? 2 * TN : 0), ti = tr + IM_OFF;
 #pragma unroll
           for (int g = 0; g < 2; ++g) {
             uint32_t v[32], u[32];
@@ -761,7 +812,7 @@ __global__ void __launch_bounds__(256) k_gather_rows_sliced(Sliced src, const in
   const int row = blockIdx.x, atom = blockIdx.z;
   if (g >= n_groups) return;
   const int s = row_idx[(int64_t)atom * idx_stride + row];
-  const int parts = sl_parts(src.fmt);
+  const int parts = sl_parts_of(src);
   uint16_t* d = dst.base + (int64_t)atom * dst.batch_stride + sl_group_offset(dst, row, g);
   const uint16_t* q = s >= 0 ? src.base + sl_group_offset(src, s, g) : nullptr;
   for (int part = 0; part < parts; ++part)
@@ -809,12 +860,12 @@ __global__ void __launch_bounds__(256) k_crop_rows(const double* __restrict__ rh
   if (threadIdx.x == 0) counts[atom] = n;
 }
 
-template <int EPI, int FMT, bool PAIR>
+template <int EPI, int FMT, bool PAIR, bool WIDE = false>
 int32_t launch_fmt(bip_ctx* ctx, const SlParams& p) {
   // per context (= per device): the shared-memory opt-in and the occupancy of this kernel variant
-  KernelInfo& ki = ctx->kernel_info[reinterpret_cast<const void*>(&k_sliced_contract<EPI, FMT, PAIR>)];
+  KernelInfo& ki = ctx->kernel_info[reinterpret_cast<const void*>(&k_sliced_contract<EPI, FMT, PAIR, WIDE>)];
   if (!ki.attr_set) {
-    BIP_CUDA(ctx, cudaFuncSetAttribute(k_sliced_contract<EPI, FMT, PAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<EPI, FMT, PAIR>()));
+    BIP_CUDA(ctx, cudaFuncSetAttribute(k_sliced_contract<EPI, FMT, PAIR, WIDE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<EPI, FMT, PAIR, WIDE>()));
     ki.attr_set = true;
   }
   SlParams q = p;
@@ -827,13 +878,13 @@ int32_t launch_fmt(bip_ctx* ctx, const SlParams& p) {
   if (q.n_items <= 0) return BIP_OK;
   q.chunk_steps = Cfg<FMT>::CHUNK_STEPS;                 // fixed: the exactness of the leading sums depends on it
   q.dgroup = std::max(1, tune_int("BIP_TUNE_DGROUP", DGROUP_DEFAULT));
-  q.lag_max = std::min(std::max(1, tune_int("BIP_TUNE_LAG", Cfg<FMT>::LAG_MAX)), n_stages<EPI, FMT, PAIR>() - 1);
+  q.lag_max = std::min(std::max(1, tune_int("BIP_TUNE_LAG", Cfg<FMT>::LAG_MAX)), n_stages<EPI, FMT, PAIR, WIDE>() - 1);
   int workers = std::max(1, std::min(q.n_items, PAIR ? ctx->sm_count / 2 : ctx->sm_count));
   workers = std::max(1, std::min(workers, tune_int("BIP_TUNE_WORKERS", workers)));
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = dim3(PAIR ? 2 * workers : workers);
   cfg.blockDim = dim3(NUM_THREADS);
-  cfg.dynamicSmemBytes = smem_bytes<EPI, FMT, PAIR>();
+  cfg.dynamicSmemBytes = smem_bytes<EPI, FMT, PAIR, WIDE>();
   cfg.stream = ctx->stream;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeClusterDimension;
@@ -843,7 +894,7 @@ int32_t launch_fmt(bip_ctx* ctx, const SlParams& p) {
   // this launch configuration (once per context and kernel variant).  The wait itself is bounded (lockstep_arrive_wait).
   if (ki.max_clusters < 0) {
     int n = 0;
-    if (cudaOccupancyMaxActiveClusters(&n, k_sliced_contract<EPI, FMT, PAIR>, &cfg) != cudaSuccess) { cudaGetLastError(); n = 0; }
+    if (cudaOccupancyMaxActiveClusters(&n, k_sliced_contract<EPI, FMT, PAIR, WIDE>, &cfg) != cudaSuccess) { cudaGetLastError(); n = 0; }
     ki.max_clusters = n;
   }
   q.sync_counter = nullptr;
@@ -853,14 +904,19 @@ int32_t launch_fmt(bip_ctx* ctx, const SlParams& p) {
     q.sync_counter = reinterpret_cast<unsigned int*>(ctx->Sync.p) + (ctx->sync_slot++ & 63);
     BIP_CUDA(ctx, cudaMemsetAsync(q.sync_counter, 0, sizeof(unsigned int), ctx->stream));
   }
-  BIP_CUDA(ctx, cudaLaunchKernelEx(&cfg, k_sliced_contract<EPI, FMT, PAIR>, q));
+  BIP_CUDA(ctx, cudaLaunchKernelEx(&cfg, k_sliced_contract<EPI, FMT, PAIR, WIDE>, q));
   ctx->timing.kernel_launches++;
   return BIP_OK;
 }
 
 template <int EPI>
-int32_t launch(bip_ctx* ctx, const SlParams& p, int fmt) {
+int32_t launch(bip_ctx* ctx, const SlParams& p, int fmt, bool y_neg) {
   const bool pair = tune_int("BIP_TUNE_PAIR", 1) != 0, tile = tune_int("BIP_TUNE_TILEACC", 1) != 0;
+  if (y_neg) {   // the Y operand carries the negated imaginary slices: the N = 256 formulation (FP16X4 on CTA pairs)
+    if (!pair || fmt != SL_FMT_FP16X4) return fail(ctx, BIP_ERR_INVALID, "contraction: a Y operand with negated imaginary slices needs the FP16X4 pair kernel");
+    if (tile && EPI == EPI_GEMM2 && p.mode != BIP_MODE_MAP) return launch_fmt<EPI_GEMM2_TILE, SL_FMT_FP16X4, true, true>(ctx, p);
+    return launch_fmt<EPI, SL_FMT_FP16X4, true, true>(ctx, p);
+  }
   if (pair && tile && EPI == EPI_GEMM2 && p.mode != BIP_MODE_MAP)
     return fmt == SL_FMT_FP16X4 ? launch_fmt<EPI_GEMM2_TILE, SL_FMT_FP16X4, true>(ctx, p) : launch_fmt<EPI_GEMM2_TILE, SL_FMT_BF16X6, true>(ctx, p);
   if (pair) return fmt == SL_FMT_FP16X4 ? launch_fmt<EPI, SL_FMT_FP16X4, true>(ctx, p) : launch_fmt<EPI, SL_FMT_BF16X6, true>(ctx, p);
@@ -870,7 +926,7 @@ int32_t launch(bip_ctx* ctx, const SlParams& p, int fmt) {
 }  // namespace
 
 int32_t launch_gemm1_sliced(bip_ctx* ctx, const Gemm1SlArgs& a) {
-  if (a.A.fmt != a.R1t.fmt) return fail(ctx, BIP_ERR_INVALID, "gemm1: operand formats differ");
+  if (a.A.fmt != a.R1t.fmt || a.A.neg_im) return fail(ctx, BIP_ERR_INVALID, "gemm1: operand formats differ");
   SlParams p{};
   p.X = a.A.base; p.sx = a.A.scale; p.x_batch_stride = a.A.batch_stride; p.sx_batch_stride = a.A.scale_batch_stride;
   p.Y = a.R1t.base; p.sy = a.R1t.scale; p.y_batch_stride = a.R1t.batch_stride; p.sy_batch_stride = a.R1t.scale_batch_stride;
@@ -882,7 +938,7 @@ int32_t launch_gemm1_sliced(bip_ctx* ctx, const Gemm1SlArgs& a) {
   p.drop_tiny = a.drop_tiny;
   p.n_rows = a.n_rho; p.n_cols = a.w2; p.rows_pad = (int)a.A.rows_pad;
   p.Psi = a.Psi; p.psi_ld = a.psi_ld; p.psi_batch_stride = a.psi_batch_stride;
-  return launch<EPI_GEMM1>(ctx, p, a.A.fmt);
+  return launch<EPI_GEMM1>(ctx, p, a.A.fmt, a.R1t.neg_im != 0);
 }
 
 int32_t launch_crop_rows(bip_ctx* ctx, const int32_t* origin_dev, int32_t n_atoms, int32_t w, int32_t* row_idx, int64_t idx_stride, int32_t* counts) {
@@ -912,7 +968,7 @@ int32_t launch_quantize_phi(bip_ctx* ctx, const float2* Psi, int64_t psi_ld, int
 }
 
 int32_t launch_gemm2_sliced(bip_ctx* ctx, const Gemm2SlArgs& a) {
-  if (a.Phi.fmt != a.R2.fmt) return fail(ctx, BIP_ERR_INVALID, "gemm2: operand formats differ");
+  if (a.Phi.fmt != a.R2.fmt || a.Phi.neg_im) return fail(ctx, BIP_ERR_INVALID, "gemm2: operand formats differ");
   SlParams p{};
   p.X = a.Phi.base; p.sx = a.Phi.scale; p.x_batch_stride = a.Phi.batch_stride; p.sx_batch_stride = a.Phi.scale_batch_stride;
   p.Y = a.R2.base; p.sy = a.R2.scale; p.y_batch_stride = a.R2.batch_stride; p.sy_batch_stride = a.R2.scale_batch_stride;
@@ -927,7 +983,7 @@ int32_t launch_gemm2_sliced(bip_ctx* ctx, const Gemm2SlArgs& a) {
   p.n_out_cols = a.n_out_cols > 0 ? a.n_out_cols : a.n_det;
   p.mode = a.mode; p.inv_G = a.inv_G; p.bin_of_det = a.bin_of_det; p.n_bins = a.n_bins; p.out = a.out;
   p.row_idx = a.row_idx; p.row_idx_stride = a.row_idx_stride;
-  return launch<EPI_GEMM2>(ctx, p, a.Phi.fmt);
+  return launch<EPI_GEMM2>(ctx, p, a.Phi.fmt, a.R2.neg_im != 0);
 }
 
 }  // namespace bip

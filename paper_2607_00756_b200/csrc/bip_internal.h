@@ -30,6 +30,10 @@ inline int tune_int(const char* name, int dflt) {
   return dflt;
 }
 
+// FP16X4 runs on the N = 256 formulation of the CTA-pair kernel, whose Y operands carry the negated imaginary slices
+// (bip_sliced.cuh).  BIP_TUNE_WIDE=0 (tuning builds only) selects the N = 128 formulation for A/B measurements.
+inline bool sliced_wide(int fmt) { return fmt == SL_FMT_FP16X4 && tune_int("BIP_TUNE_WIDE", 1) != 0 && tune_int("BIP_TUNE_PAIR", 1) != 0; }
+
 }  // namespace bip
 
 #ifdef __CUDACC__
@@ -121,7 +125,7 @@ struct bip_ctx {
   void* P_dev = nullptr;           // Fresnel propagator / G as double2 [ny][nx]
   void* ms_work = nullptr;         // double2 workspace of the cuFFT slice steps [plan_batch][ny][nx], allocated on first use
   // native fused slice step for power-of-two grids (bip_fft.cu)
-  float2 *fft_rooty = nullptr, *fft_rootx = nullptr, *fft_P = nullptr;
+  float4 *fft_rooty = nullptr, *fft_rootx = nullptr, *fft_P = nullptr;   // double-float (hi, lo) twiddles and propagator
   int32_t *fft_permy = nullptr, *fft_permx = nullptr;   // true frequency index of every stored (digit-reversed) position
   int fft_lines = 0, fft_cols = 0;
   bool fft_native = false;         // route in use (bip_set_fft_backend)

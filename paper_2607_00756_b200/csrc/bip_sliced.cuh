@@ -17,6 +17,10 @@
 // truncation, no bias; the chunk sums are added in fp32 round-to-nearest by the epilogue warps.  The small products
 // (<= 2^-8 of the leading ones) go to a second accumulator, whose truncation is 2^-8 smaller and harmless.
 //
+// Y operands of the FP16X4 CTA-pair kernel carry two more parts, the NEGATED imaginary slices (-im1, -im2; the sign flip
+// of an fp16 is exact): the kernel forms [Cr | Ci] with N = 256 MMAs, x_re . [y_re ; y_im] and x_im . [-y_im ; y_re],
+// which halves the shared-memory operand reads per flop (bip_gemm_sliced.cu).
+//
 // Memory layout (what one cp.async.bulk brings in): [batch][row tile of 128][k-step of 16][part][128 x 16 tile],
 // parts = (re1, re2, im1, im2) or (re1, re2, re3, im1, im2, im3), each 128 x 16 tile in the canonical K-major
 // no-swizzle UMMA layout (8-row x 16-byte core matrices: SBO = 256 B between 8-row groups, LBO = 128 B between the
@@ -40,6 +44,7 @@ __host__ __device__ constexpr int sl_step_el(int fmt) { return sl_parts(fmt) * S
 
 struct Sliced {
   uint16_t* base = nullptr;          // fp16 or bf16 bit patterns
+  int32_t neg_im = 0;                // 1: two extra parts (-im1, -im2) after the regular ones (FP16X4 Y operands)
   float* scale = nullptr;            // [batch][rows_pad] power-of-two row scale: value = stored * scale
   int64_t rows = 0, rows_pad = 0;    // valid rows; padded to a multiple of 128
   int64_t k = 0, ksteps = 0;         // valid k; ceil(k / 16)
@@ -48,11 +53,14 @@ struct Sliced {
   int32_t fmt = SL_FMT_FP16X4;
 };
 
+__host__ __device__ inline int sl_parts_of(const Sliced& S) { return sl_parts(S.fmt) + (S.neg_im ? 2 : 0); }
+__host__ __device__ inline int sl_step_el_of(const Sliced& S) { return sl_parts_of(S) * SL_TILE_EL; }
+
 #ifdef __CUDACC__
 // element offset of (row, k-group g of 8 consecutive k) for part 0; add part * SL_TILE_EL; 8 elements (16 B) contiguous
 __device__ __forceinline__ int64_t sl_group_offset(const Sliced& S, int64_t row, int64_t g) {
   const int64_t tile = row >> 7, r = row & 127, ks = g >> 1, half = g & 1;
-  return (tile * S.ksteps + ks) * sl_step_el(S.fmt) + (r >> 3) * 128 + half * 64 + (r & 7) * 8;
+  return (tile * S.ksteps + ks) * sl_step_el_of(S) + (r >> 3) * 128 + half * 64 + (r & 7) * 8;
 }
 
 // power-of-two scale > m (m >= 0); 1 for an all-zero row
@@ -94,6 +102,14 @@ __device__ __forceinline__ void sl_store_group(const Sliced& S, int64_t batch, i
     }
 #pragma unroll
     for (int part = 0; part < 4; ++part) *reinterpret_cast<uint4*>(p + part * SL_TILE_EL) = *reinterpret_cast<const uint4*>(out[part]);
+    if (S.neg_im) {
+#pragma unroll
+      for (int part = 2; part < 4; ++part) {
+        uint4 v = *reinterpret_cast<const uint4*>(out[part]);
+        v.x ^= 0x80008000u; v.y ^= 0x80008000u; v.z ^= 0x80008000u; v.w ^= 0x80008000u;     // -im: flip the fp16 sign bits
+        *reinterpret_cast<uint4*>(p + (part + 2) * SL_TILE_EL) = v;
+      }
+    }
   } else {
     __align__(16) uint16_t out[6][8];
 #pragma unroll

@@ -50,7 +50,7 @@ def test_native_slice_step_matches_oracle(name, scale, nz):
 def test_native_route_is_refused_on_a_grid_that_is_not_a_power_of_two():
     import paper_2607_00756_b200 as B
     from bip_inputs.specimen import tiny_random_workload
-    wl = tiny_random_workload(3)                                   # 16 x 12
+    wl = tiny_random_workload(3, W=8)                              # 16 x 12
     ctx, geo, ids = gpu_context(wl, [wl.edges[0]], parent_factor=(1, 1))
     with pytest.raises(B.BipError) as ei:
         ctx.set_fft_backend(B.FFT_NATIVE)
