@@ -393,7 +393,7 @@ def main():
     ap.add_argument("--workload", default="cfg2")
     ap.add_argument("--scale", type=int, default=1, help="shrink cells and grid together (debug; 1 = BASELINE size)")
     ap.add_argument("--atoms", type=int, default=32, help="ionised atoms per step per GPU (per edge)")
-    ap.add_argument("--planes", type=int, default=4, help="ionisation planes the atoms of a step are spread over")
+    ap.add_argument("--planes", type=int, default=2, help="ionisation planes the atoms of a step are spread over")
     ap.add_argument("--precision", default=os.environ.get("BIP_BENCH_PRECISION", "fp16x4"), choices=["fp16x4", "fp16x3", "bf16x6", "tf32x3", "fp32_simt"])
     ap.add_argument("--recon", default="magphase", choices=["linear", "magphase"])
     ap.add_argument("--mode", default="map", choices=["map", "qeels_x", "cube"])

@@ -279,6 +279,26 @@ BIP_API int32_t bip_set_scratch_budget(bip_ctx* ctx, size_t bytes);
 typedef enum { BIP_FFT_NATIVE = 0, BIP_FFT_CUFFT_F64 = 1 } bip_fft_backend;
 BIP_API int32_t bip_set_fft_backend(bip_ctx* ctx, int32_t backend);
 
+/* NEXT-4, S1 focal back-propagation (section 2.2.3.1; the paper leaves the plane and the padding open --
+ * DESIGN.md reading c20): with on != 0 the S1 side of every site is reconstructed through the scattering-centroid plane of
+ * the slices above it.  The de-tilted parent envelopes on the padded window (side 2^ceil(log2(w + 16))) are carried back by
+ * d_i = i dz - z_c(i) with the free-space transfer function of their own carrier, interpolated there (eq. 15 / eq. 11),
+ * carried forward beam by beam, re-tilted and cropped.  z_c(i) = sum_{j<i} m_j (j + 1/2) dz / sum_{j<i} m_j,
+ * m_j = sum_r |T_j(r) - 1|^2.  Exact PRISM in the full-parent limit, identical to the plain reconstruction where d_i = 0.
+ * S2 is untouched ("focal back-propagation is applied to S1 alone").  Probe-first association and
+ * tensor-core precisions only; one site at a time on the S1 side (1 GB of envelopes per site at configs[1]). */
+BIP_API int32_t bip_set_focal(bip_ctx* ctx, int32_t on);
+
+/* d_i of ionisation plane `plane` (0..nz), Angstrom, as the library computed it from T. */
+BIP_API int32_t bip_get_focal_distance(const bip_ctx* ctx, int32_t plane, double* d_out);
+
+/* Frozen-phonon averaging re-uses the pipeline once per displaced configuration: replace the
+ * transmission functions (same layout and rules as in bip_create; the scattering matrices must be rebuilt:
+ * bip_build_S1 / bip_build_S2), and let bip_map ADD to its output (on != 0) instead of zeroing it; the caller divides by
+ * the number of configurations. */
+BIP_API int32_t bip_set_transmission(bip_ctx* ctx, const void* T, int32_t T_on_device);
+BIP_API int32_t bip_set_accumulate(bip_ctx* ctx, int32_t on);
+
 /* Opt in (allow != 0) to BIP_PREC_TF32X3, which misses the 1e-6 summed-intensity bound (see bip_precision). */
 BIP_API int32_t bip_allow_tf32x3(bip_ctx* ctx, int32_t allow);
 

@@ -64,14 +64,17 @@ def illumination(c, beams, scan, ny, nx):
     return c[None, :] * np.exp(-2j * np.pi * ph)
 
 
-def atom_amplitudes(S1, S2, p1_h, p2_h, ap_beams, det_beams, w1, w2, A, H, centre, ny, nx, recon, crops=None):
+def atom_amplitudes(S1, S2, p1_h, p2_h, ap_beams, det_beams, w1, w2, A, H, centre, ny, nx, recon, crops=None, R1=None):
     """Steps a1-a7 for one ionised atom: amplitudes a[n, rho, d] (eq. 13 in the probe-first association).
+    ``R1`` may hand in the reconstructed S1 window [B, W*W] (oracle.focal reconstructs it through the scattering-centroid
+    plane); everything after the reconstruction is unchanged.
 
     Psi[rho, s] = sum_b c_b(rho) S1^b|Omega (eq. 7 on the window);  Phi_n = H_n . Psi (eq. 3);
     a_d = G^-1/2 sum_s S2^d|Omega[s] Phi_n[s]  (eq. 12-13, unitary F: SURVEY c3)."""
     W = H.shape[1]
     c1, c2 = crops if crops is not None else (None, None)
-    R1 = reconstruct_window(S1, p1_h, ap_beams, w1, centre, W, ny, nx, +1, recon, c1)     # [B, W^2]
+    if R1 is None:
+        R1 = reconstruct_window(S1, p1_h, ap_beams, w1, centre, W, ny, nx, +1, recon, c1)     # [B, W^2]
     R2 = reconstruct_window(S2, p2_h, det_beams, w2, centre, W, ny, nx, -1, recon, c2)    # [K, W^2]
     Psi = A @ R1                                                                       # [n_rho, W^2]
     a = np.empty((H.shape[0], A.shape[0], det_beams.shape[0]), dtype=np.complex128)

@@ -66,7 +66,8 @@ ABI_SYMBOLS = (
     "bip_output_size", "bip_map", "bip_map_host", "bip_map_all", "bip_get_windows", "bip_get_qeels_bins",
     "bip_seek_plane", "bip_copy_S", "bip_debug_reconstruct", "bip_get_timing", "bip_version", "bip_prism_subsample",
     "bip_set_crop", "bip_set_association", "bip_prism_coeffs", "bip_partition", "bip_set_scratch_budget", "bip_allow_tf32x3",
-    "bip_get_parents", "bip_get_weights", "bip_set_fft_backend", "bip_cube_alg3",
+    "bip_get_parents", "bip_get_weights", "bip_set_fft_backend", "bip_cube_alg3", "bip_set_focal", "bip_get_focal_distance",
+    "bip_set_transmission", "bip_set_accumulate",
 )
 
 _lib: Optional[C.CDLL] = None
@@ -295,6 +296,31 @@ class Context:
     def set_fft_backend(self, backend: int):
         """Slice-step route: FFT_NATIVE (fused fp32 kernels, power-of-two grids) or FFT_CUFFT_F64."""
         self._ck(self._lib.bip_set_fft_backend(self._ctx, int(backend)))
+
+    def set_focal(self, on: bool = True):
+        """S1 focal back-propagation to the scattering-centroid plane (NEXT-4; include/bip.h)."""
+        self._ck(self._lib.bip_set_focal(self._ctx, int(bool(on))))
+
+    def get_focal_distance(self, plane: int) -> float:
+        d = C.c_double(0.0)
+        self._ck(self._lib.bip_get_focal_distance(self._ctx, int(plane), C.byref(d)))
+        return d.value
+
+    def set_accumulate(self, on: bool = True):
+        self._ck(self._lib.bip_set_accumulate(self._ctx, int(bool(on))))
+
+    def set_transmission(self, T):
+        """Replace the transmission functions (frozen-phonon configurations); S1 / S2 must be rebuilt afterwards."""
+        import torch
+        g = self.g
+        if isinstance(T, np.ndarray):
+            T = np.ascontiguousarray(T, dtype=np.complex64)
+            assert T.shape == (g.nz, g.ny, g.nx)
+            self._ck(self._lib.bip_set_transmission(self._ctx, C.c_void_p(T.ctypes.data), 0))
+        else:
+            assert T.is_cuda and T.dtype == torch.complex64 and T.is_contiguous() and tuple(T.shape) == (g.nz, g.ny, g.nx)
+            self._ck(self._lib.bip_set_transmission(self._ctx, C.c_void_p(T.data_ptr()), 1))
+        self._T = T
 
     def allow_tf32x3(self, allow: bool = True):
         self._ck(self._lib.bip_allow_tf32x3(self._ctx, int(bool(allow))))

@@ -287,6 +287,7 @@ static int32_t contract_coupling(bip_ctx* ctx, Edge& e, const int32_t* org, int3
 // Which association runs for this edge (bip_set_association): the cost model of include/bip.h.
 static bool use_coupling(const bip_ctx* ctx, const Edge& e, double rows_per_site, size_t budget) {
   if (ctx->assoc == BIP_ASSOC_PROBE) return false;
+  if (ctx->focal && ctx->assoc == BIP_ASSOC_AUTO) return false;       // focal back-propagation lives on the probe-first path
   const double w2 = (double)e.w * e.w, nd = (double)e.n_ch * e.n_det, B = ctx->n_ap;
   if (ctx->assoc == BIP_ASSOC_AUTO) {
     const double probe = rows_per_site * w2 * (B + nd), coup = nd * B * (w2 + rows_per_site);
@@ -301,11 +302,33 @@ static bool use_coupling(const bip_ctx* ctx, const Edge& e, double rows_per_site
 static int32_t probe_at_sites(bip_ctx* ctx, Edge& e, const int32_t* org, int32_t nb, int recon, bool drop_tiny, const Sliced& Ax,
                               int32_t n_rows, const Sliced& R1t, Gemm1SlArgs* g1_out) {
   const int w2 = e.w * e.w;
-  BIP_TRY(ensure(ctx, ctx->D1, (size_t)nb * ctx->n_p1 * w2 * sizeof(float2), "D1 (de-tilted S1 windows)"));
   BIP_TRY(ensure(ctx, ctx->Psi, (size_t)nb * n_rows * w2 * sizeof(float2), "Psi (probe at the atom)"));
-  BIP_TRY(launch_crop_detilt(ctx, ctx->S1, ctx->p1_h_dev, ctx->n_p1, +1, org, nb, e.w, (float2*)ctx->D1.p));          // a1
-  BIP_TRY(launch_recon_t_sliced(ctx, (const float2*)ctx->D1.p, ctx->n_p1, ctx->ap_h_dev, ctx->n_ap, ctx->w1_idx_dev, ctx->w1_w_dev,
-                                ctx->nn1, +1, recon, org, nb, e.w, R1t));                                                   // a2
+  const double d_focal = ctx->focal ? ctx->focal_d[ctx->plane1] : 0.0;
+  if (d_focal > 0.0) {
+    // NEXT-4 (reading c20): per site, de-tilted parent envelopes on the padded window -> Fresnel step back to
+    // the scattering-centroid plane -> NNW interpolation (eq. 15 / eq. 11) -> Fresnel step forward, beam by beam ->
+    // re-tilt, crop, slice into R1^T
+    const int Wp = focal_padded_window(e.w), shift = (Wp - e.w) / 2;
+    if (Wp > std::min(ctx->g.ny, ctx->g.nx)) return fail(ctx, BIP_ERR_UNSUPPORTED, "focal back-propagation: padded window %d exceeds the grid", Wp);
+    BIP_TRY(ensure(ctx, ctx->D1p, (size_t)ctx->n_p1 * Wp * Wp * sizeof(float2), "padded de-tilted S1 windows"));
+    BIP_TRY(ensure(ctx, ctx->Env, (size_t)ctx->n_ap * Wp * Wp * sizeof(float2), "interpolated beam envelopes"));
+    std::vector<int32_t> oh(2 * (size_t)nb);
+    BIP_CUDA(ctx, cudaMemcpyAsync(oh.data(), org, sizeof(int32_t) * 2 * nb, cudaMemcpyDeviceToHost, ctx->stream));
+    BIP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    for (int32_t a = 0; a < nb; ++a) {
+      BIP_TRY(launch_crop_detilt(ctx, ctx->S1, ctx->p1_h_dev, ctx->n_p1, +1, org + 2 * (int64_t)a, 1, Wp, (float2*)ctx->D1p.p, shift));
+      BIP_TRY(focal_window_fresnel(ctx, (float2*)ctx->D1p.p, ctx->n_p1, ctx->p1_h_dev, ctx->n_p1, Wp, -d_focal));
+      BIP_TRY(launch_recon_c64(ctx, (const float2*)ctx->D1p.p, ctx->n_p1, ctx->ap_h_dev, ctx->n_ap, ctx->w1_idx_dev, ctx->w1_w_dev, ctx->nn1, +1,
+                               recon, org + 2 * (int64_t)a, 0, Wp, (float2*)ctx->Env.p, shift, /*retilt=*/false));
+      BIP_TRY(focal_window_fresnel(ctx, (float2*)ctx->Env.p, ctx->n_ap, ctx->ap_h_dev, ctx->n_ap, Wp, +d_focal));
+      BIP_TRY(focal_env_to_r1t(ctx, (const float2*)ctx->Env.p, oh[2 * a], oh[2 * a + 1], e.w, Wp, R1t, a));
+    }
+  } else {
+    BIP_TRY(ensure(ctx, ctx->D1, (size_t)nb * ctx->n_p1 * w2 * sizeof(float2), "D1 (de-tilted S1 windows)"));
+    BIP_TRY(launch_crop_detilt(ctx, ctx->S1, ctx->p1_h_dev, ctx->n_p1, +1, org, nb, e.w, (float2*)ctx->D1.p));          // a1
+    BIP_TRY(launch_recon_t_sliced(ctx, (const float2*)ctx->D1.p, ctx->n_p1, ctx->ap_h_dev, ctx->n_ap, ctx->w1_idx_dev, ctx->w1_w_dev,
+                                  ctx->nn1, +1, recon, org, nb, e.w, R1t));                                                 // a2
+  }
   Gemm1SlArgs g1;                                                                                                            // a3-a4
   g1.A = Ax; g1.R1t = R1t; g1.Psi = (float2*)ctx->Psi.p; g1.psi_ld = w2; g1.psi_batch_stride = (int64_t)n_rows * w2;
   g1.n_rho = n_rows; g1.w2 = w2; g1.n_atoms = nb; g1.drop_tiny = drop_tiny;
@@ -497,7 +520,10 @@ static int32_t run_edges(bip_ctx* ctx, const std::vector<int32_t>& ids, int mode
   sp.adv.clear(); sp.contract.clear(); sp.gemm2.clear();
   sp.pool_map.reset();
   ctx->timing.gemm2_launches = 0; ctx->timing.kernel_launches = 0; ctx->timing.amplitudes = 0; ctx->timing.flops = 0;
-  for (size_t k = 0; k < ids.size(); ++k) BIP_CUDA(ctx, cudaMemsetAsync(outs[k], 0, outs_bytes[k], ctx->stream));
+  if (ctx->focal && ctx->assoc == BIP_ASSOC_COUPLING) return fail(ctx, BIP_ERR_UNSUPPORTED, "bip_map: focal back-propagation needs the probe-first association");
+  if (ctx->focal && sliced_fmt_of(precision) < 0) return fail(ctx, BIP_ERR_UNSUPPORTED, "bip_map: focal back-propagation needs a tensor-core precision (FP16X4, FP16X3, BF16X6)");
+  if (!ctx->accumulate)
+    for (size_t k = 0; k < ids.size(); ++k) BIP_CUDA(ctx, cudaMemsetAsync(outs[k], 0, outs_bytes[k], ctx->stream));
 
   std::vector<int32_t> planes;
   for (int32_t id : ids) for (int32_t s : ctx->edges[id].slice) planes.push_back(s);
@@ -697,6 +723,7 @@ int32_t bip_create(bip_ctx** out, const bip_grid* g, const void* T, int32_t T_on
     BIP_TRY(ms_max_modulus_deviation(ctx, ctx->T_dev, (int64_t)G * g->nz, &dev));
     if (!(dev <= 1e-4f)) return fail(ctx, BIP_ERR_INVALID, "bip_create: transmission functions are not unimodular (max ||T|^2 - 1| = %.3g); "
                                      "absorptive slices are not supported (PAPER.md:372)", dev);
+    BIP_TRY(focal_init(ctx));
     return BIP_OK;
   };
   int32_t st = build();
@@ -721,11 +748,12 @@ int32_t bip_destroy(bip_ctx* ctx) {
   cudaStreamSynchronize(ctx->stream);
   bip_clear_edges(ctx);
   ms_release(ctx);
+  focal_release(ctx);
   ctx->spans.pool_map.destroy(); ctx->spans.pool_b1.destroy(); ctx->spans.pool_b2.destroy();
   if (ctx->T_owned) cudaFree((void*)ctx->T_dev);
   void* ptrs[] = {ctx->ap_h_dev, ctx->p1_h_dev, ctx->p2_h_dev, ctx->ap_c_dev, ctx->w1_idx_dev, ctx->w1_w_dev, ctx->rooty_dev,
                   ctx->rootx_dev, ctx->P_dev, ctx->ms_work, ctx->S1, ctx->S2, ctx->D1.p, ctx->D2.p, ctx->R1.p, ctx->R2.p, ctx->Psi.p,
-                  ctx->Phi.p, ctx->R1s.p, ctx->R2s.p, ctx->Phis.p, ctx->Scl.p, ctx->Sync.p, ctx->Fields.p, ctx->RowIdx.p, ctx->Acrop.p, ctx->Pmax.p, ctx->R1r.p, ctx->HR2.p, ctx->Mc.p, ctx->Ms.p, ctx->rho_dev};
+                  ctx->Phi.p, ctx->R1s.p, ctx->R2s.p, ctx->Phis.p, ctx->Scl.p, ctx->Sync.p, ctx->Fields.p, ctx->D1p.p, ctx->Env.p, ctx->RowIdx.p, ctx->Acrop.p, ctx->Pmax.p, ctx->R1r.p, ctx->HR2.p, ctx->Mc.p, ctx->Ms.p, ctx->rho_dev};
   free_illumination(ctx);
   for (void* p : ptrs) if (p) cudaFree(p);
   cudaGetLastError();
@@ -1016,6 +1044,44 @@ int32_t bip_get_weights(const bip_ctx* ctx, int32_t edge_id, int32_t* n_rows, in
   if (nn_idx_out) std::copy(idx.begin(), idx.end(), nn_idx_out);
   if (nn_w_out) std::copy(w.begin(), w.end(), nn_w_out);
   return BIP_OK;
+}
+
+int32_t bip_set_focal(bip_ctx* ctx, int32_t on) {
+  if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
+  ctx->focal = on != 0;
+  return BIP_OK;
+}
+
+int32_t bip_get_focal_distance(const bip_ctx* ctx, int32_t plane, double* d_out) {
+  if (!ctx || !d_out) return fail(nullptr, BIP_ERR_INVALID, "bip_get_focal_distance: NULL argument");
+  if (plane < 0 || plane > ctx->g.nz) return fail(const_cast<bip_ctx*>(ctx), BIP_ERR_INVALID, "plane %d outside 0..%d", plane, ctx->g.nz);
+  *d_out = ctx->focal_d[plane];
+  return BIP_OK;
+}
+
+int32_t bip_set_accumulate(bip_ctx* ctx, int32_t on) {
+  if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
+  ctx->accumulate = on != 0;
+  return BIP_OK;
+}
+
+int32_t bip_set_transmission(bip_ctx* ctx, const void* T, int32_t T_on_device) {
+  if (!ctx || !T) return fail(ctx, BIP_ERR_INVALID, "bip_set_transmission: NULL argument");
+  const size_t n = (size_t)ctx->g.ny * ctx->g.nx * ctx->g.nz;
+  BIP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+  if (T_on_device) {
+    if (ctx->T_owned) cudaFree((void*)ctx->T_dev);
+    ctx->T_dev = (const float2*)T; ctx->T_owned = false;
+  } else {
+    if (!ctx->T_owned) { float2* t = nullptr; BIP_TRY(dev_alloc(ctx, (void**)&t, n * sizeof(float2), "transmission functions")); ctx->T_dev = t; ctx->T_owned = true; }
+    BIP_CUDA(ctx, cudaMemcpyAsync((void*)ctx->T_dev, T, n * sizeof(float2), cudaMemcpyHostToDevice, ctx->stream));
+    BIP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+  }
+  ctx->s1_built = ctx->s2_built = false;                       // the scattering matrices belong to the previous configuration
+  float dev = 0.f;
+  BIP_TRY(ms_max_modulus_deviation(ctx, ctx->T_dev, (int64_t)n, &dev));
+  if (!(dev <= 1e-4f)) return fail(ctx, BIP_ERR_INVALID, "bip_set_transmission: transmission functions are not unimodular (max ||T|^2 - 1| = %.3g)", dev);
+  return focal_init(ctx);
 }
 
 int32_t bip_set_fft_backend(bip_ctx* ctx, int32_t backend) {

@@ -19,13 +19,14 @@
 //   GEMM1 (a4):    Psi[rho][s] = sx[rho] sy[s] C           -> c64, quantised to Phi_n = H_n Psi by k_quantize_phi (a5)
 //   GEMM2 (a7-a8): |a_n[rho][d]|^2 / G summed over channels and reduced per output mode
 //
-// WIDE variant (FP16X4 on CTA pairs, the product path): the same arithmetic issued as N = 256 MMAs.  With the accumulator
-// columns laid out as [Cr | Ci] of the CTA's 64 detector columns, x_re . [y_re ; y_im] and x_im . [-y_im ; y_re] give both
-// components in one instruction each, so a k-step takes 8 MMAs of N = 256 instead of 16 of N = 128: every X slice is read
-// from shared memory half as often (64 KB instead of 96 KB of operand reads per k-step and CTA, against a shared-memory
-// bandwidth of 128 B / clk that the N = 128 form of FP16X3 saturated: profiles/r02_wide_mma.md).  The Y operand carries the
-// negated imaginary slices for it (bip_sliced.cuh); a stage holds, per slice, the 64-row blocks [-y_im][y_re][y_im], so
-// both 128-row B operands are contiguous.
+// WIDE variant (FP16X4 on CTA pairs; A/B only, tuning builds): the same arithmetic issued as N = 256 MMAs.  With the
+// accumulator columns laid out as [Cr | Ci] of the CTA's 64 detector columns, x_re . [y_re ; y_im] and x_im . [-y_im ; y_re]
+// give both components in one instruction each, so a k-step takes 8 MMAs of N = 256 instead of 16 of N = 128.  The idea
+// was to read every X slice from shared memory half as often (the N = 128 form of FP16X3 saturates the 128 B / clk of
+// shared-memory bandwidth).  Measured on B200 it is SLOWER, 3.4 % for FP16X4 and 5.5 % for FP16X3
+// (profiles/r02_wide_mma.md): an N = 256 MMA evidently re-reads its A operand per 128 columns, and the Y operand grows
+// by the negated imaginary slices (bip_sliced.cuh; per slice the 64-row blocks [-y_im][y_re][y_im] in a stage).  Kept
+// as the measured alternative; the shipped build never launches it.
 //
 // Warp roles: warp 0 bulk-copy producer, warp 1 TMEM owner + MMA issuer, warps 2-9 epilogue (TMEM lane quarter =
 // warp % 4, column half = (warp - 2) / 4).

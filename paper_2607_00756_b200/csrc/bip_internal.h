@@ -30,9 +30,10 @@ inline int tune_int(const char* name, int dflt) {
   return dflt;
 }
 
-// FP16X4 runs on the N = 256 formulation of the CTA-pair kernel, whose Y operands carry the negated imaginary slices
-// (bip_sliced.cuh).  BIP_TUNE_WIDE=0 (tuning builds only) selects the N = 128 formulation for A/B measurements.
-inline bool sliced_wide(int fmt) { return fmt == SL_FMT_FP16X4 && tune_int("BIP_TUNE_WIDE", 1) != 0 && tune_int("BIP_TUNE_PAIR", 1) != 0; }
+// The N = 256 formulation of the FP16X4 CTA-pair kernel (Y operands with negated imaginary slices, bip_sliced.cuh) is an
+// A/B variant: measured 3.4 % (FP16X4) and 5.5 % (FP16X3) SLOWER than the N = 128 formulation on B200
+// (profiles/r02_wide_mma.md), so the shipped build never selects it; BIP_TUNE_WIDE=1 in a tuning build does.
+inline bool sliced_wide(int fmt) { return fmt == SL_FMT_FP16X4 && tune_int("BIP_TUNE_WIDE", 0) != 0 && tune_int("BIP_TUNE_PAIR", 1) != 0; }
 
 }  // namespace bip
 
@@ -137,6 +138,11 @@ struct bip_ctx {
   bool plan_ok = false;
   size_t scratch_budget = (size_t)12 << 30;   // bip_set_scratch_budget
   bool allow_tf32x3 = false;          // bip_allow_tf32x3
+  bool accumulate = false;            // bip_set_accumulate: bip_map adds to the output instead of zeroing it (frozen phonons)
+  bool focal = false;                 // bip_set_focal: S1 reconstructed through the scattering-centroid plane (NEXT-4)
+  std::vector<double> focal_d;        // [nz + 1] back-propagation distance of every plane (reading c20)
+  std::map<int, std::pair<void*, void*>> focal_tables;   // per padded-window size: twiddles, digit-reversal permutation
+  bip::DevBuf D1p, Env;               // padded de-tilted parent windows; interpolated beam envelopes (one site)
   bip::Spans spans;                   // CUDA-event spans behind bip_get_timing
   std::map<const void*, bip::KernelInfo> kernel_info;
   std::map<uint64_t, bip::AutoTable> auto_w2;
@@ -208,17 +214,24 @@ int32_t fft_slice_op(bip_ctx* ctx, float2* S, int n_cols, const float2* Tj, int 
 int32_t fft_detect(bip_ctx* ctx, float2* fields, int n_rho, int n_ch, float* out);
 void fft_release(bip_ctx* ctx);
 
+// ---- S1 focal back-propagation (bip_focal.cu) ----
+int32_t focal_padded_window(int32_t w);
+int32_t focal_init(bip_ctx* ctx);
+int32_t focal_window_fresnel(bip_ctx* ctx, float2* E, int64_t n_win, const int32_t* h_dev, int n_beams, int Wp, double d);
+int32_t focal_env_to_r1t(bip_ctx* ctx, const float2* Env, int32_t oy, int32_t ox, int32_t w, int32_t Wp, const Sliced& out, int32_t atom);
+void focal_release(bip_ctx* ctx);
+
 // ---- reconstruction (bip_recon.cu) ----
 // a1: D[a][p][s] = S_p(r) * exp(-carrier 2 pi i h_p.r/N) on the atoms' windows
 int32_t launch_crop_detilt(bip_ctx* ctx, const float2* S, const int32_t* ph_dev, int32_t n_par, int carrier,
-                           const int32_t* origin_dev, int32_t n_atoms, int32_t w, float2* D);
+                           const int32_t* origin_dev, int32_t n_atoms, int32_t w, float2* D, int32_t origin_shift = 0);
 // a2/a6: R[a][beam][s] (or transposed [a][s][beam]) split planes from D with ELL weights, re-tilted
 int32_t launch_recon(bip_ctx* ctx, const float2* D, int32_t n_par, const int32_t* bh_dev, int32_t n_beams,
                      const int32_t* nn_idx, const float* nn_w, int32_t max_nn, int carrier, int recon,
                      const int32_t* origin_dev, int32_t n_atoms, int32_t w, bool transpose, Planes out);
 int32_t launch_recon_c64(bip_ctx* ctx, const float2* D, int32_t n_par, const int32_t* bh_dev, int32_t n_beams,
                          const int32_t* nn_idx, const float* nn_w, int32_t max_nn, int carrier, int recon,
-                         const int32_t* origin_dev, int32_t atom, int32_t w, float2* out);
+                         const int32_t* origin_dev, int32_t atom, int32_t w, float2* out, int32_t origin_shift = 0, bool retilt = true);
 // a3: illumination planes A[rho][b] = c_b exp(-2 pi i h_b.rho/N)
 int32_t launch_illumination(bip_ctx* ctx, const double* rho_dev, int32_t n_rho, Planes out);
 

@@ -27,10 +27,10 @@ __device__ __forceinline__ float2 tilt(const float2* __restrict__ rooty, const f
 __global__ void k_crop_detilt(const float2* __restrict__ S, const int32_t* __restrict__ ph, int carrier,
                               const int32_t* __restrict__ origin, int w, int ny, int nx,
                               const float2* __restrict__ rooty, const float2* __restrict__ rootx,
-                              float2* __restrict__ D, int n_par) {
+                              float2* __restrict__ D, int n_par, int shift) {
   const int a = blockIdx.z, p = blockIdx.y;
   const int w2 = w * w;
-  const int oy = origin[2 * a], ox = origin[2 * a + 1];
+  const int oy = (origin[2 * a] - shift + ny) % ny, ox = (origin[2 * a + 1] - shift + nx) % nx;   // shift: margin of a padded window
   const int hyp = ((ph[2 * p] % ny) + ny) % ny, hxp = ((ph[2 * p + 1] % nx) + nx) % nx;
   const float2* col = S + (int64_t)p * ny * nx;
   float2* out = D + ((int64_t)a * n_par + p) * w2;
@@ -141,16 +141,16 @@ __global__ void k_recon_transposed(const float2* __restrict__ D, int n_par, cons
 __global__ void k_recon_c64(const float2* __restrict__ D, int n_par, const int32_t* __restrict__ bh, int n_beams,
                             const int32_t* __restrict__ nn_idx, const float* __restrict__ nn_w, int max_nn,
                             int carrier, int recon, const int32_t* __restrict__ origin, int atom, int w, int ny, int nx,
-                            const float2* __restrict__ rooty, const float2* __restrict__ rootx, float2* __restrict__ out) {
+                            const float2* __restrict__ rooty, const float2* __restrict__ rootx, float2* __restrict__ out, int shift, int retilt) {
   const int b = blockIdx.y;
   const int w2 = w * w;
-  const int oy = origin[2 * atom], ox = origin[2 * atom + 1];
+  const int oy = (origin[2 * atom] - shift + ny) % ny, ox = (origin[2 * atom + 1] - shift + nx) % nx;
   const int hyp = ((bh[2 * b] % ny) + ny) % ny, hxp = ((bh[2 * b + 1] % nx) + nx) % nx;
   for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < w2; s += gridDim.x * blockDim.x) {
     const int sy = s / w, sx = s - sy * w;
     int ry = oy + sy; if (ry >= ny) ry -= ny;
     int rx = ox + sx; if (rx >= nx) rx -= nx;
-    float2 t = tilt(rooty, rootx, hyp, hxp, ry, rx, ny, nx);
+    float2 t = retilt ? tilt(rooty, rootx, hyp, hxp, ry, rx, ny, nx) : make_float2(1.f, 0.f);   // retilt == 0: the bare envelope
     if (carrier < 0) t.y = -t.y;
     out[(int64_t)b * w2 + s] = recon_elem(D, nn_idx + (int64_t)b * max_nn, nn_w + (int64_t)b * max_nn, max_nn, w2, s, recon, t);
   }
@@ -340,10 +340,10 @@ __global__ void __launch_bounds__(256) k_illumination_sliced(const double* __res
 }  // namespace
 
 int32_t launch_crop_detilt(bip_ctx* ctx, const float2* S, const int32_t* ph_dev, int32_t n_par, int carrier,
-                           const int32_t* origin_dev, int32_t n_atoms, int32_t w, float2* D) {
+                           const int32_t* origin_dev, int32_t n_atoms, int32_t w, float2* D, int32_t origin_shift) {
   dim3 grid((unsigned)((w * w + 255) / 256), (unsigned)n_par, (unsigned)n_atoms);
   k_crop_detilt<<<grid, 256, 0, ctx->stream>>>(S, ph_dev, carrier, origin_dev, w, ctx->g.ny, ctx->g.nx,
-                                               ctx->rooty_dev, ctx->rootx_dev, D, n_par);
+                                               ctx->rooty_dev, ctx->rootx_dev, D, n_par, origin_shift);
   BIP_CUDA(ctx, cudaGetLastError());
   ctx->timing.kernel_launches++;
   return BIP_OK;
@@ -378,14 +378,14 @@ int32_t launch_recon(bip_ctx* ctx, const float2* D, int32_t n_par, const int32_t
 
 int32_t launch_recon_c64(bip_ctx* ctx, const float2* D, int32_t n_par, const int32_t* bh_dev, int32_t n_beams,
                          const int32_t* nn_idx, const float* nn_w, int32_t max_nn, int carrier, int recon,
-                         const int32_t* origin_dev, int32_t atom, int32_t w, float2* out) {
+                         const int32_t* origin_dev, int32_t atom, int32_t w, float2* out, int32_t origin_shift, bool retilt) {
   for (int b0 = 0; b0 < n_beams; b0 += 65535) {
     const int nb = std::min(65535, n_beams - b0);
     dim3 grid((unsigned)((w * w + 255) / 256), (unsigned)nb);
     k_recon_c64<<<grid, 256, 0, ctx->stream>>>(D, n_par, bh_dev + 2 * (int64_t)b0, nb, nn_idx + (int64_t)b0 * max_nn,
                                                nn_w + (int64_t)b0 * max_nn, max_nn, carrier, recon, origin_dev, atom, w,
                                                ctx->g.ny, ctx->g.nx, ctx->rooty_dev, ctx->rootx_dev,
-                                               out + (int64_t)b0 * w * w);
+                                               out + (int64_t)b0 * w * w, origin_shift, retilt ? 1 : 0);
     BIP_CUDA(ctx, cudaGetLastError());
   }
   return BIP_OK;
