@@ -292,6 +292,7 @@ def run_ours(args):
     line = None
     if rank == 0:
         cpu = cpu_baseline(args) if world == 1 and not args.no_cpu_baseline else None
+        extra = extra_legs(args) if world == 1 else None
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -316,11 +317,46 @@ def run_ours(args):
             "fp32_equiv_tflops_contract": float(ctx.get_timing()["flops"]) * 1.0 / (contract_ms / args.steps * 1e-3) / 1e12 if contract_ms else None,
             "cpu_baseline": cpu,
         }
+        if extra:
+            line["extra"] = extra
         print(json.dumps(line))
     ctx.close()
     if world > 1:
         dist.destroy_process_group()
     return line
+
+
+def extra_legs(args):
+    """Short legs on other BASELINE.json configs, each in a fresh process after this one has released the GPU memory it
+    needs, embedded under "extra" of the main line (the driver parses the LAST line, which stays configs[1]).  Default:
+    configs[3] in the paper's own regime (FePt nanoparticle, PRISM f = 8 beam lists + crop mask) and the
+    FP16X3 arithmetic on the default workload."""
+    out = {}
+    for spec in [x for x in args.extra.split(",") if x and x != "none"]:
+        name, _, n = spec.partition(":")
+        base = [sys.executable, os.path.abspath(__file__), "--steps", "2", "--warmup", "1", "--no-cpu-baseline", "--extra", "none"]
+        if name == "fp16x3":        # the three-product arithmetic (reduced outputs only) on the default workload
+            cmd = base + ["--precision", "fp16x3", "--atoms", n or "16", "--planes", "2"]
+        elif name == "cfg3":        # five edges in one plane loop, the largest config that fits one GPU
+            cmd = base + ["--workload", "cfg3", "--edges", "all", "--atoms", n or "2", "--planes", "1"]
+        else:
+            cmd = base + ["--workload", name, "--atoms", n or "256", "--planes", "8", "--assoc", "auto"]
+        try:
+            r = subprocess.run(cmd, capture_output=True, text=True, timeout=900, env=dict(os.environ, WORLD_SIZE="1", RANK="0", LOCAL_RANK="0"))
+            lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+            d = json.loads(lines[-1]) if r.returncode == 0 and lines else None
+        except Exception as ex:                      # a leg that fails must not take the main line with it
+            d, r = None, None
+            out[name] = {"error": repr(ex)[:200]}
+            continue
+        if d is None:
+            out[name] = {"error": (r.stderr or r.stdout)[-300:]}
+            continue
+        out[name] = {"value": d["value"], "unit": d["unit"], "dtype": d["dtype"], "e2e": d["e2e"]["value"], "ms_per_step": d["ms_per_step"], "workload": d["config"]["workload"],
+                     "association_ran": d["config"]["association_ran"], "crop_mask": d["config"]["crop_mask"],
+                     "atoms_per_step": d["config"]["atoms_per_step_per_gpu"], "phases_ms_per_step": d["phases_ms_per_step"],
+                     "roofline_frac": d["roofline"]["frac"], "gemm2_tflops_fp32_equiv": d["roofline"]["achieved"], "clocks": d["clocks"]}
+    return out or None
 
 
 def oracle_sample_setup(args, n_scan=256):
@@ -402,7 +438,11 @@ def main():
     ap.add_argument("--assoc", default="probe", choices=["probe", "coupling", "auto"], help="association of the contraction (bip_set_association)")
     ap.add_argument("--crop", type=int, default=0, help="override the workload's crop-mask factor (0 = the workload's own)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--extra", default=None, help="comma list of short extra legs embedded under 'extra' (workload[:atoms]); default cfg4:256 for "
+                    "the default workload, none otherwise")
     args = ap.parse_args()
+    if args.extra is None:
+        args.extra = "cfg4:256,fp16x3:16" if args.workload == "cfg2" and args.scale == 1 and args.precision == "fp16x4" else "none"
     if args.impl == "reference":
         run_reference(args)
         return

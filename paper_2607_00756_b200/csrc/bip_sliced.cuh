@@ -53,7 +53,13 @@ struct Sliced {
   int32_t fmt = SL_FMT_FP16X4;
 };
 
-__host__ __device__ inline int sl_parts_of(const Sliced& S) { return sl_parts(S.fmt) + (S.neg_im ? 2 : 0); }
+__host__ __device__ inline int sl_parts_of(const Sliced& S) {
+#ifdef BIP_TUNING
+  return sl_parts(S.fmt) + (S.neg_im ? 2 : 0);
+#else
+  return sl_parts(S.fmt);                  // the shipped build never sets neg_im (N = 256 A/B variant only)
+#endif
+}
 __host__ __device__ inline int sl_step_el_of(const Sliced& S) { return sl_parts_of(S) * SL_TILE_EL; }
 
 #ifdef __CUDACC__
@@ -102,6 +108,7 @@ __device__ __forceinline__ void sl_store_group(const Sliced& S, int64_t batch, i
     }
 #pragma unroll
     for (int part = 0; part < 4; ++part) *reinterpret_cast<uint4*>(p + part * SL_TILE_EL) = *reinterpret_cast<const uint4*>(out[part]);
+#ifdef BIP_TUNING                    // only the N = 256 A/B variant reads these parts; the shipped build never sets neg_im
     if (S.neg_im) {
 #pragma unroll
       for (int part = 2; part < 4; ++part) {
@@ -110,6 +117,7 @@ __device__ __forceinline__ void sl_store_group(const Sliced& S, int64_t batch, i
         *reinterpret_cast<uint4*>(p + (part + 2) * SL_TILE_EL) = v;
       }
     }
+#endif
   } else {
     __align__(16) uint16_t out[6][8];
 #pragma unroll
