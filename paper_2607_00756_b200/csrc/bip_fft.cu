@@ -146,9 +146,7 @@ int32_t fft_init(bip_ctx* ctx) {
   const int ny = ctx->g.ny, nx = ctx->g.nx;
   const int64_t G = (int64_t)ny * nx;
   auto dd = [](double re, double im) { return dd_pair(re, im); };
-  std::vector<float4> ry(ny), rx(nx), P(G);
-  for (int t = 0; t < ny; ++t) ry[t] = dd(std::cos(-2.0 * M_PI * t / ny), std::sin(-2.0 * M_PI * t / ny));
-  for (int t = 0; t < nx; ++t) rx[t] = dd(std::cos(-2.0 * M_PI * t / nx), std::sin(-2.0 * M_PI * t / nx));
+  std::vector<float4> ry = make_twiddle_table(ny), rx = make_twiddle_table(nx), P(G);
   // Fresnel propagator P(q) = exp(-i pi lambda dz |q|^2) / G (eq. 2; no band limit), in the stored (digit-reversed) order
   for (int py = 0; py < ny; ++py) {
     const int ky = dif_frequency(py, ny), hy = ky < (ny + 1) / 2 ? ky : ky - ny;
@@ -160,11 +158,11 @@ int32_t fft_init(bip_ctx* ctx) {
       P[(int64_t)py * nx + px] = dd(std::cos(ph) / (double)G, std::sin(ph) / (double)G);
     }
   }
-  BIP_TRY(dev_alloc(ctx, (void**)&ctx->fft_rooty, sizeof(float4) * ny, "fft twiddles"));
-  BIP_TRY(dev_alloc(ctx, (void**)&ctx->fft_rootx, sizeof(float4) * nx, "fft twiddles"));
+  BIP_TRY(dev_alloc(ctx, (void**)&ctx->fft_rooty, sizeof(float4) * ry.size(), "fft twiddles"));
+  BIP_TRY(dev_alloc(ctx, (void**)&ctx->fft_rootx, sizeof(float4) * rx.size(), "fft twiddles"));
   BIP_TRY(dev_alloc(ctx, (void**)&ctx->fft_P, sizeof(float4) * G, "propagator (digit-reversed order)"));
-  BIP_CUDA(ctx, cudaMemcpyAsync(ctx->fft_rooty, ry.data(), sizeof(float4) * ny, cudaMemcpyHostToDevice, ctx->stream));
-  BIP_CUDA(ctx, cudaMemcpyAsync(ctx->fft_rootx, rx.data(), sizeof(float4) * nx, cudaMemcpyHostToDevice, ctx->stream));
+  BIP_CUDA(ctx, cudaMemcpyAsync(ctx->fft_rooty, ry.data(), sizeof(float4) * ry.size(), cudaMemcpyHostToDevice, ctx->stream));
+  BIP_CUDA(ctx, cudaMemcpyAsync(ctx->fft_rootx, rx.data(), sizeof(float4) * rx.size(), cudaMemcpyHostToDevice, ctx->stream));
   BIP_CUDA(ctx, cudaMemcpyAsync(ctx->fft_P, P.data(), sizeof(float4) * G, cudaMemcpyHostToDevice, ctx->stream));
   std::vector<int32_t> py(ny), px(nx);
   for (int i = 0; i < ny; ++i) py[i] = dif_frequency(i, ny);

@@ -4,7 +4,9 @@
 #ifndef BIP_FFT_CUH_
 #define BIP_FFT_CUH_
 
+#include <cmath>
 #include <cstdint>
+#include <vector>
 #include <cuda_runtime.h>
 
 namespace bip {
@@ -66,14 +68,32 @@ __device__ __forceinline__ void dft_small(float2 (&x)[8]) {
 __device__ __forceinline__ int pad_idx(int i) { return i + (i >> 3); }
 __host__ __device__ constexpr int pad_len(int n) { return n + (n >> 3); }
 
+// Twiddle tables are stored PER STAGE, transposed: for the radix-8 stage on block length L (sub = L / 8 > 1) the entry of
+// output m (1..7) and position j (0..sub-1) is w_L^(j m) at  stage_off(L) + (m - 1) * sub + j, so that the lanes of a warp
+// (consecutive j) read consecutive 16-byte entries.  (With one table of N-th roots indexed by j m N / L every lane of a
+// warp hit its own cache line: the kernels were bound by the L1 data path, profiles/r02_fft_ncu.md.)
+// stage_off: stages run L = N, N/8, N/64, ...; the table of stage L starts after those of all longer stages.
+__host__ __device__ inline int tw_stage_off(int lN, int lL) {
+  int off = 0;
+  for (int l = lN; l > lL; l -= 3) off += 7 << (l - 3);
+  return off;
+}
+__host__ __device__ inline int tw_table_len(int lN) {       // entries of all radix-8 stages with sub > 1
+  int n = 0;
+  for (int l = lN; l > 3; l -= 3) n += 7 << (l - 3);
+  return n > 0 ? n : 1;
+}
+
 // One stage on block length L = 2^lL with radix R over all lines of the block.  Forward (DIF): butterfly, then twiddle
 // w_L^(j m); inverse (DIT): conjugate twiddle, then inverse butterfly.  Element (line, i) lives at sm[line * pitch + pad_idx(i)].
-// All sizes are powers of two: shifts and masks, no integer division.  A stage with L == R has j = 0 only: no twiddles.
+// All sizes are powers of two: shifts and masks, no integer division.  A stage with L == R has j = 0 only: no twiddles
+// (the radix-4 / radix-2 remainder stages are always of that kind).
 template <int R, bool INV>
 __device__ __forceinline__ void fft_stage(float2* sm, int lN, int lL, int n_lines, int pitch, const float4* __restrict__ root, int tid, int nthr) {
   constexpr int lR = R == 8 ? 3 : R == 4 ? 2 : 1;
-  const int lsub = lL - lR, sub = 1 << lsub, lper = lN - lR, N = 1 << lN, ltw = lN - lL;
+  const int lsub = lL - lR, sub = 1 << lsub, lper = lN - lR;
   const int total = n_lines << lper;
+  const float4* tw = root + tw_stage_off(lN, lL);
   for (int u = tid; u < total; u += nthr) {
     const int line = u >> lper, v = u & ((1 << lper) - 1);
     const int blk = v >> lsub, j = v & (sub - 1);
@@ -82,14 +102,14 @@ __device__ __forceinline__ void fft_stage(float2* sm, int lN, int lL, int n_line
     float2 x[8];
 #pragma unroll
     for (int k = 0; k < R; ++k) x[k] = p[pad_idx(i0 + (k << lsub))];
-    if (INV && lsub > 0) {
+    if (INV && R == 8 && lsub > 0) {
 #pragma unroll
-      for (int m = 1; m < R; ++m) x[m] = cmulc_dd(x[m], __ldg(root + (((j * m) << ltw) & (N - 1))));
+      for (int m = 1; m < R; ++m) x[m] = cmulc_dd(x[m], __ldg(tw + ((m - 1) << lsub) + j));
     }
     dft_small<R, INV>(x);
-    if (!INV && lsub > 0) {
+    if (!INV && R == 8 && lsub > 0) {
 #pragma unroll
-      for (int m = 1; m < R; ++m) x[m] = cmul_dd(x[m], __ldg(root + (((j * m) << ltw) & (N - 1))));
+      for (int m = 1; m < R; ++m) x[m] = cmul_dd(x[m], __ldg(tw + ((m - 1) << lsub) + j));
     }
 #pragma unroll
     for (int k = 0; k < R; ++k) p[pad_idx(i0 + (k << lsub))] = x[k];
@@ -134,6 +154,22 @@ inline int dif_frequency(int pos, int N) {
 inline float4 dd_pair(double re, double im) {
   const float hr = (float)re, hi = (float)im;
   return make_float4(hr, hi, (float)(re - (double)hr), (float)(im - (double)hi));
+}
+
+
+// per-stage transposed twiddle table of a length-N transform (see tw_stage_off): entries exp(-2 pi i j m / L)
+inline std::vector<float4> make_twiddle_table(int N) {
+  const int lN = ilog2(N);
+  std::vector<float4> t((size_t)fftdev::tw_table_len(lN), make_float4(1.f, 0.f, 0.f, 0.f));
+  for (int lL = lN; lL > 3; lL -= 3) {
+    const int L = 1 << lL, sub = L >> 3, off = fftdev::tw_stage_off(lN, lL);
+    for (int m = 1; m < 8; ++m)
+      for (int j = 0; j < sub; ++j) {
+        const double a = -2.0 * M_PI * (double)((int64_t)j * m % L) / (double)L;
+        t[(size_t)off + (size_t)(m - 1) * sub + j] = dd_pair(std::cos(a), std::sin(a));
+      }
+  }
+  return t;
 }
 
 }  // namespace bip

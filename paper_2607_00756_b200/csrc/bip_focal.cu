@@ -153,13 +153,13 @@ int32_t focal_init(bip_ctx* ctx) {
 static int32_t window_tables(bip_ctx* ctx, int Wp, const float4** root, const int32_t** perm) {
   auto it = ctx->focal_tables.find(Wp);
   if (it == ctx->focal_tables.end()) {
-    std::vector<float4> r(Wp);
+    std::vector<float4> r = make_twiddle_table(Wp);
     std::vector<int32_t> p(Wp);
-    for (int t = 0; t < Wp; ++t) { r[t] = dd_pair(std::cos(-2.0 * M_PI * t / Wp), std::sin(-2.0 * M_PI * t / Wp)); p[t] = dif_frequency(t, Wp); }
+    for (int t = 0; t < Wp; ++t) p[t] = dif_frequency(t, Wp);
     void* rd = nullptr; void* pd = nullptr;
-    BIP_TRY(dev_alloc(ctx, &rd, sizeof(float4) * Wp, "window twiddles"));
+    BIP_TRY(dev_alloc(ctx, &rd, sizeof(float4) * r.size(), "window twiddles"));
     BIP_TRY(dev_alloc(ctx, &pd, sizeof(int32_t) * Wp, "window permutation"));
-    BIP_CUDA(ctx, cudaMemcpyAsync(rd, r.data(), sizeof(float4) * Wp, cudaMemcpyHostToDevice, ctx->stream));
+    BIP_CUDA(ctx, cudaMemcpyAsync(rd, r.data(), sizeof(float4) * r.size(), cudaMemcpyHostToDevice, ctx->stream));
     BIP_CUDA(ctx, cudaMemcpyAsync(pd, p.data(), sizeof(int32_t) * Wp, cudaMemcpyHostToDevice, ctx->stream));
     BIP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     it = ctx->focal_tables.emplace(Wp, std::make_pair(rd, pd)).first;
