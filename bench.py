@@ -326,6 +326,51 @@ def run_ours(args):
     return line
 
 
+def run_alg3(args):
+    """NEXT-3 leg: Algorithm 3 (bip_cube_alg3; S1-partitioned cube on all G exit beams, per-scan exit multislice) on --atoms
+    sites of the workload.  One JSON line; amplitudes = scan positions x sites x channels x G exit beams."""
+    import torch
+    import paper_2607_00756_b200 as B
+    assert torch.cuda.is_available()
+    wl, edges = build_problem(args, 0)
+    edge = edges[0]
+    g = B.Grid(wl.ny, wl.nx, wl.ly, wl.lx, wl.nz, wl.dz, wl.lam)
+    geo = B.plan_geometry(g, wl.alpha_mrad, edge.det_mrad, wl.defocus, wl.parent_factor, prism=wl.prism)
+    ctx = B.Context(g, torch.from_numpy(wl.T).cuda(), geo.ap_h, geo.ap_c, geo.p1_h, geo.w1, geo.p2_h)
+    ctx.build_S1()
+    ctx.set_scan(wl.scan)
+    ctx.add_edge(edge.slice, edge.centre, edge.H, geo.det_h, geo.w2)
+    recon = {"linear": B.RECON_LINEAR, "magphase": B.RECON_MAGPHASE}[args.recon]
+    out = torch.empty((ctx.n_rho, wl.ny, wl.nx), dtype=torch.float32, device="cuda")
+    for _ in range(args.warmup):
+        ctx.cube_alg3(0, recon, B.PREC_FP16X4, out=out)
+    torch.cuda.synchronize()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    adv = con = 0.0
+    for _ in range(args.steps):
+        ctx.cube_alg3(0, recon, B.PREC_FP16X4, out=out)
+        t = ctx.get_timing()
+        adv += t["advance_peel_ms"]; con += t["contract_ms"]
+    ev1.record()
+    torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1) / args.steps
+    amps = float(ctx.n_rho) * edge.n_atoms * edge.n_ch * wl.ny * wl.nx
+    slices_below = float(np.mean(wl.nz - edge.slice))
+    G = wl.ny * wl.nx
+    line = {"metric": METRIC.replace("detector-beam", "exit-beam"), "value": amps / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "dtype": "f32(c64) wavefields, fp16x4 probe contraction", "data": "synthetic",
+            "config": {"workload": f"Algorithm 3 on BASELINE configs[{CONFIG_INDEX.get(args.workload, '?')}] ({wl.name}): {wl.ny}x{wl.nx} grid, {wl.nz} slices, "
+                                   f"B={geo.ap_h.shape[0]}, parents={ctx.n_p1}, W={edge.W}, N_ch={edge.n_ch}, N_rho={ctx.n_rho}, all {G} exit beams",
+                       "atoms_per_step": edge.n_atoms, "mean_slices_to_exit": slices_below},
+            "phases_ms_per_step": {"s1_advance": adv / args.steps, "probe_exit_detect": con / args.steps},
+            "wavefield_slice_steps_per_s": ctx.n_rho * edge.n_atoms * edge.n_ch * slices_below * args.steps / (con * 1e-3) if con else None,
+            "hbm_GBps_of_slice_steps": (ctx.n_rho * edge.n_atoms * edge.n_ch * slices_below * G * 48.0 * args.steps / (con * 1e-3) / 1e9) if con else None}
+    print(json.dumps(line))
+    ctx.close()
+    return line
+
+
 def extra_legs(args):
     """Short legs on other BASELINE.json configs, each in a fresh process after this one has released the GPU memory it
     needs, embedded under "extra" of the main line (the driver parses the LAST line, which stays configs[1]).  Default:
@@ -337,6 +382,8 @@ def extra_legs(args):
         base = [sys.executable, os.path.abspath(__file__), "--steps", "2", "--warmup", "1", "--no-cpu-baseline", "--extra", "none"]
         if name == "fp16x3":        # the three-product arithmetic (reduced outputs only) on the default workload
             cmd = base + ["--precision", "fp16x3", "--atoms", n or "16", "--planes", "2"]
+        elif name == "alg3":        # NEXT-3: Algorithm 3 on the configs[4] geometry
+            cmd = base + ["--workload", "cfg5", "--mode", "cube_alg3", "--atoms", n or "2", "--planes", "1"]
         elif name == "cfg3":        # five edges in one plane loop, the largest config that fits one GPU
             cmd = base + ["--workload", "cfg3", "--edges", "all", "--atoms", n or "2", "--planes", "1"]
         else:
@@ -351,6 +398,9 @@ def extra_legs(args):
             continue
         if d is None:
             out[name] = {"error": (r.stderr or r.stdout)[-300:]}
+            continue
+        if name == "alg3":
+            out[name] = {k: d[k] for k in ("value", "unit", "ms_per_step", "config", "phases_ms_per_step", "wavefield_slice_steps_per_s", "hbm_GBps_of_slice_steps")}
             continue
         out[name] = {"value": d["value"], "unit": d["unit"], "dtype": d["dtype"], "e2e": d["e2e"]["value"], "ms_per_step": d["ms_per_step"], "workload": d["config"]["workload"],
                      "association_ran": d["config"]["association_ran"], "crop_mask": d["config"]["crop_mask"],
@@ -432,7 +482,7 @@ def main():
     ap.add_argument("--planes", type=int, default=2, help="ionisation planes the atoms of a step are spread over")
     ap.add_argument("--precision", default=os.environ.get("BIP_BENCH_PRECISION", "fp16x4"), choices=["fp16x4", "fp16x3", "bf16x6", "tf32x3", "fp32_simt"])
     ap.add_argument("--recon", default="magphase", choices=["linear", "magphase"])
-    ap.add_argument("--mode", default="map", choices=["map", "qeels_x", "cube"])
+    ap.add_argument("--mode", default="map", choices=["map", "qeels_x", "cube", "cube_alg3"])
     ap.add_argument("--edges", default="first", choices=["first", "all"], help="all: every edge of the workload shares one plane loop (configs[2])")
     ap.add_argument("--parent-factor", type=float, default=0.0, help="override the workload's parent factor (configs[4] sweeps 1/2/4/8)")
     ap.add_argument("--assoc", default="probe", choices=["probe", "coupling", "auto"], help="association of the contraction (bip_set_association)")
@@ -442,7 +492,7 @@ def main():
                     "the default workload, none otherwise")
     args = ap.parse_args()
     if args.extra is None:
-        args.extra = "cfg4:256,fp16x3:16" if args.workload == "cfg2" and args.scale == 1 and args.precision == "fp16x4" else "none"
+        args.extra = "cfg4:256,fp16x3:16,alg3:2" if args.workload == "cfg2" and args.scale == 1 and args.precision == "fp16x4" else "none"
     if args.impl == "reference":
         run_reference(args)
         return
@@ -456,6 +506,9 @@ def main():
         cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
                "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
         sys.exit(subprocess.call(cmd))
+    if args.mode == "cube_alg3":
+        run_alg3(args)
+        return
     if world != args.gpus:
         sys.exit(f"bench.py: --gpus {args.gpus} does not match WORLD_SIZE = {world} (launch with torchrun --nproc-per-node {args.gpus})")
     run_ours(args)

@@ -41,7 +41,7 @@ __device__ __forceinline__ float2 apply_t(float2 v, const float2* __restrict__ T
 // Passes 1 and 3: LINES rows per block.  tmode: 0 none, 1 multiply by T, 2 by conj T (before the forward transform /
 // after the inverse one).
 template <bool INV>
-__global__ void __launch_bounds__(1024) k_ms_rows(float2* __restrict__ S, const float2* __restrict__ T, int tmode, int ny, int lnx, int lines,
+__global__ void __launch_bounds__(256, 3) k_ms_rows(float2* __restrict__ S, const float2* __restrict__ T, int tmode, int ny, int lnx, int lines,
                                                   const float4* __restrict__ rootx) {
   extern __shared__ float2 sm_rows[];
   const int nx = 1 << lnx, pitch = pad_len(nx);
@@ -68,7 +68,7 @@ __global__ void __launch_bounds__(1024) k_ms_rows(float2* __restrict__ S, const 
 
 // Pass 2: a tile of `cols` columns (consecutive stored x positions) x ny rows per block; forward along y, spectrum
 // multiply with the digit-reversed propagator table (conjugated when conj_p), inverse along y.
-__global__ void __launch_bounds__(1024) k_ms_cols(float2* __restrict__ S, const float4* __restrict__ Pperm, int conj_p, int lny, int nx, int lcols,
+__global__ void __launch_bounds__(256, 3) k_ms_cols(float2* __restrict__ S, const float4* __restrict__ Pperm, int conj_p, int lny, int nx, int lcols,
                                                   const float4* __restrict__ rooty) {
   extern __shared__ float2 sm_cols[];
   const int ny = 1 << lny, cols = 1 << lcols;
@@ -102,7 +102,7 @@ __global__ void __launch_bounds__(1024) k_ms_cols(float2* __restrict__ S, const 
 //     out[rho][ky][kx] += sum_n |F psi_n|^2 / G
 // at the TRUE frequency (ky, kx) of the stored position (permy / permx undo the digit reversal).  A block owns the
 // (all y, its x tile) outputs of its scan position, so the read-modify-write needs no atomics.
-__global__ void __launch_bounds__(1024) k_ms_cols_detect(const float2* __restrict__ F, int n_ch, float* __restrict__ out, float inv_G, int lny, int nx,
+__global__ void __launch_bounds__(256, 2) k_ms_cols_detect(const float2* __restrict__ F, int n_ch, float* __restrict__ out, float inv_G, int lny, int nx,
                                                          int lcols, const float4* __restrict__ rooty, const int32_t* __restrict__ permy,
                                                          const int32_t* __restrict__ permx) {
   extern __shared__ float2 sm_det[];
@@ -134,6 +134,14 @@ __global__ void __launch_bounds__(1024) k_ms_cols_detect(const float2* __restric
     const int64_t k = (int64_t)__ldg(permy + y) * nx + __ldg(permx + x0 + c);
     o[k] += acc[i] * inv_G;
   }
+}
+
+// threads per block: a power of two, a quarter of the butterflies of a stage (lines * N / 8), within 64 .. 256
+int fft_threads(int lines, int n) {
+  const int reuse = std::max(1, tune_int("BIP_TUNE_FFT_REUSE", 4));
+  int t = 64;
+  while (t < 256 && t * reuse < lines * n / 8) t <<= 1;
+  return t;
 }
 
 }  // namespace
@@ -172,9 +180,12 @@ int32_t fft_init(bip_ctx* ctx) {
   BIP_CUDA(ctx, cudaMemcpyAsync(ctx->fft_permy, py.data(), sizeof(int32_t) * ny, cudaMemcpyHostToDevice, ctx->stream));
   BIP_CUDA(ctx, cudaMemcpyAsync(ctx->fft_permx, px.data(), sizeof(int32_t) * nx, cudaMemcpyHostToDevice, ctx->stream));
   BIP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-  // launch shapes: ~32 KB of rows per block, ~64 KB of columns per block (at least 4 columns: whole 32-byte sectors)
-  ctx->fft_lines = std::max(1, std::min(ny, 4096 / nx));
-  ctx->fft_cols = std::max(4, std::min(nx, 8192 / ny));
+  // launch shapes: ~64 KB of rows or columns per block (at least 4 columns: whole 32-byte sectors), and a quarter as many
+  // threads as butterflies per stage, so that every thread re-uses its twiddles over 4 lines (fft_stage)
+  ctx->fft_lines = std::max(1, std::min(ny, tune_int("BIP_TUNE_FFT_ROW_EL", 8192) / nx));
+  ctx->fft_cols = std::max(tune_int("BIP_TUNE_FFT_MINCOLS", 4), std::min(nx, tune_int("BIP_TUNE_FFT_COL_EL", 8192) / ny));
+  BIP_CUDA(ctx, cudaFuncSetAttribute(k_ms_rows<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_rows_bytes(ctx->fft_lines, nx)));
+  BIP_CUDA(ctx, cudaFuncSetAttribute(k_ms_rows<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_rows_bytes(ctx->fft_lines, nx)));
   const size_t smem_cols = smem_cols_bytes(ctx->fft_cols, ny);
   BIP_CUDA(ctx, cudaFuncSetAttribute(k_ms_cols, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cols));
   BIP_CUDA(ctx, cudaFuncSetAttribute(k_ms_cols_detect, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(smem_cols + (size_t)ctx->fft_cols * ny * sizeof(float))));
@@ -185,7 +196,7 @@ int32_t fft_init(bip_ctx* ctx) {
 int32_t fft_slice_op(bip_ctx* ctx, float2* S, int n_cols, const float2* Tj, int pre, int conj_p, int post) {
   const int ny = ctx->g.ny, nx = ctx->g.nx;
   const int lines = ctx->fft_lines, cols = ctx->fft_cols;
-  const int thr_rows = std::max(32, std::min(1024, lines * nx / 8)), thr_cols = std::max(32, std::min(1024, cols * ny / 8));
+  const int thr_rows = fft_threads(lines, nx), thr_cols = fft_threads(cols, ny);
   const size_t smem_rows = smem_rows_bytes(lines, nx), smem_cols = smem_cols_bytes(cols, ny);
   const int lnx = ilog2(nx), lny = ilog2(ny), lcols = ilog2(cols);
   for (int c0 = 0; c0 < n_cols; c0 += 65535) {                // gridDim.y limit
@@ -203,7 +214,7 @@ int32_t fft_slice_op(bip_ctx* ctx, float2* S, int n_cols, const float2* Tj, int 
 int32_t fft_detect(bip_ctx* ctx, float2* fields, int n_rho, int n_ch, float* out) {
   const int ny = ctx->g.ny, nx = ctx->g.nx;
   const int lines = ctx->fft_lines, cols = ctx->fft_cols;
-  const int thr_rows = std::max(32, std::min(1024, lines * nx / 8)), thr_cols = std::max(32, std::min(1024, cols * ny / 8));
+  const int thr_rows = fft_threads(lines, nx), thr_cols = fft_threads(cols, ny);
   const size_t smem_rows = smem_rows_bytes(lines, nx);
   const size_t smem_det = smem_cols_bytes(cols, ny) + (size_t)cols * ny * sizeof(float);
   const int lnx = ilog2(nx), lny = ilog2(ny), lcols = ilog2(cols);

@@ -91,28 +91,39 @@ __host__ __device__ inline int tw_table_len(int lN) {       // entries of all ra
 template <int R, bool INV>
 __device__ __forceinline__ void fft_stage(float2* sm, int lN, int lL, int n_lines, int pitch, const float4* __restrict__ root, int tid, int nthr) {
   constexpr int lR = R == 8 ? 3 : R == 4 ? 2 : 1;
-  const int lsub = lL - lR, sub = 1 << lsub, lper = lN - lR;
-  const int total = n_lines << lper;
+  const int lsub = lL - lR, sub = 1 << lsub, lper = lN - lR, nv = 1 << lper;
   const float4* tw = root + tw_stage_off(lN, lL);
-  for (int u = tid; u < total; u += nthr) {
-    const int line = u >> lper, v = u & ((1 << lper) - 1);
+  // thread <-> butterfly position v inside a line (consecutive lanes = consecutive v: coalesced twiddle reads, conflict-free
+  // shared-memory accesses); the thread keeps the 7 twiddles of its position in registers and loops over the LINES of the
+  // block with them -- every line of a block needs the same twiddles, and fetching them per line made the twiddle reads
+  // half of the L1 traffic of these kernels (profiles/r02_fft_ncu.md)
+  const int lthr = 31 - __clz(nthr), lv = lthr < lper ? lthr : lper;       // nthr is a power of two
+  const int line0 = tid >> lv, line_step = nthr >> lv;
+  for (int v = tid & ((1 << lv) - 1); v < nv; v += 1 << lv) {
     const int blk = v >> lsub, j = v & (sub - 1);
-    float2* p = sm + line * pitch;
     const int i0 = (blk << lL) + j;
-    float2 x[8];
+    float4 w[8];
+    if (R == 8 && lsub > 0) {
 #pragma unroll
-    for (int k = 0; k < R; ++k) x[k] = p[pad_idx(i0 + (k << lsub))];
-    if (INV && R == 8 && lsub > 0) {
-#pragma unroll
-      for (int m = 1; m < R; ++m) x[m] = cmulc_dd(x[m], __ldg(tw + ((m - 1) << lsub) + j));
+      for (int m = 1; m < R; ++m) w[m] = __ldg(tw + ((m - 1) << lsub) + j);
     }
-    dft_small<R, INV>(x);
-    if (!INV && R == 8 && lsub > 0) {
+    for (int line = line0; line < n_lines; line += line_step) {
+      float2* p = sm + line * pitch;
+      float2 x[8];
 #pragma unroll
-      for (int m = 1; m < R; ++m) x[m] = cmul_dd(x[m], __ldg(tw + ((m - 1) << lsub) + j));
+      for (int k = 0; k < R; ++k) x[k] = p[pad_idx(i0 + (k << lsub))];
+      if (INV && R == 8 && lsub > 0) {
+#pragma unroll
+        for (int m = 1; m < R; ++m) x[m] = cmulc_dd(x[m], w[m]);
+      }
+      dft_small<R, INV>(x);
+      if (!INV && R == 8 && lsub > 0) {
+#pragma unroll
+        for (int m = 1; m < R; ++m) x[m] = cmul_dd(x[m], w[m]);
+      }
+#pragma unroll
+      for (int k = 0; k < R; ++k) p[pad_idx(i0 + (k << lsub))] = x[k];
     }
-#pragma unroll
-    for (int k = 0; k < R; ++k) p[pad_idx(i0 + (k << lsub))] = x[k];
   }
 }
 

@@ -34,7 +34,7 @@ __global__ void k_slice_strength(const float2* __restrict__ T, int64_t G, double
 
 // E[e] <- F_w^-1[ exp(-i pi lambda d |q_w + q_h|^2) F_w E[e] ] for window e; its carrier is beam h[e % n_beams].
 // pld = pi lambda d (signed); q_w = k / (W_p pixel); stored positions after the forward transforms are digit-reversed (perm).
-__global__ void __launch_bounds__(1024) k_window_fresnel(float2* __restrict__ E, const int32_t* __restrict__ h, int n_beams, int lW, double pld,
+__global__ void __launch_bounds__(256, 2) k_window_fresnel(float2* __restrict__ E, const int32_t* __restrict__ h, int n_beams, int lW, double pld,
                                                          double inv_ly, double inv_lx, double inv_wy, double inv_wx,
                                                          const float4* __restrict__ root, const int32_t* __restrict__ perm) {
   extern __shared__ float2 sm_win[];
@@ -178,7 +178,7 @@ int32_t focal_window_fresnel(bip_ctx* ctx, float2* E, int64_t n_win, const int32
   BIP_TRY(window_tables(ctx, Wp, &root, &perm));
   const int lW = ilog2(Wp);
   const size_t smem = (size_t)Wp * (pad_len(Wp) + 1) * sizeof(float2) + 2 * (size_t)Wp * sizeof(float4);
-  const int thr = std::max(64, std::min(1024, Wp * Wp / 8));
+  const int thr = std::max(64, std::min(256, Wp * Wp / 32));       // a quarter of the butterflies per stage: twiddle re-use over 4 lines
   const double py = ctx->g.ly / ctx->g.ny, px = ctx->g.lx / ctx->g.nx;
   for (int64_t e0 = 0; e0 < n_win; e0 += (int64_t)n_beams * 1024) {          // whole beam sets per launch: e % n_beams stays the beam
     const int64_t ne = std::min<int64_t>((int64_t)n_beams * 1024, n_win - e0);

@@ -220,8 +220,15 @@ def test_call_order_and_argument_errors():
     ctx.close()
 
 
+@pytest.fixture(scope="module")
+def cfg2_sample():
+    """The oracle's sample of the full-size configs[1] launch (built once for both arithmetics: 100 s of fp64 parent columns)."""
+    smp = OracleSample("cfg2", nz=2, n_atoms=2, n_scan=64)
+    return smp, smp.run("magphase")["map"]
+
+
 @pytest.mark.parametrize("prec_name", ["fp16x4", "fp16x3"])
-def test_full_size_cfg2_sampled_pixels(prec_name):
+def test_full_size_cfg2_sampled_pixels(prec_name, cfg2_sample):
     """BASELINE.json configs[1] at FULL contraction size, in the launch configuration bench.py times (512^2 grid,
     B = 30 909, K = 79 105, parents (1951, 4921), W = 48, 9 channels, all 4096 scan positions, MAGPHASE, map output,
     two atoms per launch): the oracle computes 64 sampled map pixels one by one (every channel and detector beam);
@@ -229,9 +236,8 @@ def test_full_size_cfg2_sampled_pixels(prec_name):
     Properties that hold at any size on the rest: non-negative, finite, window origins bit-exact."""
     import torch
     import paper_2607_00756_b200 as B
-    smp = OracleSample("cfg2", nz=2, n_atoms=2, n_scan=64)
+    smp, want = cfg2_sample
     wl, e = smp.wl, smp.e
-    want = smp.run("magphase")["map"]
     ctx, geo, ids = gpu_context(wl, [e])
     assert geo.ap_h.shape[0] == 30909 and geo.det_h.shape[0] == 79105 and (ctx.n_p1, ctx.n_p2) == (1951, 4921)
     assert np.array_equal(geo.ap_h, smp.orc.ap) and np.array_equal(geo.det_h, smp.orc.det)          # beam lists bit-exact
@@ -318,7 +324,7 @@ def test_cfg4_fept_quarter_clone_prism_regime():
 def test_cfg5_factor_one_against_conventional_multislice_at_scale():
     """BASELINE.json configs[4] at parent factor 1 (parents = all 7721 aperture and 19 797 detector beams, w = I): the
     GPU path against Algorithm 1 itself -- conventional transition-potential multislice per scan position, the ground
-    truth -- at the full 256^2 size, on 16 sampled scan positions: full cube rows and map
+    truth -- at the full 256^2 size, on 10 sampled scan positions: full cube rows and map
     pixels.  No BiP oracle code in between.  Slab truncated to 3 slices (site in slice 1: one slice above, two through
     the exit) so that the 27 518 parent columns build quickly."""
     import torch
@@ -331,7 +337,7 @@ def test_cfg5_factor_one_against_conventional_multislice_at_scale():
     ap, det = ob.beams_in_disc(wl.ny, wl.nx, wl.ly, wl.lx, qa), ob.beams_in_disc(wl.ny, wl.nx, wl.ly, wl.lx, qd)
     c = ob.aperture_coefficients(ap, wl.ny, wl.nx, wl.ly, wl.lx, wl.lam, wl.defocus)
     P = oms.fresnel_propagator(wl.ny, wl.nx, wl.ly, wl.lx, wl.lam, wl.dz)
-    sub = np.array([0, 273, 546, 819, 1000, 1365, 1638, 1911, 2079, 2457, 2730, 3003, 3276, 3549, 3822, 4095])
+    sub = np.array([0, 546, 1000, 1365, 1911, 2079, 2730, 3276, 3822, 4095])
     I1 = oms.conventional_cube(c, ap, wl.T.astype(np.complex128), P, wl.scan[sub], e.slice, e.centre, e.H.astype(complex), det)
     ctx, geo, ids = gpu_context(wl, [e])
     assert (ctx.n_p1, ctx.n_p2) == (7721, 19797) and geo.det_h.shape[0] == 19797
