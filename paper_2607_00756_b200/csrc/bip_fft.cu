@@ -31,69 +31,256 @@ namespace {
 
 using namespace fftdev;
 
-__device__ __forceinline__ float2 apply_t(float2 v, const float2* __restrict__ T, int64_t i, int mode) {
-  if (mode == 0) return v;
-  float2 t = __ldg(T + i);
-  if (mode == 2) t.y = -t.y;
-  return cmulf(v, t);
+// ---------------------------------------------------------------------------------------------------------------------
+// Compile-time-sized transforms.  Everything about a stage -- its radix, the stride of its butterflies, the shared-memory
+// offsets of its eight elements -- is a template constant, so the inner loops are loads, floating-point work and stores
+// with immediate offsets (the run-time-sized version spent 45 % of its instructions on index arithmetic and a third of its
+// shared-memory wavefronts on bank conflicts; profiles/r02_fft_ncu.md).
+//
+// Shared-memory layout of a line of N = 2^LN elements: element i lives at slot  i ^ g(i),  g = XOR of a 4-bit mask per set
+// bit 4, 5, 6 of i (masks by LN mod 3, found by exhaustive search).  With it the 16 lanes of a half-warp hit 16 different
+// 8-byte bank pairs in EVERY access pattern of the transform: contiguous runs (copies, long-stride stages), the
+// short-stride radix-8 stages and the final radix-8 / 4 / 2 stage.  The map is XOR-linear, so the slot of element
+// i0 + (k << LSUB) is slot(i0) ^ const_k.  A tile of columns adds a per-line key (c & 15) so that the same holds when the
+// lanes of a warp run over 16 lines at one position.
+// ---------------------------------------------------------------------------------------------------------------------
+constexpr int NT = 256;                    // threads per block
+constexpr int TILE_EL = 8192;              // elements per block tile (64 KB)
+
+template <int LN> struct Swz {
+  static constexpr uint32_t M4 = (LN % 3 == 1) ? 3u : 1u;
+  static constexpr uint32_t M5 = (LN % 3 == 0) ? 2u : (LN % 3 == 1) ? 4u : 6u;
+  static constexpr uint32_t M6 = (LN % 3 == 0) ? 12u : 8u;
+};
+template <int LN> __host__ __device__ constexpr uint32_t swz_g(uint32_t i) {
+  return (LN > 4 ? ((i >> 4) & 1u) * Swz<LN>::M4 : 0u) ^ (LN > 5 ? ((i >> 5) & 1u) * Swz<LN>::M5 : 0u) ^
+         (LN > 6 ? ((i >> 6) & 1u) * Swz<LN>::M6 : 0u);
+}
+template <int LN> __host__ __device__ constexpr uint32_t slot(uint32_t i) { return i ^ swz_g<LN>(i); }
+// XOR key of line c of a column tile (a line shorter than 16 elements keeps the key inside the line)
+template <int LN> __host__ __device__ constexpr uint32_t key_mask() { return LN >= 4 ? 15u : (1u << LN) - 1u; }
+
+// the tile: dynamic shared memory, always addressed as sm + offset so that every access is an LDS / STS with an
+// immediate offset (its start is 1024-byte aligned: the bank of an offset is the bank of the address)
+extern __shared__ __align__(1024) char sm[];
+constexpr size_t tile_smem_bytes() { return (size_t)TILE_EL * sizeof(float2); }
+__device__ __forceinline__ float2 lds2(uint32_t off) { return *reinterpret_cast<const float2*>(sm + off); }
+__device__ __forceinline__ void sts2(uint32_t off, float2 v) { *reinterpret_cast<float2*>(sm + off) = v; }
+// asynchronous 8-byte copy global -> shared (LDGSTS): no register staging, as many in flight as the loop issues
+__device__ __forceinline__ void cp_async8(uint32_t off, const float2* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(sm + off)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory"); }
+
+// radix-R butterfly with its twiddles: forward (DIF) butterfly then w_L^(j m); inverse (DIT) conj twiddle then butterfly
+template <int R, bool INV, bool TW>
+__device__ __forceinline__ void bfly(float2 (&x)[8], const float4 (&w)[8]) {
+  if (INV && TW) {
+#pragma unroll
+    for (int m = 1; m < R; ++m) x[m] = cmulc_dd(x[m], w[m]);
+  }
+  dft_small<R, INV>(x);
+  if (!INV && TW) {
+#pragma unroll
+    for (int m = 1; m < R; ++m) x[m] = cmul_dd(x[m], w[m]);
+  }
 }
 
-// Passes 1 and 3: LINES rows per block.  tmode: 0 none, 1 multiply by T, 2 by conj T (before the forward transform /
-// after the inverse one).
-template <bool INV>
-__global__ void __launch_bounds__(256, 3) k_ms_rows(float2* __restrict__ S, const float2* __restrict__ T, int tmode, int ny, int lnx, int lines,
-                                                  const float4* __restrict__ rootx) {
-  extern __shared__ float2 sm_rows[];
-  const int nx = 1 << lnx, pitch = pad_len(nx);
-  const int64_t G = (int64_t)ny * nx;
-  float2* col = S + (int64_t)blockIdx.y * G;
-  const int y0 = blockIdx.x * lines;
-  const int n_lines = min(lines, ny - y0);
-  const int tid = threadIdx.x, nthr = blockDim.x;
-  for (int i = tid; i < (n_lines << lnx); i += nthr) {
-    const int64_t g = (int64_t)y0 * nx + i;
-    float2 v = col[g];
-    if (!INV) v = apply_t(v, T, g, tmode);
-    sm_rows[(i >> lnx) * pitch + pad_idx(i & (nx - 1))] = v;
-  }
-  __syncthreads();
-  fft_lines<INV>(sm_rows, lnx, n_lines, pitch, rootx, tid, nthr);
-  for (int i = tid; i < (n_lines << lnx); i += nthr) {
-    const int64_t g = (int64_t)y0 * nx + i;
-    float2 v = sm_rows[(i >> lnx) * pitch + pad_idx(i & (nx - 1))];
-    if (INV) v = apply_t(v, T, g, tmode);
-    col[g] = v;
+// byte offsets of element k of a butterfly relative to element 0: an XOR part (the swizzle bits, and the k field itself
+// when it lies inside the low index bits) and an ADD part (the k field above them) -- both compile-time constants
+template <int LN, int LSUB> __host__ __device__ constexpr uint32_t xk(int k) {
+  return LSUB >= 4 ? 8u * swz_g<LN>((uint32_t)k << LSUB) : 8u * slot<LN>((uint32_t)k << LSUB);
+}
+template <int LN, int LSUB> __host__ __device__ constexpr uint32_t ak(int k) { return LSUB >= 4 ? 8u * ((uint32_t)k << LSUB) : 0u; }
+
+enum { IO_SMEM = 0, IO_GLOBAL = 1 };
+
+// One radix-R stage on block length 2^LL of n_lines transforms of length 2^LN (lines 8 N bytes apart in the tile).
+// Thread <-> butterfly position v, consecutive lanes = consecutive v; the thread keeps the twiddles of its position in
+// registers and loops over the lines with them.  SRC / DST = IO_GLOBAL (only for the stage on the whole line, LL == LN):
+// the elements are read from / written to global memory in natural order, line l at g + l N, times
+// T[(line index mod ny) N + i] (tmode 1) or its conjugate (tmode 2) -- the row passes touch global memory directly in the
+// stage whose butterflies stride over the whole row (unit stride across the lanes).  The T values of a line are requested
+// before its butterfly, so that their latency hides behind it.  KEYED: line c carries the XOR key 8 (c & 15) (column tiles).
+template <int LN, int LL, int R, bool INV, int SRC, int DST, bool KEYED>
+__device__ __forceinline__ void stage(int n_lines, const float4* __restrict__ root, int tid, float2* __restrict__ g = nullptr,
+                                      const float2* __restrict__ T = nullptr, int tmode = 0, int64_t line0_global = 0, int ny_mask = 0) {
+  constexpr int LR = R == 8 ? 3 : R == 4 ? 2 : 1;
+  constexpr int LSUB = LL - LR, SUB = 1 << LSUB, NV = 1 << (LN - LR), N = 1 << LN;
+  constexpr int NVT = NV < NT ? NV : NT, LSTEP = NT / NVT;
+  constexpr bool TW = R == 8 && LSUB > 0;
+  static_assert((SRC == IO_SMEM && DST == IO_SMEM) || LL == LN, "global access only in the stage on the whole line");
+  const float4* tw = root + tw_stage_off(LN, LL);
+  const int l0 = tid / NVT;
+  for (int v = tid % NVT; v < NV; v += NVT) {
+    const int blk = v >> LSUB, j = v & (SUB - 1);
+    const uint32_t i0 = ((uint32_t)blk << LL) + (uint32_t)j;
+    float4 w[8];
+    if (TW) {
+#pragma unroll
+      for (int m = 1; m < R; ++m) w[m] = __ldg(tw + ((m - 1) << LSUB) + j);
+    }
+    const uint32_t p0 = 8u * slot<LN>(i0);
+    for (int line = l0; line < n_lines; line += LSTEP) {
+      const uint32_t q = ((uint32_t)line * (8u * N) + p0) ^ (KEYED ? 8u * ((uint32_t)line & key_mask<LN>()) : 0u);
+      float2 x[8], t[8];
+      if (SRC == IO_GLOBAL || DST == IO_GLOBAL) {
+        if (tmode) {
+          const float2* tp = T + (((line0_global + line) & ny_mask) << LN) + i0;
+#pragma unroll
+          for (int k = 0; k < R; ++k) t[k] = __ldg(tp + (k << LSUB));
+        }
+      }
+      if (SRC == IO_GLOBAL) {
+        const float2* gp = g + (int64_t)line * N + i0;
+#pragma unroll
+        for (int k = 0; k < R; ++k) x[k] = gp[k << LSUB];
+        if (tmode) {
+#pragma unroll
+          for (int k = 0; k < R; ++k) x[k] = cmulf(x[k], make_float2(t[k].x, tmode == 2 ? -t[k].y : t[k].y));
+        }
+      } else {
+#pragma unroll
+        for (int k = 0; k < R; ++k) x[k] = lds2((q ^ xk<LN, LSUB>(k)) + ak<LN, LSUB>(k));
+      }
+      bfly<R, INV, TW>(x, w);
+      if (DST == IO_GLOBAL) {
+        float2* gp = g + (int64_t)line * N + i0;
+        if (tmode) {
+#pragma unroll
+          for (int k = 0; k < R; ++k) x[k] = cmulf(x[k], make_float2(t[k].x, tmode == 2 ? -t[k].y : t[k].y));
+        }
+#pragma unroll
+        for (int k = 0; k < R; ++k) gp[k << LSUB] = x[k];
+      } else {
+#pragma unroll
+        for (int k = 0; k < R; ++k) sts2((q ^ xk<LN, LSUB>(k)) + ak<LN, LSUB>(k), x[k]);
+      }
+    }
   }
 }
 
-// Pass 2: a tile of `cols` columns (consecutive stored x positions) x ny rows per block; forward along y, spectrum
-// multiply with the digit-reversed propagator table (conjugated when conj_p), inverse along y.
-__global__ void __launch_bounds__(256, 3) k_ms_cols(float2* __restrict__ S, const float4* __restrict__ Pperm, int conj_p, int lny, int nx, int lcols,
+// radix sequence of a length-2^LN transform: LN / 3 radix-8 stages on L = N, N/8, ..., then radix 4 or 2 on what is left
+template <int LN> struct Seq {
+  static constexpr int N8 = LN / 3, REM = LN % 3, NS = N8 + (REM ? 1 : 0);
+  static constexpr int RL = REM == 2 ? 4 : REM == 1 ? 2 : 8;         // radix of the last forward stage
+  static constexpr int LRL = REM ? REM : 3;                         // its block length (log2): L == R
+};
+
+// forward stages S .. LAST (0-based, inclusive) of every line of the tile, a block barrier after each
+template <int LN, bool KEYED, int S, int LAST>
+__device__ __forceinline__ void fwd_stages(int n_lines, const float4* __restrict__ root, int tid) {
+  if constexpr (S <= LAST) {
+    if constexpr (S < Seq<LN>::N8) stage<LN, LN - 3 * S, 8, false, IO_SMEM, IO_SMEM, KEYED>(n_lines, root, tid);
+    else stage<LN, Seq<LN>::LRL, Seq<LN>::RL, false, IO_SMEM, IO_SMEM, KEYED>(n_lines, root, tid);
+    __syncthreads();
+    fwd_stages<LN, KEYED, S + 1, LAST>(n_lines, root, tid);
+  }
+}
+// inverse stages S, S - 1, ..., FIRST (the forward stages backwards)
+template <int LN, bool KEYED, int S, int FIRST>
+__device__ __forceinline__ void inv_stages(int n_lines, const float4* __restrict__ root, int tid) {
+  if constexpr (S >= FIRST) {
+    if constexpr (S < Seq<LN>::N8) stage<LN, LN - 3 * S, 8, true, IO_SMEM, IO_SMEM, KEYED>(n_lines, root, tid);
+    else stage<LN, Seq<LN>::LRL, Seq<LN>::RL, true, IO_SMEM, IO_SMEM, KEYED>(n_lines, root, tid);
+    __syncthreads();
+    inv_stages<LN, KEYED, S - 1, FIRST>(n_lines, root, tid);
+  }
+}
+
+// Passes 1 and 3: a block takes LINES = TILE_EL / nx consecutive rows of the flat [n_cols * ny][nx] array (rows of
+// consecutive columns are consecutive in memory).  Forward: the first stage reads global memory (x pre, coalesced: its
+// butterflies stride over the whole row) and the digit-reversed result leaves through a coalesced copy; inverse: an
+// asynchronous coalesced copy comes first and the last stage (x post) writes global memory.
+// tmode: 0 none, 1 multiply by T, 2 by conj T.
+template <int LN, bool INV>
+__global__ void __launch_bounds__(NT, 3) k_ms_rows(float2* __restrict__ S, const float2* __restrict__ T, int tmode, int64_t n_lines_total,
+                                                  int ny_mask, const float4* __restrict__ rootx) {
+  constexpr int N = 1 << LN, LINES = TILE_EL / N, NS = Seq<LN>::NS;
+  const int tid = threadIdx.x;
+  const int64_t line0 = (int64_t)blockIdx.x * LINES;
+  const int n_lines = (int)min((int64_t)LINES, n_lines_total - line0);
+  float2* g = S + line0 * N;
+  const int n_el = n_lines << LN;
+  // flat copy: element e of the tile at slot e ^ g(e); g depends on bits 4-6 of e only, i.e. on tid (NT is a multiple of 128)
+  const uint32_t c0 = 8u * ((uint32_t)tid ^ swz_g<LN>((uint32_t)tid));
+  if (!INV) {
+    stage<LN, LN, 8, false, IO_GLOBAL, IO_SMEM, false>(n_lines, rootx, tid, g, T, tmode, line0, ny_mask);
+    __syncthreads();
+    fwd_stages<LN, false, 1, NS - 1>(n_lines, rootx, tid);
+#pragma unroll 8
+    for (int e = tid; e < n_el; e += NT) g[e] = lds2(c0 + 8u * (uint32_t)(e - tid));
+  } else {
+#pragma unroll 8
+    for (int e = tid; e < n_el; e += NT) cp_async8(c0 + 8u * (uint32_t)(e - tid), g + e);
+    cp_async_wait_all();
+    __syncthreads();
+    inv_stages<LN, false, NS - 1, 1>(n_lines, rootx, tid);
+    stage<LN, LN, 8, true, IO_SMEM, IO_GLOBAL, false>(n_lines, rootx, tid, g, T, tmode, line0, ny_mask);
+  }
+}
+
+// slot of row y of column c of a column tile (line c, key c & 15), in bytes
+template <int LN> __device__ __forceinline__ uint32_t col_off(uint32_t c, uint32_t y) {
+  return c * (8u << LN) + 8u * (slot<LN>(y) ^ (c & key_mask<LN>()));
+}
+
+// Pass 2: a tile of COLS = 2^LC columns (consecutive stored x positions) x ny rows per block.  Asynchronous coalesced copy
+// in (lanes run over the columns), forward stages along y, then ONE stage that does the last forward butterfly, the spectrum
+// multiply with the digit-reversed propagator table (conjugated when conj_p) and the first inverse butterfly in registers
+// -- both work on the same R consecutive elements -- with the lanes over the columns, so that the propagator reads are
+// coalesced (and requested before the shared-memory loads, so that the butterfly hides them); inverse stages, coalesced
+// copy out.  LCT >= 0: the tile width is the compile-time 2^LCT (TILE_EL / ny columns: every grid with ny nx >= TILE_EL);
+// LCT < 0: run-time width 2^lc_rt (small grids).
+template <int LN, int LCT>
+__global__ void __launch_bounds__(NT, 3) k_ms_cols(float2* __restrict__ S, const float4* __restrict__ Pperm, int conj_p, int nx, int lc_rt,
                                                   const float4* __restrict__ rooty) {
-  extern __shared__ float2 sm_cols[];
-  const int ny = 1 << lny, cols = 1 << lcols;
-  const int64_t G = (int64_t)ny * nx;
-  float2* col = S + (int64_t)blockIdx.y * G;
-  const int x0 = blockIdx.x << lcols;
-  const int pitch = pad_len(ny) + 1;
-  const int tid = threadIdx.x, nthr = blockDim.x;
-  for (int i = tid; i < (ny << lcols); i += nthr) {
-    const int y = i >> lcols, c = i & (cols - 1);
-    sm_cols[c * pitch + pad_idx(y)] = col[(int64_t)y * nx + x0 + c];
+  constexpr int N = 1 << LN, NS = Seq<LN>::NS, RL = Seq<LN>::RL;
+  const int tid = threadIdx.x, lc = LCT >= 0 ? LCT : lc_rt, cols = 1 << lc;
+  float2* col = S + (int64_t)blockIdx.y * N * nx + ((int64_t)blockIdx.x << lc);
+  const int n_el = N << lc;
+  if (cols <= NT) {
+    const uint32_t c = (uint32_t)tid & (uint32_t)(cols - 1), yy = (uint32_t)tid >> lc, ystep = (uint32_t)NT >> lc;
+    const float2* src = col + (int64_t)yy * nx + c;
+#pragma unroll 8
+    for (uint32_t y = yy; y < (uint32_t)N; y += ystep, src += (int64_t)ystep * nx) cp_async8(col_off<LN>(c, y), src);
+  } else {                                   // more columns than threads (short columns of a small grid)
+    for (int i = tid; i < n_el; i += NT) cp_async8(col_off<LN>((uint32_t)i & (uint32_t)(cols - 1), (uint32_t)i >> lc), col + (int64_t)(i >> lc) * nx + (i & (cols - 1)));
+  }
+  cp_async_wait_all();
+  __syncthreads();
+  fwd_stages<LN, true, 0, NS - 2>(cols, rooty, tid);
+  {
+    const float4 w[8] = {};
+    const uint32_t n_b = ((uint32_t)N / RL) << lc;                     // butterflies of the tile, lanes over the columns first
+    const float4* Pc = Pperm + ((int64_t)blockIdx.x << lc);
+    for (uint32_t u = (uint32_t)tid; u < n_b; u += NT) {
+      const uint32_t cc = u & (uint32_t)(cols - 1), b = u >> lc;
+      const uint32_t q = col_off<LN>(cc, b * RL);
+      const float4* pp = Pc + (int64_t)(b * RL) * nx + cc;
+      float4 p[8];
+#pragma unroll
+      for (int k = 0; k < RL; ++k) p[k] = __ldg(pp + (int64_t)k * nx);
+      float2 x[8];
+#pragma unroll
+      for (int k = 0; k < RL; ++k) x[k] = lds2(q ^ (8u * k));
+      bfly<RL, false, false>(x, w);
+#pragma unroll
+      for (int k = 0; k < RL; ++k) x[k] = conj_p ? cmulc_dd(x[k], p[k]) : cmul_dd(x[k], p[k]);
+      bfly<RL, true, false>(x, w);
+#pragma unroll
+      for (int k = 0; k < RL; ++k) sts2(q ^ (8u * k), x[k]);
+    }
   }
   __syncthreads();
-  fft_lines<false>(sm_cols, lny, cols, pitch, rooty, tid, nthr);
-  for (int i = tid; i < (ny << lcols); i += nthr) {
-    const int y = i >> lcols, c = i & (cols - 1);
-    const float4 p = __ldg(Pperm + (int64_t)y * nx + x0 + c);
-    float2* e = sm_cols + c * pitch + pad_idx(y);
-    *e = conj_p ? cmulc_dd(*e, p) : cmul_dd(*e, p);
-  }
-  __syncthreads();
-  fft_lines<true>(sm_cols, lny, cols, pitch, rooty, tid, nthr);
-  for (int i = tid; i < (ny << lcols); i += nthr) {
-    const int y = i >> lcols, c = i & (cols - 1);
-    col[(int64_t)y * nx + x0 + c] = sm_cols[c * pitch + pad_idx(y)];
+  inv_stages<LN, true, NS - 2, 0>(cols, rooty, tid);
+  if (cols <= NT) {
+    const uint32_t c = (uint32_t)tid & (uint32_t)(cols - 1), yy = (uint32_t)tid >> lc, ystep = (uint32_t)NT >> lc;
+    float2* dst = col + (int64_t)yy * nx + c;
+#pragma unroll 8
+    for (uint32_t y = yy; y < (uint32_t)N; y += ystep, dst += (int64_t)ystep * nx) *dst = lds2(col_off<LN>(c, y));
+  } else {
+    for (int i = tid; i < n_el; i += NT) col[(int64_t)(i >> lc) * nx + (i & (cols - 1))] = lds2(col_off<LN>((uint32_t)i & (uint32_t)(cols - 1), (uint32_t)i >> lc));
   }
 }
 
@@ -102,46 +289,68 @@ __global__ void __launch_bounds__(256, 3) k_ms_cols(float2* __restrict__ S, cons
 //     out[rho][ky][kx] += sum_n |F psi_n|^2 / G
 // at the TRUE frequency (ky, kx) of the stored position (permy / permx undo the digit reversal).  A block owns the
 // (all y, its x tile) outputs of its scan position, so the read-modify-write needs no atomics.
-__global__ void __launch_bounds__(256, 2) k_ms_cols_detect(const float2* __restrict__ F, int n_ch, float* __restrict__ out, float inv_G, int lny, int nx,
-                                                         int lcols, const float4* __restrict__ rooty, const int32_t* __restrict__ permy,
+template <int LN>
+__global__ void __launch_bounds__(NT, 2) k_ms_cols_detect(const float2* __restrict__ F, int n_ch, float* __restrict__ out, float inv_G, int nx, int lc,
+                                                         const float4* __restrict__ rooty, const int32_t* __restrict__ permy,
                                                          const int32_t* __restrict__ permx) {
-  extern __shared__ float2 sm_det[];
-  const int ny = 1 << lny, cols = 1 << lcols;
-  const int64_t G = (int64_t)ny * nx;
-  const int x0 = blockIdx.x << lcols, rho = blockIdx.y;
-  const int pitch = pad_len(ny) + 1;
-  float* acc = reinterpret_cast<float*>(sm_det + (size_t)cols * pitch);       // [ny * cols], element i of the tile loop
-  const int tid = threadIdx.x, nthr = blockDim.x;
-  for (int i = tid; i < (ny << lcols); i += nthr) acc[i] = 0.f;
+  constexpr int N = 1 << LN, NS = Seq<LN>::NS;
+  const int tid = threadIdx.x, cols = 1 << lc;
+  const int64_t G = (int64_t)N * nx;
+  const int x0 = blockIdx.x << lc, rho = blockIdx.y;
+  float* acc = reinterpret_cast<float*>(sm + (size_t)TILE_EL * sizeof(float2));       // [N * cols], element i of the tile loop
+  const int n_el = N << lc;
+  for (int i = tid; i < n_el; i += NT) acc[i] = 0.f;
   for (int n = 0; n < n_ch; ++n) {
-    const float2* col = F + ((int64_t)rho * n_ch + n) * G;
+    const float2* col = F + ((int64_t)rho * n_ch + n) * G + x0;
     __syncthreads();
-    for (int i = tid; i < (ny << lcols); i += nthr) {
-      const int y = i >> lcols, c = i & (cols - 1);
-      sm_det[c * pitch + pad_idx(y)] = col[(int64_t)y * nx + x0 + c];
+#pragma unroll 8
+    for (int i = tid; i < n_el; i += NT) {
+      const uint32_t y = (uint32_t)i >> lc, c = (uint32_t)i & (uint32_t)(cols - 1);
+      cp_async8(col_off<LN>(c, y), col + (int64_t)y * nx + c);
     }
+    cp_async_wait_all();
     __syncthreads();
-    fft_lines<false>(sm_det, lny, cols, pitch, rooty, tid, nthr);
-    for (int i = tid; i < (ny << lcols); i += nthr) {
-      const int y = i >> lcols, c = i & (cols - 1);
-      const float2 v = sm_det[c * pitch + pad_idx(y)];
+    fwd_stages<LN, true, 0, NS - 1>(cols, rooty, tid);
+    for (int i = tid; i < n_el; i += NT) {
+      const uint32_t y = (uint32_t)i >> lc, c = (uint32_t)i & (uint32_t)(cols - 1);
+      const float2 v = lds2(col_off<LN>(c, y));
       acc[i] += v.x * v.x + v.y * v.y;
     }
   }
   float* o = out + (int64_t)rho * G;
-  for (int i = tid; i < (ny << lcols); i += nthr) {
-    const int y = i >> lcols, c = i & (cols - 1);
+  for (int i = tid; i < n_el; i += NT) {
+    const int y = i >> lc, c = i & (cols - 1);
     const int64_t k = (int64_t)__ldg(permy + y) * nx + __ldg(permx + x0 + c);
     o[k] += acc[i] * inv_G;
   }
 }
 
-// threads per block: a power of two, a quarter of the butterflies of a stage (lines * N / 8), within 64 .. 256
-int fft_threads(int lines, int n) {
-  const int reuse = std::max(1, tune_int("BIP_TUNE_FFT_REUSE", 4));
-  int t = 64;
-  while (t < 256 && t * reuse < lines * n / 8) t <<= 1;
-  return t;
+// ---- dispatch on the (power-of-two) transform length ----
+#define BIP_FFT_SWITCH(ln, CALL)                                                                                        \
+  switch (ln) {                                                                                                         \
+    case 3: { constexpr int LN_ = 3; CALL; } break;   case 4: { constexpr int LN_ = 4; CALL; } break;                     \
+    case 5: { constexpr int LN_ = 5; CALL; } break;   case 6: { constexpr int LN_ = 6; CALL; } break;                     \
+    case 7: { constexpr int LN_ = 7; CALL; } break;   case 8: { constexpr int LN_ = 8; CALL; } break;                     \
+    case 9: { constexpr int LN_ = 9; CALL; } break;   case 10: { constexpr int LN_ = 10; CALL; } break;                   \
+    case 11: { constexpr int LN_ = 11; CALL; } break; case 12: { constexpr int LN_ = 12; CALL; } break;                   \
+    default: return fail(ctx, BIP_ERR_UNSUPPORTED, "native FFT: length 2^%d outside 8 .. 4096", ln);                    \
+  }
+
+template <int LN> int32_t set_attrs(bip_ctx* ctx) {
+  const int bytes = (int)tile_smem_bytes();
+  BIP_CUDA(ctx, cudaFuncSetAttribute(k_ms_rows<LN, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  BIP_CUDA(ctx, cudaFuncSetAttribute(k_ms_rows<LN, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  BIP_CUDA(ctx, cudaFuncSetAttribute(k_ms_cols<LN, 13 - LN>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  BIP_CUDA(ctx, cudaFuncSetAttribute(k_ms_cols<LN, -1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  BIP_CUDA(ctx, cudaFuncSetAttribute(k_ms_cols_detect<LN>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes + TILE_EL * (int)sizeof(float)));
+  return BIP_OK;
+}
+
+template <int LN, bool INV>
+void launch_rows(bip_ctx* ctx, float2* S, const float2* T, int tmode, int64_t n_lines_total, int ny) {
+  constexpr int LINES = TILE_EL >> LN;
+  const int64_t blocks = (n_lines_total + LINES - 1) / LINES;
+  k_ms_rows<LN, INV><<<(unsigned)blocks, NT, tile_smem_bytes(), ctx->stream>>>(S, T, tmode, n_lines_total, ny - 1, ctx->fft_rootx);
 }
 
 }  // namespace
@@ -180,56 +389,52 @@ int32_t fft_init(bip_ctx* ctx) {
   BIP_CUDA(ctx, cudaMemcpyAsync(ctx->fft_permy, py.data(), sizeof(int32_t) * ny, cudaMemcpyHostToDevice, ctx->stream));
   BIP_CUDA(ctx, cudaMemcpyAsync(ctx->fft_permx, px.data(), sizeof(int32_t) * nx, cudaMemcpyHostToDevice, ctx->stream));
   BIP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-  // launch shapes: ~64 KB of rows or columns per block (at least 4 columns: whole 32-byte sectors), and a quarter as many
-  // threads as butterflies per stage, so that every thread re-uses its twiddles over 4 lines (fft_stage)
-  ctx->fft_lines = std::max(1, std::min(ny, tune_int("BIP_TUNE_FFT_ROW_EL", 8192) / nx));
-  ctx->fft_cols = std::max(tune_int("BIP_TUNE_FFT_MINCOLS", 4), std::min(nx, tune_int("BIP_TUNE_FFT_COL_EL", 8192) / ny));
-  BIP_CUDA(ctx, cudaFuncSetAttribute(k_ms_rows<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_rows_bytes(ctx->fft_lines, nx)));
-  BIP_CUDA(ctx, cudaFuncSetAttribute(k_ms_rows<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_rows_bytes(ctx->fft_lines, nx)));
-  const size_t smem_cols = smem_cols_bytes(ctx->fft_cols, ny);
-  BIP_CUDA(ctx, cudaFuncSetAttribute(k_ms_cols, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cols));
-  BIP_CUDA(ctx, cudaFuncSetAttribute(k_ms_cols_detect, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(smem_cols + (size_t)ctx->fft_cols * ny * sizeof(float))));
+  // launch shapes: tiles of TILE_EL elements (64 KB): TILE_EL / nx rows per block in the row passes, min(nx, TILE_EL / ny)
+  // columns per block in the column pass
+  const int lnx = ilog2(nx), lny = ilog2(ny);
+  ctx->fft_lines = TILE_EL / nx;
+  ctx->fft_cols = std::min(nx, TILE_EL / ny);
+  BIP_FFT_SWITCH(lnx, BIP_TRY(set_attrs<LN_>(ctx)));
+  if (lny != lnx) BIP_FFT_SWITCH(lny, BIP_TRY(set_attrs<LN_>(ctx)));
   return BIP_OK;
 }
 
 // S <- post . F^-1[ P . F[ pre . S ] ] on n_cols columns (modes as in bip_multislice.cu: 0 = 1, 1 = T_j, 2 = conj T_j)
 int32_t fft_slice_op(bip_ctx* ctx, float2* S, int n_cols, const float2* Tj, int pre, int conj_p, int post) {
   const int ny = ctx->g.ny, nx = ctx->g.nx;
-  const int lines = ctx->fft_lines, cols = ctx->fft_cols;
-  const int thr_rows = fft_threads(lines, nx), thr_cols = fft_threads(cols, ny);
-  const size_t smem_rows = smem_rows_bytes(lines, nx), smem_cols = smem_cols_bytes(cols, ny);
-  const int lnx = ilog2(nx), lny = ilog2(ny), lcols = ilog2(cols);
+  const int lnx = ilog2(nx), lny = ilog2(ny), lc = ilog2(ctx->fft_cols);
+  const int64_t n_lines = (int64_t)n_cols * ny;
+  BIP_FFT_SWITCH(lnx, (launch_rows<LN_, false>(ctx, S, Tj, pre, n_lines, ny)));
   for (int c0 = 0; c0 < n_cols; c0 += 65535) {                // gridDim.y limit
     const int nc = std::min(65535, n_cols - c0);
     float2* Sc = S + (int64_t)c0 * ny * nx;
-    k_ms_rows<false><<<dim3((unsigned)((ny + lines - 1) / lines), (unsigned)nc), thr_rows, smem_rows, ctx->stream>>>(Sc, Tj, pre, ny, lnx, lines, ctx->fft_rootx);
-    k_ms_cols<<<dim3((unsigned)(nx / cols), (unsigned)nc), thr_cols, smem_cols, ctx->stream>>>(Sc, ctx->fft_P, conj_p, lny, nx, lcols, ctx->fft_rooty);
-    k_ms_rows<true><<<dim3((unsigned)((ny + lines - 1) / lines), (unsigned)nc), thr_rows, smem_rows, ctx->stream>>>(Sc, Tj, post, ny, lnx, lines, ctx->fft_rootx);
-    BIP_CUDA(ctx, cudaGetLastError());
+    const dim3 grid((unsigned)(nx >> lc), (unsigned)nc);
+    if (lc == 13 - lny) {         // the compile-time tile width (every grid with ny nx >= TILE_EL)
+      BIP_FFT_SWITCH(lny, (k_ms_cols<LN_, 13 - LN_><<<grid, NT, tile_smem_bytes(), ctx->stream>>>(Sc, ctx->fft_P, conj_p, nx, lc, ctx->fft_rooty)));
+    } else {
+      BIP_FFT_SWITCH(lny, (k_ms_cols<LN_, -1><<<grid, NT, tile_smem_bytes(), ctx->stream>>>(Sc, ctx->fft_P, conj_p, nx, lc, ctx->fft_rooty)));
+    }
   }
+  BIP_FFT_SWITCH(lnx, (launch_rows<LN_, true>(ctx, S, Tj, post, n_lines, ny)));
+  BIP_CUDA(ctx, cudaGetLastError());
   return BIP_OK;
 }
 
 // out[rho][ky][kx] += sum_n |F fields[rho][n]|^2 / G for n_rho scan positions x n_ch channel fields (destroys the fields)
 int32_t fft_detect(bip_ctx* ctx, float2* fields, int n_rho, int n_ch, float* out) {
   const int ny = ctx->g.ny, nx = ctx->g.nx;
-  const int lines = ctx->fft_lines, cols = ctx->fft_cols;
-  const int thr_rows = fft_threads(lines, nx), thr_cols = fft_threads(cols, ny);
-  const size_t smem_rows = smem_rows_bytes(lines, nx);
-  const size_t smem_det = smem_cols_bytes(cols, ny) + (size_t)cols * ny * sizeof(float);
-  const int lnx = ilog2(nx), lny = ilog2(ny), lcols = ilog2(cols);
+  const int lnx = ilog2(nx), lny = ilog2(ny), lc = ilog2(ctx->fft_cols);
   const int64_t G = (int64_t)ny * nx;
-  for (int r0 = 0; r0 < n_rho; r0 += 4096) {                  // gridDim.y limit (n_ch fields per scan position)
-    const int nr = std::min(4096, n_rho - r0);
-    float2* Fc = fields + (int64_t)r0 * n_ch * G;
-    for (int f0 = 0; f0 < nr * n_ch; f0 += 65535) {
-      const int nf = std::min(65535, nr * n_ch - f0);
-      k_ms_rows<false><<<dim3((unsigned)((ny + lines - 1) / lines), (unsigned)nf), thr_rows, smem_rows, ctx->stream>>>(Fc + (int64_t)f0 * G, nullptr, 0, ny, lnx, lines, ctx->fft_rootx);
-    }
-    k_ms_cols_detect<<<dim3((unsigned)(nx / cols), (unsigned)nr), thr_cols, smem_det, ctx->stream>>>(Fc, n_ch, out + (int64_t)r0 * G, (float)(1.0 / (double)G), lny, nx, lcols,
-                                                                                                   ctx->fft_rooty, ctx->fft_permy, ctx->fft_permx);
-    BIP_CUDA(ctx, cudaGetLastError());
+  BIP_FFT_SWITCH(lnx, (launch_rows<LN_, false>(ctx, fields, nullptr, 0, (int64_t)n_rho * n_ch * ny, ny)));
+  const size_t smem_det = tile_smem_bytes() + (size_t)TILE_EL * sizeof(float);
+  for (int r0 = 0; r0 < n_rho; r0 += 65535) {                 // gridDim.y limit
+    const int nr = std::min(65535, n_rho - r0);
+    const dim3 grid((unsigned)(nx >> lc), (unsigned)nr);
+    BIP_FFT_SWITCH(lny, (k_ms_cols_detect<LN_><<<grid, NT, smem_det, ctx->stream>>>(fields + (int64_t)r0 * n_ch * G, n_ch, out + (int64_t)r0 * G,
+                                                                                   (float)(1.0 / (double)G), nx, lc, ctx->fft_rooty,
+                                                                                   ctx->fft_permy, ctx->fft_permx)));
   }
+  BIP_CUDA(ctx, cudaGetLastError());
   return BIP_OK;
 }
 

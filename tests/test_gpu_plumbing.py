@@ -47,6 +47,38 @@ def test_native_slice_step_matches_oracle(name, scale, nz):
     ctx.close()
 
 
+@pytest.mark.parametrize("ny,nx", [(8, 8), (16, 64), (32, 8), (64, 256), (128, 32), (256, 1024), (1024, 64), (2048, 16), (16, 4096)])
+def test_native_slice_step_on_every_transform_length(ny, nx):
+    """Every compile-time transform length of the native route (8 ... 4096 along either axis, all three radix tails, row
+    tiles that span several columns, column tiles wider than a block) on a random-phase slab: S1 and S2 parents at two
+    planes against the oracle's fp64 multislice (eq. 6, eq. 12)."""
+    import paper_2607_00756_b200 as B
+    from bip_inputs.specimen import tiny_random_workload
+    wl = tiny_random_workload(11, ny=ny, nx=nx, nz=3, W=8, n_atoms=2, n_scan=2)
+    # a few dozen beams whatever the shape of the grid, all of them below the Nyquist index of both axes
+    q = min(np.sqrt(40.0 / (np.pi * wl.ly * wl.lx)), 0.9 * (ny / 2 - 1) / wl.ly, 0.9 * (nx / 2 - 1) / wl.lx)
+    wl.alpha_mrad = 1e3 * wl.lam * q
+    e = wl.edges[0]
+    e.det_mrad = 1.2 * wl.alpha_mrad
+    ctx, geo, ids = gpu_context(wl, [e], parent_factor=(1, 1))
+    ctx.set_fft_backend(B.FFT_NATIVE)
+    ctx.build_S1(); ctx.build_S2()
+    orc = OracleSetup(wl, e, parent_factor=(1, 1))
+    T = wl.T.astype(np.complex128)
+    S1 = oms.build_S1(orc.ap[orc.p1_pos], ny, nx)
+    S2 = oms.build_S2(orc.det[orc.p2_pos], T, orc.P)
+    want = {0: (S1, S2)}
+    for i in range(wl.nz):
+        S1 = oms.advance_S1(S1, T[i], orc.P)
+        S2 = oms.peel_S2(S2, T[i], orc.P)
+        want[i + 1] = (S1, S2)
+    for plane in (0, 3, 1):
+        ctx.seek_plane(plane)
+        assert np.abs(ctx.copy_S(1, 0, ctx.n_p1) - want[plane][0]).max() < 2e-5, plane
+        assert np.abs(ctx.copy_S(2, 0, ctx.n_p2) - want[plane][1]).max() < 2e-5, plane
+    ctx.close()
+
+
 def test_native_route_is_refused_on_a_grid_that_is_not_a_power_of_two():
     import paper_2607_00756_b200 as B
     from bip_inputs.specimen import tiny_random_workload
