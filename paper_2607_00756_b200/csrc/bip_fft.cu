@@ -57,8 +57,15 @@ template <int LN> __host__ __device__ constexpr uint32_t swz_g(uint32_t i) {
          (LN > 6 ? ((i >> 6) & 1u) * Swz<LN>::M6 : 0u);
 }
 template <int LN> __host__ __device__ constexpr uint32_t slot(uint32_t i) { return i ^ swz_g<LN>(i); }
-// XOR key of line c of a column tile (a line shorter than 16 elements keeps the key inside the line)
+// XOR key (4 bits) of line c of a column tile 2^lc columns wide.  16 or more columns: c & 15 -- the 16 lanes of a half-warp
+// that run over 16 columns at one row hit 16 different slots.  Narrower tiles (long columns): a half-warp covers 2^lc
+// columns x 2^(4-lc) consecutive rows (copies) or consecutive final-stage butterflies (the fused stage), whose row bits sit
+// at the bottom resp. just above the butterfly's own bits; c is therefore XORed in twice, shifted above the row bits and
+// unshifted, which keeps both patterns conflict-free.  A line shorter than 16 elements keeps the key inside the line.
 template <int LN> __host__ __device__ constexpr uint32_t key_mask() { return LN >= 4 ? 15u : (1u << LN) - 1u; }
+template <int LN> __host__ __device__ constexpr uint32_t line_key(uint32_t c, int lc) {
+  return (lc >= 4 ? c : ((c << (4 - lc)) | (c & ((1u << (4 - lc)) - 1u)))) & key_mask<LN>();
+}
 
 // the tile: dynamic shared memory, always addressed as sm + offset so that every access is an LDS / STS with an
 // immediate offset (its start is 1024-byte aligned: the bank of an offset is the bank of the address)
@@ -103,7 +110,7 @@ enum { IO_SMEM = 0, IO_GLOBAL = 1 };
 // stage whose butterflies stride over the whole row (unit stride across the lanes).  The T values of a line are requested
 // before its butterfly, so that their latency hides behind it.  KEYED: line c carries the XOR key 8 (c & 15) (column tiles).
 template <int LN, int LL, int R, bool INV, int SRC, int DST, bool KEYED>
-__device__ __forceinline__ void stage(int n_lines, const float4* __restrict__ root, int tid, float2* __restrict__ g = nullptr,
+__device__ __forceinline__ void stage(int n_lines, int lc, const float4* __restrict__ root, int tid, float2* __restrict__ g = nullptr,
                                       const float2* __restrict__ T = nullptr, int tmode = 0, int64_t line0_global = 0, int ny_mask = 0) {
   constexpr int LR = R == 8 ? 3 : R == 4 ? 2 : 1;
   constexpr int LSUB = LL - LR, SUB = 1 << LSUB, NV = 1 << (LN - LR), N = 1 << LN;
@@ -122,7 +129,7 @@ __device__ __forceinline__ void stage(int n_lines, const float4* __restrict__ ro
     }
     const uint32_t p0 = 8u * slot<LN>(i0);
     for (int line = l0; line < n_lines; line += LSTEP) {
-      const uint32_t q = ((uint32_t)line * (8u * N) + p0) ^ (KEYED ? 8u * ((uint32_t)line & key_mask<LN>()) : 0u);
+      const uint32_t q = ((uint32_t)line * (8u * N) + p0) ^ (KEYED ? 8u * line_key<LN>((uint32_t)line, lc) : 0u);
       float2 x[8], t[8];
       if (SRC == IO_GLOBAL || DST == IO_GLOBAL) {
         if (tmode) {
@@ -169,22 +176,22 @@ template <int LN> struct Seq {
 
 // forward stages S .. LAST (0-based, inclusive) of every line of the tile, a block barrier after each
 template <int LN, bool KEYED, int S, int LAST>
-__device__ __forceinline__ void fwd_stages(int n_lines, const float4* __restrict__ root, int tid) {
+__device__ __forceinline__ void fwd_stages(int n_lines, int lc, const float4* __restrict__ root, int tid) {
   if constexpr (S <= LAST) {
-    if constexpr (S < Seq<LN>::N8) stage<LN, LN - 3 * S, 8, false, IO_SMEM, IO_SMEM, KEYED>(n_lines, root, tid);
-    else stage<LN, Seq<LN>::LRL, Seq<LN>::RL, false, IO_SMEM, IO_SMEM, KEYED>(n_lines, root, tid);
+    if constexpr (S < Seq<LN>::N8) stage<LN, LN - 3 * S, 8, false, IO_SMEM, IO_SMEM, KEYED>(n_lines, lc, root, tid);
+    else stage<LN, Seq<LN>::LRL, Seq<LN>::RL, false, IO_SMEM, IO_SMEM, KEYED>(n_lines, lc, root, tid);
     __syncthreads();
-    fwd_stages<LN, KEYED, S + 1, LAST>(n_lines, root, tid);
+    fwd_stages<LN, KEYED, S + 1, LAST>(n_lines, lc, root, tid);
   }
 }
 // inverse stages S, S - 1, ..., FIRST (the forward stages backwards)
 template <int LN, bool KEYED, int S, int FIRST>
-__device__ __forceinline__ void inv_stages(int n_lines, const float4* __restrict__ root, int tid) {
+__device__ __forceinline__ void inv_stages(int n_lines, int lc, const float4* __restrict__ root, int tid) {
   if constexpr (S >= FIRST) {
-    if constexpr (S < Seq<LN>::N8) stage<LN, LN - 3 * S, 8, true, IO_SMEM, IO_SMEM, KEYED>(n_lines, root, tid);
-    else stage<LN, Seq<LN>::LRL, Seq<LN>::RL, true, IO_SMEM, IO_SMEM, KEYED>(n_lines, root, tid);
+    if constexpr (S < Seq<LN>::N8) stage<LN, LN - 3 * S, 8, true, IO_SMEM, IO_SMEM, KEYED>(n_lines, lc, root, tid);
+    else stage<LN, Seq<LN>::LRL, Seq<LN>::RL, true, IO_SMEM, IO_SMEM, KEYED>(n_lines, lc, root, tid);
     __syncthreads();
-    inv_stages<LN, KEYED, S - 1, FIRST>(n_lines, root, tid);
+    inv_stages<LN, KEYED, S - 1, FIRST>(n_lines, lc, root, tid);
   }
 }
 
@@ -205,9 +212,9 @@ __global__ void __launch_bounds__(NT, 3) k_ms_rows(float2* __restrict__ S, const
   // flat copy: element e of the tile at slot e ^ g(e); g depends on bits 4-6 of e only, i.e. on tid (NT is a multiple of 128)
   const uint32_t c0 = 8u * ((uint32_t)tid ^ swz_g<LN>((uint32_t)tid));
   if (!INV) {
-    stage<LN, LN, 8, false, IO_GLOBAL, IO_SMEM, false>(n_lines, rootx, tid, g, T, tmode, line0, ny_mask);
+    stage<LN, LN, 8, false, IO_GLOBAL, IO_SMEM, false>(n_lines, 0, rootx, tid, g, T, tmode, line0, ny_mask);
     __syncthreads();
-    fwd_stages<LN, false, 1, NS - 1>(n_lines, rootx, tid);
+    fwd_stages<LN, false, 1, NS - 1>(n_lines, 0, rootx, tid);
 #pragma unroll 8
     for (int e = tid; e < n_el; e += NT) g[e] = lds2(c0 + 8u * (uint32_t)(e - tid));
   } else {
@@ -215,26 +222,27 @@ __global__ void __launch_bounds__(NT, 3) k_ms_rows(float2* __restrict__ S, const
     for (int e = tid; e < n_el; e += NT) cp_async8(c0 + 8u * (uint32_t)(e - tid), g + e);
     cp_async_wait_all();
     __syncthreads();
-    inv_stages<LN, false, NS - 1, 1>(n_lines, rootx, tid);
-    stage<LN, LN, 8, true, IO_SMEM, IO_GLOBAL, false>(n_lines, rootx, tid, g, T, tmode, line0, ny_mask);
+    inv_stages<LN, false, NS - 1, 1>(n_lines, 0, rootx, tid);
+    stage<LN, LN, 8, true, IO_SMEM, IO_GLOBAL, false>(n_lines, 0, rootx, tid, g, T, tmode, line0, ny_mask);
   }
 }
 
 // slot of row y of column c of a column tile (line c, key c & 15), in bytes
-template <int LN> __device__ __forceinline__ uint32_t col_off(uint32_t c, uint32_t y) {
-  return c * (8u << LN) + 8u * (slot<LN>(y) ^ (c & key_mask<LN>()));
+template <int LN> __device__ __forceinline__ uint32_t col_off(uint32_t c, uint32_t y, int lc) {
+  return c * (8u << LN) + 8u * (slot<LN>(y) ^ line_key<LN>(c, lc));
 }
 
 // Pass 2: a tile of COLS = 2^LC columns (consecutive stored x positions) x ny rows per block.  Asynchronous coalesced copy
 // in (lanes run over the columns), forward stages along y, then ONE stage that does the last forward butterfly, the spectrum
-// multiply with the digit-reversed propagator table (conjugated when conj_p) and the first inverse butterfly in registers
-// -- both work on the same R consecutive elements -- with the lanes over the columns, so that the propagator reads are
-// coalesced (and requested before the shared-memory loads, so that the butterfly hides them); inverse stages, coalesced
-// copy out.  LCT >= 0: the tile width is the compile-time 2^LCT (TILE_EL / ny columns: every grid with ny nx >= TILE_EL);
+// multiply and the first inverse butterfly in registers -- both butterflies work on the same R consecutive elements.  The
+// propagator is separable, P(q) / G = Ey[qy] Ex[qx] (eq. 2: the phase is a sum of a qy^2 and a qx^2 term): two 1-D tables in
+// the digit-reversed order of their axis, conjugated when conj_p, instead of a G-entry table that falls out of L2 on a
+// 2048^2 grid (64 MB, re-read from DRAM by every column: measured 3 x the DRAM reads of the pass).  Inverse stages,
+// coalesced copy out.  LCT >= 0: the tile width is the compile-time 2^LCT (TILE_EL / ny columns: every grid with ny nx >= TILE_EL);
 // LCT < 0: run-time width 2^lc_rt (small grids).
 template <int LN, int LCT>
-__global__ void __launch_bounds__(NT, 3) k_ms_cols(float2* __restrict__ S, const float4* __restrict__ Pperm, int conj_p, int nx, int lc_rt,
-                                                  const float4* __restrict__ rooty) {
+__global__ void __launch_bounds__(NT, 3) k_ms_cols(float2* __restrict__ S, const float4* __restrict__ Ey, const float4* __restrict__ Ex, int conj_p, int nx,
+                                                  int lc_rt, const float4* __restrict__ rooty) {
   constexpr int N = 1 << LN, NS = Seq<LN>::NS, RL = Seq<LN>::RL;
   const int tid = threadIdx.x, lc = LCT >= 0 ? LCT : lc_rt, cols = 1 << lc;
   float2* col = S + (int64_t)blockIdx.y * N * nx + ((int64_t)blockIdx.x << lc);
@@ -243,44 +251,44 @@ __global__ void __launch_bounds__(NT, 3) k_ms_cols(float2* __restrict__ S, const
     const uint32_t c = (uint32_t)tid & (uint32_t)(cols - 1), yy = (uint32_t)tid >> lc, ystep = (uint32_t)NT >> lc;
     const float2* src = col + (int64_t)yy * nx + c;
 #pragma unroll 8
-    for (uint32_t y = yy; y < (uint32_t)N; y += ystep, src += (int64_t)ystep * nx) cp_async8(col_off<LN>(c, y), src);
+    for (uint32_t y = yy; y < (uint32_t)N; y += ystep, src += (int64_t)ystep * nx) cp_async8(col_off<LN>(c, y, lc), src);
   } else {                                   // more columns than threads (short columns of a small grid)
-    for (int i = tid; i < n_el; i += NT) cp_async8(col_off<LN>((uint32_t)i & (uint32_t)(cols - 1), (uint32_t)i >> lc), col + (int64_t)(i >> lc) * nx + (i & (cols - 1)));
+    for (int i = tid; i < n_el; i += NT) cp_async8(col_off<LN>((uint32_t)i & (uint32_t)(cols - 1), (uint32_t)i >> lc, lc), col + (int64_t)(i >> lc) * nx + (i & (cols - 1)));
   }
   cp_async_wait_all();
   __syncthreads();
-  fwd_stages<LN, true, 0, NS - 2>(cols, rooty, tid);
+  fwd_stages<LN, true, 0, NS - 2>(cols, lc, rooty, tid);
   {
     const float4 w[8] = {};
     const uint32_t n_b = ((uint32_t)N / RL) << lc;                     // butterflies of the tile, lanes over the columns first
-    const float4* Pc = Pperm + ((int64_t)blockIdx.x << lc);
+    const float4* ex = Ex + ((int64_t)blockIdx.x << lc);
     for (uint32_t u = (uint32_t)tid; u < n_b; u += NT) {
       const uint32_t cc = u & (uint32_t)(cols - 1), b = u >> lc;
-      const uint32_t q = col_off<LN>(cc, b * RL);
-      const float4* pp = Pc + (int64_t)(b * RL) * nx + cc;
-      float4 p[8];
+      const uint32_t q = col_off<LN>(cc, b * RL, lc);
+      const float4 px = __ldg(ex + cc);                                // a thread keeps its column when the tile is narrower than the block
+      float4 py[8];
 #pragma unroll
-      for (int k = 0; k < RL; ++k) p[k] = __ldg(pp + (int64_t)k * nx);
+      for (int k = 0; k < RL; ++k) py[k] = __ldg(Ey + b * RL + k);
       float2 x[8];
 #pragma unroll
       for (int k = 0; k < RL; ++k) x[k] = lds2(q ^ (8u * k));
       bfly<RL, false, false>(x, w);
 #pragma unroll
-      for (int k = 0; k < RL; ++k) x[k] = conj_p ? cmulc_dd(x[k], p[k]) : cmul_dd(x[k], p[k]);
+      for (int k = 0; k < RL; ++k) x[k] = conj_p ? cmulc_dd(cmulc_dd(x[k], py[k]), px) : cmul_dd(cmul_dd(x[k], py[k]), px);
       bfly<RL, true, false>(x, w);
 #pragma unroll
       for (int k = 0; k < RL; ++k) sts2(q ^ (8u * k), x[k]);
     }
   }
   __syncthreads();
-  inv_stages<LN, true, NS - 2, 0>(cols, rooty, tid);
+  inv_stages<LN, true, NS - 2, 0>(cols, lc, rooty, tid);
   if (cols <= NT) {
     const uint32_t c = (uint32_t)tid & (uint32_t)(cols - 1), yy = (uint32_t)tid >> lc, ystep = (uint32_t)NT >> lc;
     float2* dst = col + (int64_t)yy * nx + c;
 #pragma unroll 8
-    for (uint32_t y = yy; y < (uint32_t)N; y += ystep, dst += (int64_t)ystep * nx) *dst = lds2(col_off<LN>(c, y));
+    for (uint32_t y = yy; y < (uint32_t)N; y += ystep, dst += (int64_t)ystep * nx) *dst = lds2(col_off<LN>(c, y, lc));
   } else {
-    for (int i = tid; i < n_el; i += NT) col[(int64_t)(i >> lc) * nx + (i & (cols - 1))] = lds2(col_off<LN>((uint32_t)i & (uint32_t)(cols - 1), (uint32_t)i >> lc));
+    for (int i = tid; i < n_el; i += NT) col[(int64_t)(i >> lc) * nx + (i & (cols - 1))] = lds2(col_off<LN>((uint32_t)i & (uint32_t)(cols - 1), (uint32_t)i >> lc, lc));
   }
 }
 
@@ -306,14 +314,14 @@ __global__ void __launch_bounds__(NT, 2) k_ms_cols_detect(const float2* __restri
 #pragma unroll 8
     for (int i = tid; i < n_el; i += NT) {
       const uint32_t y = (uint32_t)i >> lc, c = (uint32_t)i & (uint32_t)(cols - 1);
-      cp_async8(col_off<LN>(c, y), col + (int64_t)y * nx + c);
+      cp_async8(col_off<LN>(c, y, lc), col + (int64_t)y * nx + c);
     }
     cp_async_wait_all();
     __syncthreads();
-    fwd_stages<LN, true, 0, NS - 1>(cols, rooty, tid);
+    fwd_stages<LN, true, 0, NS - 1>(cols, lc, rooty, tid);
     for (int i = tid; i < n_el; i += NT) {
       const uint32_t y = (uint32_t)i >> lc, c = (uint32_t)i & (uint32_t)(cols - 1);
-      const float2 v = lds2(col_off<LN>(c, y));
+      const float2 v = lds2(col_off<LN>(c, y, lc));
       acc[i] += v.x * v.x + v.y * v.y;
     }
   }
@@ -363,24 +371,27 @@ int32_t fft_init(bip_ctx* ctx) {
   const int ny = ctx->g.ny, nx = ctx->g.nx;
   const int64_t G = (int64_t)ny * nx;
   auto dd = [](double re, double im) { return dd_pair(re, im); };
-  std::vector<float4> ry = make_twiddle_table(ny), rx = make_twiddle_table(nx), P(G);
-  // Fresnel propagator P(q) = exp(-i pi lambda dz |q|^2) / G (eq. 2; no band limit), in the stored (digit-reversed) order
+  std::vector<float4> ry = make_twiddle_table(ny), rx = make_twiddle_table(nx), Ey(ny), Ex(nx);
+  // Fresnel propagator P(q) = exp(-i pi lambda dz |q|^2) / G (eq. 2; no band limit) = Ey[qy] Ex[qx], each factor in the
+  // stored (digit-reversed) order of its axis; the 1 / G of the unnormalised transform pair sits in Ey
   for (int py = 0; py < ny; ++py) {
     const int ky = dif_frequency(py, ny), hy = ky < (ny + 1) / 2 ? ky : ky - ny;
-    const double qy = hy / ctx->g.ly;
-    for (int px = 0; px < nx; ++px) {
-      const int kx = dif_frequency(px, nx), hx = kx < (nx + 1) / 2 ? kx : kx - nx;
-      const double qx = hx / ctx->g.lx;
-      const double ph = -M_PI * ctx->g.lambda * ctx->g.dz * (qy * qy + qx * qx);
-      P[(int64_t)py * nx + px] = dd(std::cos(ph) / (double)G, std::sin(ph) / (double)G);
-    }
+    const double qy = hy / ctx->g.ly, ph = -M_PI * ctx->g.lambda * ctx->g.dz * qy * qy;
+    Ey[py] = dd(std::cos(ph) / (double)G, std::sin(ph) / (double)G);
+  }
+  for (int px = 0; px < nx; ++px) {
+    const int kx = dif_frequency(px, nx), hx = kx < (nx + 1) / 2 ? kx : kx - nx;
+    const double qx = hx / ctx->g.lx, ph = -M_PI * ctx->g.lambda * ctx->g.dz * qx * qx;
+    Ex[px] = dd(std::cos(ph), std::sin(ph));
   }
   BIP_TRY(dev_alloc(ctx, (void**)&ctx->fft_rooty, sizeof(float4) * ry.size(), "fft twiddles"));
   BIP_TRY(dev_alloc(ctx, (void**)&ctx->fft_rootx, sizeof(float4) * rx.size(), "fft twiddles"));
-  BIP_TRY(dev_alloc(ctx, (void**)&ctx->fft_P, sizeof(float4) * G, "propagator (digit-reversed order)"));
+  BIP_TRY(dev_alloc(ctx, (void**)&ctx->fft_Ey, sizeof(float4) * ny, "propagator factor along y (digit-reversed order)"));
+  BIP_TRY(dev_alloc(ctx, (void**)&ctx->fft_Ex, sizeof(float4) * nx, "propagator factor along x (digit-reversed order)"));
   BIP_CUDA(ctx, cudaMemcpyAsync(ctx->fft_rooty, ry.data(), sizeof(float4) * ry.size(), cudaMemcpyHostToDevice, ctx->stream));
   BIP_CUDA(ctx, cudaMemcpyAsync(ctx->fft_rootx, rx.data(), sizeof(float4) * rx.size(), cudaMemcpyHostToDevice, ctx->stream));
-  BIP_CUDA(ctx, cudaMemcpyAsync(ctx->fft_P, P.data(), sizeof(float4) * G, cudaMemcpyHostToDevice, ctx->stream));
+  BIP_CUDA(ctx, cudaMemcpyAsync(ctx->fft_Ey, Ey.data(), sizeof(float4) * ny, cudaMemcpyHostToDevice, ctx->stream));
+  BIP_CUDA(ctx, cudaMemcpyAsync(ctx->fft_Ex, Ex.data(), sizeof(float4) * nx, cudaMemcpyHostToDevice, ctx->stream));
   std::vector<int32_t> py(ny), px(nx);
   for (int i = 0; i < ny; ++i) py[i] = dif_frequency(i, ny);
   for (int i = 0; i < nx; ++i) px[i] = dif_frequency(i, nx);
@@ -410,9 +421,9 @@ int32_t fft_slice_op(bip_ctx* ctx, float2* S, int n_cols, const float2* Tj, int 
     float2* Sc = S + (int64_t)c0 * ny * nx;
     const dim3 grid((unsigned)(nx >> lc), (unsigned)nc);
     if (lc == 13 - lny) {         // the compile-time tile width (every grid with ny nx >= TILE_EL)
-      BIP_FFT_SWITCH(lny, (k_ms_cols<LN_, 13 - LN_><<<grid, NT, tile_smem_bytes(), ctx->stream>>>(Sc, ctx->fft_P, conj_p, nx, lc, ctx->fft_rooty)));
+      BIP_FFT_SWITCH(lny, (k_ms_cols<LN_, 13 - LN_><<<grid, NT, tile_smem_bytes(), ctx->stream>>>(Sc, ctx->fft_Ey, ctx->fft_Ex, conj_p, nx, lc, ctx->fft_rooty)));
     } else {
-      BIP_FFT_SWITCH(lny, (k_ms_cols<LN_, -1><<<grid, NT, tile_smem_bytes(), ctx->stream>>>(Sc, ctx->fft_P, conj_p, nx, lc, ctx->fft_rooty)));
+      BIP_FFT_SWITCH(lny, (k_ms_cols<LN_, -1><<<grid, NT, tile_smem_bytes(), ctx->stream>>>(Sc, ctx->fft_Ey, ctx->fft_Ex, conj_p, nx, lc, ctx->fft_rooty)));
     }
   }
   BIP_FFT_SWITCH(lnx, (launch_rows<LN_, true>(ctx, S, Tj, post, n_lines, ny)));
@@ -439,8 +450,8 @@ int32_t fft_detect(bip_ctx* ctx, float2* fields, int n_rho, int n_ch, float* out
 }
 
 void fft_release(bip_ctx* ctx) {
-  cudaFree(ctx->fft_rooty); cudaFree(ctx->fft_rootx); cudaFree(ctx->fft_P); cudaFree(ctx->fft_permy); cudaFree(ctx->fft_permx);
-  ctx->fft_rooty = ctx->fft_rootx = ctx->fft_P = nullptr;
+  cudaFree(ctx->fft_rooty); cudaFree(ctx->fft_rootx); cudaFree(ctx->fft_Ey); cudaFree(ctx->fft_Ex); cudaFree(ctx->fft_permy); cudaFree(ctx->fft_permx);
+  ctx->fft_rooty = ctx->fft_rootx = ctx->fft_Ey = ctx->fft_Ex = nullptr;
   ctx->fft_permy = ctx->fft_permx = nullptr;
 }
 

@@ -126,7 +126,7 @@ struct bip_ctx {
   void* P_dev = nullptr;           // Fresnel propagator / G as double2 [ny][nx]
   void* ms_work = nullptr;         // double2 workspace of the cuFFT slice steps [plan_batch][ny][nx], allocated on first use
   // native fused slice step for power-of-two grids (bip_fft.cu)
-  float4 *fft_rooty = nullptr, *fft_rootx = nullptr, *fft_P = nullptr;   // double-float (hi, lo) twiddles and propagator
+  float4 *fft_rooty = nullptr, *fft_rootx = nullptr, *fft_Ey = nullptr, *fft_Ex = nullptr;   // double-float (hi, lo) twiddles and the two 1-D factors of the propagator
   int32_t *fft_permy = nullptr, *fft_permx = nullptr;   // true frequency index of every stored (digit-reversed) position
   int fft_lines = 0, fft_cols = 0;
   bool fft_native = false;         // route in use (bip_set_fft_backend)
