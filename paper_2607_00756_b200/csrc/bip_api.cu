@@ -216,7 +216,7 @@ static int32_t seek_S1(bip_ctx* ctx, int32_t plane) {
   }
   while (ctx->plane1 < plane) { BIP_TRY(ms_step_S1(ctx, ctx->plane1, +1)); ctx->plane1++; }
   while (ctx->plane1 > plane) { BIP_TRY(ms_step_S1(ctx, ctx->plane1 - 1, -1)); ctx->plane1--; }
-  return BIP_OK;
+  return ms_flush(ctx);
 }
 
 static int32_t seek(bip_ctx* ctx, int32_t plane) {
@@ -224,7 +224,7 @@ static int32_t seek(bip_ctx* ctx, int32_t plane) {
   BIP_TRY(seek_S1(ctx, plane));
   while (ctx->plane2 < plane) { BIP_TRY(ms_step_S2(ctx, ctx->plane2, +1)); ctx->plane2++; }
   while (ctx->plane2 > plane) { BIP_TRY(ms_step_S2(ctx, ctx->plane2 - 1, -1)); ctx->plane2--; }
-  return BIP_OK;
+  return ms_flush(ctx);
 }
 
 // Steps a1-a8 on the sliced 16-bit operands (BIP_PREC_FP16X4 / BIP_PREC_BF16X6).
@@ -780,6 +780,7 @@ int32_t bip_build_S2(bip_ctx* ctx) {
     BIP_TRY(ms_plane_waves(ctx, ctx->S2, ctx->p2_h_dev, ctx->n_p2, -1));
     ctx->plane2 = ctx->g.nz;
     while (ctx->plane2 > 0) { ctx->plane2--; BIP_TRY(ms_step_S2(ctx, ctx->plane2, -1)); }
+    BIP_TRY(ms_flush(ctx));
   }
   ctx->s2_built = true;
   return BIP_OK;
@@ -1089,6 +1090,7 @@ int32_t bip_set_fft_backend(bip_ctx* ctx, int32_t backend) {
   if (backend != BIP_FFT_NATIVE && backend != BIP_FFT_CUFFT_F64) return fail(ctx, BIP_ERR_INVALID, "bip_set_fft_backend: unknown backend %d", backend);
   if (backend == BIP_FFT_NATIVE && !fft_supported(ctx))
     return fail(ctx, BIP_ERR_UNSUPPORTED, "bip_set_fft_backend: the native slice step needs a power-of-two grid (8..4096), this one is %d x %d", ctx->g.ny, ctx->g.nx);
+  BIP_TRY(ms_flush(ctx));
   ctx->fft_native = backend == BIP_FFT_NATIVE;
   return BIP_OK;
 }

@@ -227,6 +227,80 @@ __global__ void __launch_bounds__(NT, 3) k_ms_rows(float2* __restrict__ S, const
   }
 }
 
+// The stage on the whole line of the inverse transform of one slice step and of the forward transform of the NEXT one, in
+// registers: conj twiddle, inverse butterfly, x post (of this step) x pre (of the next), forward butterfly, twiddle -- both
+// butterflies work on the same eight elements i0 + k N/8.
+template <int LN>
+__device__ __forceinline__ void stage_both(int n_lines, const float4* __restrict__ root, int tid, const float2* __restrict__ Ta, int mode_a,
+                                           const float2* __restrict__ Tb, int mode_b, int64_t line0_global, int ny_mask) {
+  constexpr int LSUB = LN - 3, SUB = 1 << LSUB, NV = 1 << LSUB, N = 1 << LN;
+  constexpr int NVT = NV < NT ? NV : NT, LSTEP = NT / NVT;
+  constexpr bool TW = LSUB > 0;
+  const float4* tw = root + tw_stage_off(LN, LN);
+  const int l0 = tid / NVT;
+  for (int v = tid % NVT; v < NV; v += NVT) {
+    const uint32_t i0 = (uint32_t)v;
+    float4 w[8];
+    if (TW) {
+#pragma unroll
+      for (int m = 1; m < 8; ++m) w[m] = __ldg(tw + ((m - 1) << LSUB) + v);
+    }
+    const uint32_t p0 = 8u * slot<LN>(i0);
+    for (int line = l0; line < n_lines; line += LSTEP) {
+      const uint32_t q = (uint32_t)line * (8u * N) + p0;
+      const int64_t trow = (((line0_global + line) & ny_mask) << LN) + i0;
+      float2 x[8], t[8];
+      if (mode_a) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) { t[k] = __ldg(Ta + trow + (k << LSUB)); if (mode_a == 2) t[k].y = -t[k].y; }
+      }
+      if (mode_b) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          float2 u = __ldg(Tb + trow + (k << LSUB));
+          if (mode_b == 2) u.y = -u.y;
+          t[k] = mode_a ? cmulf(t[k], u) : u;
+        }
+      }
+#pragma unroll
+      for (int k = 0; k < 8; ++k) x[k] = lds2((q ^ xk<LN, LSUB>(k)) + ak<LN, LSUB>(k));
+      bfly<8, true, TW>(x, w);
+      if (mode_a || mode_b) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) x[k] = cmulf(x[k], t[k]);
+      }
+      bfly<8, false, TW>(x, w);
+#pragma unroll
+      for (int k = 0; k < 8; ++k) sts2((q ^ xk<LN, LSUB>(k)) + ak<LN, LSUB>(k), x[k]);
+    }
+  }
+  (void)SUB;
+}
+
+// Pass 3 of one slice step and pass 1 of the next on the same rows in one kernel (consecutive steps of a build, of a cursor
+// move over several slices, of the exit multislice of Algorithm 3): k chained steps take 2 k + 1 passes instead of 3 k.
+template <int LN>
+__global__ void __launch_bounds__(NT, 3) k_ms_rows_both(float2* __restrict__ S, const float2* __restrict__ Ta, int mode_a, const float2* __restrict__ Tb,
+                                                       int mode_b, int64_t n_lines_total, int ny_mask, const float4* __restrict__ rootx) {
+  constexpr int N = 1 << LN, LINES = TILE_EL / N, NS = Seq<LN>::NS;
+  const int tid = threadIdx.x;
+  const int64_t line0 = (int64_t)blockIdx.x * LINES;
+  const int n_lines = (int)min((int64_t)LINES, n_lines_total - line0);
+  float2* g = S + line0 * N;
+  const int n_el = n_lines << LN;
+  const uint32_t c0 = 8u * ((uint32_t)tid ^ swz_g<LN>((uint32_t)tid));
+#pragma unroll 8
+  for (int e = tid; e < n_el; e += NT) cp_async8(c0 + 8u * (uint32_t)(e - tid), g + e);
+  cp_async_wait_all();
+  __syncthreads();
+  inv_stages<LN, false, NS - 1, 1>(n_lines, 0, rootx, tid);
+  stage_both<LN>(n_lines, rootx, tid, Ta, mode_a, Tb, mode_b, line0, ny_mask);
+  __syncthreads();
+  fwd_stages<LN, false, 1, NS - 1>(n_lines, 0, rootx, tid);
+#pragma unroll 8
+  for (int e = tid; e < n_el; e += NT) g[e] = lds2(c0 + 8u * (uint32_t)(e - tid));
+}
+
 // slot of row y of column c of a column tile (line c, key c & 15), in bytes
 template <int LN> __device__ __forceinline__ uint32_t col_off(uint32_t c, uint32_t y, int lc) {
   return c * (8u << LN) + 8u * (slot<LN>(y) ^ line_key<LN>(c, lc));
@@ -348,6 +422,7 @@ template <int LN> int32_t set_attrs(bip_ctx* ctx) {
   const int bytes = (int)tile_smem_bytes();
   BIP_CUDA(ctx, cudaFuncSetAttribute(k_ms_rows<LN, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
   BIP_CUDA(ctx, cudaFuncSetAttribute(k_ms_rows<LN, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  BIP_CUDA(ctx, cudaFuncSetAttribute(k_ms_rows_both<LN>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
   BIP_CUDA(ctx, cudaFuncSetAttribute(k_ms_cols<LN, 13 - LN>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
   BIP_CUDA(ctx, cudaFuncSetAttribute(k_ms_cols<LN, -1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
   BIP_CUDA(ctx, cudaFuncSetAttribute(k_ms_cols_detect<LN>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes + TILE_EL * (int)sizeof(float)));
@@ -359,6 +434,13 @@ void launch_rows(bip_ctx* ctx, float2* S, const float2* T, int tmode, int64_t n_
   constexpr int LINES = TILE_EL >> LN;
   const int64_t blocks = (n_lines_total + LINES - 1) / LINES;
   k_ms_rows<LN, INV><<<(unsigned)blocks, NT, tile_smem_bytes(), ctx->stream>>>(S, T, tmode, n_lines_total, ny - 1, ctx->fft_rootx);
+}
+
+template <int LN>
+void launch_rows_both(bip_ctx* ctx, float2* S, const float2* Ta, int mode_a, const float2* Tb, int mode_b, int64_t n_lines_total, int ny) {
+  constexpr int LINES = TILE_EL >> LN;
+  const int64_t blocks = (n_lines_total + LINES - 1) / LINES;
+  k_ms_rows_both<LN><<<(unsigned)blocks, NT, tile_smem_bytes(), ctx->stream>>>(S, Ta, mode_a, Tb, mode_b, n_lines_total, ny - 1, ctx->fft_rootx);
 }
 
 }  // namespace
@@ -415,7 +497,16 @@ int32_t fft_slice_op(bip_ctx* ctx, float2* S, int n_cols, const float2* Tj, int 
   const int ny = ctx->g.ny, nx = ctx->g.nx;
   const int lnx = ilog2(nx), lny = ilog2(ny), lc = ilog2(ctx->fft_cols);
   const int64_t n_lines = (int64_t)n_cols * ny;
-  BIP_FFT_SWITCH(lnx, (launch_rows<LN_, false>(ctx, S, Tj, pre, n_lines, ny)));
+  // the inverse row pass of the previous step on the same columns is still owed (fft_flush): it runs together with this step's
+  // forward row pass in one kernel
+  FftPending& pd = ctx->fft_pending;
+  if (pd.active && pd.S == S && pd.n_cols == n_cols) {
+    BIP_FFT_SWITCH(lnx, (launch_rows_both<LN_>(ctx, S, pd.T, pd.post, Tj, pre, n_lines, ny)));
+    pd.active = false;
+  } else {
+    BIP_TRY(fft_flush(ctx));
+    BIP_FFT_SWITCH(lnx, (launch_rows<LN_, false>(ctx, S, Tj, pre, n_lines, ny)));
+  }
   for (int c0 = 0; c0 < n_cols; c0 += 65535) {                // gridDim.y limit
     const int nc = std::min(65535, n_cols - c0);
     float2* Sc = S + (int64_t)c0 * ny * nx;
@@ -426,7 +517,19 @@ int32_t fft_slice_op(bip_ctx* ctx, float2* S, int n_cols, const float2* Tj, int 
       BIP_FFT_SWITCH(lny, (k_ms_cols<LN_, -1><<<grid, NT, tile_smem_bytes(), ctx->stream>>>(Sc, ctx->fft_Ey, ctx->fft_Ex, conj_p, nx, lc, ctx->fft_rooty)));
     }
   }
-  BIP_FFT_SWITCH(lnx, (launch_rows<LN_, true>(ctx, S, Tj, post, n_lines, ny)));
+  BIP_CUDA(ctx, cudaGetLastError());
+  pd.S = S; pd.n_cols = n_cols; pd.T = Tj; pd.post = post; pd.active = true;      // pass 3 is owed: the next step on S or fft_flush runs it
+  return BIP_OK;
+}
+
+// Run the inverse row pass that the last fft_slice_op left owing.  Every caller of a sequence of slice steps ends it with
+// ms_flush (bip_api.cu: seek, bip_build_S2); fft_detect takes the owed pass into its own forward row pass.
+int32_t fft_flush(bip_ctx* ctx) {
+  FftPending& pd = ctx->fft_pending;
+  if (!pd.active) return BIP_OK;
+  pd.active = false;
+  const int ny = ctx->g.ny, lnx = ilog2(ctx->g.nx);
+  BIP_FFT_SWITCH(lnx, (launch_rows<LN_, true>(ctx, pd.S, pd.T, pd.post, (int64_t)pd.n_cols * ny, ny)));
   BIP_CUDA(ctx, cudaGetLastError());
   return BIP_OK;
 }
@@ -436,7 +539,14 @@ int32_t fft_detect(bip_ctx* ctx, float2* fields, int n_rho, int n_ch, float* out
   const int ny = ctx->g.ny, nx = ctx->g.nx;
   const int lnx = ilog2(nx), lny = ilog2(ny), lc = ilog2(ctx->fft_cols);
   const int64_t G = (int64_t)ny * nx;
-  BIP_FFT_SWITCH(lnx, (launch_rows<LN_, false>(ctx, fields, nullptr, 0, (int64_t)n_rho * n_ch * ny, ny)));
+  FftPending& pd = ctx->fft_pending;
+  if (pd.active && pd.S == fields && pd.n_cols == n_rho * n_ch) {      // the exit multislice's last inverse row pass + this forward one
+    BIP_FFT_SWITCH(lnx, (launch_rows_both<LN_>(ctx, fields, pd.T, pd.post, nullptr, 0, (int64_t)n_rho * n_ch * ny, ny)));
+    pd.active = false;
+  } else {
+    BIP_TRY(fft_flush(ctx));
+    BIP_FFT_SWITCH(lnx, (launch_rows<LN_, false>(ctx, fields, nullptr, 0, (int64_t)n_rho * n_ch * ny, ny)));
+  }
   const size_t smem_det = tile_smem_bytes() + (size_t)TILE_EL * sizeof(float);
   for (int r0 = 0; r0 < n_rho; r0 += 65535) {                 // gridDim.y limit
     const int nr = std::min(65535, n_rho - r0);

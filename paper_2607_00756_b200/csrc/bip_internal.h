@@ -101,6 +101,9 @@ struct KernelInfo { bool attr_set = false; int max_clusters = -1; };   // per (c
 
 }  // namespace bip
 
+// Inverse row pass of a native slice step that has not run yet (bip_fft.cu: consecutive steps on the same columns share it)
+struct FftPending { float2* S = nullptr; int n_cols = 0; const float2* T = nullptr; int post = 0; bool active = false; };
+
 struct bip_ctx {
   bip_grid g{};
   cudaStream_t stream = nullptr;
@@ -129,6 +132,7 @@ struct bip_ctx {
   float4 *fft_rooty = nullptr, *fft_rootx = nullptr, *fft_Ey = nullptr, *fft_Ex = nullptr;   // double-float (hi, lo) twiddles and the two 1-D factors of the propagator
   int32_t *fft_permy = nullptr, *fft_permx = nullptr;   // true frequency index of every stored (digit-reversed) position
   int fft_lines = 0, fft_cols = 0;
+  FftPending fft_pending;          // inverse row pass owed by the last native slice step (fft_flush)
   bool fft_native = false;         // route in use (bip_set_fft_backend)
   float2 *S1 = nullptr, *S2 = nullptr;
   bool s1_built = false, s2_built = false;
@@ -206,12 +210,14 @@ int32_t ms_step_S2(bip_ctx* ctx, int32_t j, int dir);
 int32_t ms_exit_step(bip_ctx* ctx, float2* fields, int n, int32_t j);
 // out[rho][ky][kx] += sum_n |F fields[rho][n]|^2 / G (unitary F, corner-origin order); fields are destroyed
 int32_t ms_detect(bip_ctx* ctx, float2* fields, int n_rho, int n_ch, float* out);
+int32_t ms_flush(bip_ctx* ctx);       // end of a sequence of slice steps: every column is complete in memory afterwards
 
 // ---- native fused slice step for power-of-two grids (bip_fft.cu) ----
 bool fft_supported(const bip_ctx* ctx);
 int32_t fft_init(bip_ctx* ctx);
 int32_t fft_slice_op(bip_ctx* ctx, float2* S, int n_cols, const float2* Tj, int pre, int conj_p, int post);
 int32_t fft_detect(bip_ctx* ctx, float2* fields, int n_rho, int n_ch, float* out);
+int32_t fft_flush(bip_ctx* ctx);      // run the inverse row pass the last fft_slice_op left owing (chained slice steps share row passes)
 void fft_release(bip_ctx* ctx);
 
 // ---- S1 focal back-propagation (bip_focal.cu) ----

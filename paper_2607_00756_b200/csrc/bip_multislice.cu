@@ -106,6 +106,7 @@ int32_t get_plan(bip_ctx* ctx, int batch, cufftHandle* out) {
 //   pre / post: 0 = identity, 1 = T_j, 2 = conj T_j ;  conj_p: multiply the spectrum by conj(P) instead of P
 int32_t slice_op(bip_ctx* ctx, float2* S, int n_cols, const float2* Tj, int pre, int conj_p, int post) {
   if (ctx->fft_native) return fft_slice_op(ctx, S, n_cols, Tj, pre, conj_p, post);
+  BIP_TRY(fft_flush(ctx));                      // the backend was switched in the middle of a sequence
   const int64_t G = (int64_t)ctx->g.ny * ctx->g.nx;
   const int chunk = ctx->plan_batch;
   if (!ctx->ms_work) BIP_TRY(dev_alloc(ctx, &ctx->ms_work, (size_t)ctx->plan_batch * G * sizeof(double2), "multislice workspace"));
@@ -149,8 +150,11 @@ int32_t ms_exit_step(bip_ctx* ctx, float2* fields, int n, int32_t j) {
   return slice_op(ctx, fields, n, Tj, /*pre=*/1, /*conj_p=*/0, /*post=*/0);      // psi <- P[T_j psi] (eq. 6 on a wavefield)
 }
 
+int32_t ms_flush(bip_ctx* ctx) { return fft_flush(ctx); }   // the cuFFT route never leaves a pass owing
+
 int32_t ms_detect(bip_ctx* ctx, float2* fields, int n_rho, int n_ch, float* out) {
   if (ctx->fft_native) return fft_detect(ctx, fields, n_rho, n_ch, out);
+  BIP_TRY(fft_flush(ctx));
   const int64_t G = (int64_t)ctx->g.ny * ctx->g.nx;
   if (!ctx->ms_work) BIP_TRY(dev_alloc(ctx, &ctx->ms_work, (size_t)ctx->plan_batch * G * sizeof(double2), "multislice workspace"));
   double2* W = reinterpret_cast<double2*>(ctx->ms_work);
