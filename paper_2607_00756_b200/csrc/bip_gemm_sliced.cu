@@ -93,6 +93,9 @@ struct SlParams {
   int lag_max;             // the leading products may trail the small ones by up to this many k-steps (< STAGES)
   int dgroup;              // column tiles per raster group
   int drop_tiny;           // FP16X3: the x2 y2 products (<= 2^-18 of the leading ones) are not issued
+#ifdef BIP_TUNING
+  int probe_x;             // timing probes (wrong results): 1 = X loaded only in the first k-step of a segment, 2 = every worker streams the X of row tile 0
+#endif
   unsigned int* sync_counter;   // lockstep of the workers (below); NULL = free-running
   int sync_steps;               // ... every this many k-steps of a segment
   // GEMM1 epilogue
@@ -186,6 +189,14 @@ __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr) {
   return d;                                           // layout type 0 = no swizzle
 }
 
+// The same descriptor from its low word: within one stage every operand slice differs from the stage base only in the start
+// address, so the issuing thread forms  lo = umma_desc_lo(stage base)  once per k-step and each descriptor is lo + (offset >> 4)
+// (one uniform add instead of add / shift / mask / or per descriptor: the issue loop, not the tensor pipe, paces FP16X3).
+__device__ __forceinline__ uint32_t umma_desc_lo(uint32_t saddr) { return ((saddr & 0x3FFFF) >> 4) | ((uint32_t)(128 >> 4) << 16); }
+__device__ __forceinline__ uint64_t umma_desc_at(uint32_t lo, uint32_t byte_off) {
+  return ((uint64_t)((256u >> 4) | (1u << 14)) << 32) | (uint64_t)(lo + (byte_off >> 4));
+}
+
 // cute::UMMA::InstrDescriptor for kind::f16 (fp16 or bf16 operands), fp32 accumulate, K-major A and B;
 // M = 128 (one CTA) or 256 (CTA pair, cta_group::2), N = 128 or 256
 __host__ __device__ constexpr uint32_t umma_idesc(uint32_t ab_format, bool neg_a, bool pair, int n = TN) {
@@ -256,21 +267,10 @@ __device__ __forceinline__ void mbar_arrive_cluster(uint64_t* bar, uint32_t rank
       "}" ::"r"(smem_u32(bar)), "r"(rank)
       : "memory");
 }
-// wait on a barrier that threads of the peer CTA arrive on
-__device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity) {
-  uint32_t done = 0;
-  while (!done) {
-    asm volatile(
-        "{\n\t"
-        ".reg .pred P1;\n\t"
-        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 P1, [%1], %2;\n\t"
-        "selp.b32 %0, 1, 0, P1;\n\t"
-        "}"
-        : "=r"(done)
-        : "r"(smem_u32(bar)), "r"(parity)
-        : "memory");
-  }
-}
+// Barriers that threads of the peer CTA arrive on (peer_full, c0_empty, c12_empty) are waited on with the plain CTA-scope
+// mbar_wait: what those arrivals publish is read by the tensor core or lives in tensor memory and is ordered by
+// tcgen05.fence::after_thread_sync; a cluster-scope acquire costs an L1 invalidation (CCTL.IVALL) per wait -- once per k-step
+// in the issue loop, its largest single stall (profiles/r02_gemm2_probes.md).
 
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
   asm volatile(
@@ -311,8 +311,9 @@ __device__ __forceinline__ void issue_small(uint32_t t12r, uint32_t t12i, uint32
   constexpr int YP = PAIR ? PART_BYTES / 2 : PART_BYTES;      // a CTA of a pair holds 64 of the 128 Y rows of every part
   auto umma = [](uint32_t d, uint64_t da, uint64_t db, uint32_t id, uint32_t ac) { umma_f16<PAIR>(d, da, db, id, ac); };
   if (FMT == SL_FMT_FP16X4) {
-    const uint64_t xr1 = umma_desc(a0), xr2 = umma_desc(a0 + PART_BYTES), xi1 = umma_desc(a0 + 2 * PART_BYTES), xi2 = umma_desc(a0 + 3 * PART_BYTES);
-    const uint64_t yr1 = umma_desc(b0), yr2 = umma_desc(b0 + YP), yi1 = umma_desc(b0 + 2 * YP), yi2 = umma_desc(b0 + 3 * YP);
+    const uint32_t al = umma_desc_lo(a0), bl = umma_desc_lo(b0);
+    const uint64_t xr1 = umma_desc_at(al, 0), xr2 = umma_desc_at(al, PART_BYTES), xi1 = umma_desc_at(al, 2 * PART_BYTES), xi2 = umma_desc_at(al, 3 * PART_BYTES);
+    const uint64_t yr1 = umma_desc_at(bl, 0), yr2 = umma_desc_at(bl, YP), yi1 = umma_desc_at(bl, 2 * YP), yi2 = umma_desc_at(bl, 3 * YP);
     // tiniest first: x2 y2 (FP16X3 leaves them out), then x1 y2 + x2 y1
     uint32_t acc_r = acc, acc_i = acc;
     if (!drop_tiny) {
@@ -334,10 +335,11 @@ __device__ __forceinline__ void issue_small(uint32_t t12r, uint32_t t12i, uint32
     umma(t12i, xi1, yr2, id_pos, 1u);
     umma(t12i, xi2, yr1, id_pos, 1u);
   } else {
-    const uint64_t xr1 = umma_desc(a0), xr2 = umma_desc(a0 + PART_BYTES), xr3 = umma_desc(a0 + 2 * PART_BYTES);
-    const uint64_t xi1 = umma_desc(a0 + 3 * PART_BYTES), xi2 = umma_desc(a0 + 4 * PART_BYTES), xi3 = umma_desc(a0 + 5 * PART_BYTES);
-    const uint64_t yr1 = umma_desc(b0), yr2 = umma_desc(b0 + YP), yr3 = umma_desc(b0 + 2 * YP);
-    const uint64_t yi1 = umma_desc(b0 + 3 * YP), yi2 = umma_desc(b0 + 4 * YP), yi3 = umma_desc(b0 + 5 * YP);
+    const uint32_t al = umma_desc_lo(a0), bl = umma_desc_lo(b0);
+    const uint64_t xr1 = umma_desc_at(al, 0), xr2 = umma_desc_at(al, PART_BYTES), xr3 = umma_desc_at(al, 2 * PART_BYTES);
+    const uint64_t xi1 = umma_desc_at(al, 3 * PART_BYTES), xi2 = umma_desc_at(al, 4 * PART_BYTES), xi3 = umma_desc_at(al, 5 * PART_BYTES);
+    const uint64_t yr1 = umma_desc_at(bl, 0), yr2 = umma_desc_at(bl, YP), yr3 = umma_desc_at(bl, 2 * YP);
+    const uint64_t yi1 = umma_desc_at(bl, 3 * YP), yi2 = umma_desc_at(bl, 4 * YP), yi3 = umma_desc_at(bl, 5 * YP);
     // C12r = sum over (i + j in {3, 4}) of xr_i yr_j - xi_i yi_j
     umma(t12r, xr1, yr3, id_pos, acc);
     umma(t12r, xr2, yr2, id_pos, 1u);
@@ -370,7 +372,8 @@ __device__ __forceinline__ void issue_lead(uint32_t t0r, uint32_t t0i, uint32_t 
   constexpr int YP = PAIR ? PART_BYTES / 2 : PART_BYTES;
   constexpr int IM = (Cfg<FMT>::PARTS / 2) * PART_BYTES, IMY = (Cfg<FMT>::PARTS / 2) * YP;   // first imaginary slice
   auto umma = [](uint32_t d, uint64_t da, uint64_t db, uint32_t id, uint32_t ac) { umma_f16<PAIR>(d, da, db, id, ac); };
-  const uint64_t xr1 = umma_desc(a0), xi1 = umma_desc(a0 + IM), yr1 = umma_desc(b0), yi1 = umma_desc(b0 + IMY);
+  const uint32_t al = umma_desc_lo(a0), bl = umma_desc_lo(b0);
+  const uint64_t xr1 = umma_desc_at(al, 0), xi1 = umma_desc_at(al, IM), yr1 = umma_desc_at(bl, 0), yi1 = umma_desc_at(bl, IMY);
   umma(t0r, xr1, yr1, id_pos, acc);
   umma(t0r, xi1, yi1, id_neg, 1u);
   umma(t0i, xr1, yi1, id_pos, acc);
@@ -476,14 +479,28 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
             const int s = it % STAGES;
             mbar_wait(&empty[s], ((it / STAGES) & 1) ^ 1);
             uint8_t* st = smem + s * STAGE_BYTES;
+#ifdef BIP_TUNING
+            if (p.probe_x == 1 && ks > 0) {
+              mbar_expect_tx(&full[s], STAGE_BYTES - X_BYTES);
+            } else {
+              mbar_expect_tx(&full[s], STAGE_BYTES);
+              const uint16_t* xs = p.probe_x == 2 ? p.X + (int64_t)atom * p.x_batch_stride + ((int64_t)n * p.n_rt_x + (PAIR ? (int)rank : 0)) * p.ksteps * STEP_EL : xsrc;
+              bulk_load(st, xs + (int64_t)ks * STEP_EL, X_BYTES, &full[s]);
+            }
+#else
             mbar_expect_tx(&full[s], STAGE_BYTES);
             bulk_load(st, xsrc + (int64_t)ks * STEP_EL, X_BYTES, &full[s]);
+#endif
             if (WIDE) {
               // parts in memory: re1 re2 im1 im2 -im1 -im2; blocks in the stage: [-im1][re1][im1][-im2][re2][im2]
               constexpr int dst_block[6] = {1, 4, 2, 5, 0, 3};
 #pragma unroll
               for (int part = 0; part < 6; ++part)
                 bulk_load(st + X_BYTES + dst_block[part] * YB, ysrc + (int64_t)ks * STEP_EL_Y + part * SL_TILE_EL, YB, &full[s]);
+#ifdef BIP_TUNING
+            } else if (PAIR && p.probe_x == 3) {          // timing probe (wrong data): the CTA's Y half as ONE copy instead of one per slice
+              bulk_load(st + X_BYTES, ysrc + (int64_t)ks * STEP_EL, Y_BYTES, &full[s]);
+#endif
             } else if (PAIR) {
 #pragma unroll
               for (int part = 0; part < C::PARTS; ++part)
@@ -527,7 +544,7 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
     uint32_t s_small = 0, ph_small = 0;            // stage and phase of the small-product cursor
     uint32_t ks_s = 0, seg_par = 0;                // its k-step inside the segment; segment parity
     uint32_t s_lead = 0, ks_l = 0, in_chunk = 0, chunk_par = 0, pending = 0;   // leading-product cursor
-    auto wait_epi = [&](uint64_t* bar, uint32_t parity) { if (PAIR) mbar_wait_cluster(bar, parity); else mbar_wait(bar, parity); };
+    auto wait_epi = [&](uint64_t* bar, uint32_t parity) { mbar_wait(bar, parity); };
     auto lead = [&]() {
       if (in_chunk == 0) {
         wait_epi(c0_empty, chunk_par ^ 1);                           // epilogue has drained the previous chunk's C0
@@ -550,7 +567,7 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
     };
     for (uint32_t g = 0; g < total; ++g) {
       mbar_wait(&full[s_small], ph_small);
-      if (PAIR) mbar_wait_cluster(&peer_full[s_small], ph_small);
+      if (PAIR) mbar_wait(&peer_full[s_small], ph_small);
       if (ks_s == 0) {
         while (pending) lead();
         wait_epi(c12_empty, seg_par ^ 1);                            // epilogue has drained the previous segment's C12
@@ -878,6 +895,12 @@ int32_t launch_fmt(bip_ctx* ctx, const SlParams& p) {
   q.n_items = p.n_items / p.n_rt * q.n_rt;
   if (q.n_items <= 0) return BIP_OK;
   q.chunk_steps = Cfg<FMT>::CHUNK_STEPS;                 // fixed: the exactness of the leading sums depends on it
+#ifdef BIP_TUNING
+  q.chunk_steps = std::max(1, tune_int("BIP_TUNE_CHUNK", q.chunk_steps));   // timing probe only: longer chunks are no longer exact
+#endif
+#ifdef BIP_TUNING
+  q.probe_x = tune_int("BIP_TUNE_PROBE_X", 0);
+#endif
   q.dgroup = std::max(1, tune_int("BIP_TUNE_DGROUP", DGROUP_DEFAULT));
   q.lag_max = std::min(std::max(1, tune_int("BIP_TUNE_LAG", Cfg<FMT>::LAG_MAX)), n_stages<EPI, FMT, PAIR, WIDE>() - 1);
   int workers = std::max(1, std::min(q.n_items, PAIR ? ctx->sm_count / 2 : ctx->sm_count));
