@@ -18,9 +18,15 @@ __device__ __forceinline__ float tf32_hi(float x) {
 
 // exp(+2 pi i h.r/N) for non-negative reduced beam index (hyp, hxp) at global pixel (ry, rx): exact phase from the
 // root tables, (h r mod N) reduced in integers (SURVEY "Phases exactly").
+// a mod n for 0 <= a: a mask when n is a power of two (every BASELINE grid; the branch is uniform), else the division
+__device__ __forceinline__ int mod_n(int a, int n) { return (n & (n - 1)) == 0 ? (a & (n - 1)) : a % n; }
+
+// non-negative index of a signed beam component (|h| < n / 2 is checked when the beam lists are registered)
+__device__ __forceinline__ int beam_idx(int h, int n) { return h < 0 ? h + n : h; }
+
 __device__ __forceinline__ float2 tilt(const float2* __restrict__ rooty, const float2* __restrict__ rootx,
                                        int hyp, int hxp, int ry, int rx, int ny, int nx) {
-  return cmul(rooty[(hyp * ry) % ny], rootx[(hxp * rx) % nx]);
+  return cmul(rooty[mod_n(hyp * ry, ny)], rootx[mod_n(hxp * rx, nx)]);
 }
 
 // a1: D[a][p][s] = S_p(r) exp(-carrier 2 pi i h_p.r/N), r = (origin_a + s) mod N
@@ -31,7 +37,7 @@ __global__ void k_crop_detilt(const float2* __restrict__ S, const int32_t* __res
   const int a = blockIdx.z, p = blockIdx.y;
   const int w2 = w * w;
   const int oy = (origin[2 * a] - shift + ny) % ny, ox = (origin[2 * a + 1] - shift + nx) % nx;   // shift: margin of a padded window
-  const int hyp = ((ph[2 * p] % ny) + ny) % ny, hxp = ((ph[2 * p + 1] % nx) + nx) % nx;
+  const int hyp = beam_idx(ph[2 * p], ny), hxp = beam_idx(ph[2 * p + 1], nx);
   const float2* col = S + (int64_t)p * ny * nx;
   float2* out = D + ((int64_t)a * n_par + p) * w2;
   for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < w2; s += gridDim.x * blockDim.x) {
@@ -81,7 +87,7 @@ __global__ void k_recon_rows(const float2* __restrict__ D, int n_par, const int3
   }
   __syncthreads();
   const int oy = origin[2 * a], ox = origin[2 * a + 1];
-  const int hyp = ((bh[2 * b] % ny) + ny) % ny, hxp = ((bh[2 * b + 1] % nx) + nx) % nx;
+  const int hyp = beam_idx(bh[2 * b], ny), hxp = beam_idx(bh[2 * b + 1], nx);
   const float2* Da = D + (int64_t)a * n_par * w2;
   const int64_t row = (int64_t)a * out.batch_stride + (int64_t)b * out.ld;
   for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < w2; s += gridDim.x * blockDim.x) {
@@ -116,7 +122,7 @@ __global__ void k_recon_transposed(const float2* __restrict__ D, int n_par, cons
       const int sy = s / w, sx = s - sy * w;
       int ry = oy + sy; if (ry >= ny) ry -= ny;
       int rx = ox + sx; if (rx >= nx) rx -= nx;
-      const int hyp = ((bh[2 * b] % ny) + ny) % ny, hxp = ((bh[2 * b + 1] % nx) + nx) % nx;
+      const int hyp = beam_idx(bh[2 * b], ny), hxp = beam_idx(bh[2 * b + 1], nx);
       float2 t = tilt(rooty, rootx, hyp, hxp, ry, rx, ny, nx);
       if (carrier < 0) t.y = -t.y;
       v = recon_elem(Da, nn_idx + (int64_t)b * max_nn, nn_w + (int64_t)b * max_nn, max_nn, w2, s, recon, t);
@@ -145,7 +151,7 @@ __global__ void k_recon_c64(const float2* __restrict__ D, int n_par, const int32
   const int b = blockIdx.y;
   const int w2 = w * w;
   const int oy = (origin[2 * atom] - shift + ny) % ny, ox = (origin[2 * atom + 1] - shift + nx) % nx;
-  const int hyp = ((bh[2 * b] % ny) + ny) % ny, hxp = ((bh[2 * b + 1] % nx) + nx) % nx;
+  const int hyp = beam_idx(bh[2 * b], ny), hxp = beam_idx(bh[2 * b + 1], nx);
   for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < w2; s += gridDim.x * blockDim.x) {
     const int sy = s / w, sx = s - sy * w;
     int ry = oy + sy; if (ry >= ny) ry -= ny;
@@ -203,6 +209,21 @@ __global__ void __launch_bounds__(256) k_recon_t_sliced(const float2* __restrict
   const int a = blockIdx.z;
   const int w2 = w * w;
   const int s = blockIdx.x * 32 + threadIdx.x, g = blockIdx.y * 8 + threadIdx.y;
+  // neighbour lists of the block's 64 beams, read once per block instead of once per (beam, window pixel)
+  __shared__ int32_t s_idx[64][BIP_MAX_NN];
+  __shared__ float s_w[64][BIP_MAX_NN];
+  __shared__ int32_t s_h[64][2];
+  for (int i = threadIdx.y * 32 + threadIdx.x; i < 64 * max_nn; i += 256) {
+    const int bb = i / max_nn, j = i - bb * max_nn, b = blockIdx.y * 64 + bb;
+    s_idx[bb][j] = b < n_beams ? nn_idx[(int64_t)b * max_nn + j] : -1;
+    s_w[bb][j] = b < n_beams ? nn_w[(int64_t)b * max_nn + j] : 0.f;
+  }
+  if (threadIdx.y < 2) {
+    const int bb = threadIdx.y * 32 + threadIdx.x, b = blockIdx.y * 64 + bb;
+    s_h[bb][0] = b < n_beams ? beam_idx(bh[2 * b], ny) : 0;
+    s_h[bb][1] = b < n_beams ? beam_idx(bh[2 * b + 1], nx) : 0;
+  }
+  __syncthreads();
   if (s >= w2 || g >= 2 * out.ksteps) return;
   const int oy = origin[2 * a], ox = origin[2 * a + 1];
   const int sy = s / w, sx = s - sy * w;
@@ -212,13 +233,12 @@ __global__ void __launch_bounds__(256) k_recon_t_sliced(const float2* __restrict
   float re[8], im[8];
 #pragma unroll
   for (int j = 0; j < 8; ++j) {
-    const int b = g * 8 + j;
+    const int b = g * 8 + j, bb = threadIdx.y * 8 + j;
     float2 v = make_float2(0.f, 0.f);
     if (b < n_beams) {
-      const int hyp = ((bh[2 * b] % ny) + ny) % ny, hxp = ((bh[2 * b + 1] % nx) + nx) % nx;
-      float2 t = tilt(rooty, rootx, hyp, hxp, ry, rx, ny, nx);
+      float2 t = tilt(rooty, rootx, s_h[bb][0], s_h[bb][1], ry, rx, ny, nx);
       if (carrier < 0) t.y = -t.y;
-      v = recon_elem(Da, nn_idx + (int64_t)b * max_nn, nn_w + (int64_t)b * max_nn, max_nn, w2, s, recon, t);
+      v = recon_elem(Da, s_idx[bb], s_w[bb], max_nn, w2, s, recon, t);
     }
     re[j] = v.x; im[j] = v.y;
   }
@@ -274,24 +294,60 @@ __global__ void __launch_bounds__(256) k_recon_rows_sliced(const float2* __restr
     for (int n = 0; n < n_rep; ++n)
       out.scale[(int64_t)a * out.scale_batch_stride + (int64_t)n * n_beams + b] = sl_pow2_scale(1.001f * bound * (H ? hmax[n] : 1.f));
   const int oy = origin[2 * a], ox = origin[2 * a + 1];
-  const int hyp = ((bh[2 * b] % ny) + ny) % ny, hxp = ((bh[2 * b + 1] % nx) + nx) % nx;
+  const int hyp = beam_idx(bh[2 * b], ny), hxp = beam_idx(bh[2 * b + 1], nx);
   const float2* Da = D + (int64_t)a * n_par * w2;
   const int n_groups = 2 * (int)out.ksteps;
   for (int g = gl; g < n_groups; g += 32) {
+    // the 8 window pixels s0 .. s0 + 7 of this k-group: neighbours in the outer loop (index and weight read once per
+    // group, the parent window read as 4 x 16 bytes), eq. 15 / eq. 11 sums in registers, then re-tilt
+    const int s0 = g * 8;
+    const bool whole = s0 + 8 <= w2;
+    float zr[8], zi[8], mg[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { zr[j] = 0.f; zi[j] = 0.f; mg[j] = 0.f; }
+    for (int jn = 0; jn < max_nn; ++jn) {
+      const int p = s_idx[r][jn];
+      if (p < 0) break;
+      const float wj = s_w[r][jn];
+      const float2* dp = Da + (int64_t)p * w2 + s0;
+      float2 d[8];
+      if (whole) {                                   // w is even: rows of D and s0 are 16-byte aligned
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const float4 q = __ldg(reinterpret_cast<const float4*>(dp) + j);
+          d[2 * j] = make_float2(q.x, q.y); d[2 * j + 1] = make_float2(q.z, q.w);
+        }
+      } else {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) d[j] = s0 + j < w2 ? __ldg(dp + j) : make_float2(0.f, 0.f);
+      }
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        zr[j] = fmaf(wj, d[j].x, zr[j]);
+        zi[j] = fmaf(wj, d[j].y, zi[j]);
+        if (recon == BIP_RECON_MAGPHASE) mg[j] = fmaf(wj, sqrtf(d[j].x * d[j].x + d[j].y * d[j].y), mg[j]);
+      }
+    }
     float re[8], im[8];
+    int sy = s0 / w, sx = s0 - sy * w;
 #pragma unroll
     for (int j = 0; j < 8; ++j) {
-      const int s = g * 8 + j;
       float2 v = make_float2(0.f, 0.f);
-      if (s < w2) {
-        const int sy = s / w, sx = s - sy * w;
+      if (s0 + j < w2) {
         int ry = oy + sy; if (ry >= ny) ry -= ny;
         int rx = ox + sx; if (rx >= nx) rx -= nx;
         float2 t = tilt(rooty, rootx, hyp, hxp, ry, rx, ny, nx);
         if (carrier < 0) t.y = -t.y;
-        v = recon_elem(Da, s_idx[r], s_w[r], max_nn, w2, s, recon, t);
+        float ar = zr[j], ai = zi[j];
+        if (recon == BIP_RECON_MAGPHASE) {
+          const float az = sqrtf(ar * ar + ai * ai);
+          const float sc = az >= 1e-30f ? mg[j] / az : 0.f;   // eq. 11; |z| < 1e-30 -> 0
+          ar *= sc; ai *= sc;
+        }
+        v = cmul(make_float2(ar, ai), t);
       }
       re[j] = v.x; im[j] = v.y;
+      if (++sx == w) { sx = 0; ++sy; }
     }
     if (!H) {
       sl_store_group(out, a, b, g, re, im, 1.f / sl_pow2_scale(1.001f * bound));
