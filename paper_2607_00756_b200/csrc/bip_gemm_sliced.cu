@@ -306,7 +306,7 @@ __device__ __forceinline__ void decode_item(const SlParams& p, int item, int& at
 
 // The small products of one k-step (accumulators C12r, C12i): everything except x1 y1.
 template <int FMT, bool PAIR>
-__device__ __forceinline__ void issue_small(uint32_t t12r, uint32_t t12i, uint32_t a0, uint32_t b0, uint32_t acc, bool drop_tiny) {
+__device__ __forceinline__ void issue_small(uint32_t t12r, uint32_t t12i, uint32_t a0, uint32_t b0, uint32_t acc, bool drop_tiny, bool alt_order = false) {
   constexpr uint32_t id_pos = umma_idesc(Cfg<FMT>::AB_FORMAT, false, PAIR), id_neg = umma_idesc(Cfg<FMT>::AB_FORMAT, true, PAIR);
   constexpr int YP = PAIR ? PART_BYTES / 2 : PART_BYTES;      // a CTA of a pair holds 64 of the 128 Y rows of every part
   auto umma = [](uint32_t d, uint64_t da, uint64_t db, uint32_t id, uint32_t ac) { umma_f16<PAIR>(d, da, db, id, ac); };
@@ -321,6 +321,19 @@ __device__ __forceinline__ void issue_small(uint32_t t12r, uint32_t t12i, uint32
       umma(t12r, xi2, yi2, id_neg, 1u);
       acc_r = 1u;
     }
+#ifdef BIP_TUNING
+    if (drop_tiny && alt_order) {                     // timing probe: same products, consecutive MMAs share the X slice and alternate the accumulator
+      umma(t12r, xr1, yr2, id_pos, acc);
+      umma(t12i, xr1, yi2, id_pos, acc);
+      umma(t12r, xr2, yr1, id_pos, 1u);
+      umma(t12i, xr2, yi1, id_pos, 1u);
+      umma(t12r, xi1, yi2, id_neg, 1u);
+      umma(t12i, xi1, yr2, id_pos, 1u);
+      umma(t12r, xi2, yi1, id_neg, 1u);
+      umma(t12i, xi2, yr1, id_pos, 1u);
+      return;
+    }
+#endif
     umma(t12r, xr1, yr2, id_pos, acc_r);
     umma(t12r, xr2, yr1, id_pos, 1u);
     umma(t12r, xi1, yi2, id_neg, 1u);
@@ -480,7 +493,10 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
             mbar_wait(&empty[s], ((it / STAGES) & 1) ^ 1);
             uint8_t* st = smem + s * STAGE_BYTES;
 #ifdef BIP_TUNING
-            if (p.probe_x == 1 && ks > 0) {
+            if (p.probe_x == 4 && ks > 0) {               // no operand traffic at all: issue + MMA only
+              mbar_expect_tx(&full[s], 0);
+              continue;
+            } else if (p.probe_x == 1 && ks > 0) {
               mbar_expect_tx(&full[s], STAGE_BYTES - X_BYTES);
             } else {
               mbar_expect_tx(&full[s], STAGE_BYTES);
@@ -577,7 +593,11 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
       if (elect_one()) {
         const uint32_t a0 = smem_base + s_small * STAGE_BYTES;
         if (WIDE) issue_small_wide(t12r, a0, a0 + X_BYTES, ks_s ? 1u : 0u, drop_tiny);
+#ifdef BIP_TUNING
+        else issue_small<FMT, PAIR>(t12r, t12i, a0, a0 + X_BYTES, ks_s ? 1u : 0u, drop_tiny, p.probe_x == 5);
+#else
         else issue_small<FMT, PAIR>(t12r, t12i, a0, a0 + X_BYTES, ks_s ? 1u : 0u, drop_tiny);
+#endif
         if (seg_end) umma_commit<PAIR>(c12_full);
       }
       __syncwarp();
