@@ -5,13 +5,16 @@
 // in THREE passes over the column instead of the eleven of the cuFFT route (load/convert, 2 x 2 cuFFT passes, spectrum
 // multiply, store/convert, each reading and writing the whole column):
 //
-//   pass 1  rows:     load S[y][.] (x pre),  forward FFT along x in shared memory,           store
-//   pass 2  columns:  load a tile of columns, forward FFT along y, x P(q) / G, inverse FFT along y, store
-//   pass 3  rows:     load, inverse FFT along x, (x post), store
+//   pass 1  rows:     load S[y][.] (x pre),  forward FFT along x in shared memory,           store      k_ms_rows<LN, fwd>
+//   pass 2  columns:  load a tile of columns, forward FFT along y, x P(q) / G, inverse FFT along y, store   k_ms_cols<LN, LC>
+//   pass 3  rows:     load, inverse FFT along x, (x post), store                                         k_ms_rows<LN, inv>
 //
-// i.e. 48 bytes of HBM traffic per pixel and slice step.  The forward transforms are decimation-in-frequency (natural
-// order in, digit-reversed order out), the inverse ones decimation-in-time (digit-reversed in, natural out), so no
-// reordering pass exists at all: the propagator table is stored once in the digit-reversed order of both axes.
+// i.e. 48 bytes of HBM traffic per pixel and slice step -- and 32 when slice steps follow one another on the same columns
+// (a build, a cursor move over several slices, the exit multislice of Algorithm 3): pass 3 of step j and pass 1 of step
+// j + 1 work on the same rows and run as ONE kernel (k_ms_rows_both; fft_slice_op leaves pass 3 owing, the next step or
+// fft_flush runs it).  The forward transforms are decimation-in-frequency (natural order in, digit-reversed order out),
+// the inverse ones decimation-in-time (digit-reversed in, natural out), so no reordering pass exists at all: the
+// propagator -- separable, P(q) / G = Ey[q_y] Ex[q_x] -- is stored as two 1-D tables in the digit-reversed order of their axis.
 // Butterflies are radix-8 in registers (radix 4 / 2 for the last stage), fp32 with round-to-nearest throughout.
 // Every CONSTANT the data is multiplied by -- twiddles, sqrt(1/2), the propagator -- is held as a double-float pair
 // hi + lo (hi = fp32(c), lo = fp32(c - hi)) and applied with the small terms first inside one FMA chain.  A twiddle

@@ -1,5 +1,7 @@
-// Device building blocks of the library's own power-of-two FFTs (bip_fft.cu: slice steps on the whole grid; bip_focal.cu:
-// Fresnel steps on padded windows): radix-8 butterflies in registers, double-float constants, padded shared-memory lines.
+// Device building blocks of the library's own power-of-two FFTs: the radix-8 / 4 / 2 butterflies and double-float constant
+// products shared by both users, the per-stage twiddle tables, and the run-time-sized transform on padded shared-memory lines
+// that bip_focal.cu uses for the Fresnel steps on padded windows (bip_fft.cu has its own compile-time-sized stages for the
+// slice steps on the whole grid).
 // See the header comment of bip_fft.cu for why every constant is a hi + lo pair.
 #ifndef BIP_FFT_CUH_
 #define BIP_FFT_CUH_
