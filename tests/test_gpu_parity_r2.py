@@ -63,18 +63,18 @@ def test_cfg3_interface_clone_five_edges_one_plane_loop():
 @pytest.mark.slow
 def test_full_size_cfg2_site_deep_in_the_slab():
     """BASELINE.json configs[1] at full size with a REAL slab: one B site in slice 19 (S1 has channelled through 19 slices;
-    the slab is cut at 26 slices, so S2 holds the 7 below -- the S2 side through a thick slab is the cfg3 / cfg1 clones'
+    the slab is cut at 22 slices, so S2 holds the 3 below -- the S2 side through a thick slab is the cfg3 / cfg1 clones'
     job, and every further slice costs the oracle 10 s of fp64 FFTs), all 4096 scan positions on the GPU, MAGPHASE; the
     oracle builds the fp64 parent windows for that site (1951 + 4921 parent columns, in chunks) and computes 64 sampled
     map pixels."""
     import torch
     import paper_2607_00756_b200 as B
-    wl0 = make_workload("cfg2", nz=26)
+    wl0 = make_workload("cfg2", nz=22)
     deep = np.nonzero(wl0.edges[0].slice == 19)[0]
     assert deep.size == 400
-    smp = OracleSample("cfg2", nz=26, n_scan=64, atom_idx=deep[[137]])
+    smp = OracleSample("cfg2", nz=22, n_scan=64, atom_idx=deep[[137]])
     wl, e = smp.wl, smp.e
-    assert wl.nz == 26 and int(e.slice[0]) == 19
+    assert wl.nz == 22 and int(e.slice[0]) == 19
     want = smp.run("magphase")["map"]
     ctx, geo, ids = gpu_context(wl, [e])
     m = ctx.map(0, B.MODE_MAP, B.RECON_MAGPHASE, B.PREC_FP16X4)
