@@ -186,7 +186,8 @@ BIP_API const char* bip_last_error(const bip_ctx* ctx);
 BIP_API int32_t bip_build_S1(bip_ctx* ctx);
 
 /* S2 parents <- exp(-2 pi i h_p.r/N) at the exit surface, then u <- T_j . P[u] for j = nz-1 .. 0 (eq. 12,
- * PAPER.md:209-212): the adjoint detector columns at plane 0.  cuFFT; timed separately (bip_get_timing). */
+ * PAPER.md:209-212): the adjoint detector columns at plane 0.  Slice steps by the route of bip_set_fft_backend; timed
+ * separately (bip_get_timing). */
 BIP_API int32_t bip_build_S2(bip_ctx* ctx);
 
 /* Scan positions rho [n_rho][2] in pixels, any real value.  Builds the illumination matrix
@@ -272,8 +273,8 @@ BIP_API int32_t bip_cube_alg3(bip_ctx* ctx, int32_t edge_id, int32_t recon, int3
 BIP_API int32_t bip_set_scratch_budget(bip_ctx* ctx, size_t bytes);
 
 /* Route of the slice steps (bip_build_S2, ADVANCETO, PEELTO; plumbing, timed separately):
- *   BIP_FFT_NATIVE     the library's own fused fp32 slice step, three passes over a column (power-of-two grids 8..4096;
- *                      the default there);
+ *   BIP_FFT_NATIVE     the library's own fused fp32 slice step, three passes over a column -- two when steps follow one
+ *                      another on the same columns (power-of-two grids 8..4096; the default there);
  *   BIP_FFT_CUFFT_F64  cuFFT Z2Z on a double-precision workspace, columns rounded to c64 once per slice (any grid; the
  *                      default for grids that are not powers of two, and the A/B reference of the native route). */
 typedef enum { BIP_FFT_NATIVE = 0, BIP_FFT_CUFFT_F64 = 1 } bip_fft_backend;
