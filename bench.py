@@ -377,10 +377,10 @@ def run_alg3(args):
 
 
 def extra_legs(args):
-    """Short legs on other BASELINE.json configs, each in a fresh process after this one has released the GPU memory it
-    needs, embedded under "extra" of the main line (the driver parses the LAST line, which stays configs[1]).  Default:
-    configs[3] in the paper's own regime (FePt nanoparticle, PRISM f = 8 beam lists + crop mask) and the
-    FP16X3 arithmetic on the default workload."""
+    """Short legs on other BASELINE.json configs, each in a fresh process, embedded under "extra" of the main line (the driver
+    parses the LAST line, which stays configs[1]).  Default: configs[3] in the paper's own regime (FePt nanoparticle, PRISM
+    f = 8 beam lists + crop mask), the FP16X3 arithmetic on the default workload, Algorithm 3 on the
+    configs[4] geometry, and configs[2] (five edges in one plane loop, the largest config that fits one GPU)."""
     out = {}
     for spec in [x for x in args.extra.split(",") if x and x != "none"]:
         name, _, n = spec.partition(":")
@@ -497,7 +497,7 @@ def main():
                     "the default workload, none otherwise")
     args = ap.parse_args()
     if args.extra is None:
-        args.extra = "cfg4:256,fp16x3:16,alg3:2" if args.workload == "cfg2" and args.scale == 1 and args.precision == "fp16x4" else "none"
+        args.extra = "cfg4:256,fp16x3:16,alg3:2,cfg3:2" if args.workload == "cfg2" and args.scale == 1 and args.precision == "fp16x4" else "none"
     if args.impl == "reference":
         run_reference(args)
         return
