@@ -257,13 +257,17 @@ __device__ __forceinline__ uint32_t cluster_ctarank() {
 __device__ __forceinline__ void cluster_sync_all() {
   asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
-// arrive on the barrier at the same shared-memory offset in CTA `rank` of the cluster
+// arrive on the barrier at the same shared-memory offset in CTA `rank` of the cluster.  RELAXED: nothing these arrivals
+// publish goes through generic-proxy memory (operands land by bulk copy and are read by the tensor core; accumulators are
+// read with tcgen05.ld + tcgen05.wait::ld before the arrival), and a release at cluster scope costs a MEMBAR.ALL.GPU per
+// arrival -- in the peer's per-k-step "operands landed" forward that fence capped the pair at one k-step per ~1000 clocks
+// whatever the number of MMAs (profiles/r02_gemm2_probes.md)
 __device__ __forceinline__ void mbar_arrive_cluster(uint64_t* bar, uint32_t rank) {
   asm volatile(
       "{\n\t"
       ".reg .b32 ra;\n\t"
       "mapa.shared::cluster.u32 ra, %0, %1;\n\t"
-      "mbarrier.arrive.release.cluster.shared::cluster.b64 _, [ra];\n\t"
+      "mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [ra];\n\t"
       "}" ::"r"(smem_u32(bar)), "r"(rank)
       : "memory");
 }
