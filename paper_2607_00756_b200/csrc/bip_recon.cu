@@ -259,7 +259,7 @@ __global__ void __launch_bounds__(256) k_parent_rowmax(const float2* __restrict_
   if (lane == 0) pmax[(int64_t)a * n_par + p] = sqrtf(m);
 }
 
-__global__ void __launch_bounds__(256) k_recon_rows_sliced(const float2* __restrict__ D, int n_par, const int32_t* __restrict__ bh, int n_beams,
+__global__ void __launch_bounds__(256, 3) k_recon_rows_sliced(const float2* __restrict__ D, int n_par, const int32_t* __restrict__ bh, int n_beams,
                                     const int32_t* __restrict__ nn_idx, const float* __restrict__ nn_w, int max_nn, int carrier,
                                     int recon, const int32_t* __restrict__ origin, int w, int ny, int nx,
                                     const float2* __restrict__ rooty, const float2* __restrict__ rootx,
