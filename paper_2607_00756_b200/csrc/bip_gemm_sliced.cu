@@ -772,7 +772,7 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) k_sliced_contract(const SlPara
 // slice groups of the 8 rows of one k-group land in one contiguous 128-byte line (the blocked layout puts rows r .. r+7
 // of a k-group side by side): every store instruction writes whole lines.
 constexpr int QCH = 9;
-__global__ void __launch_bounds__(256) k_quantize_phi(const float2* __restrict__ Psi, int64_t psi_ld, int64_t psi_batch_stride,
+__global__ void __launch_bounds__(256, 4) k_quantize_phi(const float2* __restrict__ Psi, int64_t psi_ld, int64_t psi_batch_stride,
                                                       const float2* __restrict__ H, Sliced Phi, int n_rho, int rows_pad, int w2, int n_ch) {
   __shared__ float inv_s[8][QCH];
   __shared__ int s_max[8][QCH];                      // row maxima as bit patterns (non-negative floats order like ints)
