@@ -862,44 +862,53 @@ __global__ void __launch_bounds__(256) k_gather_rows_sliced(Sliced src, const in
   if (g == 0) dst.scale[(int64_t)atom * dst.scale_batch_stride + row] = s >= 0 ? src.scale[s] : 1.f;
 }
 
-// Crop mask (reading c19): the scan rows of every site, in ascending scan order.  One block per site walks
-// the scan list in chunks of 256 with an ordered block compaction.  fp64, the oracle's expression order:
+constexpr int CROP_THREADS = 1024;
+// Crop mask (reading c19): the scan rows of every site, in ascending scan order.  One block of 32 warps per site; warp w owns
+// the contiguous scans [w S, (w + 1) S), S = ceil(n_rho / 1024) * 32, and walks them 32 at a time (coalesced reads of the scan
+// list): a first sweep counts the scans inside the window, the 32 warp totals give every warp its offset, a second sweep writes
+// the rows with ballot-ordered offsets -- no block barrier inside the sweeps (the one-chunk-of-256-at-a-time version needed
+// three per chunk; each iteration is one L2 round trip, so the sweeps are latency-bound and want many warps).  fp64, the oracle's expression order:
 // d = ((rho - c + N/2) mod N) - N/2, inside iff |d_y| < N_y / (2 f_y) and |d_x| < N_x / (2 f_x).
-__global__ void __launch_bounds__(256) k_crop_rows(const double* __restrict__ rho, int n_rho, const int32_t* __restrict__ origin, int w,
+__global__ void __launch_bounds__(CROP_THREADS) k_crop_rows(const double* __restrict__ rho, int n_rho, const int32_t* __restrict__ origin, int w,
                                                    int ny, int nx, int fy, int fx, int32_t* __restrict__ row_idx, int64_t idx_stride,
                                                    int32_t* __restrict__ counts) {
-  __shared__ int warp_sum[8];
-  __shared__ int base;
-  const int atom = blockIdx.x, lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  __shared__ int warp_tot[CROP_THREADS / 32];
+  const int atom = blockIdx.x, t = threadIdx.x, lane = t & 31, wid = t >> 5;
   const double cy = (double)((origin[2 * atom] + w / 2) % ny), cx = (double)((origin[2 * atom + 1] + w / 2) % nx);
   const double hy = ny / (2.0 * fy), hx = nx / (2.0 * fx);
   int32_t* out = row_idx ? row_idx + (int64_t)atom * idx_stride : nullptr;   // NULL: count only
-  if (threadIdx.x == 0) base = 0;
+  const int S = ((n_rho + CROP_THREADS - 1) / CROP_THREADS) * 32, r0 = wid * S, r1 = min(n_rho, r0 + S);
+  // fmod(a, n) for a power-of-two n: a - n trunc(a (1 / n)), every step exact (a scaling, an integer, a difference whose bits are
+  // the low bits of a) and therefore bit-identical to fmod, at a tenth of its cost; any other n takes fmod itself
+  const bool pow2 = (ny & (ny - 1)) == 0 && (nx & (nx - 1)) == 0;
+  const double inv_ny = 1.0 / ny, inv_nx = 1.0 / nx;      // exact for powers of two: the quotient is a product (fp64 division costs ~30 instructions)
+  auto fmod_n = [&](double a, int n, double inv_n) { return pow2 ? a - (double)n * trunc(a * inv_n) : fmod(a, (double)n); };
+  auto inside = [&](int r) {
+    if (r >= r1) return false;
+    const double2 p = *reinterpret_cast<const double2*>(rho + 2 * (int64_t)r);
+    double dy = fmod_n(p.x - cy + ny / 2.0, ny, inv_ny);
+    double dx = fmod_n(p.y - cx + nx / 2.0, nx, inv_nx);
+    if (dy < 0) dy += ny;
+    if (dx < 0) dx += nx;
+    dy -= ny / 2.0; dx -= nx / 2.0;
+    return fabs(dy) < hy && fabs(dx) < hx;
+  };
+  int n = 0;
+  for (int r = r0 + lane; r < r0 + S; r += 32) n += __popc(__ballot_sync(0xffffffffu, inside(r)));
+  if (lane == 0) warp_tot[wid] = n;
   __syncthreads();
-  for (int r0 = 0; r0 < n_rho; r0 += 256) {
-    const int r = r0 + threadIdx.x;
-    bool in = false;
-    if (r < n_rho) {
-      double dy = fmod(rho[2 * (int64_t)r] - cy + ny / 2.0, (double)ny);
-      double dx = fmod(rho[2 * (int64_t)r + 1] - cx + nx / 2.0, (double)nx);
-      if (dy < 0) dy += ny;
-      if (dx < 0) dx += nx;
-      dy -= ny / 2.0; dx -= nx / 2.0;
-      in = fabs(dy) < hy && fabs(dx) < hx;
+  int off = 0, total = 0;
+  for (int k = 0; k < CROP_THREADS / 32; ++k) { if (k < wid) off += warp_tot[k]; total += warp_tot[k]; }
+  if (out) {
+    for (int r = r0 + lane; r < r0 + S; r += 32) {
+      const bool in = inside(r);
+      const unsigned m = __ballot_sync(0xffffffffu, in);
+      if (in) out[off + __popc(m & ((1u << lane) - 1u))] = r;
+      off += __popc(m);
     }
-    const unsigned m = __ballot_sync(0xffffffffu, in);
-    if (lane == 0) warp_sum[wid] = __popc(m);
-    __syncthreads();
-    int off = base;
-    for (int k = 0; k < wid; ++k) off += warp_sum[k];
-    if (in && out) out[off + __popc(m & ((1u << lane) - 1u))] = r;
-    __syncthreads();
-    if (threadIdx.x == 0) { int t = 0; for (int k = 0; k < 8; ++k) t += warp_sum[k]; base += t; }
-    __syncthreads();
+    for (int64_t i = total + t; i < idx_stride; i += CROP_THREADS) out[i] = -1;
   }
-  const int n = base;
-  if (out) for (int64_t i = n + threadIdx.x; i < idx_stride; i += 256) out[i] = -1;
-  if (threadIdx.x == 0) counts[atom] = n;
+  if (t == 0) counts[atom] = total;
 }
 
 template <int EPI, int FMT, bool PAIR, bool WIDE = false>
@@ -990,7 +999,7 @@ int32_t launch_gemm1_sliced(bip_ctx* ctx, const Gemm1SlArgs& a) {
 }
 
 int32_t launch_crop_rows(bip_ctx* ctx, const int32_t* origin_dev, int32_t n_atoms, int32_t w, int32_t* row_idx, int64_t idx_stride, int32_t* counts) {
-  k_crop_rows<<<(unsigned)n_atoms, 256, 0, ctx->stream>>>(ctx->rho_dev, ctx->n_rho, origin_dev, w, ctx->g.ny, ctx->g.nx, ctx->crop_fy,
+  k_crop_rows<<<(unsigned)n_atoms, CROP_THREADS, 0, ctx->stream>>>(ctx->rho_dev, ctx->n_rho, origin_dev, w, ctx->g.ny, ctx->g.nx, ctx->crop_fy,
                                                           ctx->crop_fx, row_idx, idx_stride, counts);
   BIP_CUDA(ctx, cudaGetLastError());
   ctx->timing.kernel_launches++;
