@@ -37,6 +37,34 @@ int32_t dev_alloc(bip_ctx* ctx, void** p, size_t bytes, const char* what) {
   return BIP_OK;
 }
 
+// Recycled device blocks for per-call objects: best fit among the context's released blocks (at most twice the request), else
+// a fresh cudaMalloc.  Released blocks are kept until bip_destroy.
+int32_t pool_alloc(bip_ctx* ctx, void** p, size_t bytes, const char* what) {
+  if (bytes == 0) bytes = 16;
+  int best = -1;
+  for (int i = 0; i < (int)ctx->pool_free.size(); ++i) {
+    const size_t sz = ctx->pool_free[i].second;
+    if (sz >= bytes && sz <= 2 * bytes + 256 && (best < 0 || sz < ctx->pool_free[best].second)) best = i;
+  }
+  if (best >= 0) {
+    *p = ctx->pool_free[best].first;
+    ctx->pool_size[*p] = ctx->pool_free[best].second;
+    ctx->pool_free.erase(ctx->pool_free.begin() + best);
+    return BIP_OK;
+  }
+  BIP_TRY(dev_alloc(ctx, p, bytes, what));
+  ctx->pool_size[*p] = bytes;
+  return BIP_OK;
+}
+
+void pool_release(bip_ctx* ctx, void* p) {
+  if (!p) return;
+  auto it = ctx->pool_size.find(p);
+  if (it == ctx->pool_size.end()) { cudaFree(p); return; }
+  ctx->pool_free.emplace_back(p, it->second);
+  ctx->pool_size.erase(it);
+}
+
 int32_t ensure(bip_ctx* ctx, DevBuf& b, size_t bytes, const char* what) {
   if (b.bytes >= bytes && b.p) return BIP_OK;
   if (b.p) { cudaStreamSynchronize(ctx->stream); cudaFree(b.p); b.p = nullptr; b.bytes = 0; }
@@ -126,6 +154,14 @@ static void free_illumination(bip_ctx* ctx) {
 template <class T>
 static int32_t upload(bip_ctx* ctx, T** dst, const T* src, size_t n, const char* what) {
   BIP_TRY(dev_alloc(ctx, (void**)dst, n * sizeof(T), what));
+  if (n) BIP_CUDA(ctx, cudaMemcpyAsync(*dst, src, n * sizeof(T), cudaMemcpyHostToDevice, ctx->stream));
+  return BIP_OK;
+}
+
+// the same into a recycled block (edge tables: registered and cleared once per end-to-end step)
+template <class T>
+static int32_t upload_pooled(bip_ctx* ctx, T** dst, const T* src, size_t n, const char* what) {
+  BIP_TRY(pool_alloc(ctx, (void**)dst, n * sizeof(T), what));
   if (n) BIP_CUDA(ctx, cudaMemcpyAsync(*dst, src, n * sizeof(T), cudaMemcpyHostToDevice, ctx->stream));
   return BIP_OK;
 }
@@ -736,8 +772,8 @@ int32_t bip_clear_edges(bip_ctx* ctx) {
   if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
   cudaStreamSynchronize(ctx->stream);
   for (Edge& e : ctx->edges) {
-    cudaFree(e.H_dev); cudaFree(e.hmax_dev); cudaFree(e.det_h_dev); cudaFree(e.nn_idx_dev); cudaFree(e.nn_w_dev);
-    cudaFree(e.bin_of_det_x_dev); cudaFree(e.bin_of_det_y_dev); cudaFree(e.origin_dev);
+    void* blocks[] = {e.H_dev, e.hmax_dev, e.det_h_dev, e.nn_idx_dev, e.nn_w_dev, e.bin_of_det_x_dev, e.bin_of_det_y_dev, e.origin_dev};
+    for (void* b : blocks) pool_release(ctx, b);
   }
   ctx->edges.clear();
   return BIP_OK;
@@ -756,6 +792,8 @@ int32_t bip_destroy(bip_ctx* ctx) {
                   ctx->Phi.p, ctx->R1s.p, ctx->R2s.p, ctx->Phis.p, ctx->Scl.p, ctx->Sync.p, ctx->Fields.p, ctx->D1p.p, ctx->Env.p, ctx->RowIdx.p, ctx->Acrop.p, ctx->Pmax.p, ctx->R1r.p, ctx->HR2.p, ctx->Mc.p, ctx->Ms.p, ctx->rho_dev};
   free_illumination(ctx);
   for (void* p : ptrs) if (p) cudaFree(p);
+  for (auto& b : ctx->pool_free) cudaFree(b.first);
+  for (auto& b : ctx->pool_size) cudaFree(b.first);
   cudaGetLastError();
   delete ctx;
   return BIP_OK;
@@ -882,20 +920,20 @@ int32_t bip_add_edge(bip_ctx* ctx, int32_t n_atoms, const int32_t* slice, const 
     bx[d] = (int32_t)(std::lower_bound(e.binx.begin(), e.binx.end(), bx[d]) - e.binx.begin());
     by[d] = (int32_t)(std::lower_bound(e.biny.begin(), e.biny.end(), by[d]) - e.biny.begin());
   }
-  BIP_TRY(upload(ctx, (float**)&e.H_dev, H, 2 * (size_t)n_ch * w * w, "H windows"));
+  BIP_TRY(upload_pooled(ctx, (float**)&e.H_dev, H, 2 * (size_t)n_ch * w * w, "H windows"));
   std::vector<float> hmax(n_ch, 0.f);
   for (int n = 0; n < n_ch; ++n)
     for (size_t s = 0; s < (size_t)w * w; ++s) {
       const float* h = H + 2 * ((size_t)n * w * w + s);
       hmax[n] = std::max(hmax[n], 1.0001f * std::hypot(h[0], h[1]));
     }
-  BIP_TRY(upload(ctx, &e.hmax_dev, hmax.data(), (size_t)n_ch, "H maxima"));
-  BIP_TRY(upload(ctx, &e.det_h_dev, det_h, 2 * (size_t)n_det, "detector beams"));
-  BIP_TRY(upload(ctx, &e.nn_idx_dev, e.w2_idx.data(), e.w2_idx.size(), "w2 indices"));
-  BIP_TRY(upload(ctx, &e.nn_w_dev, e.w2_w.data(), e.w2_w.size(), "w2 weights"));
-  BIP_TRY(upload(ctx, &e.bin_of_det_x_dev, bx.data(), (size_t)n_det, "qEELS bins"));
-  BIP_TRY(upload(ctx, &e.bin_of_det_y_dev, by.data(), (size_t)n_det, "qEELS bins"));
-  BIP_TRY(upload(ctx, &e.origin_dev, e.origin.data(), 2 * (size_t)n_atoms, "window origins"));
+  BIP_TRY(upload_pooled(ctx, &e.hmax_dev, hmax.data(), (size_t)n_ch, "H maxima"));
+  BIP_TRY(upload_pooled(ctx, &e.det_h_dev, det_h, 2 * (size_t)n_det, "detector beams"));
+  BIP_TRY(upload_pooled(ctx, &e.nn_idx_dev, e.w2_idx.data(), e.w2_idx.size(), "w2 indices"));
+  BIP_TRY(upload_pooled(ctx, &e.nn_w_dev, e.w2_w.data(), e.w2_w.size(), "w2 weights"));
+  BIP_TRY(upload_pooled(ctx, &e.bin_of_det_x_dev, bx.data(), (size_t)n_det, "qEELS bins"));
+  BIP_TRY(upload_pooled(ctx, &e.bin_of_det_y_dev, by.data(), (size_t)n_det, "qEELS bins"));
+  BIP_TRY(upload_pooled(ctx, &e.origin_dev, e.origin.data(), 2 * (size_t)n_atoms, "window origins"));
   BIP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));     // host sources may go away after return
   ctx->edges.push_back(std::move(e));
   if (edge_id) *edge_id = (int32_t)ctx->edges.size() - 1;
@@ -931,7 +969,7 @@ int32_t bip_map_host(bip_ctx* ctx, int32_t edge_id, int32_t mode, int32_t recon,
   if (!ctx) return fail(nullptr, BIP_ERR_INVALID, "ctx is NULL");
   if (!out_host) return fail(ctx, BIP_ERR_INVALID, "bip_map_host: output is NULL");
   void* d = nullptr;
-  BIP_TRY(dev_alloc(ctx, &d, out_bytes, "host-call output staging"));
+  BIP_TRY(pool_alloc(ctx, &d, out_bytes, "host-call output staging"));
   int32_t st = bip_map(ctx, edge_id, mode, recon, precision, d, out_bytes);
   if (st == BIP_OK) {
     cudaError_t e = cudaMemcpyAsync(out_host, d, out_bytes, cudaMemcpyDeviceToHost, ctx->stream);
@@ -939,7 +977,7 @@ int32_t bip_map_host(bip_ctx* ctx, int32_t edge_id, int32_t mode, int32_t recon,
     if (e != cudaSuccess) st = fail(ctx, BIP_ERR_CUDA, "bip_map_host: %s", cudaGetErrorString(e));
   }
   cudaStreamSynchronize(ctx->stream);
-  cudaFree(d);
+  pool_release(ctx, d);
   return st;
 }
 

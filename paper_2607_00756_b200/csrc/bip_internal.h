@@ -132,6 +132,10 @@ struct bip_ctx {
   float4 *fft_rooty = nullptr, *fft_rootx = nullptr, *fft_Ey = nullptr, *fft_Ex = nullptr;   // double-float (hi, lo) twiddles and the two 1-D factors of the propagator
   int32_t *fft_permy = nullptr, *fft_permx = nullptr;   // true frequency index of every stored (digit-reversed) position
   int fft_lines = 0, fft_cols = 0;
+  // device blocks of per-call objects (edge tables, the staging buffer of bip_map_host), recycled instead of freed: a
+  // cudaFree / cudaMalloc pair per bip_add_edge / bip_clear_edges cost up to 0.8 s of driver time in the end-to-end step
+  std::vector<std::pair<void*, size_t>> pool_free;
+  std::map<void*, size_t> pool_size;
   FftPending fft_pending;          // inverse row pass owed by the last native slice step (fft_flush)
   bool fft_native = false;         // route in use (bip_set_fft_backend)
   float2 *S1 = nullptr, *S2 = nullptr;
@@ -210,6 +214,8 @@ int32_t ms_step_S2(bip_ctx* ctx, int32_t j, int dir);
 int32_t ms_exit_step(bip_ctx* ctx, float2* fields, int n, int32_t j);
 // out[rho][ky][kx] += sum_n |F fields[rho][n]|^2 / G (unitary F, corner-origin order); fields are destroyed
 int32_t ms_detect(bip_ctx* ctx, float2* fields, int n_rho, int n_ch, float* out);
+int32_t pool_alloc(bip_ctx* ctx, void** p, size_t bytes, const char* what);   // recycled device block (bip_api.cu)
+void pool_release(bip_ctx* ctx, void* p);
 int32_t ms_flush(bip_ctx* ctx);       // end of a sequence of slice steps: every column is complete in memory afterwards
 
 // ---- native fused slice step for power-of-two grids (bip_fft.cu) ----
