@@ -332,6 +332,24 @@ BIP_API int32_t bip_copy_S(bip_ctx* ctx, int32_t which, int32_t p0, int32_t np, 
 BIP_API int32_t bip_debug_reconstruct(bip_ctx* ctx, int32_t edge_id, int32_t atom, int32_t which, int32_t recon,
                               void* out_host);
 
+/* The ONE entry point that allocates nothing: for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it).  Same result as bip_debug_reconstruct -- the reconstructed windows of one site at
+ * the current plane (steps a1-a2 / a6; eq. 15, or eq. 11): which = 1: S1^b|Omega c64
+ * [n_ap][w*w]; which = 2: S2^d|Omega c64 [n_det][w*w] -- but written to the caller's DEVICE buffer out_dev (out_bytes =
+ * rows * w * w * 8, checked), and with the intermediate de-tilted parent windows D[p][s] in a static device array of
+ * BIP_NOALLOC_SCRATCH_BYTES inside the library instead of an allocated buffer.
+ *   - n_parent * w * w * 8 bytes must fit the array (n_parent = the S1 / S2 parent count): larger requests fail with
+ *     BIP_ERR_UNSUPPORTED and touch nothing.  Every GPU that loads the library holds the array until the process exits.
+ *   - The call makes no cudaMalloc / cudaFree and calls no allocating routine; it enqueues two kernels on the context's
+ *     stream and returns without synchronising (the caller syncs before reading out_dev).  The first call on a device
+ *     resolves the array's address (cudaGetSymbolAddress): make one call before starting a capture.
+ *   - Every call on a GPU, from any context or stream, shares the array, which keeps the last call's contents (nothing in it
+ *     has to start at zero: each call overwrites what it reads).  Calls that overlap on the GPU race on it: serialise them.
+ *   - The plane cursor is not moved (bip_seek_plane first); edge and atom as registered by bip_add_edge. */
+#define BIP_NOALLOC_SCRATCH_BYTES (4u << 20)
+BIP_API int32_t bip_reconstruct_noalloc(bip_ctx* ctx, int32_t edge_id, int32_t atom, int32_t which, int32_t recon, void* out_dev,
+                                        size_t out_bytes);
+
 BIP_API int32_t bip_get_timing(const bip_ctx* ctx, bip_timing* out);
 
 /* Library / device description ("libbip <version>; device <name> sm_XY; SMs n"); never NULL. */

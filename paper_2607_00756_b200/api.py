@@ -67,7 +67,7 @@ ABI_SYMBOLS = (
     "bip_seek_plane", "bip_copy_S", "bip_debug_reconstruct", "bip_get_timing", "bip_version", "bip_prism_subsample",
     "bip_set_crop", "bip_set_association", "bip_prism_coeffs", "bip_partition", "bip_set_scratch_budget", "bip_allow_tf32x3",
     "bip_get_parents", "bip_get_weights", "bip_set_fft_backend", "bip_cube_alg3", "bip_set_focal", "bip_get_focal_distance",
-    "bip_set_transmission", "bip_set_accumulate",
+    "bip_set_transmission", "bip_set_accumulate", "bip_reconstruct_noalloc",
 )
 
 _lib: Optional[C.CDLL] = None
@@ -431,6 +431,19 @@ class Context:
         rows = self.n_ap if which == 1 else n_det
         out = np.empty((rows, w * w), dtype=np.complex64)
         self._ck(self._lib.bip_debug_reconstruct(self._ctx, edge_id, atom, which, recon, C.c_void_p(out.ctypes.data)))
+        return out
+
+    def reconstruct_noalloc(self, edge_id: int, atom: int, which: int, recon: int = RECON_LINEAR, out=None):
+        """bip_reconstruct_noalloc: as debug_reconstruct, into the caller's DEVICE tensor ``out`` (complex64 [rows][w*w]; made
+        here when None -- the library itself allocates nothing), enqueued on the context's stream without synchronising."""
+        import torch
+        n_at, n_ch, w, n_det = self._edges[edge_id]
+        rows = self.n_ap if which == 1 else n_det
+        if out is None:
+            out = torch.empty((rows, w * w), dtype=torch.complex64, device="cuda")
+        assert out.is_cuda and out.is_contiguous() and out.dtype == torch.complex64
+        self._ck(self._lib.bip_reconstruct_noalloc(self._ctx, edge_id, atom, which, recon, C.c_void_p(out.data_ptr()),
+                                                   C.c_size_t(out.numel() * out.element_size())))
         return out
 
     def get_timing(self) -> dict:

@@ -23,7 +23,7 @@ LIB = os.path.join(HERE, "libbip.so")
 CUDA_HOME = os.environ.get("CUDA_HOME", "/usr/local/cuda")
 NVCC = os.path.join(CUDA_HOME, "bin", "nvcc")
 
-SOURCES = ["bip_api.cu", "bip_multislice.cu", "bip_fft.cu", "bip_focal.cu", "bip_recon.cu", "bip_gemm_simt.cu", "bip_gemm_tc.cu", "bip_gemm_sliced.cu", "bip_geometry.cpp"]
+SOURCES = ["bip_api.cu", "bip_multislice.cu", "bip_fft.cu", "bip_focal.cu", "bip_recon.cu", "bip_gemm_simt.cu", "bip_gemm_tc.cu", "bip_gemm_sliced.cu", "bip_noalloc.cu", "bip_geometry.cpp"]
 COMMON = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
           "-Xcompiler", "-fPIC,-fvisibility=hidden,-ffp-contract=off,-Wall,-Wno-unknown-pragmas", "-I", os.path.join(HERE, "..", "include")]
 
